@@ -1,0 +1,211 @@
+/*
+ * kvarn.h -- C ABI of the KVarN hot path for NVIDIA B200 (sm_100a).
+ *
+ * KVarN (arxiv/paper_2606_03458; cited as P:<line> of PAPER.md) compresses the
+ * KV cache tile by tile: every (head_dim=128 x 128-token) tile of one KV head
+ * is Hadamard-rotated along head_dim (Fig. 2), variance-normalised
+ * along both axes by Algorithm 1 "VarN", quantised by
+ * asymmetric round-to-nearest -- K per channel, V per token, Eq. 1 --
+ * and stored as packed 2-bit (or 4-bit) codes plus, per 128 elements, two FP8
+ * scales and one FP16 zero-point = 2.25 bit/element.  Decoding reads
+ * that cache directly (P:9): kvarn_decode_attention computes
+ * softmax(q K^T * sm_scale) V over [dequantised chunks ; raw residual tokens]
+ * without ever materialising a dequantised cache.
+ *
+ * Conventions
+ *   - "DEVICE" pointers are CUDA device memory owned by the caller; "HOST"
+ *     pointers are ordinary (preferably pinned) host memory.  The library
+ *     allocates no device memory, keeps no global state and never synchronises
+ *     the device: every call only enqueues work on the caller's `stream`
+ *     (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *   - All calls return a kvarn_status (0 = OK, negative = error); nothing is
+ *     enqueued when a negative status is returned.  No C++ exception crosses
+ *     this boundary.  Non-finite inputs give undefined codes but never fault.
+ *   - A "tile" is 128 tokens x 128 channels of ONE KV head, row-major
+ *     [token][channel], of K or of V.  A "record" is the stored form of one
+ *     tile; its internal packing is opaque (use kvarn_unpack_record_host).
+ */
+#ifndef KVARN_H_
+#define KVARN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define KVARN_API __attribute__((visibility("default")))
+#else
+#define KVARN_API
+#endif
+
+#define KVARN_HEAD_DIM 128
+#define KVARN_CHUNK 128
+#define KVARN_MAX_ITERS 16
+
+typedef enum {
+  KVARN_OK = 0,
+  KVARN_INVALID_ARG = -1,         /* null pointer, non-positive size, Hq % Hkv != 0 */
+  KVARN_UNSUPPORTED = -2,         /* head_dim/chunk != 128, bits not in {2,4}, g not in 1..8, dtype */
+  KVARN_MISALIGNED = -3,          /* a pointer or stride is not 16-byte aligned */
+  KVARN_WORKSPACE_TOO_SMALL = -4, /* ws_bytes < kvarn_decode_workspace_bytes(...) */
+  KVARN_CAPACITY = -5,            /* host-checkable capacity bound violated */
+  KVARN_CUDA = -6                 /* cudaGetLastError() after a launch / copy was not cudaSuccess */
+} kvarn_status;
+
+typedef enum { KVARN_BF16 = 0, KVARN_F32 = 1 } kvarn_dtype;
+typedef enum { KVARN_KIND_K = 0, KVARN_KIND_V = 1 } kvarn_kind;
+
+/* Method parameters (POD, caller-filled; kvarn_default_params gives the paper's). */
+typedef struct {
+  int32_t head_dim;  /* must be 128 */
+  int32_t chunk;     /* tokens per quantisation group G; must be 128 */
+  int32_t bits;      /* 2 (paper) or 4 */
+  int32_t iters;     /* Algorithm 1's K; 8 in Sec. 4.2; 0..KVARN_MAX_ITERS */
+  float var_min;     /* c_min of Alg. 1: lower clamp on variances; default 1e-8 */
+  float var_max;     /* c_max of Alg. 1; default 1e8 */
+  float log_lo;      /* lower clamp of the log-scales, -0.3 */
+  float log_hi;      /* upper clamp of the log-scales, 10.0 */
+  int32_t rotate_k;  /* 1: Hadamard-rotate K tiles (and q inside decode) */
+  int32_t rotate_v;  /* 1: Hadamard-rotate V tiles (and un-rotate the output) */
+  int32_t in_dtype;  /* kvarn_dtype of K, V, q and of the residual window */
+  int32_t out_dtype; /* kvarn_dtype of the attention output */
+  int32_t splits;    /* decode split-K factor over chunks; 0 = choose automatically */
+  int32_t reserved;
+} kvarn_params;
+
+/* Byte layout of one record (fixed by bits).  codes: K records hold one row
+ * per TOKEN (128 channels), V records one row per CHANNEL (128 tokens).
+ * s1 = FP8-E4M3 absorbed scale of the RTN group (K: per channel, V: per token),
+ * s2 = FP8-E4M3 second (Sinkhorn) scale of the other axis, z = FP16 zero-point
+ * of the RTN group (Eq. 1: x_dq = (code + z) * s1 * s2). */
+typedef struct {
+  size_t record_bytes; /* 4608 at 2-bit, 8704 at 4-bit (=> 2.25 / 4.25 bit per element) */
+  size_t codes_off, codes_bytes;
+  size_t s1_off, s2_off, z_off; /* 128 x u8, 128 x u8, 128 x f16 */
+} kvarn_layout_info;
+
+/* The cache of one attention layer (quantised body of 128-token groups
+ * followed by the trailing not-yet-quantised tokens).  All DEVICE pointers. */
+typedef struct {
+  void* k_records;      /* [B][Hkv][max_chunks][record_bytes], 16-B aligned */
+  void* v_records;      /* same shape */
+  void* k_resid;        /* [B][Hkv][128][128] in_dtype: raw (un-rotated) residual tokens */
+  void* v_resid;        /* same shape */
+  int32_t* seq_lens;    /* [B] tokens held per sequence: chunks = len/128, residual = len%128 */
+  int32_t* ticket;      /* [B] scratch for kvarn_append, zero-initialised by the caller once */
+  int32_t B, Hkv, max_chunks;
+  int32_t reserved;
+} kvarn_cache;
+
+/* Optional per-tile debug outputs of the quantizer (all DEVICE, each nullable).
+ * Index [kind][tile] with kind 0 = K, 1 = V.  Values are the fp32 numbers
+ * BEFORE FP8/FP16 storage rounding, so tests can compare against the oracle at
+ * the iterate the kernel kept (Alg. 1 line 18 is degenerate between iterates
+ * whose imbalance agrees to rounding). */
+typedef struct {
+  int32_t* k_best; /* [2][n_tiles]            iterate kept by the "<=" rule (0..iters) */
+  float* imb;      /* [2][n_tiles][KVARN_MAX_ITERS+1] imbalance I_k, k = 0..iters */
+  float* aux_f32;  /* [2][n_tiles][3][128]    s1, s2, z as fp32 (indexing as in the record) */
+} kvarn_debug;
+
+KVARN_API void kvarn_default_params(kvarn_params* p, int32_t bits);
+KVARN_API const char* kvarn_status_string(int status);
+KVARN_API int kvarn_version(void);
+
+/* Record layout for p->bits.  Returns KVARN_UNSUPPORTED for other bit widths. */
+KVARN_API int kvarn_layout(const kvarn_params* p, kvarn_layout_info* out);
+
+/* Bytes of DEVICE workspace kvarn_decode_attention needs for this shape. */
+KVARN_API size_t kvarn_decode_workspace_bytes(const kvarn_params* p, int32_t B, int32_t Hq, int32_t Hkv,
+                                    int32_t max_chunks);
+
+/*
+ * kvarn_quantize_chunk -- the write path for a batch of tiles in ONE launch
+ * (Fig. 2: rotate -> VarN -> RTN -> store codes + scale + zero + second
+ * scale).  Tile i of K is the 128x128 block at k + i*tile_stride (elements of
+ * in_dtype), its token t at + t*tok_stride, channels contiguous; likewise V.
+ * Record i is written at k_rec + i*rec_stride (bytes) / v_rec + i*rec_stride.
+ *   k, v        DEVICE, in_dtype, 16-B aligned; strides multiples of 8 elements
+ *   k_rec,v_rec DEVICE, 16-B aligned; rec_stride >= record_bytes, multiple of 16
+ *   dbg         nullable
+ * Either of (k, k_rec) or (v, v_rec) may be NULL to quantise only one kind.
+ */
+KVARN_API int kvarn_quantize_chunk(const kvarn_params* p, const void* k, const void* v, int64_t n_tiles,
+                         int64_t tile_stride, int64_t tok_stride, void* k_rec, void* v_rec,
+                         int64_t rec_stride, const kvarn_debug* dbg, void* stream);
+
+/*
+ * kvarn_prefill -- bulk-load a cache: quantise the first floor(n_tok/128)
+ * chunks of every (sequence, KV head) of k, v = [B][Hkv][n_tok][128] into the
+ * cache's records, copy the remaining n_tok%128 tokens into the residual window
+ * and set seq_lens[b] = n_tok.  Same kernel as kvarn_quantize_chunk.
+ */
+KVARN_API int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, const void* k, const void* v,
+                  int32_t n_tok, void* stream);
+
+/*
+ * kvarn_append -- on-the-fly compression during decoding (P:17, P:53, P:83,
+ * P:350): append ONE new token per sequence.  k_new, v_new = [B][Hkv][128]
+ * in_dtype (DEVICE).  The token goes to residual slot len%128; a residual that
+ * thereby reaches 128 tokens is quantised at once into chunk slot len/128 (bit
+ * for bit what kvarn_quantize_chunk gives on those 128 tokens) and the residual
+ * becomes empty.  seq_lens[b] is read and advanced ON DEVICE (no host round
+ * trip).  A sequence already holding max_chunks*128 + 127 tokens is left
+ * unchanged (its token is dropped); the caller bounds lengths on the host.
+ */
+KVARN_API int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_new,
+                 const void* v_new, void* stream);
+
+/*
+ * kvarn_decode_attention -- out[b][h] = softmax(q[b][h] K^T * sm_scale) V over
+ * all seq_lens[b] tokens of KV head h / (Hq/Hkv): the quantised chunks, read as
+ * packed codes + scales + zero-points (Eq. 1 with the second scale fused,
+ * P:45), then the raw residual window.  The Hadamard
+ * rotation and the per-channel scales are folded into q and the output.
+ *   q    DEVICE [B][Hq][128] in_dtype          out  DEVICE [B][Hq][128] out_dtype
+ *   ws   DEVICE scratch of >= kvarn_decode_workspace_bytes(...) bytes, 16-B aligned
+ * A sequence of length 0 yields zeros.  Hq/Hkv must be in 1..8.
+ */
+KVARN_API int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                           int32_t Hq, float sm_scale, void* out, void* ws, size_t ws_bytes,
+                           void* stream);
+
+/*
+ * Host-buffer forms (end-to-end measurement; HOST pointers in, HOST out).
+ * They copy host->device into caller-provided DEVICE staging, run the device
+ * call above and copy the result back, all enqueued on `stream`; the caller
+ * synchronises the stream before reading the host outputs.
+ *   kvarn_quantize_chunk_host: k_host, v_host contiguous [n_tiles][128][128];
+ *     dev_in_k / dev_in_v DEVICE staging of the same size; dev_rec_k / dev_rec_v
+ *     DEVICE records [n_tiles][record_bytes] (kept: they are the cache);
+ *     k_rec_host / v_rec_host nullable HOST copies of the records.
+ *   kvarn_decode_attention_host: q_host [B][Hq][128] -> out_host [B][Hq][128];
+ *     dev_q / dev_out DEVICE staging.
+ */
+KVARN_API int kvarn_quantize_chunk_host(const kvarn_params* p, const void* k_host, const void* v_host,
+                              int64_t n_tiles, void* dev_in_k, void* dev_in_v, void* dev_rec_k,
+                              void* dev_rec_v, void* k_rec_host, void* v_rec_host, void* stream);
+KVARN_API int kvarn_decode_attention_host(const kvarn_params* p, const kvarn_cache* cache,
+                                const void* q_host, int32_t Hq, float sm_scale, void* out_host,
+                                void* dev_q, void* dev_out, void* ws, size_t ws_bytes,
+                                void* stream);
+
+/*
+ * Test hooks (pure host code, HOST pointers): convert one record to / from the
+ * canonical form  codes[t][c] (u8, 128x128, token-major for BOTH kinds),
+ * s1[128], s2[128], z[128] as fp32 (exact values of the stored FP8/FP16).
+ * s1 and z are indexed by the RTN group (K: channel, V: token), s2 by the
+ * other axis.  pack rounds s1/s2 to FP8-E4M3 and z to FP16 (RNE, saturating).
+ */
+KVARN_API int kvarn_unpack_record_host(const kvarn_params* p, int32_t kind, const void* record,
+                             uint8_t* codes, float* s1, float* s2, float* z);
+KVARN_API int kvarn_pack_record_host(const kvarn_params* p, int32_t kind, const uint8_t* codes,
+                           const float* s1, const float* s2, const float* z, void* record);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KVARN_H_ */

@@ -1,0 +1,430 @@
+// C-ABI entry points of libkvarn (include/kvarn.h): argument validation, kernel
+// launches on the caller's stream, host-side record pack/unpack test hooks.
+#include <cstdio>
+#include <cstring>
+
+#include "kvarn_common.cuh"
+#include "kvarn_decode_ref.cuh"
+#include "kvarn_quantize.cuh"
+
+namespace kvarn {
+
+// ------------------------------------------------------------------ kernels
+struct QuantArgs {
+  const void* in[2];
+  uint8_t* rec[2];
+  long long n_inner;
+  long long in_outer_stride, in_tile_stride, tok_stride;  // elements
+  long long rec_outer_stride, rec_stride;                 // bytes
+  long long n_tiles;
+  int kind_base;
+  int rotate[2];
+  VarnConsts vc;
+  int32_t* dbg_kbest;
+  float* dbg_imb;
+  float* dbg_aux;
+};
+
+template <int BITS, typename InT>
+__global__ void __launch_bounds__(256, 2) quantize_kernel(const QuantArgs A) {
+  __shared__ QuantSmem<BITS> sm;
+  const int kind = A.kind_base + blockIdx.y;
+  const long long tile = blockIdx.x;
+  const long long outer = tile / A.n_inner, inner = tile - outer * A.n_inner;
+  const InT* src = reinterpret_cast<const InT*>(A.in[kind]) + outer * A.in_outer_stride +
+                   inner * A.in_tile_stride;
+  uint8_t* dst = A.rec[kind] + outer * A.rec_outer_stride + inner * A.rec_stride;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int c0 = 8 * (lane & 15), t0 = 16 * warp + 8 * (lane >> 4);
+  float2 x[8][4];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) load_row8<InT>(src + (long long)(t0 + i) * A.tok_stride + c0, x[i]);
+  QuantDebug dbg;
+  dbg.k_best = A.dbg_kbest ? A.dbg_kbest + (long long)kind * A.n_tiles : nullptr;
+  dbg.imb = A.dbg_imb ? A.dbg_imb + (long long)kind * A.n_tiles * (KVARN_MAX_ITERS + 1) : nullptr;
+  dbg.aux = A.dbg_aux ? A.dbg_aux + (long long)kind * A.n_tiles * 384 : nullptr;
+  quantize_tile<BITS>(x, kind, A.rotate[kind] != 0, A.vc, dst, dbg, tile, sm);
+}
+
+struct AppendArgs {
+  uint8_t* rec[2];
+  void* resid[2];
+  const void* tok[2];
+  int32_t* seq_lens;
+  int32_t* ticket;
+  int B, Hkv, max_chunks;
+  int rotate[2];
+  VarnConsts vc;
+};
+
+// One CTA per (sequence, KV head, kind).  The decision to quantise is taken on
+// the device from seq_lens (no host round trip).
+template <int BITS, typename InT>
+__global__ void __launch_bounds__(256, 2) append_kernel(const AppendArgs A) {
+  __shared__ QuantSmem<BITS> sm;
+  const int kind = blockIdx.y, bh = blockIdx.x, b = bh / A.Hkv;
+  const int tid = threadIdx.x;
+  const int len = A.seq_lens[b];
+  const int r = len & 127, chunk = len >> 7;
+  const bool full = (r == 127);
+  const bool can_store = full ? (chunk < A.max_chunks) : (chunk <= A.max_chunks);
+  InT* resid = reinterpret_cast<InT*>(A.resid[kind]) + (size_t)bh * G * D;
+  const InT* tok = reinterpret_cast<const InT*>(A.tok[kind]) + (size_t)bh * D;
+  if (can_store && !full) {
+    if (tid < D) resid[(size_t)r * D + tid] = tok[tid];
+  } else if (can_store) {
+    const int lane = tid & 31, warp = tid >> 5;
+    const int c0 = 8 * (lane & 15), t0 = 16 * warp + 8 * (lane >> 4);
+    float2 x[8][4];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int t = t0 + i;
+      const InT* row = (t == 127) ? tok : resid + (size_t)t * D;
+      load_row8<InT>(row + c0, x[i]);
+    }
+    uint8_t* dst = A.rec[kind] + ((size_t)bh * A.max_chunks + chunk) * record_bytes(BITS);
+    QuantDebug dbg{nullptr, nullptr, nullptr};
+    quantize_tile<BITS>(x, kind, A.rotate[kind] != 0, A.vc, dst, dbg, 0, sm);
+  }
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    const int old = atomicAdd(&A.ticket[b], 1);
+    if (old == 2 * A.Hkv - 1) {  // last CTA of this sequence: every CTA has read seq_lens[b]
+      A.ticket[b] = 0;
+      if (can_store) A.seq_lens[b] = len + 1;
+    }
+  }
+}
+
+struct TailArgs {
+  const void* in[2];
+  void* resid[2];
+  int32_t* seq_lens;
+  int B, Hkv, n_tok, n_full;
+};
+template <typename InT>
+__global__ void prefill_tail_kernel(const TailArgs A) {
+  const int bh = blockIdx.x, kind = blockIdx.y;
+  const int r = A.n_tok - A.n_full * G;
+  const InT* src = reinterpret_cast<const InT*>(A.in[kind]) + ((size_t)bh * A.n_tok + (size_t)A.n_full * G) * D;
+  InT* dst = reinterpret_cast<InT*>(A.resid[kind]) + (size_t)bh * G * D;
+  for (int i = threadIdx.x; i < r * D; i += blockDim.x) dst[i] = src[i];
+  if (kind == 0 && threadIdx.x == 0 && (bh % A.Hkv) == 0) A.seq_lens[bh / A.Hkv] = A.n_tok;
+}
+
+// ------------------------------------------------------------------ host helpers
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+static int check_params(const kvarn_params* p) {
+  if (!p) return KVARN_INVALID_ARG;
+  if (p->head_dim != D || p->chunk != G) return KVARN_UNSUPPORTED;
+  if (p->bits != 2 && p->bits != 4) return KVARN_UNSUPPORTED;
+  if (p->iters < 0 || p->iters > KVARN_MAX_ITERS) return KVARN_INVALID_ARG;
+  if (p->in_dtype != KVARN_BF16 && p->in_dtype != KVARN_F32) return KVARN_UNSUPPORTED;
+  if (p->out_dtype != KVARN_BF16 && p->out_dtype != KVARN_F32) return KVARN_UNSUPPORTED;
+  if (!(p->var_min > 0.f) || !(p->var_max >= p->var_min) || !(p->log_hi >= p->log_lo)) return KVARN_INVALID_ARG;
+  return KVARN_OK;
+}
+
+static VarnConsts varn_consts(const kvarn_params* p) {
+  VarnConsts vc;
+  vc.iters = p->iters; vc.var_min = p->var_min; vc.var_max = p->var_max;
+  vc.log_lo = p->log_lo; vc.log_hi = p->log_hi;
+  return vc;
+}
+
+static int last_cuda() { return cudaGetLastError() == cudaSuccess ? KVARN_OK : KVARN_CUDA; }
+
+static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kinds, cudaStream_t st) {
+  if (A.n_tiles == 0) return KVARN_OK;
+  dim3 grid((unsigned)A.n_tiles, (unsigned)n_kinds), block(256);
+  const bool f32 = p->in_dtype == KVARN_F32;
+  if (p->bits == 2) {
+    if (f32) quantize_kernel<2, float><<<grid, block, 0, st>>>(A);
+    else quantize_kernel<2, __nv_bfloat16><<<grid, block, 0, st>>>(A);
+  } else {
+    if (f32) quantize_kernel<4, float><<<grid, block, 0, st>>>(A);
+    else quantize_kernel<4, __nv_bfloat16><<<grid, block, 0, st>>>(A);
+  }
+  return last_cuda();
+}
+
+static int auto_splits(const kvarn_params* p, int B, int Hkv, int max_chunks) {
+  if (p->splits > 0) return p->splits < max_chunks ? p->splits : (max_chunks > 0 ? max_chunks : 1);
+  const int bh = B * Hkv;
+  int s = (148 * 4 + bh - 1) / bh;
+  if (s > 64) s = 64;
+  if (s > max_chunks) s = max_chunks;
+  if (s < 1) s = 1;
+  return s;
+}
+
+template <int BITS, typename InT>
+static void launch_decode_ref(const DecodeArgs& A, int g, cudaStream_t st) {
+  dim3 grid(A.B * A.Hkv, A.splits), block(128);
+  switch (g) {
+    case 1: decode_partial_ref_kernel<BITS, 1, InT><<<grid, block, 0, st>>>(A); break;
+    case 2: decode_partial_ref_kernel<BITS, 2, InT><<<grid, block, 0, st>>>(A); break;
+    case 3: decode_partial_ref_kernel<BITS, 3, InT><<<grid, block, 0, st>>>(A); break;
+    case 4: decode_partial_ref_kernel<BITS, 4, InT><<<grid, block, 0, st>>>(A); break;
+    case 5: decode_partial_ref_kernel<BITS, 5, InT><<<grid, block, 0, st>>>(A); break;
+    case 6: decode_partial_ref_kernel<BITS, 6, InT><<<grid, block, 0, st>>>(A); break;
+    case 7: decode_partial_ref_kernel<BITS, 7, InT><<<grid, block, 0, st>>>(A); break;
+    default: decode_partial_ref_kernel<BITS, 8, InT><<<grid, block, 0, st>>>(A); break;
+  }
+}
+
+}  // namespace kvarn
+
+using namespace kvarn;
+
+// ------------------------------------------------------------------ C ABI
+extern "C" {
+
+void kvarn_default_params(kvarn_params* p, int32_t bits) {
+  if (!p) return;
+  memset(p, 0, sizeof(*p));
+  p->head_dim = D; p->chunk = G; p->bits = bits; p->iters = 8;
+  p->var_min = 1e-8f; p->var_max = 1e8f; p->log_lo = -0.3f; p->log_hi = 10.0f;
+  p->rotate_k = 1; p->rotate_v = 1;
+  p->in_dtype = KVARN_BF16; p->out_dtype = KVARN_F32; p->splits = 0;
+}
+
+const char* kvarn_status_string(int status) {
+  switch (status) {
+    case KVARN_OK: return "KVARN_OK";
+    case KVARN_INVALID_ARG: return "KVARN_INVALID_ARG";
+    case KVARN_UNSUPPORTED: return "KVARN_UNSUPPORTED";
+    case KVARN_MISALIGNED: return "KVARN_MISALIGNED";
+    case KVARN_WORKSPACE_TOO_SMALL: return "KVARN_WORKSPACE_TOO_SMALL";
+    case KVARN_CAPACITY: return "KVARN_CAPACITY";
+    case KVARN_CUDA: return "KVARN_CUDA";
+    default: return "KVARN_UNKNOWN_STATUS";
+  }
+}
+
+int kvarn_version(void) { return 1; }
+
+int kvarn_layout(const kvarn_params* p, kvarn_layout_info* out) {
+  if (!p || !out) return KVARN_INVALID_ARG;
+  if (p->bits != 2 && p->bits != 4) return KVARN_UNSUPPORTED;
+  out->record_bytes = record_bytes(p->bits);
+  out->codes_off = 0; out->codes_bytes = codes_bytes(p->bits);
+  out->s1_off = s1_off(p->bits); out->s2_off = s2_off(p->bits); out->z_off = z_off(p->bits);
+  return KVARN_OK;
+}
+
+size_t kvarn_decode_workspace_bytes(const kvarn_params* p, int32_t B, int32_t Hq, int32_t Hkv,
+                                    int32_t max_chunks) {
+  if (!p || B <= 0 || Hq <= 0 || Hkv <= 0) return 0;
+  const int s = auto_splits(p, B, Hkv, max_chunks);
+  return (size_t)B * Hq * s * WS_STRIDE * sizeof(float);
+}
+
+int kvarn_quantize_chunk(const kvarn_params* p, const void* k, const void* v, int64_t n_tiles,
+                         int64_t tile_stride, int64_t tok_stride, void* k_rec, void* v_rec,
+                         int64_t rec_stride, const kvarn_debug* dbg, void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if (n_tiles == 0) return KVARN_OK;
+  const bool do_k = k && k_rec, do_v = v && v_rec;
+  if (n_tiles < 0 || (!do_k && !do_v) || (k && !k_rec) || (v && !v_rec) || (!k && k_rec) || (!v && v_rec))
+    return KVARN_INVALID_ARG;
+  if (n_tiles > 0x7fffffffLL) return KVARN_CAPACITY;
+  if (tok_stride < D || tile_stride < 0) return KVARN_INVALID_ARG;
+  if ((tok_stride % 8) || (tile_stride % 8) || (rec_stride % 16) || !aligned16(k) || !aligned16(v) ||
+      !aligned16(k_rec) || !aligned16(v_rec))
+    return KVARN_MISALIGNED;
+  if (rec_stride < (int64_t)record_bytes(p->bits)) return KVARN_INVALID_ARG;
+  QuantArgs A{};
+  A.in[0] = k; A.in[1] = v; A.rec[0] = (uint8_t*)k_rec; A.rec[1] = (uint8_t*)v_rec;
+  A.n_inner = n_tiles > 0 ? n_tiles : 1; A.in_outer_stride = 0; A.in_tile_stride = tile_stride;
+  A.tok_stride = tok_stride; A.rec_outer_stride = 0; A.rec_stride = rec_stride; A.n_tiles = n_tiles;
+  A.kind_base = do_k ? 0 : 1;
+  A.rotate[0] = p->rotate_k; A.rotate[1] = p->rotate_v;
+  A.vc = varn_consts(p);
+  if (dbg) { A.dbg_kbest = dbg->k_best; A.dbg_imb = dbg->imb; A.dbg_aux = dbg->aux_f32; }
+  return launch_quantize(p, A, (do_k && do_v) ? 2 : 1, (cudaStream_t)stream);
+}
+
+static int check_cache(const kvarn_cache* c) {
+  if (!c || !c->k_records || !c->v_records || !c->k_resid || !c->v_resid || !c->seq_lens) return KVARN_INVALID_ARG;
+  if (c->B <= 0 || c->Hkv <= 0 || c->max_chunks < 0) return KVARN_INVALID_ARG;
+  if (!aligned16(c->k_records) || !aligned16(c->v_records) || !aligned16(c->k_resid) || !aligned16(c->v_resid))
+    return KVARN_MISALIGNED;
+  return KVARN_OK;
+}
+
+int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, const void* k, const void* v,
+                  int32_t n_tok, void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if ((st = check_cache(cache))) return st;
+  if (n_tok < 0 || ((!k || !v) && n_tok > 0)) return KVARN_INVALID_ARG;
+  if (!aligned16(k) || !aligned16(v)) return KVARN_MISALIGNED;
+  const int n_full = n_tok / G;
+  if (n_full > cache->max_chunks) return KVARN_CAPACITY;
+  const long long BH = (long long)cache->B * cache->Hkv;
+  if (BH * n_full > 0x7fffffffLL) return KVARN_CAPACITY;
+  cudaStream_t s = (cudaStream_t)stream;
+  QuantArgs A{};
+  A.in[0] = k; A.in[1] = v; A.rec[0] = (uint8_t*)cache->k_records; A.rec[1] = (uint8_t*)cache->v_records;
+  A.n_inner = n_full > 0 ? n_full : 1;
+  A.in_outer_stride = (long long)n_tok * D; A.in_tile_stride = (long long)G * D; A.tok_stride = D;
+  A.rec_outer_stride = (long long)cache->max_chunks * record_bytes(p->bits);
+  A.rec_stride = record_bytes(p->bits);
+  A.n_tiles = BH * n_full; A.kind_base = 0;
+  A.rotate[0] = p->rotate_k; A.rotate[1] = p->rotate_v; A.vc = varn_consts(p);
+  if ((st = launch_quantize(p, A, 2, s))) return st;
+  TailArgs T{};
+  T.in[0] = k; T.in[1] = v; T.resid[0] = cache->k_resid; T.resid[1] = cache->v_resid;
+  T.seq_lens = cache->seq_lens; T.B = cache->B; T.Hkv = cache->Hkv; T.n_tok = n_tok; T.n_full = n_full;
+  dim3 grid((unsigned)BH, 2);
+  if (p->in_dtype == KVARN_F32) prefill_tail_kernel<float><<<grid, 256, 0, s>>>(T);
+  else prefill_tail_kernel<__nv_bfloat16><<<grid, 256, 0, s>>>(T);
+  return last_cuda();
+}
+
+int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_new,
+                 const void* v_new, void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if ((st = check_cache(cache))) return st;
+  if (!k_new || !v_new || !cache->ticket) return KVARN_INVALID_ARG;
+  if (!aligned16(k_new) || !aligned16(v_new)) return KVARN_MISALIGNED;
+  AppendArgs A{};
+  A.rec[0] = (uint8_t*)cache->k_records; A.rec[1] = (uint8_t*)cache->v_records;
+  A.resid[0] = cache->k_resid; A.resid[1] = cache->v_resid;
+  A.tok[0] = k_new; A.tok[1] = v_new;
+  A.seq_lens = cache->seq_lens; A.ticket = cache->ticket;
+  A.B = cache->B; A.Hkv = cache->Hkv; A.max_chunks = cache->max_chunks;
+  A.rotate[0] = p->rotate_k; A.rotate[1] = p->rotate_v; A.vc = varn_consts(p);
+  dim3 grid((unsigned)(cache->B * cache->Hkv), 2), block(256);
+  cudaStream_t s = (cudaStream_t)stream;
+  const bool f32 = p->in_dtype == KVARN_F32;
+  if (p->bits == 2) {
+    if (f32) append_kernel<2, float><<<grid, block, 0, s>>>(A);
+    else append_kernel<2, __nv_bfloat16><<<grid, block, 0, s>>>(A);
+  } else {
+    if (f32) append_kernel<4, float><<<grid, block, 0, s>>>(A);
+    else append_kernel<4, __nv_bfloat16><<<grid, block, 0, s>>>(A);
+  }
+  return last_cuda();
+}
+
+int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                           int32_t Hq, float sm_scale, void* out, void* ws, size_t ws_bytes,
+                           void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if ((st = check_cache(cache))) return st;
+  if (!q || !out || !ws || Hq <= 0 || (Hq % cache->Hkv) != 0) return KVARN_INVALID_ARG;
+  const int g = Hq / cache->Hkv;
+  if (g > 8) return KVARN_UNSUPPORTED;
+  if (!aligned16(q) || !aligned16(out) || !aligned16(ws)) return KVARN_MISALIGNED;
+  const size_t need = kvarn_decode_workspace_bytes(p, cache->B, Hq, cache->Hkv, cache->max_chunks);
+  if (ws_bytes < need) return KVARN_WORKSPACE_TOO_SMALL;
+  DecodeArgs A{};
+  A.k_records = (const uint8_t*)cache->k_records; A.v_records = (const uint8_t*)cache->v_records;
+  A.k_resid = cache->k_resid; A.v_resid = cache->v_resid; A.seq_lens = cache->seq_lens;
+  A.q = q; A.out = out; A.ws = (float*)ws;
+  A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.max_chunks = cache->max_chunks;
+  A.splits = auto_splits(p, cache->B, cache->Hkv, cache->max_chunks);
+  A.q_scale = sm_scale * 1.4426950408889634f;
+  A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
+  cudaStream_t s = (cudaStream_t)stream;
+  const bool f32 = p->in_dtype == KVARN_F32;
+  if (p->bits == 2) {
+    if (f32) launch_decode_ref<2, float>(A, g, s); else launch_decode_ref<2, __nv_bfloat16>(A, g, s);
+  } else {
+    if (f32) launch_decode_ref<4, float>(A, g, s); else launch_decode_ref<4, __nv_bfloat16>(A, g, s);
+  }
+  if ((st = last_cuda())) return st;
+  decode_merge_kernel<<<A.B * A.Hq, 32, 0, s>>>(A);
+  return last_cuda();
+}
+
+int kvarn_quantize_chunk_host(const kvarn_params* p, const void* k_host, const void* v_host,
+                              int64_t n_tiles, void* dev_in_k, void* dev_in_v, void* dev_rec_k,
+                              void* dev_rec_v, void* k_rec_host, void* v_rec_host, void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if (!k_host || !v_host || !dev_in_k || !dev_in_v || !dev_rec_k || !dev_rec_v || n_tiles < 0) return KVARN_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t esz = p->in_dtype == KVARN_F32 ? 4 : 2;
+  const size_t in_bytes = (size_t)n_tiles * G * D * esz, rec_b = (size_t)n_tiles * record_bytes(p->bits);
+  if (cudaMemcpyAsync(dev_in_k, k_host, in_bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) return KVARN_CUDA;
+  if (cudaMemcpyAsync(dev_in_v, v_host, in_bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) return KVARN_CUDA;
+  st = kvarn_quantize_chunk(p, dev_in_k, dev_in_v, n_tiles, (int64_t)G * D, D, dev_rec_k, dev_rec_v,
+                            record_bytes(p->bits), nullptr, stream);
+  if (st) return st;
+  if (k_rec_host && cudaMemcpyAsync(k_rec_host, dev_rec_k, rec_b, cudaMemcpyDeviceToHost, s) != cudaSuccess) return KVARN_CUDA;
+  if (v_rec_host && cudaMemcpyAsync(v_rec_host, dev_rec_v, rec_b, cudaMemcpyDeviceToHost, s) != cudaSuccess) return KVARN_CUDA;
+  return KVARN_OK;
+}
+
+int kvarn_decode_attention_host(const kvarn_params* p, const kvarn_cache* cache,
+                                const void* q_host, int32_t Hq, float sm_scale, void* out_host,
+                                void* dev_q, void* dev_out, void* ws, size_t ws_bytes,
+                                void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if (!cache || !q_host || !out_host || !dev_q || !dev_out || Hq <= 0) return KVARN_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t n = (size_t)cache->B * Hq * D;
+  const size_t qb = n * (p->in_dtype == KVARN_F32 ? 4 : 2), ob = n * (p->out_dtype == KVARN_F32 ? 4 : 2);
+  if (cudaMemcpyAsync(dev_q, q_host, qb, cudaMemcpyHostToDevice, s) != cudaSuccess) return KVARN_CUDA;
+  st = kvarn_decode_attention(p, cache, dev_q, Hq, sm_scale, dev_out, ws, ws_bytes, stream);
+  if (st) return st;
+  if (cudaMemcpyAsync(out_host, dev_out, ob, cudaMemcpyDeviceToHost, s) != cudaSuccess) return KVARN_CUDA;
+  return KVARN_OK;
+}
+
+int kvarn_unpack_record_host(const kvarn_params* p, int32_t kind, const void* record,
+                             uint8_t* codes, float* s1, float* s2, float* z) {
+  if (!p || !record || !codes || !s1 || !s2 || !z) return KVARN_INVALID_ARG;
+  if (p->bits != 2 && p->bits != 4) return KVARN_UNSUPPORTED;
+  if (kind != KVARN_KIND_K && kind != KVARN_KIND_V) return KVARN_INVALID_ARG;
+  const int bits = p->bits, lv = (1 << bits) - 1, per_byte = 8 / bits, rowb = row_bytes(bits);
+  const uint8_t* r = (const uint8_t*)record;
+  for (int row = 0; row < 128; ++row)
+    for (int e = 0; e < 128; ++e) {
+      const uint8_t byte = r[row * rowb + e / per_byte];
+      const uint8_t code = (byte >> (bits * (e % per_byte))) & lv;
+      if (kind == KVARN_KIND_K) codes[row * 128 + e] = code;   // row = token, e = channel
+      else codes[e * 128 + row] = code;                        // row = channel, e = token
+    }
+  for (int i = 0; i < 128; ++i) {
+    s1[i] = e4m3_to_f32(r[s1_off(bits) + i]);
+    s2[i] = e4m3_to_f32(r[s2_off(bits) + i]);
+    uint16_t zb;
+    memcpy(&zb, r + z_off(bits) + 2 * i, 2);
+    z[i] = f16_bits_to_f32(zb);
+  }
+  return KVARN_OK;
+}
+
+int kvarn_pack_record_host(const kvarn_params* p, int32_t kind, const uint8_t* codes,
+                           const float* s1, const float* s2, const float* z, void* record) {
+  if (!p || !record || !codes || !s1 || !s2 || !z) return KVARN_INVALID_ARG;
+  if (p->bits != 2 && p->bits != 4) return KVARN_UNSUPPORTED;
+  if (kind != KVARN_KIND_K && kind != KVARN_KIND_V) return KVARN_INVALID_ARG;
+  const int bits = p->bits, lv = (1 << bits) - 1, per_byte = 8 / bits, rowb = row_bytes(bits);
+  uint8_t* r = (uint8_t*)record;
+  memset(r, 0, record_bytes(bits));
+  for (int row = 0; row < 128; ++row)
+    for (int e = 0; e < 128; ++e) {
+      const uint8_t code = (kind == KVARN_KIND_K ? codes[row * 128 + e] : codes[e * 128 + row]) & lv;
+      r[row * rowb + e / per_byte] |= (uint8_t)(code << (bits * (e % per_byte)));
+    }
+  for (int i = 0; i < 128; ++i) {
+    r[s1_off(bits) + i] = f32_to_e4m3(s1[i]);
+    r[s2_off(bits) + i] = f32_to_e4m3(s2[i]);
+    const uint16_t zb = f32_to_f16_bits(z[i]);
+    memcpy(r + z_off(bits) + 2 * i, &zb, 2);
+  }
+  return KVARN_OK;
+}
+
+}  // extern "C"

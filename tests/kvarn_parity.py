@@ -1,0 +1,84 @@
+"""Shared helpers of the GPU parity tests: everything here calls the oracle for
+expected values and the CUDA binding only for the values under test."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from oracle import kvarn_oracle as O
+
+# Tolerances (BASELINE.json north_star)
+CODE_MISMATCH_FRAC = 1e-4     # codes bit-exact except fp32 rounding ties, each off by one level
+SCALE_RTOL = 1e-5             # pre-storage scales and zero-points vs the oracle at the kernel's k
+IMB_ACCEPT = 1e-5             # reading R10: any iterate within this of the best imbalance is valid
+ATTN_RTOL = 2e-3              # per (b, q head): max|out - ref| / max|ref|
+
+
+def tile_f64(x: torch.Tensor) -> np.ndarray:
+    return x.detach().to(torch.float64).cpu().numpy()
+
+
+def check_quantized_tile(kv, p, kind: int, X: np.ndarray, rec: np.ndarray, k_gpu: int,
+                         imb_gpu: np.ndarray, aux_gpu: np.ndarray, stats: dict):
+    """Compare one GPU record (+ debug outputs) against the oracle on tile X[t, c]."""
+    kname = "k" if kind == 0 else "v"
+    codes, s1, s2, z = kv.unpack_record(p, kind, rec)
+    ref_free = O.quantize_tile(X, kname, bits=p.bits, iters=p.iters,
+                               rotate_on=bool(p.rotate_k if kind == 0 else p.rotate_v))
+    I = np.array(ref_free.varn.I)
+    # (1) the iterate kept by the kernel is a valid choice of Alg. 1 line 18 (R10)
+    assert 0 <= k_gpu <= p.iters
+    assert I[k_gpu] <= I.min() * (1 + IMB_ACCEPT), (k_gpu, I)
+    # (2) imbalance trajectory
+    n = p.iters + 1
+    assert np.allclose(imb_gpu[:n], I[:n], rtol=2e-4), (imb_gpu[:n], I[:n])
+    # (3) pre-storage scales / zero-points at the kernel's k
+    ref = O.quantize_tile(X, kname, bits=p.bits, iters=p.iters, at_k=k_gpu,
+                          rotate_on=bool(p.rotate_k if kind == 0 else p.rotate_v))
+    s1_f, s2_f, z_f = aux_gpu[0].astype(np.float64), aux_gpu[1].astype(np.float64), aux_gpu[2].astype(np.float64)
+    assert np.allclose(s1_f, ref.s1_f, rtol=SCALE_RTOL, atol=0), np.abs(s1_f / ref.s1_f - 1).max()
+    assert np.allclose(s2_f, ref.s2_f, rtol=SCALE_RTOL, atol=0), np.abs(s2_f / ref.s2_f - 1).max()
+    # z = mn / s is O(1..10) in code units; tolerance relative to the code range
+    assert np.allclose(z_f, ref.z_f, rtol=SCALE_RTOL, atol=SCALE_RTOL * (1 << p.bits)), np.abs(z_f - ref.z_f).max()
+    # (4) stored bytes = storage rounding of the kernel's own fp32 values
+    st_mis = int((s1.astype(np.float64) != O.round_fp8_e4m3(s1_f)).sum()
+                 + (s2.astype(np.float64) != O.round_fp8_e4m3(s2_f)).sum()
+                 + (z.astype(np.float64) != O.round_fp16(z_f)).sum())
+    assert st_mis == 0
+    # ... and equal the oracle's stored values except at rounding ties
+    aux_mis = int((s1 != ref.s1).sum() + (s2 != ref.s2).sum() + (z != ref.z).sum())
+    # (5) codes
+    diff = codes.astype(np.int32) - ref.codes.astype(np.int32)
+    assert np.abs(diff).max() <= 1
+    stats["codes"] = stats.get("codes", 0) + diff.size
+    stats["code_mismatch"] = stats.get("code_mismatch", 0) + int((diff != 0).sum())
+    stats["aux"] = stats.get("aux", 0) + 384
+    stats["aux_mismatch"] = stats.get("aux_mismatch", 0) + aux_mis
+    return codes, s1, s2, z
+
+
+def assert_mismatch_budget(stats: dict):
+    frac = stats["code_mismatch"] / max(stats["codes"], 1)
+    assert frac <= CODE_MISMATCH_FRAC, f"code mismatch fraction {frac:.2e}"
+    # stored aux values differ from the oracle's only at FP8/FP16 rounding ties
+    assert stats["aux_mismatch"] <= max(2, 2e-3 * stats["aux"]), stats
+
+
+def oracle_attention_from_records(kv, p, k_recs, v_recs, k_resid, v_resid, q, sm_scale=None):
+    """Oracle steps 5-6 applied to GPU-produced record bytes (reading R17).
+
+    k_recs / v_recs: uint8 arrays [n_chunks, record_bytes]; k_resid / v_resid:
+    float64 [r, 128]; q: float64 [g, 128]."""
+    kt = [kv.unpack_record(p, 0, r) for r in k_recs]
+    vt = [kv.unpack_record(p, 1, r) for r in v_recs]
+    kt = [tuple(np.asarray(a, dtype=np.float64) if i else a for i, a in enumerate(t)) for t in kt]
+    vt = [tuple(np.asarray(a, dtype=np.float64) if i else a for i, a in enumerate(t)) for t in vt]
+    return O.decode_attention(q, kt, vt, k_resid, v_resid, sm_scale=sm_scale,
+                              rotate_k=bool(p.rotate_k), rotate_v=bool(p.rotate_v))
+
+
+def attn_rel_err(out: np.ndarray, ref: np.ndarray) -> float:
+    """per head max|out-ref| / max|ref|, maximum over heads (reading R16)."""
+    num = np.abs(out - ref).max(axis=-1)
+    den = np.maximum(np.abs(ref).max(axis=-1), 1e-30)
+    return float((num / den).max())

@@ -1,0 +1,145 @@
+"""GPU parity: kvarn_quantize_chunk (through the C ABI) vs the oracle, element by
+element on the same seeded inputs (BASELINE.json configs 0 and 3, edge cases)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_03458_b200 import workloads as W
+import kvarn_parity as P
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def kv():
+    from paper_2606_03458_b200 import kvarn
+    return kvarn
+
+
+def _run_and_check(kv, p, K, V, stats=None):
+    """K, V torch [n, 128, 128] on cuda.  Checks every tile of both kinds."""
+    k_rec, v_rec, dbg = kv.quantize_chunk(p, K, V, debug=True)
+    torch.cuda.synchronize()
+    stats = {} if stats is None else stats
+    kb, imb, aux = dbg.k_best.cpu().numpy(), dbg.imb.cpu().numpy(), dbg.aux.cpu().numpy()
+    recs = (k_rec.cpu().numpy(), v_rec.cpu().numpy())
+    for kind, X in ((0, K), (1, V)):
+        for i in range(X.shape[0]):
+            P.check_quantized_tile(kv, p, kind, P.tile_f64(X[i]), recs[kind][i], int(kb[kind, i]),
+                                   imb[kind, i], aux[kind, i], stats)
+    return stats, recs, kb
+
+
+def test_config0_single_tile_fp32(kv):
+    # BASELINE.json configs[0]: K with 4 outlier channels x20 and token 0 x10
+    K, V, q, oc = W.config0()
+    p = kv.default_params(2)
+    Kt, Vt = torch.tensor(K, device="cuda")[None], torch.tensor(V, device="cuda")[None]
+    stats, recs, kb = _run_and_check(kv, p, Kt, Vt)
+    P.assert_mismatch_budget(stats)
+    assert recs[0].shape == (1, 4608)
+    # token 0 (x10) carries the largest per-token second scale of the K tile
+    _, _, s2, _ = kv.unpack_record(p, 0, recs[0][0])
+    assert int(np.argmax(s2)) == 0
+
+
+@pytest.mark.parametrize("bits", [2, 4])
+def test_config3_sample_bf16(kv, bits):
+    # config 3 recipe (log-normal channel scales, 1 % token outliers x8), a
+    # multi-tile launch spanning several waves' worth of CTAs with a ragged count
+    K, V = W.quantizer_sweep_tiles(Hkv=8, n_tok=128 * 37, seed=3, device="cuda")
+    Kt = K.reshape(-1, 128, 128).contiguous()
+    Vt = V.reshape(-1, 128, 128).contiguous()
+    assert Kt.shape[0] == 296
+    p = kv.default_params(bits)
+    k_rec, v_rec, dbg = kv.quantize_chunk(p, Kt, Vt, debug=True)
+    torch.cuda.synchronize()
+    kb, imb, aux = dbg.k_best.cpu().numpy(), dbg.imb.cpu().numpy(), dbg.aux.cpu().numpy()
+    recs = (k_rec.cpu().numpy(), v_rec.cpu().numpy())
+    stats = {}
+    rng = np.random.default_rng(0)
+    sample = sorted(set([0, 1, 147, 148, 295]) | set(rng.choice(296, 19, replace=False).tolist()))
+    for kind, X in ((0, Kt), (1, Vt)):
+        for i in sample:
+            P.check_quantized_tile(kv, p, kind, P.tile_f64(X[i]), recs[kind][i], int(kb[kind, i]),
+                                   imb[kind, i], aux[kind, i], stats)
+    P.assert_mismatch_budget(stats)
+
+
+def test_deterministic_and_k_only_v_only(kv):
+    K, V = W.quantizer_sweep_tiles(Hkv=2, n_tok=128 * 3, seed=5, device="cuda")
+    Kt, Vt = K.reshape(-1, 128, 128).contiguous(), V.reshape(-1, 128, 128).contiguous()
+    p = kv.default_params(2)
+    a = kv.quantize_chunk(p, Kt, Vt)
+    b = kv.quantize_chunk(p, Kt, Vt)
+    assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
+    ko, _ = kv.quantize_chunk(p, Kt, None)
+    _, vo = kv.quantize_chunk(p, None, Vt)
+    assert torch.equal(ko, a[0]) and torch.equal(vo, a[1])
+
+
+def test_offset_tile_variance_is_mean_centred(kv):
+    # P:127 "in some cases have large offsets": channels with mean >> std
+    X = W.offset_tile(seed=11, offset=6.0, device="cuda")
+    p = kv.default_params(2)
+    stats, _, _ = _run_and_check(kv, p, X[None], X[None].clone())
+    P.assert_mismatch_budget(stats)
+
+
+@pytest.mark.parametrize("opts", [dict(iters=0), dict(iters=1), dict(iters=3), dict(rotate_k=0, rotate_v=0),
+                                  dict(iters=0, rotate_k=0, rotate_v=0)])
+def test_ablation_switches(kv, opts):
+    # KIVI (RTN only), HK (Hadamard + RTN), VarN(K) -- the same kernel with flags
+    K, V, _, _ = W.config0()
+    p = kv.default_params(2, **opts)
+    Kt, Vt = torch.tensor(K, device="cuda")[None], torch.tensor(V, device="cuda")[None]
+    stats, _, kb = _run_and_check(kv, p, Kt, Vt)
+    P.assert_mismatch_budget(stats)
+    if p.iters == 0:
+        assert kb.max() == 0
+
+
+def test_degenerate_tiles_do_not_fault(kv):
+    p = kv.default_params(2)
+    Z = torch.zeros((1, 128, 128), device="cuda", dtype=torch.bfloat16)
+    Cst = torch.full((1, 128, 128), 1.5, device="cuda", dtype=torch.bfloat16)
+    for X in (Z, Cst):
+        k_rec, v_rec = kv.quantize_chunk(p, X, X.clone())
+        torch.cuda.synchronize()
+        for kind, rec in ((0, k_rec), (1, v_rec)):
+            codes, s1, s2, z = kv.unpack_record(p, kind, rec[0].cpu().numpy())
+            assert np.isfinite(s1).all() and np.isfinite(s2).all() and np.isfinite(z).all()
+    # all-zero tile: every variance 0 -> clamped, L = -0.3 on both axes; RTN
+    # groups degenerate -> codes 0, z = 0, dequant = 0 exactly
+    codes, s1, s2, z = kv.unpack_record(p, 0, kv.quantize_chunk(p, Z, Z.clone())[0][0].cpu().numpy())
+    assert codes.sum() == 0 and np.all(z == 0)
+    # non-finite input: undefined values, no fault
+    X = torch.randn((2, 128, 128), device="cuda").to(torch.bfloat16)
+    X[0, 3, 7] = float("inf"); X[1, 5, 5] = float("nan")
+    kv.quantize_chunk(p, X, X.clone())
+    torch.cuda.synchronize()
+
+
+def test_strided_input_and_record_stride(kv):
+    # tokens of a tile need not be contiguous with the next tile: [Hkv][n_tok][128]
+    # viewed per head with a padded token stride
+    import ctypes as C
+    K, V = W.quantizer_sweep_tiles(Hkv=1, n_tok=128 * 4, seed=9, device="cuda")
+    pad = torch.zeros((4 * 128, 256), device="cuda", dtype=torch.bfloat16)
+    pad[:, :128] = K[0]
+    p = kv.default_params(2)
+    rec_s = torch.zeros((4, 4608 + 64), dtype=torch.uint8, device="cuda")
+    st = kv.lib.kvarn_quantize_chunk(C.byref(p), C.c_void_p(pad.data_ptr()), None, 4, 128 * 256, 256,
+                                     C.c_void_p(rec_s.data_ptr()), None, 4608 + 64, None,
+                                     C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    assert st == 0
+    ref, _ = kv.quantize_chunk(p, K[0].reshape(4, 128, 128).contiguous(), None)
+    torch.cuda.synchronize()
+    assert torch.equal(rec_s[:, :4608], ref) and int(rec_s[:, 4608:].sum()) == 0
+
+
+def test_zero_tiles_is_a_noop(kv):
+    p = kv.default_params(2)
+    E = torch.empty((0, 128, 128), device="cuda", dtype=torch.bfloat16)
+    k_rec, v_rec = kv.quantize_chunk(p, E, E.clone())
+    assert k_rec.shape == (0, 4608)
