@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py -- KVarN hot path on B200: BASELINE.json configs[1] (Llama-3.1-8B-
+shaped decode layer: B=8, 32 q / 8 KV heads, head_dim 128, ctx 8192 = 64 chunks,
+2-bit), one JSON line.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+  write path  kvarn_quantize_chunk over the batch's 2 x 4096 K/V tiles (one launch)
+  read path   kvarn_decode_attention over a 64-chunk packed cache (2 launches)
+The bench cycles through L = 8 distinct "layers" (input + cache copies, 2.4 GB
+of inputs, 302 MB of records: far larger than the 126 MB L2); the read path of
+step i reads the cache written L/2 steps earlier, so neither kernel ever finds
+its input in L2.  Each kernel is timed with CUDA events on the launching
+stream inside the timed region.
+
+  metric/value  2-bit decode-attention GB/s  (algorithmic bytes / decode time)
+  also          quantize tokens/s, us/step, HBM / ALU roofline fractions,
+                the oracle timed on the host cores (cpu_baseline), and the same
+                step through the host-buffer C-ABI calls (e2e).
+
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample instead.
+Under torchrun (N > 1) every rank runs an independent replica of the workload
+(the path has no cross-sequence exchange: DESIGN.md "Multi-GPU").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+D, G = 128, 128
+FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12  # SMs x lanes x FMA x max clock
+# Algorithmic fp32 flops of the write path per tile:
+#   Hadamard 7 stages x 16384 add/sub                       = 114 688
+#   Alg. 1, K=8: 18 variance passes x 16384 x (mul+add+fma) = 1 179 648  (4 flop / element / pass)
+#   balance (2 mul) + RTN (min, max, fma, round, 2 clamp)    =   131 072
+QUANT_FLOPS_PER_TILE = 7 * 16384 + 18 * 16384 * 4 + 8 * 16384
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(index)], stdout=subprocess.PIPE, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(smax)) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(n_tiles: int, n_units: int, n_chunks: int, g: int, seed: int = 1):
+    """Time the oracle, as it stands, on a bounded sample of configs[1]:
+    n_tiles K tiles + n_tiles V tiles through quantize_tile, then decode attention
+    of n_units (sequence, KV head) units over n_chunks chunks each."""
+    from oracle import kvarn_oracle as O
+    from paper_2606_03458_b200 import workloads as W
+    K, V = W.kv_tokens(1, 1, n_tiles * G, seed=seed, device="cpu")
+    q = W.queries(1, g, seed=seed, device="cpu")[0].double().numpy()
+    Kt = K[0, 0].double().numpy().reshape(n_tiles, G, D)
+    Vt = V[0, 0].double().numpy().reshape(n_tiles, G, D)
+    t0 = time.perf_counter()
+    kt = [O.quantize_tile(x, "k") for x in Kt]
+    vt = [O.quantize_tile(x, "v") for x in Vt]
+    t_q = time.perf_counter() - t0
+    ks = [(t.codes, t.s1, t.s2, t.z) for t in kt]
+    vs = [(t.codes, t.s1, t.s2, t.z) for t in vt]
+    kc = [ks[i % n_tiles] for i in range(n_chunks)]
+    vc = [vs[i % n_tiles] for i in range(n_chunks)]
+    t0 = time.perf_counter()
+    for _ in range(n_units):
+        O.decode_attention(q, kc, vc, np.zeros((0, D)), np.zeros((0, D)))
+    t_d = time.perf_counter() - t0
+    return t_q, t_d
+
+
+def cpu_threads() -> int:
+    try:
+        return int(torch.get_num_threads())
+    except Exception:
+        return 1
+
+
+def run_reference(args, shape):
+    """--impl reference: the oracle on the host cores, same metric and config."""
+    n_tiles, n_units = 16, 4
+    rec_bytes = 4608
+    unit_bytes = shape.n_chunks * 2 * rec_bytes + shape.g * (D * 2 + D * 4)
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(2, 1, 4, shape.g)
+    tq = td = 0.0
+    t_all = time.perf_counter()
+    for _ in range(args.steps):
+        a, b = oracle_sample(n_tiles, n_units, shape.n_chunks, shape.g)
+        tq += a; td += b
+    wall = time.perf_counter() - t_all
+    gbs = n_units * unit_bytes * args.steps / td / 1e9
+    tok_s = n_tiles * G * args.steps / tq / shape.Hkv   # a token = one position across the 8 KV heads, K and V
+    sample = (f"per step: quantize_tile on {n_tiles} K + {n_tiles} V tiles, decode_attention on {n_units} "
+              f"(sequence, KV head) units x {shape.n_chunks} chunks (g={shape.g}); numpy float64")
+    line = {
+        "impl": "reference", "metric": "kvarn_2bit_decode_attn_GBps", "value": gbs, "unit": "GB/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": wall / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(shape, 0),
+        "quantize_tokens_per_s": tok_s,
+        "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": cpu_threads(), "kind": "oracle",
+                         "sample": sample, "quantize_tokens_per_s": tok_s},
+        "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def workload_config(shape, layers):
+    return {"workload": "BASELINE.json configs[1]: Llama-3.1-8B-shaped decode layer",
+            "B": shape.B, "Hq": shape.Hq, "Hkv": shape.Hkv, "head_dim": D, "ctx": shape.ctx,
+            "chunks": shape.n_chunks, "resid": shape.resid, "bits": shape.bits,
+            "step": "kvarn_quantize_chunk(2x%d tiles) + kvarn_decode_attention" % (shape.B * shape.Hkv * shape.n_chunks),
+            "l2": "inputs larger than L2: %d rotating layer copies, decode reads the cache written %d steps earlier"
+                  % (layers, layers // 2),
+            "parallelism": "replicas"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--warmup", type=int, default=8)
+    ap.add_argument("--impl", default="kvarn", choices=["kvarn", "reference"])
+    ap.add_argument("--layers", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "kvarn" else args.warmup
+
+    from paper_2606_03458_b200 import workloads as W
+    shape = W.CONFIG1
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, shape)
+        return
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the KVarN path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2606_03458_b200 import kvarn as kv
+    p = kv.default_params(shape.bits)
+    rb = kv.record_bytes(p)
+    L = args.layers
+    BH = shape.B * shape.Hkv
+    n_tiles = BH * shape.n_chunks
+
+    # ---- synthetic inputs, resident in HBM before the timed region -----------------
+    Ks, Vs, caches, qs = [], [], [], []
+    for l in range(L):
+        K, V = W.kv_tokens(shape.B, shape.Hkv, shape.ctx, seed=shape.seed + 100 * l + 1000 * rank, device=dev)
+        Ks.append(K.view(n_tiles, G, D)); Vs.append(V.view(n_tiles, G, D))
+        qs.append(W.queries(shape.B, shape.Hq, seed=shape.seed + 100 * l + 1000 * rank, device=dev))
+        c = kv.Cache(p, shape.B, shape.Hkv, shape.n_chunks, device=dev)
+        c.seq_lens.fill_(shape.ctx)
+        caches.append(c)
+    ws = torch.empty((kv.decode_workspace_bytes(p, shape.B, shape.Hq, shape.Hkv, shape.n_chunks),),
+                     dtype=torch.uint8, device=dev)
+    out = torch.empty((shape.B, shape.Hq, D), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step(i, ev=None):
+        lq, ld = i % L, (i + L // 2) % L
+        c = caches[lq]
+        if ev: ev[0].record(stream)
+        kv.quantize_chunk(p, Ks[lq], Vs[lq], c.k_records.view(n_tiles, rb), c.v_records.view(n_tiles, rb))
+        if ev: ev[1].record(stream)
+        kv.decode_attention(p, caches[ld], qs[ld], out=out, ws=ws)
+        if ev: ev[2].record(stream)
+
+    for l in range(L):   # fill every cache once (untimed) so decode always reads real records
+        step(l)
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    if dist: dist.barrier()
+    torch.cuda.synchronize()
+    t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+    t0.record(stream)
+    for i in range(args.steps):
+        step(i, evs[i])
+    t1.record(stream)
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    total_ms = t0.elapsed_time(t1)
+    q_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
+    d_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
+    times = torch.tensor([total_ms, q_ms, d_ms], dtype=torch.float64, device=dev)
+    if dist:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    total_ms, q_ms, d_ms = times.tolist()
+
+    # ---- algorithmic bytes --------------------------------------
+    dec_bytes = BH * shape.n_chunks * 2 * rb + shape.B * shape.Hq * (D * 2 + D * 4)
+    q_in = 2 * n_tiles * G * D * 2
+    q_bytes = q_in + 2 * n_tiles * rb
+    hbm_peak, peak_src = peaks()
+    dec_gbs = dec_bytes / (d_ms * 1e-3) / 1e9
+    q_gbs = q_bytes / (q_ms * 1e-3) / 1e9
+    q_tflops = 2 * n_tiles * QUANT_FLOPS_PER_TILE / (q_ms * 1e-3) / 1e12
+    tok_s = shape.B * shape.ctx / (q_ms * 1e-3)
+
+    # ---- e2e: the same step through the host-buffer C-ABI calls --------------------------
+    e2e = None
+    if not args.no_e2e:
+        hk = Ks[0].cpu().pin_memory(); hv = Vs[0].cpu().pin_memory()
+        hq = qs[0].cpu().pin_memory()
+        hout = torch.empty((shape.B, shape.Hq, D), dtype=torch.float32).pin_memory()
+        dq = torch.empty_like(qs[0])
+        c = caches[0]
+        def e2e_step():
+            kv.quantize_chunk_host(p, hk, hv, Ks[0], Vs[0], c.k_records.view(n_tiles, rb), c.v_records.view(n_tiles, rb))
+            kv.decode_attention_host(p, c, hq, hout, dq, out, ws)
+        n_e2e = max(3, min(args.steps, 10))
+        for _ in range(2): e2e_step()
+        torch.cuda.synchronize()
+        if dist: dist.barrier()
+        a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n_e2e): e2e_step()
+        b.record(stream)
+        torch.cuda.synchronize()
+        e_ms = torch.tensor([a.elapsed_time(b) / n_e2e], dtype=torch.float64, device=dev)
+        if dist: dist.all_reduce(e_ms, op=dist.ReduceOp.MAX)
+        e_ms = float(e_ms.item())
+        e2e = {"value": world * dec_bytes / (e_ms * 1e-3) / 1e9, "unit": "GB/s",
+               "h2d_bytes_per_step": int(hk.numel() * 2 + hv.numel() * 2 + hq.numel() * 2),
+               "d2h_bytes_per_step": int(hout.numel() * 4), "ms_per_step": e_ms,
+               "tokens_per_s": world * shape.B * shape.ctx / (e_ms * 1e-3),
+               "note": "kvarn_quantize_chunk_host + kvarn_decode_attention_host, pinned host buffers; "
+                       "value = decode algorithmic bytes / whole e2e step time (PCIe-bound by the 537 MB K/V upload)"}
+
+    if rank != 0:
+        if dist: dist.destroy_process_group()
+        return
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        n_t, n_u = 48, 16
+        tq, td = oracle_sample(n_t, n_u, shape.n_chunks, shape.g)
+        unit_bytes = shape.n_chunks * 2 * rb + shape.g * (D * 2 + D * 4)
+        cpu = {"value": n_u * unit_bytes / td / 1e9, "unit": "GB/s", "cores": cpu_threads(), "kind": "oracle",
+               "sample": f"quantize_tile on {n_t} K + {n_t} V tiles ({tq:.1f} s), decode_attention on {n_u} of "
+                         f"{BH} (sequence, KV head) units x {shape.n_chunks} chunks ({td:.1f} s); numpy float64",
+               "quantize_tokens_per_s": n_t * G / tq / shape.Hkv,
+               "gpu_over_cpu_decode": dec_gbs / (n_u * unit_bytes / td / 1e9)}
+
+    rl_quant = {"kernel": "quantize_kernel<2,bf16>", "bound": "alu", "achieved": q_tflops,
+                "peak": FP32_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s", "frac": q_tflops / FP32_PEAK_TFLOPS_NOMINAL,
+                "traffic": None, "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                "hbm_achieved_GBps": q_gbs, "hbm_frac": q_gbs / hbm_peak, "ms": q_ms}
+    rl_dec = {"kernel": "decode_partial + decode_merge", "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak,
+              "unit": "GB/s", "frac": dec_gbs / hbm_peak, "traffic": None, "peak_source": peak_src,
+              "frac_of_nominal_8TBps": dec_gbs / 8000.0, "us": d_ms * 1e3}
+    line = {
+        "metric": "kvarn_2bit_decode_attn_GBps", "value": world * dec_gbs, "unit": "GB/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": workload_config(shape, L),
+        "decode_us_per_step": d_ms * 1e3, "quantize_ms_per_step": q_ms,
+        "quantize_tokens_per_s": world * tok_s, "quantize_tiles_per_s": world * 2 * n_tiles / (q_ms * 1e-3),
+        "roofline": rl_quant if q_ms > d_ms else rl_dec,
+        "rooflines": {"quantize": rl_quant, "decode": rl_dec},
+        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": 3 * args.steps, "clocks": clocks,
+    }
+    print(json.dumps(line))
+    if dist: dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
