@@ -129,7 +129,10 @@ def cpu_threads() -> int:
 
 def run_reference(args, shape):
     """--impl reference: the oracle on the host cores, same metric and config."""
-    n_tiles, n_units = 16, 4
+    pq, pd = oracle_sample(2, 1, shape.n_chunks, shape.g)
+    budget = min(4.0, 90.0 / (2 * max(args.steps + min(args.warmup, 1), 1)))   # seconds per half-step: whole run ~ 90 s
+    n_tiles = int(min(max(budget / max(pq / 2, 1e-4), 2), 1024))
+    n_units = int(min(max(budget / max(pd, 1e-3), 1), 256))
     rec_bytes = 4608
     unit_bytes = shape.n_chunks * 2 * rec_bytes + shape.g * (D * 2 + D * 4)
     for _ in range(min(args.warmup, 1)):
@@ -295,7 +298,7 @@ def main():
                "d2h_bytes_per_step": int(hout.numel() * 4), "ms_per_step": e_ms,
                "tokens_per_s": world * shape.B * shape.ctx / (e_ms * 1e-3),
                "note": "kvarn_quantize_chunk_host + kvarn_decode_attention_host, pinned host buffers; "
-                       "value = decode algorithmic bytes / whole e2e step time (PCIe-bound by the 537 MB K/V upload)"}
+                       "value = decode algorithmic bytes / whole e2e step time (PCIe-bound by the 268 MB K/V upload)"}
 
     if rank != 0:
         if dist: dist.destroy_process_group()
@@ -303,12 +306,15 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        n_t, n_u = 48, 16
+        # size the sample for ~8 s of oracle work per half on THIS host (probe first)
+        pq, pd = oracle_sample(4, 1, shape.n_chunks, shape.g)
+        n_t = int(min(max(8.0 / max(pq / 4, 1e-4), 8), 4096))
+        n_u = int(min(max(8.0 / max(pd, 1e-3), 2), 4 * BH))
         tq, td = oracle_sample(n_t, n_u, shape.n_chunks, shape.g)
         unit_bytes = shape.n_chunks * 2 * rb + shape.g * (D * 2 + D * 4)
         cpu = {"value": n_u * unit_bytes / td / 1e9, "unit": "GB/s", "cores": cpu_threads(), "kind": "oracle",
                "sample": f"quantize_tile on {n_t} K + {n_t} V tiles ({tq:.1f} s), decode_attention on {n_u} of "
-                         f"{BH} (sequence, KV head) units x {shape.n_chunks} chunks ({td:.1f} s); numpy float64",
+                         f"the workload's {BH} (sequence, KV head) unit shapes x {shape.n_chunks} chunks ({td:.1f} s); numpy float64",
                "quantize_tokens_per_s": n_t * G / tq / shape.Hkv,
                "gpu_over_cpu_decode": dec_gbs / (n_u * unit_bytes / td / 1e9)}
 
