@@ -77,10 +77,15 @@ typedef struct {
 } kvarn_params;
 
 /* Byte layout of one record (fixed by bits).  codes: K records hold one row
- * per TOKEN (128 channels), V records one row per CHANNEL (128 tokens).
+ * per TOKEN (its 128 channels), V records one row per CHANNEL (its 128 tokens);
+ * a row is little-endian (element e at bit bits*(e % (8/bits)) of byte
+ * e*bits/8) and is stored in 16-byte segments, segment s of row r at byte
+ * s*2048 + r*16 -- the order the decode kernel's TMEM operand loader reads.
  * s1 = FP8-E4M3 absorbed scale of the RTN group (K: per channel, V: per token),
  * s2 = FP8-E4M3 second (Sinkhorn) scale of the other axis, z = FP16 zero-point
- * of the RTN group (Eq. 1: x_dq = (code + z) * s1 * s2). */
+ * of the RTN group (Eq. 1: x_dq = (code + z) * s1 * s2).  K records keep
+ * s1 and z in the tensor-core "K position" order of their channel (see
+ * csrc/kvarn_common.cuh); use kvarn_unpack_record_host for a canonical view. */
 typedef struct {
   size_t record_bytes; /* 4608 at 2-bit, 8704 at 4-bit (=> 2.25 / 4.25 bit per element) */
   size_t codes_off, codes_bytes;
@@ -96,6 +101,9 @@ typedef struct {
   void* v_resid;        /* same shape */
   int32_t* seq_lens;    /* [B] tokens held per sequence: chunks = len/128, residual = len%128 */
   int32_t* ticket;      /* [B] scratch for kvarn_append, zero-initialised by the caller once */
+  int32_t* decode_ticket; /* [B*Hkv] scratch for kvarn_decode_attention (arrival counters of the split-K
+                           * merge), zero-initialised by the caller once; every call leaves it zero.
+                           * Calls that share it must be ordered on one stream. */
   int32_t B, Hkv, max_chunks;
   int32_t reserved;
 } kvarn_cache;

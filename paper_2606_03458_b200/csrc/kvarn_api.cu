@@ -4,7 +4,7 @@
 #include <cstring>
 
 #include "kvarn_common.cuh"
-#include "kvarn_decode_ref.cuh"
+#include "kvarn_decode.cuh"
 #include "kvarn_quantize.cuh"
 
 namespace kvarn {
@@ -153,26 +153,33 @@ static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kind
 static int auto_splits(const kvarn_params* p, int B, int Hkv, int max_chunks) {
   if (p->splits > 0) return p->splits < max_chunks ? p->splits : (max_chunks > 0 ? max_chunks : 1);
   const int bh = B * Hkv;
-  int s = (148 * 4 + bh - 1) / bh;
+  int s = (148 * 4 + bh / 2) / bh;   // about one wave of 148 SMs x 4 resident CTAs
   if (s > 64) s = 64;
   if (s > max_chunks) s = max_chunks;
   if (s < 1) s = 1;
   return s;
 }
 
-template <int BITS, typename InT>
-static void launch_decode_ref(const DecodeArgs& A, int g, cudaStream_t st) {
-  dim3 grid(A.B * A.Hkv, A.splits), block(128);
-  switch (g) {
-    case 1: decode_partial_ref_kernel<BITS, 1, InT><<<grid, block, 0, st>>>(A); break;
-    case 2: decode_partial_ref_kernel<BITS, 2, InT><<<grid, block, 0, st>>>(A); break;
-    case 3: decode_partial_ref_kernel<BITS, 3, InT><<<grid, block, 0, st>>>(A); break;
-    case 4: decode_partial_ref_kernel<BITS, 4, InT><<<grid, block, 0, st>>>(A); break;
-    case 5: decode_partial_ref_kernel<BITS, 5, InT><<<grid, block, 0, st>>>(A); break;
-    case 6: decode_partial_ref_kernel<BITS, 6, InT><<<grid, block, 0, st>>>(A); break;
-    case 7: decode_partial_ref_kernel<BITS, 7, InT><<<grid, block, 0, st>>>(A); break;
-    default: decode_partial_ref_kernel<BITS, 8, InT><<<grid, block, 0, st>>>(A); break;
+template <int BITS, int GP, typename InT>
+static cudaError_t launch_decode_tc(const DecodeArgs& A, cudaStream_t st) {
+  using SM = DecSmem<BITS, GP>;
+  static bool configured = false;   // per instantiation; benign race (idempotent attribute calls)
+  auto kern = decode_tc_kernel<BITS, GP, InT>;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SM));
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    configured = true;
   }
+  dim3 grid(A.B * A.Hkv, A.splits), block(128);
+  kern<<<grid, block, sizeof(SM), st>>>(A);
+  return cudaGetLastError();
+}
+
+template <int BITS, typename InT>
+static cudaError_t launch_decode(const DecodeArgs& A, cudaStream_t st) {
+  return A.g <= 4 ? launch_decode_tc<BITS, 4, InT>(A, st) : launch_decode_tc<BITS, 8, InT>(A, st);
 }
 
 }  // namespace kvarn
@@ -319,7 +326,7 @@ int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, cons
   int st = check_params(p);
   if (st) return st;
   if ((st = check_cache(cache))) return st;
-  if (!q || !out || !ws || Hq <= 0 || (Hq % cache->Hkv) != 0) return KVARN_INVALID_ARG;
+  if (!q || !out || !ws || !cache->decode_ticket || Hq <= 0 || (Hq % cache->Hkv) != 0) return KVARN_INVALID_ARG;
   const int g = Hq / cache->Hkv;
   if (g > 8) return KVARN_UNSUPPORTED;
   if (!aligned16(q) || !aligned16(out) || !aligned16(ws)) return KVARN_MISALIGNED;
@@ -328,21 +335,18 @@ int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, cons
   DecodeArgs A{};
   A.k_records = (const uint8_t*)cache->k_records; A.v_records = (const uint8_t*)cache->v_records;
   A.k_resid = cache->k_resid; A.v_resid = cache->v_resid; A.seq_lens = cache->seq_lens;
+  A.ticket = cache->decode_ticket;
   A.q = q; A.out = out; A.ws = (float*)ws;
-  A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.max_chunks = cache->max_chunks;
+  A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;
   A.splits = auto_splits(p, cache->B, cache->Hkv, cache->max_chunks);
   A.q_scale = sm_scale * 1.4426950408889634f;
   A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
   cudaStream_t s = (cudaStream_t)stream;
   const bool f32 = p->in_dtype == KVARN_F32;
-  if (p->bits == 2) {
-    if (f32) launch_decode_ref<2, float>(A, g, s); else launch_decode_ref<2, __nv_bfloat16>(A, g, s);
-  } else {
-    if (f32) launch_decode_ref<4, float>(A, g, s); else launch_decode_ref<4, __nv_bfloat16>(A, g, s);
-  }
-  if ((st = last_cuda())) return st;
-  decode_merge_kernel<<<A.B * A.Hq, 32, 0, s>>>(A);
-  return last_cuda();
+  cudaError_t e;
+  if (p->bits == 2) e = f32 ? launch_decode<2, float>(A, s) : launch_decode<2, __nv_bfloat16>(A, s);
+  else e = f32 ? launch_decode<4, float>(A, s) : launch_decode<4, __nv_bfloat16>(A, s);
+  return e == cudaSuccess ? KVARN_OK : KVARN_CUDA;
 }
 
 int kvarn_quantize_chunk_host(const kvarn_params* p, const void* k_host, const void* v_host,
@@ -388,18 +392,21 @@ int kvarn_unpack_record_host(const kvarn_params* p, int32_t kind, const void* re
   if (kind != KVARN_KIND_K && kind != KVARN_KIND_V) return KVARN_INVALID_ARG;
   const int bits = p->bits, lv = (1 << bits) - 1, per_byte = 8 / bits, rowb = row_bytes(bits);
   const uint8_t* r = (const uint8_t*)record;
+  (void)rowb;
   for (int row = 0; row < 128; ++row)
     for (int e = 0; e < 128; ++e) {
-      const uint8_t byte = r[row * rowb + e / per_byte];
+      const uint8_t byte = r[code_off(row, e / per_byte)];
       const uint8_t code = (byte >> (bits * (e % per_byte))) & lv;
       if (kind == KVARN_KIND_K) codes[row * 128 + e] = code;   // row = token, e = channel
       else codes[e * 128 + row] = code;                        // row = channel, e = token
     }
   for (int i = 0; i < 128; ++i) {
-    s1[i] = e4m3_to_f32(r[s1_off(bits) + i]);
+    // K records keep s1 and z (per channel) in K-position order; everything else is natural
+    const int gi = (kind == KVARN_KIND_K) ? kpos_of_elem(bits, i) : i;
+    s1[i] = e4m3_to_f32(r[s1_off(bits) + gi]);
     s2[i] = e4m3_to_f32(r[s2_off(bits) + i]);
     uint16_t zb;
-    memcpy(&zb, r + z_off(bits) + 2 * i, 2);
+    memcpy(&zb, r + z_off(bits) + 2 * gi, 2);
     z[i] = f16_bits_to_f32(zb);
   }
   return KVARN_OK;
@@ -413,16 +420,18 @@ int kvarn_pack_record_host(const kvarn_params* p, int32_t kind, const uint8_t* c
   const int bits = p->bits, lv = (1 << bits) - 1, per_byte = 8 / bits, rowb = row_bytes(bits);
   uint8_t* r = (uint8_t*)record;
   memset(r, 0, record_bytes(bits));
+  (void)rowb;
   for (int row = 0; row < 128; ++row)
     for (int e = 0; e < 128; ++e) {
       const uint8_t code = (kind == KVARN_KIND_K ? codes[row * 128 + e] : codes[e * 128 + row]) & lv;
-      r[row * rowb + e / per_byte] |= (uint8_t)(code << (bits * (e % per_byte)));
+      r[code_off(row, e / per_byte)] |= (uint8_t)(code << (bits * (e % per_byte)));
     }
   for (int i = 0; i < 128; ++i) {
-    r[s1_off(bits) + i] = f32_to_e4m3(s1[i]);
+    const int gi = (kind == KVARN_KIND_K) ? kpos_of_elem(bits, i) : i;
+    r[s1_off(bits) + gi] = f32_to_e4m3(s1[i]);
     r[s2_off(bits) + i] = f32_to_e4m3(s2[i]);
     const uint16_t zb = f32_to_f16_bits(z[i]);
-    memcpy(r + z_off(bits) + 2 * i, &zb, 2);
+    memcpy(r + z_off(bits) + 2 * gi, &zb, 2);
   }
   return KVARN_OK;
 }

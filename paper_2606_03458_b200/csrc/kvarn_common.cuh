@@ -24,6 +24,25 @@ __host__ __device__ constexpr int s1_off(int bits) { return codes_bytes(bits); }
 __host__ __device__ constexpr int s2_off(int bits) { return codes_bytes(bits) + 128; }
 __host__ __device__ constexpr int z_off(int bits) { return codes_bytes(bits) + 256; }
 
+// Code rows are stored "segment-major": the 16-byte segment s of row r (a row =
+// the 128 codes of one token (K) / one channel (V), little-endian, element e at
+// bit bits*(e % (8/bits)) of byte e*bits/8) sits at  s*2048 + r*16, so that 128
+// threads reading one segment of their own row touch consecutive 16-byte words.
+__host__ __device__ constexpr int code_off(int row, int byte_in_row) {
+  return (byte_in_row >> 4) * 2048 + row * 16 + (byte_in_row & 15);
+}
+// "K position" of element e of a code row inside the tensor-core A operand:
+// the decode kernel expands a packed 32-bit word W with  W & (mask << bits*j), so
+// byte b of A column (8/bits)*w + j holds element (32/bits)*w + (8/bits)*b + j.
+// kpos = 4*column + b.  The per-channel aux arrays of K records (s1, z) are
+// stored in K-position order so the B-operand builder reads them contiguously.
+__host__ __device__ constexpr int kpos_of_elem(int bits, int e) {
+  return bits == 2 ? ((e & ~15) | ((e & 3) << 2) | ((e >> 2) & 3)) : ((e & ~7) | ((e & 1) << 2) | ((e >> 1) & 3));
+}
+__host__ __device__ constexpr int elem_of_kpos(int bits, int k) {
+  return bits == 2 ? ((k & ~15) | ((k & 3) << 2) | ((k >> 2) & 3)) : ((k & ~7) | ((k & 3) << 1) | ((k >> 2) & 1));
+}
+
 // ---- storage formats -------------------------------------------------------
 // FP8 E4M3 (finite, max 448), round-to-nearest-even, saturating (DESIGN R9).
 __host__ __device__ inline uint8_t f32_to_e4m3(float x) {

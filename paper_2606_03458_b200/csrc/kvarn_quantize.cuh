@@ -335,9 +335,10 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       const float z = mn / s;
       sm.inv_s[tid] = 1.f / s; sm.z[tid] = z;
       const float s1 = s * sm.Sr[tid], s2 = sm.Sc[tid];  // K: s1 per channel, s2 per token
-      sm.rec[s1_off(BITS) + tid] = f32_to_e4m3(s1);
+      const int kp = kpos_of_elem(BITS, tid);  // K records keep s1, z in K-position order
+      sm.rec[s1_off(BITS) + kp] = f32_to_e4m3(s1);
       sm.rec[s2_off(BITS) + tid] = f32_to_e4m3(s2);
-      reinterpret_cast<uint16_t*>(&sm.rec[z_off(BITS)])[tid] = f32_to_f16_bits(z);
+      reinterpret_cast<uint16_t*>(&sm.rec[z_off(BITS)])[kp] = f32_to_f16_bits(z);
       if (dbg.aux) {
         float* o = dbg.aux + tile_idx * 384;
         o[tid] = s1; o[128 + tid] = s2; o[256 + tid] = z;
@@ -362,9 +363,8 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
         w |= ((uint32_t)q0) << (BITS * 2 * kp);
         w |= ((uint32_t)q1) << (BITS * (2 * kp + 1));
       }
-      uint8_t* row = &sm.rec[(t0 + i) * row_bytes(BITS)];
-      if (BITS == 2) reinterpret_cast<uint16_t*>(row)[li] = (uint16_t)w;
-      else reinterpret_cast<uint32_t*>(row)[li] = w;
+      if (BITS == 2) *reinterpret_cast<uint16_t*>(&sm.rec[code_off(t0 + i, 2 * li)]) = (uint16_t)w;
+      else *reinterpret_cast<uint32_t*>(&sm.rec[code_off(t0 + i, 4 * li)]) = w;
     }
   } else {
     // group = token over the 128 channels: min / max inside the half-warp
@@ -420,9 +420,8 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       }
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      uint8_t* row = &sm.rec[(c0 + k) * row_bytes(BITS)];
-      if (BITS == 2) reinterpret_cast<uint16_t*>(row)[2 * warp + lj] = (uint16_t)w[k];
-      else reinterpret_cast<uint32_t*>(row)[2 * warp + lj] = w[k];
+      if (BITS == 2) *reinterpret_cast<uint16_t*>(&sm.rec[code_off(c0 + k, 2 * (2 * warp + lj))]) = (uint16_t)w[k];
+      else *reinterpret_cast<uint32_t*>(&sm.rec[code_off(c0 + k, 4 * (2 * warp + lj))]) = w[k];
     }
   }
   if (dbg.k_best && tid == 0) dbg.k_best[tile_idx] = k_best;

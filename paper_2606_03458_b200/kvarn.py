@@ -44,7 +44,7 @@ class LayoutInfo(C.Structure):
 class CacheDesc(C.Structure):
     _fields_ = [("k_records", C.c_void_p), ("v_records", C.c_void_p), ("k_resid", C.c_void_p),
                 ("v_resid", C.c_void_p), ("seq_lens", C.c_void_p), ("ticket", C.c_void_p),
-                ("B", C.c_int32), ("Hkv", C.c_int32), ("max_chunks", C.c_int32),
+                ("decode_ticket", C.c_void_p), ("B", C.c_int32), ("Hkv", C.c_int32), ("max_chunks", C.c_int32),
                 ("reserved", C.c_int32)]
 
 
@@ -177,9 +177,11 @@ class Cache:
         self.v_resid = torch.zeros_like(self.k_resid)
         self.seq_lens = torch.zeros((B,), dtype=torch.int32, device=device)
         self.ticket = torch.zeros((B,), dtype=torch.int32, device=device)
+        self.decode_ticket = torch.zeros((B * Hkv,), dtype=torch.int32, device=device)
         self.desc = CacheDesc(self.k_records.data_ptr(), self.v_records.data_ptr(),
                               self.k_resid.data_ptr(), self.v_resid.data_ptr(),
-                              self.seq_lens.data_ptr(), self.ticket.data_ptr(), B, Hkv, max_chunks, 0)
+                              self.seq_lens.data_ptr(), self.ticket.data_ptr(),
+                              self.decode_ticket.data_ptr(), B, Hkv, max_chunks, 0)
 
     def nbytes_read_by_decode(self, ctx: int) -> int:
         """Algorithmic bytes one decode step reads for context length ctx."""

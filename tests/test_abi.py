@@ -78,7 +78,7 @@ def test_status_strings_and_argument_validation_without_gpu(kv):
     assert kv.lib.kvarn_quantize_chunk(C.byref(p), C.c_void_p(0x1000), C.c_void_p(0x1000), 1, 16384, 128,
                                        C.c_void_p(0x2000), C.c_void_p(0x3000), 4608, None, None) == -2
     p = kv.default_params(2)
-    cache = kv.CacheDesc(0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000, 2, 8, 4, 0)
+    cache = kv.CacheDesc(0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000, 0x6800, 2, 8, 4, 0)
     # Hq not a multiple of Hkv, g > 8, workspace too small
     assert kv.lib.kvarn_decode_attention(C.byref(p), C.byref(cache), C.c_void_p(0x7000), 12, 0.1,
                                          C.c_void_p(0x8000), C.c_void_p(0x9000), 1 << 30, None) == -1
@@ -108,23 +108,38 @@ def test_pack_unpack_round_trip_and_formats(kv, bits, kind):
     assert np.array_equal(a2.astype(np.float64), O.round_fp8_e4m3(s2.astype(np.float64)))
     assert np.array_equal(zz.astype(np.float64), O.round_fp16(z.astype(np.float64)))
     info = kv.layout(p)
-    assert np.array_equal(rec[info.s1_off:info.s1_off + 128], O.fp8_e4m3_bits(O.round_fp8_e4m3(s1.astype(np.float64))))
+    stored = rec[info.s1_off:info.s1_off + 128]
+    if kind == 0:
+        # K records keep s1 (and z) in the K-position order of their channel (csrc/kvarn_common.cuh)
+        e = np.arange(128)
+        kpos = ((e & ~15) | ((e & 3) << 2) | ((e >> 2) & 3)) if bits == 2 else ((e & ~7) | ((e & 1) << 2) | ((e >> 1) & 3))
+        assert sorted(kpos.tolist()) == list(range(128))
+        stored = stored[kpos]
+    assert np.array_equal(stored, O.fp8_e4m3_bits(O.round_fp8_e4m3(s1.astype(np.float64))))
     # saturation
     rec = kv.pack_record(p, kind, codes, np.full(128, 1e6, np.float32), s2, z)
     assert np.all(kv.unpack_record(p, kind, rec)[1] == 448.0)
 
 
 def test_code_row_layout(kv):
-    # K rows are per token, V rows per channel, little-endian within a row:
-    # element e of a row sits at bit bits*(e % (8/bits)) of byte e*bits/8.
+    # include/kvarn.h: K rows are per token, V rows per channel, little-endian within
+    # a row (element e at bit bits*(e % (8/bits)) of byte e*bits/8); the 16-byte
+    # segment s of row r sits at byte s*2048 + r*16.
     p = kv.default_params(2)
     codes = np.zeros((128, 128), np.uint8)
     codes[5, 9] = 3          # token 5, channel 9
+    codes[7, 100] = 2        # token 7, channel 100 -> byte 25 of its K row = segment 1, byte 9
     ones = np.ones(128, np.float32)
     rk = kv.pack_record(p, 0, codes, ones, ones, ones)
     rv = kv.pack_record(p, 1, codes, ones, ones, ones)
-    assert rk[5 * 32 + 9 // 4] == 3 << (2 * (9 % 4)) and rk[:4096].sum() == rk[5 * 32 + 2]
-    assert rv[9 * 32 + 5 // 4] == 3 << (2 * (5 % 4)) and rv[:4096].sum() == rv[9 * 32 + 1]
+    assert rk[0 * 2048 + 5 * 16 + 9 // 4] == 3 << (2 * (9 % 4))
+    assert rk[1 * 2048 + 7 * 16 + (100 // 4 - 16)] == 2 << (2 * (100 % 4))
+    assert rk[:4096].sum() == (3 << 2) + (2 << 0)
+    assert rv[0 * 2048 + 9 * 16 + 5 // 4] == 3 << (2 * (5 % 4))
+    assert rv[0 * 2048 + 100 * 16 + 7 // 4] == 2 << (2 * (7 % 4))
+    p4 = kv.default_params(4)
+    r4 = kv.pack_record(p4, 0, codes, ones, ones, ones)
+    assert r4[(100 // 2 // 16) * 2048 + 7 * 16 + (100 // 2) % 16] == 2 << (4 * (100 % 2))
 
 
 def test_missing_library_fails_loudly(tmp_path, monkeypatch):

@@ -134,8 +134,10 @@ def test_split_count_invariance(kv):
         p = kv.default_params(2, splits=s)
         cache = _build_cache(kv, p, K, V)
         outs.append(kv.decode_attention(p, cache, q))
+    # the partials differ only by the running maximum their 18-bit fixed-point
+    # probabilities refer to: an order below ATTN_RTOL
     for o in outs[1:]:
-        assert (o - outs[0]).abs().max() <= 1e-5 * outs[0].abs().max()
+        assert (o - outs[0]).abs().max() <= 2e-4 * outs[0].abs().max()
 
 
 def test_equal_logits_give_mean_of_values_and_rotation_flags(kv):
