@@ -632,22 +632,42 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
     __syncthreads();
     if (!sm.last_flag) return;
     __threadfence();
+    // weights of the splits: warp w handles heads w, w+4; lane s handles splits s, s+32
+    float* wsp = reinterpret_cast<float*>(sm.bq);   // [GP][64] split weights (B_q is dead by now)
+    for (int h = warp; h < g; h += 4) {
+      const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * A.splits * WS_STRIDE;
+      const float m0 = lane < A.splits ? __ldcg(base + (size_t)lane * WS_STRIDE) : -INFINITY;
+      const float m1 = lane + 32 < A.splits ? __ldcg(base + (size_t)(lane + 32) * WS_STRIDE) : -INFINITY;
+      const float l0 = lane < A.splits ? __ldcg(base + (size_t)lane * WS_STRIDE + 1) : 0.f;
+      const float l1 = lane + 32 < A.splits ? __ldcg(base + (size_t)(lane + 32) * WS_STRIDE + 1) : 0.f;
+      const float mstar = warp_max(fmaxf(m0, m1));
+      const float w0 = (m0 == -INFINITY) ? 0.f : exp2f(m0 - mstar);
+      const float w1 = (m1 == -INFINITY) ? 0.f : exp2f(m1 - mstar);
+      wsp[h * 64 + lane] = w0;
+      wsp[h * 64 + lane + 32] = w1;
+      const float L = warp_sum(fmaf(w0, l0, w1 * l1));
+      if (lane == 0) sm.hs[h][1] = L;
+    }
+    __syncthreads();
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
       if (h < g) {
-        const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * A.splits * WS_STRIDE;
-        float mstar = -INFINITY;
-        for (int s = 0; s < A.splits; ++s) mstar = fmaxf(mstar, __ldcg(base + (size_t)s * WS_STRIDE));
-        float L = 0.f, rot = 0.f, res = 0.f;
-        for (int s = 0; s < A.splits; ++s) {
-          const float* p = base + (size_t)s * WS_STRIDE;
-          const float ms = __ldcg(p);
-          const float w = (ms == -INFINITY) ? 0.f : exp2f(ms - mstar);
-          L = fmaf(w, __ldcg(p + 1), L);
-          rot = fmaf(w, __ldcg(p + 4 + tid), rot);
-          res = fmaf(w, __ldcg(p + 132 + tid), res);
+        const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * A.splits * WS_STRIDE + 4 + tid;
+        float rot = 0.f, res = 0.f;
+        int s = 0;
+        for (; s + 4 <= A.splits; s += 4) {
+          float r[4], e[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) { r[j] = __ldcg(base + (size_t)(s + j) * WS_STRIDE); e[j] = __ldcg(base + (size_t)(s + j) * WS_STRIDE + 128); }
+#pragma unroll
+          for (int j = 0; j < 4; ++j) { const float w = wsp[h * 64 + s + j]; rot = fmaf(w, r[j], rot); res = fmaf(w, e[j], res); }
         }
-        Ltot[h] = L; acc[h] = rot; acc_res[h] = res;
+        for (; s < A.splits; ++s) {
+          const float w = wsp[h * 64 + s];
+          rot = fmaf(w, __ldcg(base + (size_t)s * WS_STRIDE), rot);
+          res = fmaf(w, __ldcg(base + (size_t)s * WS_STRIDE + 128), res);
+        }
+        Ltot[h] = sm.hs[h][1]; acc[h] = rot; acc_res[h] = res;
       }
     }
   } else {
