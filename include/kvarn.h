@@ -84,8 +84,8 @@ typedef struct {
  * s1 = FP8-E4M3 absorbed scale of the RTN group (K: per channel, V: per token),
  * s2 = FP8-E4M3 second (Sinkhorn) scale of the other axis, z = FP16 zero-point
  * of the RTN group (Eq. 1: x_dq = (code + z) * s1 * s2).  K records keep
- * s1 and z in the tensor-core "K position" order of their channel (see
- * csrc/kvarn_common.cuh); use kvarn_unpack_record_host for a canonical view. */
+ * s1 and z in the order the decode kernel's B-operand builder reads them (a
+ * permutation of the channels, kaux_of_elem in csrc/kvarn_common.cuh); use kvarn_unpack_record_host for a canonical view. */
 typedef struct {
   size_t record_bytes; /* 4608 at 2-bit, 8704 at 4-bit (=> 2.25 / 4.25 bit per element) */
   size_t codes_off, codes_bytes;

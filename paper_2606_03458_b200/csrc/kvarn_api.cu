@@ -402,7 +402,7 @@ int kvarn_unpack_record_host(const kvarn_params* p, int32_t kind, const void* re
     }
   for (int i = 0; i < 128; ++i) {
     // K records keep s1 and z (per channel) in K-position order; everything else is natural
-    const int gi = (kind == KVARN_KIND_K) ? kpos_of_elem(bits, i) : i;
+    const int gi = (kind == KVARN_KIND_K) ? kaux_of_elem(bits, i) : i;
     s1[i] = e4m3_to_f32(r[s1_off(bits) + gi]);
     s2[i] = e4m3_to_f32(r[s2_off(bits) + i]);
     uint16_t zb;
@@ -427,7 +427,7 @@ int kvarn_pack_record_host(const kvarn_params* p, int32_t kind, const uint8_t* c
       r[code_off(row, e / per_byte)] |= (uint8_t)(code << (bits * (e % per_byte)));
     }
   for (int i = 0; i < 128; ++i) {
-    const int gi = (kind == KVARN_KIND_K) ? kpos_of_elem(bits, i) : i;
+    const int gi = (kind == KVARN_KIND_K) ? kaux_of_elem(bits, i) : i;
     r[s1_off(bits) + gi] = f32_to_e4m3(s1[i]);
     r[s2_off(bits) + i] = f32_to_e4m3(s2[i]);
     const uint16_t zb = f32_to_f16_bits(z[i]);

@@ -34,13 +34,18 @@ __host__ __device__ constexpr int code_off(int row, int byte_in_row) {
 // "K position" of element e of a code row inside the tensor-core A operand:
 // the decode kernel expands a packed 32-bit word W with  W & (mask << bits*j), so
 // byte b of A column (8/bits)*w + j holds element (32/bits)*w + (8/bits)*b + j.
-// kpos = 4*column + b.  The per-channel aux arrays of K records (s1, z) are
-// stored in K-position order so the B-operand builder reads them contiguously.
+// kpos = 4*column + b.
 __host__ __device__ constexpr int kpos_of_elem(int bits, int e) {
   return bits == 2 ? ((e & ~15) | ((e & 3) << 2) | ((e >> 2) & 3)) : ((e & ~7) | ((e & 1) << 2) | ((e >> 1) & 3));
 }
 __host__ __device__ constexpr int elem_of_kpos(int bits, int k) {
   return bits == 2 ? ((k & ~15) | ((k & 3) << 2) | ((k >> 2) & 3)) : ((k & ~7) | ((k & 3) << 1) | ((k >> 2) & 1));
+}
+// The per-channel aux arrays of K records (s1, z) are stored so that lane l of
+// the decode kernel's B-operand builder, which owns K positions l, l+32, l+64,
+// l+96, reads its four values contiguously: index 4*(kpos & 31) + (kpos >> 5).
+__host__ __device__ constexpr int kaux_of_elem(int bits, int e) {
+  return 4 * (kpos_of_elem(bits, e) & 31) + (kpos_of_elem(bits, e) >> 5);
 }
 
 // ---- storage formats -------------------------------------------------------

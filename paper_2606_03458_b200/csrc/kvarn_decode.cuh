@@ -122,21 +122,27 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {
 }
 
 // ------------------------------------------------------------------ operand geometry
-// B operand in shared memory: K-major, no swizzle, 8-row x 16-byte core matrices.
-// Core matrices of consecutive 16-byte K blocks are 144 bytes apart (128 + 16 of
-// padding) so that a warp writing one row at 32 consecutive K words touches 32
-// different banks; 8-row groups are 8 * 144 bytes apart.
-constexpr int B_LBO = 144;
-constexpr int B_SBO = 8 * B_LBO;
-__host__ __device__ constexpr int b_bytes(int n_rows) { return (n_rows / 8) * B_SBO; }
-__device__ __forceinline__ int b_off(int n, int k) { return (n >> 3) * B_SBO + (k >> 4) * B_LBO + (n & 7) * 16 + (k & 15); }
+// B operand in shared memory: MN-major ("transposed"), no swizzle.  Canonical
+// layout ((16,m),(8,k)) : ((1,SBO),(16,LBO)) bytes: the 16 N values of one K
+// position are 16 contiguous bytes, 8 consecutive K positions are 16 bytes apart
+// (one 128-byte core matrix), groups of 8 K positions LBO = 128 bytes apart, and
+// a second panel of 16 N values (GP = 8) SBO = 2048 bytes further.  So panel p of
+// the operand is a dense [128 K positions][16 bytes] array, and the 16 bytes of
+// a K position are (head-major) the radix-256 digits of 4 heads:
+//     byte 4*(h & 3) + i of panel (h >> 2)  =  digit i of head h,
+// i.e. a thread that holds the 32-bit fixed-point value X of (head h, K position
+// k) stores X itself -- no byte transposes.  D column n = 4*h + i.
+constexpr int B_LBO = 128;
+constexpr int B_SBO = 2048;
+constexpr int B_KSTEP = 32 * 16;   // bytes per MMA K step (32 K positions)
+__host__ __device__ constexpr int b_bytes(int n_rows) { return (n_rows / 16) * B_SBO; }
 
 __device__ __forceinline__ uint64_t b_desc(uint32_t saddr) {
   return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)(B_LBO >> 4) << 16) | ((uint64_t)(B_SBO >> 4) << 32) | (1ull << 46);
 }
-// idesc (kind::i8): D = s32, A = u8, B = s8 (b_signed) or u8, both K-major, M = 128
+// idesc (kind::i8): D = s32, A = u8 (K-major, TMEM), B = s8 (b_signed) or u8, MN-major, M = 128
 __host__ __device__ constexpr uint32_t idesc_i8(int n, int b_signed) {
-  return (2u << 4) | (0u << 7) | ((uint32_t)b_signed << 10) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
+  return (2u << 4) | (0u << 7) | ((uint32_t)b_signed << 10) | (1u << 16) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
 }
 
 template <typename T> __device__ __forceinline__ float ld_in(const T* p);
@@ -191,24 +197,22 @@ struct RMax { __device__ __forceinline__ float operator()(float a, float b) cons
 
 constexpr float MAGIC_F = 12582912.0f;       // 1.5 * 2^23: (x + MAGIC) rounds x to an integer (RNE) for |x| <= 2^22
 constexpr int MAGIC_I = 0x4B400000;
-constexpr float Q_FIX = 4194304.0f;          // 2^22: fixed-point scale of qt relative to max_c |qt[h,c]|
-constexpr float P_FIX = 262143.0f;           // 2^18 - 1: fixed-point scale of pt relative to max_t s1v[t]
+constexpr float Q_FIX = 4194300.0f;          // 2^22: fixed-point scale of qt relative to max_c |qt[h,c]|
+constexpr float P_FIX = 4194304.0f;          // 2^22: fixed-point scale of pt = p s1v <= 1
 
 template <int BITS, int GP>
 struct DecSmem {
   static constexpr int RB = record_bytes(BITS);
   static constexpr int STAGES = BITS == 2 ? 3 : 2;
-  static constexpr int NQ = GP * 4;           // B rows of the QK^T MMA: 4 s8 digit planes per head
-  static constexpr int NP = GP == 4 ? 16 : 32;  // B rows of the PV MMA: 3 u8 digit planes per head, padded to 16 | 32
+  static constexpr int NB = GP * 4;           // N of both MMAs: 4 radix-256 digits per head (D column 4 h + i)
   alignas(128) uint8_t rec[STAGES][2][RB];     // [stage][K | V] records
-  alignas(128) uint8_t bq[b_bytes(NQ)];
-  alignas(128) uint8_t bp[b_bytes(NP)];
+  alignas(128) uint8_t bq[b_bytes(NB)];
+  alignas(128) uint8_t bp[b_bytes(NB)];
   alignas(16) float qrot[GP][128];             // q' (rotated, scaled); later: merged acc_rot for the inverse Hadamard
   alignas(16) float qraw[GP][128];             // q * q_scale (un-rotated, for the residual window); later p of the residual
   alignas(16) float hs[GP][2];                 // per head: {scale, beta} of the current chunk
   alignas(16) float wmax[4][GP];               // per-warp partial maxima
   alignas(16) float wz[4][GP];                 // per-warp partial zero-point sums / l sums
-  float pscale[2];                             // {P_FIX / s1vmax, s1vmax / P_FIX}
   alignas(8) uint64_t full[STAGES];
   alignas(8) uint64_t mma_bar[2];              // QK^T done, PV done
   uint32_t tmem_base;
@@ -233,13 +237,14 @@ __device__ __forceinline__ void unpack_row(const uint8_t* codes, int r, uint32_t
 }
 
 template <int BITS, int GP, typename InT>
-__global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
+__global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_tc_kernel(const DecodeArgs A) {
   using SM = DecSmem<BITS, GP>;
-  constexpr int RB = SM::RB, STAGES = SM::STAGES, NQ = SM::NQ, NP = SM::NP;
+  constexpr int RB = SM::RB, STAGES = SM::STAGES, NB = SM::NB;
   constexpr int NCLS = 8 / BITS;
   constexpr float CLS_INV = BITS == 2 ? (1.f / 64.f) : (1.f / 16.f);  // 1 / CLSMAX
   constexpr int HPW = GP / 4;                                          // heads per warp in the B_q builder
-  constexpr uint32_t TM_AK = 0, TM_AV = 32, TM_D1 = 64, TM_D2 = 96;
+  // TMEM columns: A operand (K tile, then V tile of the same chunk), D (logits, then values)
+  constexpr uint32_t TM_A = 0, TM_D = 32, TM_COLS = 64;
 
   extern __shared__ __align__(128) uint8_t smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
@@ -277,7 +282,7 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
         bulk_g2s(sm.rec[s][1], vrec + (size_t)s * RB, RB, &sm.full[s]);
       }
   }
-  if (warp == 1 && n_my > 0) tmem_alloc<128>(&sm.tmem_base);
+  if (warp == 1 && n_my > 0) tmem_alloc<TM_COLS>(&sm.tmem_base);
 
   // D1: q' = (q H / sqrt(128)) * q_scale; heads >= g are zero
   for (int hh = warp; hh < GP; hh += 4) {
@@ -299,21 +304,29 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
   __syncthreads();
   tc_fence_after();
 
-  // B_q builder role: lane = A column kg (K positions 4kg..4kg+3), warp -> heads warp, warp+4
-  // channel at K position 4kg+b:  2-bit  16*(kg>>2) + 4b + (kg&3);  4-bit  8*(kg>>1) + 2b + (kg&1)
+  // B_q builder role: warp -> heads warp (+4); lane owns K positions lane + 32 r, r = 0..3, which
+  // all sit in byte (lane & 3) of an A column of class j = (lane >> 2) & (NCLS - 1):
+  //   2-bit  channel = 32 r + 16 (lane >> 4) + 4 (lane & 3) + ((lane >> 2) & 3)
+  //   4-bit  channel = 32 r +  8 (lane >> 3) + 2 (lane & 3) + ((lane >> 2) & 1)
   float qreg[HPW][4];
   {
-    const int cbase = BITS == 2 ? 16 * (lane >> 2) + (lane & 3) : 8 * (lane >> 1) + (lane & 1);
+    const int cbase = BITS == 2 ? 16 * (lane >> 4) + 4 * (lane & 3) + ((lane >> 2) & 3)
+                                : 8 * (lane >> 3) + 2 * (lane & 3) + ((lane >> 2) & 1);
 #pragma unroll
     for (int u = 0; u < HPW; ++u)
 #pragma unroll
-      for (int bb = 0; bb < 4; ++bb) qreg[u][bb] = sm.qrot[warp + 4 * u][cbase + NCLS * bb];
+      for (int r = 0; r < 4; ++r) qreg[u][r] = sm.qrot[warp + 4 * u][cbase + 32 * r];
   }
-  const int shift_q = BITS * (NCLS - 1 - (lane & (NCLS - 1)));  // class of column `lane`
+  // fixed-point value -> digits: X = (bits(f) - MAGIC_I) << shift, balanced:  (X + 0x80808080) ^ 0x80808080
+  const int shift_q = BITS * (NCLS - 1 - ((lane >> 2) & (NCLS - 1)));
+  const uint32_t mul_q = 1u << shift_q;
+  const uint32_t add_q = 0x80808080u - ((uint32_t)MAGIC_I << shift_q);
   // token role (softmax): K position of token tid in a V code row, and its class shift
   const int kpos_t = BITS == 2 ? ((tid & ~15) | ((tid & 3) << 2) | ((tid >> 2) & 3))
                                : ((tid & ~7) | ((tid & 1) << 2) | ((tid >> 1) & 3));
   const int shift_p = BITS * (NCLS - 1 - (tid & (NCLS - 1)));
+  const uint32_t mul_p = 1u << shift_p;
+  const uint32_t add_p = 0u - ((uint32_t)MAGIC_I << shift_p);
 
   float m_run[GP], l_part[GP], acc[GP];
 #pragma unroll
@@ -334,10 +347,10 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
     {
       uint32_t a[32];
       unpack_row<BITS>(kr, tid, a);
-      tmem_st32(taddr_w + TM_AK, a);
+      tmem_st32(taddr_w + TM_A, a);
     }
     {
-      // aux of the K record in K-position order: s1p[4kg+b], zp[4kg+b]
+      // aux of the K record in builder order: s1[4 lane + r], z[4 lane + r] <-> K position lane + 32 r
       const uint32_t s1w = *reinterpret_cast<const uint32_t*>(kr + s1_off(BITS) + 4 * lane);
       const uint2 zw = *reinterpret_cast<const uint2*>(kr + z_off(BITS) + 8 * lane);
       const float2 s01 = e4m3x2_to_f32x2((uint16_t)(s1w & 0xffff)), s23 = e4m3x2_to_f32x2((uint16_t)(s1w >> 16));
@@ -345,66 +358,38 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
       const float2 z01 = __half22float2(*reinterpret_cast<const __half2*>(&zw.x));
       const float2 z23 = __half22float2(*reinterpret_cast<const __half2*>(&zw.y));
       const float z[4] = {z01.x, z01.y, z23.x, z23.y};
-      float qt[HPW][4], amax[HPW];
+      float qt[HPW][4], amax[HPW], bsum[HPW];
 #pragma unroll
       for (int u = 0; u < HPW; ++u) {
 #pragma unroll
-        for (int bb = 0; bb < 4; ++bb) qt[u][bb] = qreg[u][bb] * s1[bb];
+        for (int r = 0; r < 4; ++r) qt[u][r] = qreg[u][r] * s1[r];
         amax[u] = fmaxf(fmaxf(fabsf(qt[u][0]), fabsf(qt[u][1])), fmaxf(fabsf(qt[u][2]), fabsf(qt[u][3])));
+        // beta uses the unrounded qt: it differs from the 22-bit fixed-point value by < 2^-23 max|qt|
+        bsum[u] = fmaf(qt[u][0], z[0], fmaf(qt[u][1], z[1], fmaf(qt[u][2], z[2], qt[u][3] * z[3])));
       }
 #pragma unroll
-      for (int m = 16; m > 0; m >>= 1)
-#pragma unroll
-        for (int u = 0; u < HPW; ++u) amax[u] = fmaxf(amax[u], __shfl_xor_sync(0xffffffffu, amax[u], m));
-      float bsum[HPW];
-#pragma unroll
-      for (int u = 0; u < HPW; ++u) {
-        const float inv = amax[u] > 0.f ? Q_FIX / amax[u] : 0.f;
-        uint32_t x[4];
-        bsum[u] = 0.f;
-#pragma unroll
-        for (int bb = 0; bb < 4; ++bb) {
-          const float f = fmaf(qt[u][bb], inv, MAGIC_F);            // integer Q in the low mantissa bits
-          bsum[u] = fmaf(f - MAGIC_F, z[bb], bsum[u]);               // Q * z
-          const int Q = __float_as_int(f) - MAGIC_I;
-          const uint32_t X = (uint32_t)Q << shift_q;              // Q * CLSMAX / cls
-          x[bb] = (X + 0x80808080u) ^ 0x80808080u;                   // bytes = balanced radix-256 digits (s8)
-        }
-        // 4 x 4 byte transpose: word i = digit i of the 4 K positions
-        const uint32_t t0 = __byte_perm(x[0], x[1], 0x5140), t1 = __byte_perm(x[2], x[3], 0x5140);
-        const uint32_t t2 = __byte_perm(x[0], x[1], 0x7362), t3 = __byte_perm(x[2], x[3], 0x7362);
-        const uint32_t d0 = __byte_perm(t0, t1, 0x5410), d1 = __byte_perm(t0, t1, 0x7632);
-        const uint32_t d2 = __byte_perm(t2, t3, 0x5410), d3 = __byte_perm(t2, t3, 0x7632);
-        const int h = warp + 4 * u;
-        *reinterpret_cast<uint32_t*>(sm.bq + b_off(0 * GP + h, 4 * lane)) = d0;
-        *reinterpret_cast<uint32_t*>(sm.bq + b_off(1 * GP + h, 4 * lane)) = d1;
-        *reinterpret_cast<uint32_t*>(sm.bq + b_off(2 * GP + h, 4 * lane)) = d2;
-        *reinterpret_cast<uint32_t*>(sm.bq + b_off(3 * GP + h, 4 * lane)) = d3;
-      }
+      for (int u = 0; u < HPW; ++u)   // non-negative floats order like their bit patterns
+        amax[u] = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax[u])));
 #pragma unroll
       for (int m = 16; m > 0; m >>= 1)
 #pragma unroll
         for (int u = 0; u < HPW; ++u) bsum[u] += __shfl_xor_sync(0xffffffffu, bsum[u], m);
-      if (lane == 0) {
 #pragma unroll
-        for (int u = 0; u < HPW; ++u) {
-          const float sc = amax[u] * (1.f / Q_FIX);
-          sm.hs[warp + 4 * u][0] = sc * CLS_INV;   // logit = s2 * (acc * scale + beta)
-          sm.hs[warp + 4 * u][1] = sc * bsum[u];
+      for (int u = 0; u < HPW; ++u) {
+        const int h = warp + 4 * u;
+        const float inv = amax[u] > 0.f ? Q_FIX * __fdividef(1.f, amax[u]) : 0.f;
+        uint8_t* dst = sm.bq + (h >> 2) * B_SBO + lane * 16 + 4 * (h & 3);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          const float f = fmaf(qt[u][r], inv, MAGIC_F);            // integer Q in the low mantissa bits
+          const uint32_t X = (__float_as_uint(f) * mul_q + add_q) ^ 0x80808080u;   // balanced s8 digits of Q << shift
+          *reinterpret_cast<uint32_t*>(dst + r * 512) = X;
         }
-      }
-    }
-    if (warp == 3) {
-      // max_t s1v[t]: e4m3 bytes of positive values order like the values
-      uint32_t w = *reinterpret_cast<const uint32_t*>(vr + s1_off(BITS) + 4 * lane);
-#pragma unroll
-      for (int m = 16; m > 0; m >>= 1) w = __vmaxu4(w, __shfl_xor_sync(0xffffffffu, w, m));
-      w = __vmaxu4(w, w >> 16);
-      w = __vmaxu4(w, w >> 8);
-      if (lane == 0) {
-        const float mx = e4m3_to_f32((uint8_t)(w & 0xff));
-        sm.pscale[0] = mx > 0.f ? P_FIX / mx : 0.f;
-        sm.pscale[1] = mx * (1.f / P_FIX);
+        if (lane == 0) {
+          const float sc = amax[u] * (1.f / Q_FIX);
+          sm.hs[h][0] = sc * CLS_INV;   // logit = s2 * (acc * scale + beta)
+          sm.hs[h][1] = bsum[u];
+        }
       }
     }
     tmem_st_wait();
@@ -416,39 +401,41 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
       const uint64_t bd = b_desc(bq_addr);
 #pragma unroll
       for (int ks = 0; ks < 4; ++ks)
-        umma_i8_ts(tmem + TM_D1, tmem + TM_AK + 8 * ks, bd + (uint64_t)((2 * B_LBO * ks) >> 4), idesc_i8(NQ, 1), ks > 0);
+        umma_i8_ts(tmem + TM_D, tmem + TM_A + 8 * ks, bd + (uint64_t)((B_KSTEP * ks) >> 4), idesc_i8(NB, 1), ks > 0);
       umma_commit(&sm.mma_bar[0]);
     }
 
-    // ---- phase B: V codes -> TMEM (overlaps the QK^T MMA) ------------------------------
-    {
-      uint32_t a[32];
-      unpack_row<BITS>(vr, tid, a);
-      tmem_st32(taddr_w + TM_AV, a);
-    }
+    // ---- phase B: per-token / per-channel aux of this chunk (overlaps the QK^T MMA) -------
     const float s2t = e4m3_to_f32(kr[s2_off(BITS) + tid]);
-    const float s1v = e4m3_to_f32(vr[s1_off(BITS) + tid]);
+    const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + tid]), 9.094947e-13f);   // 2^-40: a zero scale stays harmless
     const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[tid]);
-    const float s2v = e4m3_to_f32(vr[s2_off(BITS) + tid]);          // channel role
-    const float ps0 = sm.pscale[0], ps1 = sm.pscale[1];
+    const float s2v = e4m3_to_f32(vr[s2_off(BITS) + tid]) * (1.f / P_FIX);   // channel role
+    // pt = p s1v = exp2(logit + log2 s1v - m): the running maximum is taken over the shifted logits,
+    // so pt <= 1 and its fixed-point scale is a constant
+    const float lam = __log2f(s1v), inv_s1v = __fdividef(1.f, s1v);
 
-    // ---- D3/D4: logits of token tid, online softmax ---------------------------------------
     mbar_wait(&sm.mma_bar[0], par);
     tc_fence_after();
+    {
+      uint32_t a[32];                      // V codes -> the same TMEM columns (the QK^T MMA is done with them)
+      unpack_row<BITS>(vr, tid, a);
+      tmem_st32(taddr_w + TM_A, a);
+    }
+    // ---- D3/D4: logits of token tid, online softmax ---------------------------------------
     float logit[GP];
     {
       int32_t dlo[16], dhi[16];
-      tmem_ld16(taddr_w + TM_D1, dlo);
-      if (NQ == 32) tmem_ld16(taddr_w + TM_D1 + 16, dhi);
-      auto d = [&](int n) -> int32_t { return n < 16 ? dlo[n & 15] : dhi[n & 15]; };
+      tmem_ld16(taddr_w + TM_D, dlo);
+      if (NB == 32) tmem_ld16(taddr_w + TM_D + 16, dhi);
       tmem_ld_wait();
 #pragma unroll
       for (int h = 0; h < GP; ++h) {
-        const int x01 = d(1 * GP + h) * 256 + d(0 * GP + h);
-        const int x23 = d(3 * GP + h) * 256 + d(2 * GP + h);
+        const int32_t* d = h < 4 ? &dlo[4 * h] : &dhi[4 * (h & 3)];
+        const int x01 = d[1] * 256 + d[0];
+        const int x23 = d[3] * 256 + d[2];
         const float a = fmaf(__int2float_rn(x23), 65536.f, __int2float_rn(x01));
         const float2 sb = *reinterpret_cast<const float2*>(sm.hs[h]);
-        logit[h] = s2t * fmaf(a, sb.x, sb.y);
+        logit[h] = fmaf(s2t, fmaf(a, sb.x, sb.y), lam);
       }
     }
     {
@@ -460,22 +447,22 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
     }
     __syncthreads();                                                   // barrier 2
     float corr[GP], zpart[GP];
+    uint32_t X[GP];
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
       const float mc = fmaxf(fmaxf(sm.wmax[0][h], sm.wmax[1][h]), fmaxf(sm.wmax[2][h], sm.wmax[3][h]));
       const float m_new = fmaxf(m_run[h], mc);
       corr[h] = exp2f(m_run[h] - m_new);
       m_run[h] = m_new;
-      const float p = exp2f(logit[h] - m_new);
-      l_part[h] = fmaf(l_part[h], corr[h], p);
-      // D5 prep: fixed-point pt, its radix-256 digits into B_p at this token's K position
-      const float f = fmaf(p * s1v, ps0, MAGIC_F);
+      const float pt = exp2f(logit[h] - m_new);
+      l_part[h] = fmaf(l_part[h], corr[h], pt * inv_s1v);
+      // D5 prep: fixed-point pt; its radix-256 digits are the bytes of X
+      const float f = fmaf(pt, P_FIX, MAGIC_F);
       zpart[h] = (f - MAGIC_F) * zv;
-      const uint32_t X = (uint32_t)(__float_as_int(f) - MAGIC_I) << shift_p;
-      sm.bp[b_off(0 * GP + h, kpos_t)] = (uint8_t)X;
-      sm.bp[b_off(1 * GP + h, kpos_t)] = (uint8_t)(X >> 8);
-      sm.bp[b_off(2 * GP + h, kpos_t)] = (uint8_t)(X >> 16);
+      X[h] = __float_as_uint(f) * mul_p + add_p;
     }
+    *reinterpret_cast<uint4*>(sm.bp + kpos_t * 16) = make_uint4(X[0], X[1], X[2], X[3]);
+    if (GP == 8) *reinterpret_cast<uint4*>(sm.bp + B_SBO + kpos_t * 16) = make_uint4(X[GP - 4], X[GP - 3], X[GP - 2], X[GP - 1]);
     {
       const float r = warp_reduce_multi<GP>(zpart, lane, RAdd());
       if ((lane & (32 / GP - 1)) == 0) sm.wz[warp][red_index<GP>(lane)] = r;
@@ -489,7 +476,7 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
       const uint64_t bd = b_desc(bp_addr);
 #pragma unroll
       for (int ks = 0; ks < 4; ++ks)
-        umma_i8_ts(tmem + TM_D2, tmem + TM_AV + 8 * ks, bd + (uint64_t)((2 * B_LBO * ks) >> 4), idesc_i8(NP, 0), ks > 0);
+        umma_i8_ts(tmem + TM_D, tmem + TM_A + 8 * ks, bd + (uint64_t)((B_KSTEP * ks) >> 4), idesc_i8(NB, 0), ks > 0);
       umma_commit(&sm.mma_bar[1]);
       // the record slot is free (all aux values are in registers): prefetch chunk it + STAGES
       if (it + STAGES < n_my) {
@@ -507,16 +494,16 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
     tc_fence_after();
     {
       int32_t dlo[16], dhi[16];
-      tmem_ld16(taddr_w + TM_D2, dlo);
-      if (NP == 32) tmem_ld16(taddr_w + TM_D2 + 16, dhi);
-      auto d = [&](int n) -> int32_t { return n < 16 ? dlo[n & 15] : dhi[n & 15]; };
+      tmem_ld16(taddr_w + TM_D, dlo);
+      if (NB == 32) tmem_ld16(taddr_w + TM_D + 16, dhi);
       tmem_ld_wait();
-      const float sc = s2v * ps1;
 #pragma unroll
       for (int h = 0; h < GP; ++h) {
-        const int x01 = d(1 * GP + h) * 256 + d(0 * GP + h);
-        const float a = fmaf(__int2float_rn(d(2 * GP + h)), 65536.f, __int2float_rn(x01));
-        acc[h] = fmaf(acc[h], corr[h], sc * fmaf(a, CLS_INV, zsum[h]));
+        const int32_t* d = h < 4 ? &dlo[4 * h] : &dhi[4 * (h & 3)];
+        const int x01 = d[1] * 256 + d[0];
+        const int x23 = d[3] * 256 + d[2];
+        const float a = fmaf(__int2float_rn(x23), 65536.f, __int2float_rn(x01));
+        acc[h] = fmaf(acc[h], corr[h], s2v * fmaf(a, CLS_INV, zsum[h]));
       }
     }
     tc_fence_before();
@@ -601,7 +588,7 @@ __global__ void __launch_bounds__(128, 4) decode_tc_kernel(const DecodeArgs A) {
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1 && n_my > 0) { tc_fence_after(); tmem_dealloc<128>(tmem); }
+  if (warp == 1 && n_my > 0) { tc_fence_after(); tmem_dealloc<64>(tmem); }
   float l_tot[GP];
 #pragma unroll
   for (int h = 0; h < GP; ++h) l_tot[h] = (sm.wz[0][h] + sm.wz[1][h]) + (sm.wz[2][h] + sm.wz[3][h]);

@@ -335,7 +335,7 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       const float z = mn / s;
       sm.inv_s[tid] = 1.f / s; sm.z[tid] = z;
       const float s1 = s * sm.Sr[tid], s2 = sm.Sc[tid];  // K: s1 per channel, s2 per token
-      const int kp = kpos_of_elem(BITS, tid);  // K records keep s1, z in K-position order
+      const int kp = kaux_of_elem(BITS, tid);  // K records keep s1, z in K-position order
       sm.rec[s1_off(BITS) + kp] = f32_to_e4m3(s1);
       sm.rec[s2_off(BITS) + tid] = f32_to_e4m3(s2);
       reinterpret_cast<uint16_t*>(&sm.rec[z_off(BITS)])[kp] = f32_to_f16_bits(z);

@@ -114,7 +114,7 @@ def test_pack_unpack_round_trip_and_formats(kv, bits, kind):
         e = np.arange(128)
         kpos = ((e & ~15) | ((e & 3) << 2) | ((e >> 2) & 3)) if bits == 2 else ((e & ~7) | ((e & 1) << 2) | ((e >> 1) & 3))
         assert sorted(kpos.tolist()) == list(range(128))
-        stored = stored[kpos]
+        stored = stored[4 * (kpos & 31) + (kpos >> 5)]   # lane-contiguous order of the B-operand builder
     assert np.array_equal(stored, O.fp8_e4m3_bits(O.round_fp8_e4m3(s1.astype(np.float64))))
     # saturation
     rec = kv.pack_record(p, kind, codes, np.full(128, 1e6, np.float32), s2, z)
