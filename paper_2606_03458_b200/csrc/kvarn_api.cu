@@ -150,21 +150,75 @@ static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kind
   return last_cuda();
 }
 
-static int auto_splits(const kvarn_params* p, int B, int Hkv, int max_chunks) {
-  if (p->splits > 0) return p->splits < max_chunks ? p->splits : (max_chunks > 0 ? max_chunks : 1);
+// Split-K plan of kvarn_decode_attention: `cluster` CTAs of a thread-block cluster share one
+// (sequence, KV head) and merge through DSMEM; `nclus` clusters per (sequence, KV head) merge
+// through the workspace (only when one cluster leaves most of the GPU idle on long contexts).
+struct SplitPlan { int cluster, nclus; };
+
+template <int BITS, int GP, typename InT>
+static int decode_ctas_per_sm() {
+  static int cached = 0;   // per instantiation; benign race (same value)
+  if (cached) return cached;
+  using SM = DecSmem<BITS, GP>;
+  auto kern = decode_kernel<BITS, GP, InT>;
+  int n = 0;
+  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SM));
+  cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 128, sizeof(SM)) != cudaSuccess || n < 1) {
+    cudaGetLastError();
+    n = GP == 4 ? 4 : 3;   // no device (host-only queries): a conservative constant
+    return n;
+  }
+  cached = n;
+  return n;
+}
+static int decode_slots(const kvarn_params* p, int g) {
+  int sms = 148, dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  else cudaGetLastError();
+  const bool f32 = p->in_dtype == KVARN_F32;
+  int per;
+  if (p->bits == 2) per = g <= 4 ? (f32 ? decode_ctas_per_sm<2, 4, float>() : decode_ctas_per_sm<2, 4, __nv_bfloat16>())
+                                 : (f32 ? decode_ctas_per_sm<2, 8, float>() : decode_ctas_per_sm<2, 8, __nv_bfloat16>());
+  else per = g <= 4 ? (f32 ? decode_ctas_per_sm<4, 4, float>() : decode_ctas_per_sm<4, 4, __nv_bfloat16>())
+                    : (f32 ? decode_ctas_per_sm<4, 8, float>() : decode_ctas_per_sm<4, 8, __nv_bfloat16>());
+  return sms * per;
+}
+
+static SplitPlan split_plan(const kvarn_params* p, int B, int Hkv, int g, int max_chunks) {
+  SplitPlan sp{1, 1};
+  if (max_chunks <= 1) return sp;
+  if (p->splits > 0) {   // caller-chosen total: the largest cluster size (<= 8) that divides it
+    int s = p->splits < max_chunks ? p->splits : max_chunks;
+    int cs = 8;
+    while (s % cs) --cs;
+    sp.cluster = cs; sp.nclus = s / cs;
+    if (sp.nclus > 64) sp.nclus = 64;
+    return sp;
+  }
   const int bh = B * Hkv;
-  int s = (148 * 4 + bh / 2) / bh;   // about one wave of 148 SMs x 4 resident CTAs
-  if (s > 64) s = 64;
-  if (s > max_chunks) s = max_chunks;
-  if (s < 1) s = 1;
-  return s;
+  const int slots = decode_slots(p, g);        // resident CTAs of decode_kernel on this device
+  int want = slots / bh;                        // splits that still fit in one wave
+  if (want < 1) want = 1;
+  if (want > max_chunks) want = max_chunks;
+  sp.cluster = want < 8 ? want : 8;
+  if (sp.cluster == 8) {
+    const int per = (max_chunks + 7) / 8;       // chunks per CTA with one cluster
+    if (per > 32) {
+      int nc = want / 8, cap = per / 16;
+      if (nc > cap) nc = cap;
+      if (nc > 64) nc = 64;
+      if (nc > 1) sp.nclus = nc;
+    }
+  }
+  return sp;
 }
 
 template <int BITS, int GP, typename InT>
-static cudaError_t launch_decode_tc(const DecodeArgs& A, cudaStream_t st) {
+static cudaError_t launch_decode_k(const DecodeArgs& A, cudaStream_t st) {
   using SM = DecSmem<BITS, GP>;
   static bool configured = false;   // per instantiation; benign race (idempotent attribute calls)
-  auto kern = decode_tc_kernel<BITS, GP, InT>;
+  auto kern = decode_kernel<BITS, GP, InT>;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SM));
     if (e != cudaSuccess) return e;
@@ -172,14 +226,21 @@ static cudaError_t launch_decode_tc(const DecodeArgs& A, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  dim3 grid(A.B * A.Hkv, A.splits), block(128);
-  kern<<<grid, block, sizeof(SM), st>>>(A);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(A.B * A.Hkv, A.splits, 1);
+  cfg.blockDim = dim3(128, 1, 1);
+  cfg.dynamicSmemBytes = sizeof(SM);
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 1; attr[0].val.clusterDim.y = (unsigned)A.cluster; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = A.cluster > 1 ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, A);
 }
 
 template <int BITS, typename InT>
 static cudaError_t launch_decode(const DecodeArgs& A, cudaStream_t st) {
-  return A.g <= 4 ? launch_decode_tc<BITS, 4, InT>(A, st) : launch_decode_tc<BITS, 8, InT>(A, st);
+  return A.g <= 4 ? launch_decode_k<BITS, 4, InT>(A, st) : launch_decode_k<BITS, 8, InT>(A, st);
 }
 
 }  // namespace kvarn
@@ -225,8 +286,8 @@ int kvarn_layout(const kvarn_params* p, kvarn_layout_info* out) {
 size_t kvarn_decode_workspace_bytes(const kvarn_params* p, int32_t B, int32_t Hq, int32_t Hkv,
                                     int32_t max_chunks) {
   if (!p || B <= 0 || Hq <= 0 || Hkv <= 0) return 0;
-  const int s = auto_splits(p, B, Hkv, max_chunks);
-  return (size_t)B * Hq * s * WS_STRIDE * sizeof(float);
+  const SplitPlan sp = split_plan(p, B, Hkv, Hq / Hkv, max_chunks);
+  return (size_t)B * Hq * sp.nclus * WS_STRIDE * sizeof(float);   // read and written only when nclus > 1
 }
 
 int kvarn_quantize_chunk(const kvarn_params* p, const void* k, const void* v, int64_t n_tiles,
@@ -338,7 +399,8 @@ int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, cons
   A.ticket = cache->decode_ticket;
   A.q = q; A.out = out; A.ws = (float*)ws;
   A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;
-  A.splits = auto_splits(p, cache->B, cache->Hkv, cache->max_chunks);
+  const SplitPlan sp = split_plan(p, cache->B, cache->Hkv, g, cache->max_chunks);
+  A.cluster = sp.cluster; A.nclus = sp.nclus; A.splits = sp.cluster * sp.nclus;
   A.q_scale = sm_scale * 1.4426950408889634f;
   A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
   cudaStream_t s = (cudaStream_t)stream;
@@ -395,16 +457,19 @@ int kvarn_unpack_record_host(const kvarn_params* p, int32_t kind, const void* re
   (void)rowb;
   for (int row = 0; row < 128; ++row)
     for (int e = 0; e < 128; ++e) {
-      const uint8_t byte = r[code_off(row, e / per_byte)];
+      const int slot = (kind == KVARN_KIND_K) ? slot_of_token(bits, row) : row;
+      const uint8_t byte = r[code_off(bits, slot, e / per_byte)];
       const uint8_t code = (byte >> (bits * (e % per_byte))) & lv;
       if (kind == KVARN_KIND_K) codes[row * 128 + e] = code;   // row = token, e = channel
       else codes[e * 128 + row] = code;                        // row = channel, e = token
     }
   for (int i = 0; i < 128; ++i) {
-    // K records keep s1 and z (per channel) in K-position order; everything else is natural
-    const int gi = (kind == KVARN_KIND_K) ? kaux_of_elem(bits, i) : i;
+    // K: s1, z per channel in B-operand builder order, s2 per token in row-slot order;
+    // V: s1, z per token in row-slot order, s2 per channel in natural order
+    const int gi = (kind == KVARN_KIND_K) ? kaux_of_elem(bits, i) : slot_of_token(bits, i);
+    const int si = (kind == KVARN_KIND_K) ? slot_of_token(bits, i) : i;
     s1[i] = e4m3_to_f32(r[s1_off(bits) + gi]);
-    s2[i] = e4m3_to_f32(r[s2_off(bits) + i]);
+    s2[i] = e4m3_to_f32(r[s2_off(bits) + si]);
     uint16_t zb;
     memcpy(&zb, r + z_off(bits) + 2 * gi, 2);
     z[i] = f16_bits_to_f32(zb);
@@ -424,12 +489,14 @@ int kvarn_pack_record_host(const kvarn_params* p, int32_t kind, const uint8_t* c
   for (int row = 0; row < 128; ++row)
     for (int e = 0; e < 128; ++e) {
       const uint8_t code = (kind == KVARN_KIND_K ? codes[row * 128 + e] : codes[e * 128 + row]) & lv;
-      r[code_off(row, e / per_byte)] |= (uint8_t)(code << (bits * (e % per_byte)));
+      const int slot = (kind == KVARN_KIND_K) ? slot_of_token(bits, row) : row;
+      r[code_off(bits, slot, e / per_byte)] |= (uint8_t)(code << (bits * (e % per_byte)));
     }
   for (int i = 0; i < 128; ++i) {
-    const int gi = (kind == KVARN_KIND_K) ? kaux_of_elem(bits, i) : i;
+    const int gi = (kind == KVARN_KIND_K) ? kaux_of_elem(bits, i) : slot_of_token(bits, i);
+    const int si = (kind == KVARN_KIND_K) ? slot_of_token(bits, i) : i;
     r[s1_off(bits) + gi] = f32_to_e4m3(s1[i]);
-    r[s2_off(bits) + i] = f32_to_e4m3(s2[i]);
+    r[s2_off(bits) + si] = f32_to_e4m3(s2[i]);
     const uint16_t zb = f32_to_f16_bits(z[i]);
     memcpy(r + z_off(bits) + 2 * gi, &zb, 2);
   }

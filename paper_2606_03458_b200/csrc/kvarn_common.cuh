@@ -24,29 +24,50 @@ __host__ __device__ constexpr int s1_off(int bits) { return codes_bytes(bits); }
 __host__ __device__ constexpr int s2_off(int bits) { return codes_bytes(bits) + 128; }
 __host__ __device__ constexpr int z_off(int bits) { return codes_bytes(bits) + 256; }
 
-// Code rows are stored "segment-major": the 16-byte segment s of row r (a row =
-// the 128 codes of one token (K) / one channel (V), little-endian, element e at
-// bit bits*(e % (8/bits)) of byte e*bits/8) sits at  s*2048 + r*16, so that 128
-// threads reading one segment of their own row touch consecutive 16-byte words.
-__host__ __device__ constexpr int code_off(int row, int byte_in_row) {
-  return (byte_in_row >> 4) * 2048 + row * 16 + (byte_in_row & 15);
+// ---- record layout ---------------------------------
+// The decode kernel contracts with warp-level IMMA m16n8k32 (u8 x s8/u8 -> s32):
+// the 128 code rows of a record (K: one row per token, V: one row per channel;
+// a row = 128 codes, little-endian, element e at bit bits*(e % (8/bits)) of byte
+// e*bits/8) are the M rows.  "Slot" s = 32*warp + 16*mtile + 8*rho + g names the
+// MMA row that thread (g = lane>>2, t = lane&3) of `warp` holds in A registers
+// a[rho] / a[rho+2] of m-tile `mtile`.  A packed 32-bit word W of a row expands
+// with one LOP3 per register,  W & (mask << bits*j),  into the four k-bytes of
+// one A register, so thread t needs words t, t+4 (, t+8, t+12 at 4-bit) of its
+// four rows; they are stored so that each (warp, mtile[, rho]) is one conflict-
+// free LDS.128 per lane.
+__host__ __device__ constexpr int code_off(int bits, int slot, int byte_in_row) {
+  const int wi = byte_in_row >> 2, bb = byte_in_row & 3;
+  const int w = slot >> 5, mt = (slot >> 4) & 1, rho = (slot >> 3) & 1, g = slot & 7;
+  const int t = wi & 3, q = wi >> 2;
+  return bits == 2 ? w * 1024 + mt * 512 + (4 * g + t) * 16 + rho * 8 + q * 4 + bb
+                   : w * 2048 + mt * 1024 + rho * 512 + (4 * g + t) * 16 + q * 4 + bb;
 }
-// "K position" of element e of a code row inside the tensor-core A operand:
-// the decode kernel expands a packed 32-bit word W with  W & (mask << bits*j), so
-// byte b of A column (8/bits)*w + j holds element (32/bits)*w + (8/bits)*b + j.
-// kpos = 4*column + b.
-__host__ __device__ constexpr int kpos_of_elem(int bits, int e) {
-  return bits == 2 ? ((e & ~15) | ((e & 3) << 2) | ((e >> 2) & 3)) : ((e & ~7) | ((e & 1) << 2) | ((e >> 1) & 3));
+// Position of element e of a code row in the contraction (K) dimension: k-step
+// kappa (32 positions each) and position p inside it.  All codes of one k-step
+// sit at the same bit offset bits*j inside their byte (2-bit: j = kappa, 4-bit:
+// j = kappa & 1); the B operand compensates with a power of two.
+__host__ __device__ constexpr int kstep_of_elem(int bits, int e) {
+  return bits == 2 ? (e & 3) : (2 * (e >> 6) + (e & 1));
 }
-__host__ __device__ constexpr int elem_of_kpos(int bits, int k) {
-  return bits == 2 ? ((k & ~15) | ((k & 3) << 2) | ((k >> 2) & 3)) : ((k & ~7) | ((k & 3) << 1) | ((k >> 2) & 1));
+__host__ __device__ constexpr int kpos_of_elem(int bits, int e) {   // p = 16*half + 4*t' + b
+  return bits == 2 ? (16 * (e >> 6) + 4 * ((e >> 4) & 3) + ((e >> 2) & 3))
+                   : (16 * ((e >> 5) & 1) + 4 * ((e >> 3) & 3) + ((e >> 1) & 3));
 }
-// The per-channel aux arrays of K records (s1, z) are stored so that lane l of
-// the decode kernel's B-operand builder, which owns K positions l, l+32, l+64,
-// l+96, reads its four values contiguously: index 4*(kpos & 31) + (kpos >> 5).
+// B-operand builder lane that owns element e:  lane = 8*kappa + 4*half + t',  its b-th value.
 __host__ __device__ constexpr int kaux_of_elem(int bits, int e) {
-  return 4 * (kpos_of_elem(bits, e) & 31) + (kpos_of_elem(bits, e) >> 5);
+  return 4 * (8 * kstep_of_elem(bits, e) + (kpos_of_elem(bits, e) >> 2)) + (kpos_of_elem(bits, e) & 3);
 }
+// K records: MMA row slot of token tau.  Chosen so that the four tokens a thread
+// sees in its C fragments (mtile, rho) are the four k-bytes b = 2*mtile + rho of
+// one B-operand word of the value contraction (k-step = warp, half = g>>2, t' = g&3).
+__host__ __device__ constexpr int slot_of_token(int bits, int tau) {
+  return bits == 2
+             ? 32 * (tau & 3) + 16 * ((tau >> 3) & 1) + 8 * ((tau >> 2) & 1) + ((((tau >> 6) & 1) << 2) | ((tau >> 4) & 3))
+             : 32 * ((((tau >> 6) & 1) << 1) | (tau & 1)) + 16 * ((tau >> 2) & 1) + 8 * ((tau >> 1) & 1) +
+                   ((((tau >> 5) & 1) << 2) | ((tau >> 3) & 3));
+}
+// Aux arrays: per-token arrays (K.s2, V.s1, V.z) are stored at index slot_of_token(tau);
+// K.s1 and K.z (per channel) at index kaux_of_elem(c); V.s2 (per channel) at index c.
 
 // ---- storage formats -------------------------------------------------------
 // FP8 E4M3 (finite, max 448), round-to-nearest-even, saturating (DESIGN R9).

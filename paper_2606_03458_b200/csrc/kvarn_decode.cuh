@@ -1,6 +1,7 @@
-// kvarn_decode_attention for sm_100a: split-K over 128-token chunks, the two
-// g x 128 x 128 contractions of every chunk on the 5th-gen tensor cores
-// (tcgen05.mma kind::i8, accumulators in TMEM), records staged by TMA bulk copies.
+// kvarn_decode_attention for sm_100a: split-K over 128-token chunks; records staged
+// by TMA bulk copies into a shared-memory ring; the two g x 128 x 128 contractions of
+// every chunk run on the tensor cores as integer MMAs straight on the packed codes;
+// split partials merge through distributed shared memory inside a thread-block cluster.
 // SURVEY 8(a) rows D1-D7; DESIGN.md "Decode kernel".
 //
 //   D1  q' = (q H / sqrt(128)) * sm_scale * log2(e)                    (online Q transform)
@@ -10,33 +11,41 @@
 //   D4  online softmax in the log2 domain
 //   D5  pt[h,t] = p[h,t] s1v[t];  a[h,c] = sum_t pt[h,t] (codeV[t,c] + zv[t]);  acc[h,c] += s2v[c] a[h,c]
 //   D6  residual window: raw tokens in the un-rotated space
-//   D7  split partials -> workspace; the last CTA of a (sequence, KV head) merges them
-//       (log-sum-exp), applies the inverse Hadamard and normalises.
+//   D7  split partials: reduce-scatter by head through DSMEM inside the cluster (and through
+//       the workspace when several clusters share a sequence), inverse Hadamard, normalise.
 //
 // How the contractions reach the tensor cores without a dequantised tile
 // ---------------------------------------------------------------------
-// A operand (M = 128 rows, K = 128, u8) lives in TMEM: thread r owns row r
-// (K tile: token r, V tile: channel r), reads the row's packed codes from the
-// staged record and expands them with ONE LOP3 per four codes:
-//     column(NCLS*w + j) = W[w] & (MASK0 << BITS*j)
-// i.e. the code stays where it is inside its byte and therefore carries the
-// factor cls = 2^(BITS*j).  The B operand compensates: the fixed-point value
-// of qt (or pt) at that K position is multiplied by CLSMAX / cls before it is
-// split into radix-256 digits (s8 digits for qt, u8 digits for pt).  Each digit
-// plane is one B row, so one MMA yields, per token, the exact int32 sums
-//     D[t][i*GP + h] = sum_k A[t,k] * digit_i(X[h,k])
-// and  sum_c Q[h,c] code[t,c] = (sum_i 256^i D[t][i*GP+h]) / CLSMAX  exactly.
+// A operand = the codes themselves (u8): a thread expands the packed words of its
+// MMA rows (K tile: tokens, V tile: channels) with ONE LOP3 per four codes,
+//     reg(kappa) = W & (MASK0 << BITS*j(kappa)),
+// i.e. a code stays where it is inside its byte and carries the factor 2^(BITS*j),
+// the same for every code of k-step kappa.  The B operand compensates: the
+// fixed-point value of qt (or pt) at that K position is multiplied by
+// CLSMAX / 2^(BITS*j) before it is split into radix-256 digits (s8 digits for qt,
+// u8 digits for pt).  Each digit plane is one B column, so the MMA yields, per
+// token, the exact int32 sums  D[t][(h, i)] = sum_k A[t,k] * digit_i(X[h,k])  and
+//     sum_c Q[h,c] code[t,c] = (sum_i 256^i D[t][(h,i)]) / CLSMAX   exactly.
 // The only rounding is the fixed-point conversion of qt (22 bits + sign relative
-// to max_c |qt[h,c]|) and pt (18 bits relative to max_t s1v[t]); beta and the
-// zero-point term of V use the SAME fixed-point values, so no cancellation
-// error appears between the code term and the zero-point term.
+// to max_c |qt[h,c]|) and pt (22 bits, pt <= 1); beta and the zero-point term of V
+// use the same fixed-point values, so no cancellation error appears between the
+// code term and the zero-point term.
+//
+// Why warp-level mma.sync (IMMA m16n8k32) and not tcgen05: the contraction is tiny
+// (N = 4 digits x g heads <= 32 columns) and the kernel is bound by instruction
+// issue and by the dependent chain of one chunk, not by tensor throughput.  The
+// tcgen05 version of this kernel (git history, profiles/r01b_*) paid two
+// TMEM-store -> MMA -> commit -> mbarrier -> TMEM-load round trips and a
+// single-thread issue path per chunk; register-level MMAs need 128 (g<=4) or 256
+// (g<=8) IMMA per chunk = 270 / 540 tensor-pipe cycles per SM (measured 2.1
+// clk/IMMA/SM), below the HBM time of a chunk, with no asynchronous-proxy hand-off.
 #pragma once
 
 #include "kvarn_common.cuh"
 
 namespace kvarn {
 
-constexpr int WS_STRIDE = 260;  // floats per (b, hq, split): m, l, pad, pad, acc_rot[128], acc_res[128]
+constexpr int WS_STRIDE = 260;  // floats per partial: m, l, pad, pad, acc_rot[128], acc_res[128]
 
 struct DecodeArgs {
   const uint8_t* k_records;
@@ -49,6 +58,8 @@ struct DecodeArgs {
   void* out;
   float* ws;
   int B, Hkv, Hq, g, max_chunks, splits;
+  int cluster;    // CTAs per thread-block cluster along the split axis (1, 2, 4 or 8): merged through DSMEM
+  int nclus;      // clusters per (sequence, KV head); splits = cluster * nclus; nclus > 1 -> workspace merge
   float q_scale;  // sm_scale * log2(e)
   int rotate_k, rotate_v, out_dtype;
 };
@@ -76,73 +87,48 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-template <int NCOLS>
-__device__ __forceinline__ void tmem_alloc(uint32_t* slot) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot)), "n"(NCOLS) : "memory");
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+// thread-block cluster: rank, peer shared-memory addresses (DSMEM), barrier
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
 }
-template <int NCOLS>
-__device__ __forceinline__ void tmem_dealloc(uint32_t base) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "n"(NCOLS) : "memory");
+__device__ __forceinline__ uint32_t mapa_shared(uint32_t saddr, uint32_t cta_rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(cta_rank));
+  return r;
 }
-// 32 lanes x 32 columns: thread i of the warp writes r[0..31] to columns taddr.. of its lane
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
-      "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
-      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
-        "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
-        "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
-        "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-      : "memory");
+__device__ __forceinline__ void st_cluster_f32(uint32_t addr, float v) {
+  asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
 }
-__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, int32_t (&d)[16]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-      : "=r"(d[0]), "=r"(d[1]), "=r"(d[2]), "=r"(d[3]), "=r"(d[4]), "=r"(d[5]), "=r"(d[6]), "=r"(d[7]),
-        "=r"(d[8]), "=r"(d[9]), "=r"(d[10]), "=r"(d[11]), "=r"(d[12]), "=r"(d[13]), "=r"(d[14]), "=r"(d[15])
-      : "r"(taddr) : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// D[tmem] (+)= A[tmem, u8] * B[smem desc]; int32 accumulate
-__device__ __forceinline__ void umma_i8_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t}"
-      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint64_t* bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-// ------------------------------------------------------------------ operand geometry
-// B operand in shared memory: MN-major ("transposed"), no swizzle.  Canonical
-// layout ((16,m),(8,k)) : ((1,SBO),(16,LBO)) bytes: the 16 N values of one K
-// position are 16 contiguous bytes, 8 consecutive K positions are 16 bytes apart
-// (one 128-byte core matrix), groups of 8 K positions LBO = 128 bytes apart, and
-// a second panel of 16 N values (GP = 8) SBO = 2048 bytes further.  So panel p of
-// the operand is a dense [128 K positions][16 bytes] array, and the 16 bytes of
-// a K position are (head-major) the radix-256 digits of 4 heads:
-//     byte 4*(h & 3) + i of panel (h >> 2)  =  digit i of head h,
-// i.e. a thread that holds the 32-bit fixed-point value X of (head h, K position
-// k) stores X itself -- no byte transposes.  D column n = 4*h + i.
-constexpr int B_LBO = 128;
-constexpr int B_SBO = 2048;
-constexpr int B_KSTEP = 32 * 16;   // bytes per MMA K step (32 K positions)
-__host__ __device__ constexpr int b_bytes(int n_rows) { return (n_rows / 16) * B_SBO; }
-
-__device__ __forceinline__ uint64_t b_desc(uint32_t saddr) {
-  return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)(B_LBO >> 4) << 16) | ((uint64_t)(B_SBO >> 4) << 32) | (1ull << 46);
+// D (s32, 16x8) += A (u8, 16x32, row) * B (s8 or u8, 32x8, col)
+template <bool B_SIGNED>
+__device__ __forceinline__ void imma_16832(int32_t (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  if (B_SIGNED)
+    asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.u8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+  else
+    asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.u8.u8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
-// idesc (kind::i8): D = s32, A = u8 (K-major, TMEM), B = s8 (b_signed) or u8, MN-major, M = 128
-__host__ __device__ constexpr uint32_t idesc_i8(int n, int b_signed) {
-  return (2u << 4) | (0u << 7) | ((uint32_t)b_signed << 10) | (1u << 16) | ((uint32_t)(n >> 3) << 17) | ((128u >> 4) << 24);
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+  uint32_t r;
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
+  return r;
+}
+// 4x4 byte transpose: y[d] = (byte d of x[0], x[1], x[2], x[3])
+__device__ __forceinline__ void transpose4x4(const uint32_t (&x)[4], uint32_t (&y)[4]) {
+  const uint32_t t0 = prmt(x[0], x[1], 0x5140), t1 = prmt(x[2], x[3], 0x5140);
+  const uint32_t t2 = prmt(x[0], x[1], 0x7362), t3 = prmt(x[2], x[3], 0x7362);
+  y[0] = prmt(t0, t1, 0x5410); y[1] = prmt(t0, t1, 0x7632);
+  y[2] = prmt(t2, t3, 0x5410); y[3] = prmt(t2, t3, 0x7632);
 }
 
 template <typename T> __device__ __forceinline__ float ld_in(const T* p);
@@ -164,7 +150,7 @@ __device__ __forceinline__ void ld_in8(const __nv_bfloat16* p, float (&v)[8]) {
 // Reduce NV values per lane over the 32 lanes of a warp with the exchange
 // ("transpose") scheme: every step halves the number of live values until one is
 // left, then plain butterflies.  Returns the reduced value of index
-// red_index<NV>(lane) -- every index is held by 32/NV lanes.
+// red_index<NV>(lane) -- every index is held by 32/NV lanes.  (Residual window.)
 template <int NV> __device__ __forceinline__ int red_index(int lane) {
   if (NV == 8) return ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
   if (NV == 4) return ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);
@@ -195,6 +181,11 @@ __device__ __forceinline__ float warp_reduce_multi(float (&v)[NV], int lane, Op 
 struct RAdd { __device__ __forceinline__ float operator()(float a, float b) const { return a + b; } };
 struct RMax { __device__ __forceinline__ float operator()(float a, float b) const { return fmaxf(a, b); } };
 
+// single-instruction MUFU forms (no denormal / range fix-up code around them)
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
 constexpr float MAGIC_F = 12582912.0f;       // 1.5 * 2^23: (x + MAGIC) rounds x to an integer (RNE) for |x| <= 2^22
 constexpr int MAGIC_I = 0x4B400000;
 constexpr float Q_FIX = 4194300.0f;          // 2^22: fixed-point scale of qt relative to max_c |qt[h,c]|
@@ -203,53 +194,111 @@ constexpr float P_FIX = 4194304.0f;          // 2^22: fixed-point scale of pt = 
 template <int BITS, int GP>
 struct DecSmem {
   static constexpr int RB = record_bytes(BITS);
-  static constexpr int STAGES = BITS == 2 ? 3 : 2;
-  static constexpr int NB = GP * 4;           // N of both MMAs: 4 radix-256 digits per head (D column 4 h + i)
+  static constexpr int STAGES = 2;
+  static constexpr int NT = GP / 2;            // n-tiles (8 columns each): 4 radix-256 digits x GP heads
   alignas(128) uint8_t rec[STAGES][2][RB];     // [stage][K | V] records
-  alignas(128) uint8_t bq[b_bytes(NB)];
-  alignas(128) uint8_t bp[b_bytes(NB)];
-  alignas(16) float qrot[GP][128];             // q' (rotated, scaled); later: merged acc_rot for the inverse Hadamard
+  // B operands in fragment order: word (nu, kappa, half, lane' = 4 g' + t') -> [nu][hk = kappa>>1][b_slot(lane', hk)][2 (kappa&1) + half]
+  alignas(16) uint32_t bq[NT][2][32][4];
+  alignas(16) uint32_t bp[NT][2][32][4];
+  alignas(16) float4 aux_tok[128];             // per MMA row slot of the K tile: {s2, log2 s1v, 1 / s1v, zv} of its token
+  alignas(16) float aux_ch[2][128];            // per channel: s2v / P_FIX (double-buffered by chunk parity)
+  alignas(16) float qrot[GP][128];             // q' (rotated, scaled); later: staging of acc / merged acc_rot
   alignas(16) float qraw[GP][128];             // q * q_scale (un-rotated, for the residual window); later p of the residual
   alignas(16) float hs[GP][2];                 // per head: {scale, beta} of the current chunk
-  alignas(16) float wmax[4][GP];               // per-warp partial maxima
-  alignas(16) float wz[4][GP];                 // per-warp partial zero-point sums / l sums
-  alignas(8) uint64_t full[STAGES];
-  alignas(8) uint64_t mma_bar[2];              // QK^T done, PV done
-  uint32_t tmem_base;
+  alignas(16) float hmax[GP][4];               // per head: per-warp maxima
+  alignas(16) float hz[GP][4];                 // per head: per-warp zero-point sums / l sums
+  alignas(16) float wmax[4][GP];               // residual window: per-warp maxima
+  alignas(16) float wz[4][GP];                 // residual window / final l: per-warp sums
+  alignas(8) uint64_t fullk[STAGES];
+  alignas(8) uint64_t fullv[STAGES];
   int last_flag;
 };
 
-// Expand the packed codes of row r of a staged record into A-operand columns.
+// 16-byte slot of fragment lane lane' inside a [nu][hk] block of a B operand: bit 2 is flipped by
+// (bit 3 of lane') ^ hk, which spreads the builders' 32-bit stores over twice as many banks and keeps
+// the fragment loads (one LDS.128 per lane) conflict-free
+__device__ __forceinline__ int b_slot(int lane_p, int hk) { return lane_p ^ ((((lane_p >> 3) ^ hk) & 1) << 2); }
+
+// Packed words of the four MMA rows (mtile mt; rho = 0, 1) this thread feeds: W[rho][word]
 template <int BITS>
-__device__ __forceinline__ void unpack_row(const uint8_t* codes, int r, uint32_t (&a)[32]) {
-  constexpr int NSEG = row_bytes(BITS) / 16;
-  constexpr int NCLS = 8 / BITS;
+__device__ __forceinline__ void load_row_words(const uint8_t* codes, int warp, int lane, int mt, uint32_t (&W)[2][BITS == 2 ? 2 : 4]) {
+  if constexpr (BITS == 2) {
+    const uint4 v = *reinterpret_cast<const uint4*>(codes + warp * 1024 + mt * 512 + lane * 16);
+    W[0][0] = v.x; W[0][1] = v.y; W[1][0] = v.z; W[1][1] = v.w;
+  } else {
+#pragma unroll
+    for (int rho = 0; rho < 2; ++rho) {
+      const uint4 v = *reinterpret_cast<const uint4*>(codes + warp * 2048 + mt * 1024 + rho * 512 + lane * 16);
+      W[rho][0] = v.x; W[rho][1] = v.y; W[rho][2] = v.z; W[rho][3] = v.w;
+    }
+  }
+}
+// A fragment of k-step kappa: one LOP3 per register
+template <int BITS>
+__device__ __forceinline__ void a_frag(const uint32_t (&W)[2][BITS == 2 ? 2 : 4], int kappa, uint32_t (&a)[4]) {
   constexpr uint32_t MASK0 = BITS == 2 ? 0x03030303u : 0x0F0F0F0Fu;
+  const int j = BITS == 2 ? kappa : (kappa & 1);
+  const int w0 = BITS == 2 ? 0 : 2 * (kappa >> 1);
+  const uint32_t m = MASK0 << (BITS * j);
+  a[0] = W[0][w0] & m; a[1] = W[1][w0] & m; a[2] = W[0][w0 + 1] & m; a[3] = W[1][w0 + 1] & m;
+}
+
+// D[mt][nu] = sum over the 128 K positions of codes (A) x digit planes (B fragments in shared memory);
+// the 2 x NT accumulator chains are interleaved so that no IMMA waits for the previous one
+template <int BITS, int NT, bool B_SIGNED>
+__device__ __forceinline__ void contract(const uint8_t* codes, const uint32_t (*bsm)[2][32][4], int warp, int lane,
+                                         int32_t (&d)[2][NT][4]) {
+  uint32_t W[2][2][BITS == 2 ? 2 : 4];
+  load_row_words<BITS>(codes, warp, lane, 0, W[0]);
+  load_row_words<BITS>(codes, warp, lane, 1, W[1]);
 #pragma unroll
-  for (int s = 0; s < NSEG; ++s) {
-    const uint4 w4 = *reinterpret_cast<const uint4*>(codes + s * 2048 + r * 16);
-    const uint32_t w[4] = {w4.x, w4.y, w4.z, w4.w};
+  for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
+    for (int nu = 0; nu < NT; ++nu)
 #pragma unroll
-      for (int j = 0; j < NCLS; ++j) a[NCLS * (4 * s + q) + j] = w[q] & (MASK0 << (BITS * j));
+      for (int c = 0; c < 4; ++c) d[mt][nu][c] = 0;
+#pragma unroll
+  for (int hk = 0; hk < 2; ++hk) {
+    uint4 bf[NT];
+#pragma unroll
+    for (int nu = 0; nu < NT; ++nu) bf[nu] = *reinterpret_cast<const uint4*>(&bsm[nu][hk][b_slot(lane, hk)][0]);
+#pragma unroll
+    for (int k1 = 0; k1 < 2; ++k1) {
+      const int kappa = 2 * hk + k1;
+      uint32_t a[2][4];
+      a_frag<BITS>(W[0], kappa, a[0]);
+      a_frag<BITS>(W[1], kappa, a[1]);
+#pragma unroll
+      for (int nu = 0; nu < NT; ++nu)
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt) {
+          if (k1) imma_16832<B_SIGNED>(d[mt][nu], a[mt], bf[nu].z, bf[nu].w);
+          else imma_16832<B_SIGNED>(d[mt][nu], a[mt], bf[nu].x, bf[nu].y);
+        }
+    }
   }
 }
 
+// radix-256 digits (d0 + 256 d1 + 65536 d2 + 2^24 d3) of the int32 sums -> float
+__device__ __forceinline__ float undigit(int d0, int d1, int d2, int d3) {
+  const int x01 = d1 * 256 + d0;
+  const int x23 = d3 * 256 + d2;
+  return fmaf(__int2float_rn(x23), 65536.f, __int2float_rn(x01));
+}
+
 template <int BITS, int GP, typename InT>
-__global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_tc_kernel(const DecodeArgs A) {
+__global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_kernel(const DecodeArgs A) {
   using SM = DecSmem<BITS, GP>;
-  constexpr int RB = SM::RB, STAGES = SM::STAGES, NB = SM::NB;
+  constexpr int RB = SM::RB, STAGES = SM::STAGES, NT = SM::NT;
   constexpr int NCLS = 8 / BITS;
   constexpr float CLS_INV = BITS == 2 ? (1.f / 64.f) : (1.f / 16.f);  // 1 / CLSMAX
-  constexpr int HPW = GP / 4;                                          // heads per warp in the B_q builder
-  // TMEM columns: A operand (K tile, then V tile of the same chunk), D (logits, then values)
-  constexpr uint32_t TM_A = 0, TM_D = 32, TM_COLS = 64;
+  constexpr int HPW = GP / 4;   // heads per warp in the B_q builder = heads per thread in the softmax (h = t + 4u)
 
   extern __shared__ __align__(128) uint8_t smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int fg = lane >> 2, ft = lane & 3;   // MMA fragment coordinates: row group g, thread-in-group t
   const int bh = blockIdx.x, b = bh / A.Hkv, hkv = bh - b * A.Hkv;
   const int split = blockIdx.y;
   const int g = A.g;
@@ -267,22 +316,20 @@ __global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_tc_kernel(const D
   const uint8_t* krec = A.k_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
   const uint8_t* vrec = A.v_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
 
-  // ---- setup: barriers, TMEM, first TMA loads, q ------------------------------------
+  // ---- setup: barriers, first TMA loads, q ------------------------------------------
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < STAGES; ++s) mbar_init(&sm.full[s], 1);
-    mbar_init(&sm.mma_bar[0], 1);
-    mbar_init(&sm.mma_bar[1], 1);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&sm.fullk[s], 1); mbar_init(&sm.fullv[s], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 #pragma unroll
     for (int s = 0; s < STAGES; ++s)
       if (s < n_my) {
-        mbar_expect_tx(&sm.full[s], 2 * RB);
-        bulk_g2s(sm.rec[s][0], krec + (size_t)s * RB, RB, &sm.full[s]);
-        bulk_g2s(sm.rec[s][1], vrec + (size_t)s * RB, RB, &sm.full[s]);
+        mbar_expect_tx(&sm.fullk[s], RB);
+        bulk_g2s(sm.rec[s][0], krec + (size_t)s * RB, RB, &sm.fullk[s]);
+        mbar_expect_tx(&sm.fullv[s], RB);
+        bulk_g2s(sm.rec[s][1], vrec + (size_t)s * RB, RB, &sm.fullv[s]);
       }
   }
-  if (warp == 1 && n_my > 0) tmem_alloc<TM_COLS>(&sm.tmem_base);
 
   // D1: q' = (q H / sqrt(128)) * q_scale; heads >= g are zero
   for (int hh = warp; hh < GP; hh += 4) {
@@ -300,57 +347,55 @@ __global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_tc_kernel(const D
     }
     *reinterpret_cast<float4*>(&sm.qrot[hh][4 * lane]) = make_float4(v[0], v[1], v[2], v[3]);
   }
-  tc_fence_before();
   __syncthreads();
-  tc_fence_after();
 
-  // B_q builder role: warp -> heads warp (+4); lane owns K positions lane + 32 r, r = 0..3, which
-  // all sit in byte (lane & 3) of an A column of class j = (lane >> 2) & (NCLS - 1):
-  //   2-bit  channel = 32 r + 16 (lane >> 4) + 4 (lane & 3) + ((lane >> 2) & 3)
-  //   4-bit  channel = 32 r +  8 (lane >> 3) + 2 (lane & 3) + ((lane >> 2) & 1)
+  // B_q builder role: warp -> heads warp (+4); lane = 8 kappa + 4 half + t' owns the four K positions
+  // p = 16 half + 4 t' + b (b = 0..3) of k-step kappa, i.e. one 32-bit word of a B fragment per digit
+  const int bk = lane >> 3, bhalf = (lane >> 2) & 1, btp = lane & 3;
   float qreg[HPW][4];
-  {
-    const int cbase = BITS == 2 ? 16 * (lane >> 4) + 4 * (lane & 3) + ((lane >> 2) & 3)
-                                : 8 * (lane >> 3) + 2 * (lane & 3) + ((lane >> 2) & 1);
 #pragma unroll
-    for (int u = 0; u < HPW; ++u)
+  for (int bb = 0; bb < 4; ++bb) {
+    const int ch = BITS == 2 ? 16 * btp + 4 * bb + bk + 64 * bhalf
+                             : 8 * (btp + 4 * (2 * (bk >> 1) + bhalf)) + 2 * bb + (bk & 1);
 #pragma unroll
-      for (int r = 0; r < 4; ++r) qreg[u][r] = sm.qrot[warp + 4 * u][cbase + 32 * r];
+    for (int u = 0; u < HPW; ++u) qreg[u][bb] = sm.qrot[warp + 4 * u][ch];
   }
   // fixed-point value -> digits: X = (bits(f) - MAGIC_I) << shift, balanced:  (X + 0x80808080) ^ 0x80808080
-  const int shift_q = BITS * (NCLS - 1 - ((lane >> 2) & (NCLS - 1)));
-  const uint32_t mul_q = 1u << shift_q;
-  const uint32_t add_q = 0x80808080u - ((uint32_t)MAGIC_I << shift_q);
-  // token role (softmax): K position of token tid in a V code row, and its class shift
-  const int kpos_t = BITS == 2 ? ((tid & ~15) | ((tid & 3) << 2) | ((tid >> 2) & 3))
-                               : ((tid & ~7) | ((tid & 1) << 2) | ((tid >> 1) & 3));
-  const int shift_p = BITS * (NCLS - 1 - (tid & (NCLS - 1)));
-  const uint32_t mul_p = 1u << shift_p;
-  const uint32_t add_p = 0u - ((uint32_t)MAGIC_I << shift_p);
-
-  float m_run[GP], l_part[GP], acc[GP];
+  const int jq = BITS == 2 ? bk : (bk & 1);
+  const uint32_t mul_q = 1u << (BITS * (NCLS - 1 - jq));
+  const uint32_t add_q = 0x80808080u - ((uint32_t)MAGIC_I * mul_q);
+  // column (h, d) of head h = warp + 4u: n-tile 2u + (d >> 1), g' = 2 warp + (d & 1); lane' = 4 g' + t'
+  uint32_t* bq_dst[2];
 #pragma unroll
-  for (int h = 0; h < GP; ++h) { m_run[h] = -INFINITY; l_part[h] = 0.f; acc[h] = 0.f; }
+  for (int dd = 0; dd < 2; ++dd) bq_dst[dd] = &sm.bq[0][bk >> 1][b_slot(4 * (2 * warp + dd) + btp, bk >> 1)][2 * (bk & 1) + bhalf];
+  // softmax role: thread (warp, fg, ft) sees tokens slot(mt, rho) = 32 warp + 16 mt + 8 rho + fg, heads ft + 4u;
+  // these four tokens are K positions b = 2 mt + rho of word (kappa = warp, half = fg >> 2, t' = fg & 3)
+  const int jp = BITS == 2 ? warp : (warp & 1);
+  const uint32_t mul_p = 1u << (BITS * (NCLS - 1 - jp));
+  const uint32_t add_p = 0u - ((uint32_t)MAGIC_I * mul_p);
+  // column (h, d) of head h = ft + 4u: n-tile 2u + (d >> 1), g' = 2 ft + (d & 1); lane' = 4 g' + t'
+  uint32_t* bp_dst[2];
+#pragma unroll
+  for (int dd = 0; dd < 2; ++dd) bp_dst[dd] = &sm.bp[0][warp >> 1][b_slot(4 * (2 * ft + dd) + (fg & 3), warp >> 1)][2 * (warp & 1) + (fg >> 2)];
 
-  uint32_t tmem = 0, taddr_w = 0;
-  if (n_my > 0) { tmem = sm.tmem_base; taddr_w = tmem + ((uint32_t)(warp * 32) << 16); }
-  const uint32_t bq_addr = smem_u32(sm.bq), bp_addr = smem_u32(sm.bp);
+  float mr[HPW], lp[HPW], ac[HPW][4];
+#pragma unroll
+  for (int u = 0; u < HPW; ++u) {
+    mr[u] = -INFINITY; lp[u] = 0.f;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) ac[u][i] = 0.f;
+  }
 
   for (int it = 0; it < n_my; ++it) {
     const int st = it % STAGES;
-    const uint32_t par = it & 1;
+    const uint32_t par = (it / STAGES) & 1;
     const uint8_t* kr = sm.rec[st][0];
     const uint8_t* vr = sm.rec[st][1];
-    mbar_wait(&sm.full[st], (it / STAGES) & 1);
+    mbar_wait(&sm.fullk[st], par);
 
-    // ---- phase A: K codes -> TMEM, B_q (digits of the fixed-point qt), beta -----------
+    // ---- phase A: B_q (digits of the fixed-point qt), beta, per-token / per-channel aux -----------
     {
-      uint32_t a[32];
-      unpack_row<BITS>(kr, tid, a);
-      tmem_st32(taddr_w + TM_A, a);
-    }
-    {
-      // aux of the K record in builder order: s1[4 lane + r], z[4 lane + r] <-> K position lane + 32 r
+      // aux of the K record in builder order: s1[4 lane + b], z[4 lane + b]
       const uint32_t s1w = *reinterpret_cast<const uint32_t*>(kr + s1_off(BITS) + 4 * lane);
       const uint2 zw = *reinterpret_cast<const uint2*>(kr + z_off(BITS) + 8 * lane);
       const float2 s01 = e4m3x2_to_f32x2((uint16_t)(s1w & 0xffff)), s23 = e4m3x2_to_f32x2((uint16_t)(s1w >> 16));
@@ -377,14 +422,16 @@ __global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_tc_kernel(const D
 #pragma unroll
       for (int u = 0; u < HPW; ++u) {
         const int h = warp + 4 * u;
-        const float inv = amax[u] > 0.f ? Q_FIX * __fdividef(1.f, amax[u]) : 0.f;
-        uint8_t* dst = sm.bq + (h >> 2) * B_SBO + lane * 16 + 4 * (h & 3);
+        const float inv = amax[u] > 1e-30f ? Q_FIX * rcp_approx(amax[u]) : 0.f;
+        uint32_t X[4], Y[4];
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
           const float f = fmaf(qt[u][r], inv, MAGIC_F);            // integer Q in the low mantissa bits
-          const uint32_t X = (__float_as_uint(f) * mul_q + add_q) ^ 0x80808080u;   // balanced s8 digits of Q << shift
-          *reinterpret_cast<uint32_t*>(dst + r * 512) = X;
+          X[r] = (__float_as_uint(f) * mul_q + add_q) ^ 0x80808080u;   // balanced s8 digits of Q << shift
         }
+        transpose4x4(X, Y);   // Y[d] = digit d of the four K positions = one B-fragment word of column (h, d)
+#pragma unroll
+        for (int d = 0; d < 4; ++d) bq_dst[d & 1][(2 * u + (d >> 1)) * 256] = Y[d];
         if (lane == 0) {
           const float sc = amax[u] * (1.f / Q_FIX);
           sm.hs[h][0] = sc * CLS_INV;   // logit = s2 * (acc * scale + beta)
@@ -392,121 +439,130 @@ __global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_tc_kernel(const D
         }
       }
     }
-    tmem_st_wait();
-    fence_proxy_async();
-    tc_fence_before();
+    mbar_wait(&sm.fullv[st], par);
+    {
+      // thread tid: aux of MMA row slot tid of the K tile (token-indexed arrays are stored in slot order)
+      // and of channel tid of the V tile
+      const float s2t = e4m3_to_f32(kr[s2_off(BITS) + tid]);
+      const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + tid]), 9.094947e-13f);   // 2^-40: a zero scale stays harmless
+      const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[tid]);
+      // pt = p s1v = exp2(logit + log2 s1v - m): the running maximum is taken over the shifted logits,
+      // so pt <= 1 and its fixed-point scale is a constant
+      sm.aux_tok[tid] = make_float4(s2t, lg2_approx(s1v), rcp_approx(s1v), zv);
+      sm.aux_ch[it & 1][tid] = e4m3_to_f32(vr[s2_off(BITS) + tid]) * (1.f / P_FIX);
+    }
     __syncthreads();                                                   // barrier 1
-    if (tid == 0) {
-      tc_fence_after();
-      const uint64_t bd = b_desc(bq_addr);
-#pragma unroll
-      for (int ks = 0; ks < 4; ++ks)
-        umma_i8_ts(tmem + TM_D, tmem + TM_A + 8 * ks, bd + (uint64_t)((B_KSTEP * ks) >> 4), idesc_i8(NB, 1), ks > 0);
-      umma_commit(&sm.mma_bar[0]);
+    // every warp is done with chunk it-1: refill its V slot (its K slot was refilled after barrier 2)
+    if (tid == 0 && it >= 1 && it - 1 + STAGES < n_my) {
+      const int s2 = (it - 1) % STAGES;
+      mbar_expect_tx(&sm.fullv[s2], RB);
+      bulk_g2s(sm.rec[s2][1], vrec + (size_t)(it - 1 + STAGES) * RB, RB, &sm.fullv[s2]);
     }
 
-    // ---- phase B: per-token / per-channel aux of this chunk (overlaps the QK^T MMA) -------
-    const float s2t = e4m3_to_f32(kr[s2_off(BITS) + tid]);
-    const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + tid]), 9.094947e-13f);   // 2^-40: a zero scale stays harmless
-    const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[tid]);
-    const float s2v = e4m3_to_f32(vr[s2_off(BITS) + tid]) * (1.f / P_FIX);   // channel role
-    // pt = p s1v = exp2(logit + log2 s1v - m): the running maximum is taken over the shifted logits,
-    // so pt <= 1 and its fixed-point scale is a constant
-    const float lam = __log2f(s1v), inv_s1v = __fdividef(1.f, s1v);
-
-    mbar_wait(&sm.mma_bar[0], par);
-    tc_fence_after();
+    // ---- D3: logits of this thread's 4 tokens x HPW heads --------------------------------------------
+    float logit[HPW][4];
+    float4 aux[4];
     {
-      uint32_t a[32];                      // V codes -> the same TMEM columns (the QK^T MMA is done with them)
-      unpack_row<BITS>(vr, tid, a);
-      tmem_st32(taddr_w + TM_A, a);
-    }
-    // ---- D3/D4: logits of token tid, online softmax ---------------------------------------
-    float logit[GP];
-    {
-      int32_t dlo[16], dhi[16];
-      tmem_ld16(taddr_w + TM_D, dlo);
-      if (NB == 32) tmem_ld16(taddr_w + TM_D + 16, dhi);
-      tmem_ld_wait();
+      int32_t dd[2][NT][4];
+      contract<BITS, NT, true>(kr, sm.bq, warp, lane, dd);
 #pragma unroll
-      for (int h = 0; h < GP; ++h) {
-        const int32_t* d = h < 4 ? &dlo[4 * h] : &dhi[4 * (h & 3)];
-        const int x01 = d[1] * 256 + d[0];
-        const int x23 = d[3] * 256 + d[2];
-        const float a = fmaf(__int2float_rn(x23), 65536.f, __int2float_rn(x01));
-        const float2 sb = *reinterpret_cast<const float2*>(sm.hs[h]);
-        logit[h] = fmaf(s2t, fmaf(a, sb.x, sb.y), lam);
+      for (int i = 0; i < 4; ++i) aux[i] = sm.aux_tok[32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];
+#pragma unroll
+      for (int u = 0; u < HPW; ++u) {
+        const float2 sb = *reinterpret_cast<const float2*>(sm.hs[ft + 4 * u]);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {   // i = 2 mt + rho
+          const int mt = i >> 1, c = 2 * (i & 1);
+          const float a = undigit(dd[mt][2 * u][c], dd[mt][2 * u][c + 1], dd[mt][2 * u + 1][c], dd[mt][2 * u + 1][c + 1]);
+          logit[u][i] = fmaf(aux[i].x, fmaf(a, sb.x, sb.y), aux[i].y);
+        }
       }
     }
-    {
-      float v[GP];
+    // ---- D4: online softmax -----------------------------------------------------------------------------
 #pragma unroll
-      for (int h = 0; h < GP; ++h) v[h] = logit[h];
-      const float r = warp_reduce_multi<GP>(v, lane, RMax());
-      if ((lane & (32 / GP - 1)) == 0) sm.wmax[warp][red_index<GP>(lane)] = r;
+    for (int u = 0; u < HPW; ++u) {
+      float mx = fmaxf(fmaxf(logit[u][0], logit[u][1]), fmaxf(logit[u][2], logit[u][3]));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 8));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 16));
+      if (fg == 0) sm.hmax[ft + 4 * u][warp] = mx;
     }
     __syncthreads();                                                   // barrier 2
-    float corr[GP], zpart[GP];
-    uint32_t X[GP];
+    // every warp is done with the K record of this chunk: prefetch chunk it + STAGES into its slot
+    if (tid == 0 && it + STAGES < n_my) {
+      mbar_expect_tx(&sm.fullk[st], RB);
+      bulk_g2s(sm.rec[st][0], krec + (size_t)(it + STAGES) * RB, RB, &sm.fullk[st]);
+    }
+    float corr[HPW];
 #pragma unroll
-    for (int h = 0; h < GP; ++h) {
-      const float mc = fmaxf(fmaxf(sm.wmax[0][h], sm.wmax[1][h]), fmaxf(sm.wmax[2][h], sm.wmax[3][h]));
-      const float m_new = fmaxf(m_run[h], mc);
-      corr[h] = exp2f(m_run[h] - m_new);
-      m_run[h] = m_new;
-      const float pt = exp2f(logit[h] - m_new);
-      l_part[h] = fmaf(l_part[h], corr[h], pt * inv_s1v);
-      // D5 prep: fixed-point pt; its radix-256 digits are the bytes of X
-      const float f = fmaf(pt, P_FIX, MAGIC_F);
-      zpart[h] = (f - MAGIC_F) * zv;
-      X[h] = __float_as_uint(f) * mul_p + add_p;
+    for (int u = 0; u < HPW; ++u) {
+      const float4 hm = *reinterpret_cast<const float4*>(sm.hmax[ft + 4 * u]);
+      const float m_new = fmaxf(mr[u], fmaxf(fmaxf(hm.x, hm.y), fmaxf(hm.z, hm.w)));
+      corr[u] = ex2_approx(mr[u] - m_new);
+      mr[u] = m_new;
+      uint32_t X[4], Y[4];
+      float lsum = 0.f, zpart = 0.f;
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float pt = ex2_approx(logit[u][i] - m_new);
+        lsum = fmaf(pt, aux[i].z, lsum);
+        // D5 prep: fixed-point pt; its radix-256 digits are the bytes of X
+        const float f = fmaf(pt, P_FIX, MAGIC_F);
+        zpart = fmaf(f - MAGIC_F, aux[i].w, zpart);
+        X[i] = __float_as_uint(f) * mul_p + add_p;
+      }
+      lp[u] = fmaf(lp[u], corr[u], lsum);
+      transpose4x4(X, Y);
+#pragma unroll
+      for (int d = 0; d < 4; ++d) bp_dst[d & 1][(2 * u + (d >> 1)) * 256] = Y[d];
+      zpart += __shfl_xor_sync(0xffffffffu, zpart, 4);
+      zpart += __shfl_xor_sync(0xffffffffu, zpart, 8);
+      zpart += __shfl_xor_sync(0xffffffffu, zpart, 16);
+      if (fg == 0) sm.hz[ft + 4 * u][warp] = zpart;
     }
-    *reinterpret_cast<uint4*>(sm.bp + kpos_t * 16) = make_uint4(X[0], X[1], X[2], X[3]);
-    if (GP == 8) *reinterpret_cast<uint4*>(sm.bp + B_SBO + kpos_t * 16) = make_uint4(X[GP - 4], X[GP - 3], X[GP - 2], X[GP - 1]);
-    {
-      const float r = warp_reduce_multi<GP>(zpart, lane, RAdd());
-      if ((lane & (32 / GP - 1)) == 0) sm.wz[warp][red_index<GP>(lane)] = r;
-    }
-    tmem_st_wait();
-    fence_proxy_async();
-    tc_fence_before();
     __syncthreads();                                                   // barrier 3
-    if (tid == 0) {
-      tc_fence_after();
-      const uint64_t bd = b_desc(bp_addr);
-#pragma unroll
-      for (int ks = 0; ks < 4; ++ks)
-        umma_i8_ts(tmem + TM_D, tmem + TM_A + 8 * ks, bd + (uint64_t)((B_KSTEP * ks) >> 4), idesc_i8(NB, 0), ks > 0);
-      umma_commit(&sm.mma_bar[1]);
-      // the record slot is free (all aux values are in registers): prefetch chunk it + STAGES
-      if (it + STAGES < n_my) {
-        mbar_expect_tx(&sm.full[st], 2 * RB);
-        bulk_g2s(sm.rec[st][0], krec + (size_t)(it + STAGES) * RB, RB, &sm.full[st]);
-        bulk_g2s(sm.rec[st][1], vrec + (size_t)(it + STAGES) * RB, RB, &sm.full[st]);
-      }
-    }
-    float zsum[GP];
-#pragma unroll
-    for (int h = 0; h < GP; ++h) zsum[h] = (sm.wz[0][h] + sm.wz[1][h]) + (sm.wz[2][h] + sm.wz[3][h]);
 
-    // ---- D5: channel tid of the value contraction ---------------------------------------------
-    mbar_wait(&sm.mma_bar[1], par);
-    tc_fence_after();
+    // ---- D5: this thread's 4 channels x HPW heads of the value contraction ---------------------------
     {
-      int32_t dlo[16], dhi[16];
-      tmem_ld16(taddr_w + TM_D, dlo);
-      if (NB == 32) tmem_ld16(taddr_w + TM_D + 16, dhi);
-      tmem_ld_wait();
+      int32_t dd[2][NT][4];
+      contract<BITS, NT, false>(vr, sm.bp, warp, lane, dd);
+      float s2v[4];
 #pragma unroll
-      for (int h = 0; h < GP; ++h) {
-        const int32_t* d = h < 4 ? &dlo[4 * h] : &dhi[4 * (h & 3)];
-        const int x01 = d[1] * 256 + d[0];
-        const int x23 = d[3] * 256 + d[2];
-        const float a = fmaf(__int2float_rn(x23), 65536.f, __int2float_rn(x01));
-        acc[h] = fmaf(acc[h], corr[h], s2v * fmaf(a, CLS_INV, zsum[h]));
+      for (int i = 0; i < 4; ++i) s2v[i] = sm.aux_ch[it & 1][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];
+#pragma unroll
+      for (int u = 0; u < HPW; ++u) {
+        const float4 hz = *reinterpret_cast<const float4*>(sm.hz[ft + 4 * u]);
+        const float zsum = (hz.x + hz.y) + (hz.z + hz.w);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int mt = i >> 1, c = 2 * (i & 1);
+          const float a = undigit(dd[mt][2 * u][c], dd[mt][2 * u][c + 1], dd[mt][2 * u + 1][c], dd[mt][2 * u + 1][c + 1]);
+          ac[u][i] = fmaf(ac[u][i], corr[u], s2v[i] * fmaf(a, CLS_INV, zsum));
+        }
       }
     }
-    tc_fence_before();
+  }
+
+  // ---- hand over to the per-channel layout of the residual window / merge: thread tid = channel tid ----
+  __syncthreads();
+#pragma unroll
+  for (int u = 0; u < HPW; ++u) {
+    float l = lp[u];
+    l += __shfl_xor_sync(0xffffffffu, l, 4);
+    l += __shfl_xor_sync(0xffffffffu, l, 8);
+    l += __shfl_xor_sync(0xffffffffu, l, 16);
+    if (fg == 0) { sm.hz[ft + 4 * u][warp] = l; if (warp == 0) sm.hs[ft + 4 * u][0] = mr[u]; }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) sm.qrot[ft + 4 * u][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg] = ac[u][i];
+  }
+  __syncthreads();
+  float m_run[GP], l_part[GP], acc[GP];
+#pragma unroll
+  for (int h = 0; h < GP; ++h) {
+    m_run[h] = sm.hs[h][0];
+    const float4 hz = *reinterpret_cast<const float4*>(sm.hz[h]);
+    l_part[h] = tid == 0 ? (hz.x + hz.y) + (hz.z + hz.w) : 0.f;   // thread 0 carries the sum over the chunks
+    acc[h] = sm.qrot[h][tid];
   }
 
   // ---- D6: residual window (raw tokens, un-rotated space) -------------------------------------
@@ -586,47 +642,90 @@ __global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_tc_kernel(const D
     const float r = warp_reduce_multi<GP>(v, lane, RAdd());
     if ((lane & (32 / GP - 1)) == 0) sm.wz[warp][red_index<GP>(lane)] = r;
   }
-  tc_fence_before();
   __syncthreads();
-  if (warp == 1 && n_my > 0) { tc_fence_after(); tmem_dealloc<64>(tmem); }
   float l_tot[GP];
 #pragma unroll
   for (int h = 0; h < GP; ++h) l_tot[h] = (sm.wz[0][h] + sm.wz[1][h]) + (sm.wz[2][h] + sm.wz[3][h]);
 
-  // ---- D7: partials -> workspace; last CTA of this (sequence, KV head) merges -------------------
-  float* merged_rot = &sm.qrot[0][0];   // [GP][128]
-  float Ltot[GP];
-#pragma unroll
-  for (int h = 0; h < GP; ++h) Ltot[h] = 0.f;
-  if (A.splits > 1) {
+  // ---- D7a: in-cluster merge of the split partials through distributed shared memory ----------
+  // Reduce-scatter by head: head h is merged by the CTA of cluster rank h % CS, which receives the
+  // partial of rank r in landing slot (h / CS) * CS + r.  The landing area is the record ring, dead
+  // once every CTA of the cluster has left its main loop (first cluster barrier).  Afterwards this
+  // CTA holds, in array slot j, the merged (m, l, acc, acc_res) of its owned head h = hbase + hstride j.
+  const int CS = A.cluster, NC = A.nclus;
+  int hbase = 0, hstride = 1;
+  if (CS > 1) {
+    const int crank = (int)cluster_ctarank();
+    float* land = reinterpret_cast<float*>(&sm.rec[0][0][0]);   // [<= 15][WS_STRIDE]
+    static_assert(sizeof(sm.rec) >= 15 * WS_STRIDE * sizeof(float), "landing area");
+    cluster_sync_all();
+    const uint32_t land_addr = smem_u32(land);
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
       if (h < g) {
-        float* o = A.ws + (((size_t)b * A.Hq + hkv * g + h) * A.splits + split) * WS_STRIDE;
-        if (tid == 0) { o[0] = m_run[h]; o[1] = l_tot[h]; }
-        o[4 + tid] = acc[h];
-        o[132 + tid] = acc_res[h];
+        const int j = h / CS, d = h - j * CS;
+        const uint32_t dst = mapa_shared(land_addr + (uint32_t)(j * CS + crank) * (WS_STRIDE * 4), (uint32_t)d);
+        if (tid == 0) { st_cluster_f32(dst, m_run[h]); st_cluster_f32(dst + 4, l_tot[h]); }
+        st_cluster_f32(dst + 16 + 4 * tid, acc[h]);
+        if (do_resid) st_cluster_f32(dst + 16 + 512 + 4 * tid, acc_res[h]);
+      }
+    }
+    cluster_sync_all();
+    const bool res_here = resid > 0 && split / CS == NC - 1;   // this cluster's last rank ran the residual window
+#pragma unroll
+    for (int j = 0; j < GP; ++j) {
+      const int h = crank + j * CS;
+      float mj = -INFINITY, lj = 0.f, aj = 0.f, rj = 0.f;
+      if (h < g) {
+        const float* slot0 = land + j * CS * WS_STRIDE;
+        for (int r = 0; r < CS; ++r) mj = fmaxf(mj, slot0[r * WS_STRIDE]);
+        for (int r = 0; r < CS; ++r) {
+          const float* sl = slot0 + r * WS_STRIDE;
+          const float w = (sl[0] == -INFINITY) ? 0.f : ex2_approx(sl[0] - mj);
+          lj = fmaf(w, sl[1], lj);
+          aj = fmaf(w, sl[4 + tid], aj);
+          if (res_here && r == CS - 1) rj = w * sl[132 + tid];
+        }
+      }
+      m_run[j] = mj; l_tot[j] = lj; acc[j] = aj; acc_res[j] = rj;
+    }
+    hbase = crank; hstride = CS;
+    if (hbase >= g) return;   // this rank owns no head
+  }
+
+  // ---- D7b: several clusters per (sequence, KV head): partials -> workspace, last arriver merges ----
+  if (NC > 1) {
+    const int cidx = split / CS;
+#pragma unroll
+    for (int j = 0; j < GP; ++j) {
+      const int h = hbase + hstride * j;
+      if (h < g) {
+        float* o = A.ws + (((size_t)b * A.Hq + hkv * g + h) * NC + cidx) * WS_STRIDE;
+        if (tid == 0) { o[0] = m_run[j]; o[1] = l_tot[j]; }
+        o[4 + tid] = acc[j];
+        o[132 + tid] = acc_res[j];
       }
     }
     __threadfence();
     __syncthreads();
     if (tid == 0) {
+      const int n_writers = NC * min(CS, g);   // CTAs that own at least one head
       const int old = atomicAdd(&A.ticket[bh], 1);
-      const int last = (old == A.splits - 1);
+      const int last = (old == n_writers - 1);
       if (last) A.ticket[bh] = 0;
       sm.last_flag = last;
     }
     __syncthreads();
     if (!sm.last_flag) return;
     __threadfence();
-    // weights of the splits: warp w handles heads w, w+4; lane s handles splits s, s+32
-    float* wsp = reinterpret_cast<float*>(sm.bq);   // [GP][64] split weights (B_q is dead by now)
+    // weights of the partials: warp w handles heads w, w+4; lane s handles partials s, s+32
+    float* wsp = reinterpret_cast<float*>(sm.bq);   // [GP][64] weights (B_q is dead by now)
     for (int h = warp; h < g; h += 4) {
-      const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * A.splits * WS_STRIDE;
-      const float m0 = lane < A.splits ? __ldcg(base + (size_t)lane * WS_STRIDE) : -INFINITY;
-      const float m1 = lane + 32 < A.splits ? __ldcg(base + (size_t)(lane + 32) * WS_STRIDE) : -INFINITY;
-      const float l0 = lane < A.splits ? __ldcg(base + (size_t)lane * WS_STRIDE + 1) : 0.f;
-      const float l1 = lane + 32 < A.splits ? __ldcg(base + (size_t)(lane + 32) * WS_STRIDE + 1) : 0.f;
+      const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * NC * WS_STRIDE;
+      const float m0 = lane < NC ? __ldcg(base + (size_t)lane * WS_STRIDE) : -INFINITY;
+      const float m1 = lane + 32 < NC ? __ldcg(base + (size_t)(lane + 32) * WS_STRIDE) : -INFINITY;
+      const float l0 = lane < NC ? __ldcg(base + (size_t)lane * WS_STRIDE + 1) : 0.f;
+      const float l1 = lane + 32 < NC ? __ldcg(base + (size_t)(lane + 32) * WS_STRIDE + 1) : 0.f;
       const float mstar = warp_max(fmaxf(m0, m1));
       const float w0 = (m0 == -INFINITY) ? 0.f : exp2f(m0 - mstar);
       const float w1 = (m1 == -INFINITY) ? 0.f : exp2f(m1 - mstar);
@@ -638,47 +737,51 @@ __global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_tc_kernel(const D
     __syncthreads();
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
+      float rot = 0.f, res = 0.f, L = 0.f;
       if (h < g) {
-        const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * A.splits * WS_STRIDE + 4 + tid;
-        float rot = 0.f, res = 0.f;
+        const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * NC * WS_STRIDE + 4 + tid;
         int s = 0;
-        for (; s + 4 <= A.splits; s += 4) {
+        for (; s + 4 <= NC; s += 4) {
           float r[4], e[4];
 #pragma unroll
           for (int j = 0; j < 4; ++j) { r[j] = __ldcg(base + (size_t)(s + j) * WS_STRIDE); e[j] = __ldcg(base + (size_t)(s + j) * WS_STRIDE + 128); }
 #pragma unroll
           for (int j = 0; j < 4; ++j) { const float w = wsp[h * 64 + s + j]; rot = fmaf(w, r[j], rot); res = fmaf(w, e[j], res); }
         }
-        for (; s < A.splits; ++s) {
+        for (; s < NC; ++s) {
           const float w = wsp[h * 64 + s];
           rot = fmaf(w, __ldcg(base + (size_t)s * WS_STRIDE), rot);
           res = fmaf(w, __ldcg(base + (size_t)s * WS_STRIDE + 128), res);
         }
-        Ltot[h] = sm.hs[h][1]; acc[h] = rot; acc_res[h] = res;
+        L = sm.hs[h][1];
       }
+      l_tot[h] = L; acc[h] = rot; acc_res[h] = res;
     }
-  } else {
-#pragma unroll
-    for (int h = 0; h < GP; ++h) Ltot[h] = l_tot[h];
+    hbase = 0; hstride = 1;
   }
+
+  // ---- D7c: inverse Hadamard, residual part, normalisation of the owned heads ---------------------
+  float* merged_rot = &sm.qrot[0][0];   // [GP][128]
   __syncthreads();
 #pragma unroll
-  for (int h = 0; h < GP; ++h) {
-    merged_rot[h * 128 + tid] = acc[h];
-    sm.qraw[h][tid] = (Ltot[h] > 0.f) ? acc_res[h] : 0.f;
-    if (tid == 0) sm.hs[h][0] = (Ltot[h] > 0.f) ? 1.f / Ltot[h] : 0.f;
+  for (int j = 0; j < GP; ++j) {
+    merged_rot[j * 128 + tid] = acc[j];
+    sm.qraw[j][tid] = (l_tot[j] > 0.f) ? acc_res[j] : 0.f;
+    if (tid == 0) sm.hs[j][0] = (l_tot[j] > 0.f) ? 1.f / l_tot[j] : 0.f;
   }
   __syncthreads();
-  for (int hh = warp; hh < g; hh += 4) {
-    float4 r4 = *reinterpret_cast<const float4*>(&merged_rot[hh * 128 + 4 * lane]);
+  for (int jj = warp; jj < GP; jj += 4) {
+    const int hh = hbase + hstride * jj;
+    if (hh >= g) break;
+    float4 r4 = *reinterpret_cast<const float4*>(&merged_rot[jj * 128 + 4 * lane]);
     float v[4] = {r4.x, r4.y, r4.z, r4.w};
     if (A.rotate_v) {
       fwht128_lane4(v, lane);
 #pragma unroll
       for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
     }
-    const float4 s4 = *reinterpret_cast<const float4*>(&sm.qraw[hh][4 * lane]);
-    const float inv = sm.hs[hh][0];
+    const float4 s4 = *reinterpret_cast<const float4*>(&sm.qraw[jj][4 * lane]);
+    const float inv = sm.hs[jj][0];
     const float o0 = (v[0] + s4.x) * inv, o1 = (v[1] + s4.y) * inv, o2 = (v[2] + s4.z) * inv, o3 = (v[3] + s4.w) * inv;
     const size_t off = ((size_t)b * A.Hq + hkv * g + hh) * D + 4 * lane;
     if (A.out_dtype == KVARN_F32) {

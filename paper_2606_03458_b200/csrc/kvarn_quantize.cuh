@@ -335,9 +335,9 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       const float z = mn / s;
       sm.inv_s[tid] = 1.f / s; sm.z[tid] = z;
       const float s1 = s * sm.Sr[tid], s2 = sm.Sc[tid];  // K: s1 per channel, s2 per token
-      const int kp = kaux_of_elem(BITS, tid);  // K records keep s1, z in K-position order
+      const int kp = kaux_of_elem(BITS, tid);  // K records keep s1, z in B-operand builder order
       sm.rec[s1_off(BITS) + kp] = f32_to_e4m3(s1);
-      sm.rec[s2_off(BITS) + tid] = f32_to_e4m3(s2);
+      sm.rec[s2_off(BITS) + slot_of_token(BITS, tid)] = f32_to_e4m3(s2);   // per-token arrays: MMA row-slot order
       reinterpret_cast<uint16_t*>(&sm.rec[z_off(BITS)])[kp] = f32_to_f16_bits(z);
       if (dbg.aux) {
         float* o = dbg.aux + tile_idx * 384;
@@ -363,8 +363,9 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
         w |= ((uint32_t)q0) << (BITS * 2 * kp);
         w |= ((uint32_t)q1) << (BITS * (2 * kp + 1));
       }
-      if (BITS == 2) *reinterpret_cast<uint16_t*>(&sm.rec[code_off(t0 + i, 2 * li)]) = (uint16_t)w;
-      else *reinterpret_cast<uint32_t*>(&sm.rec[code_off(t0 + i, 4 * li)]) = w;
+      const int slot = slot_of_token(BITS, t0 + i);
+      if (BITS == 2) *reinterpret_cast<uint16_t*>(&sm.rec[code_off(2, slot, 2 * li)]) = (uint16_t)w;
+      else *reinterpret_cast<uint32_t*>(&sm.rec[code_off(4, slot, 4 * li)]) = w;
     }
   } else {
     // group = token over the 128 channels: min / max inside the half-warp
@@ -388,8 +389,9 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     if (li < 8) {
       sm.inv_s[tok_own] = 1.f / s; sm.z[tok_own] = z;
       const float s1 = s * sm.Sc[tok_own];  // V: s1 per token
-      sm.rec[s1_off(BITS) + tok_own] = f32_to_e4m3(s1);
-      reinterpret_cast<uint16_t*>(&sm.rec[z_off(BITS)])[tok_own] = f32_to_f16_bits(z);
+      const int slot = slot_of_token(BITS, tok_own);
+      sm.rec[s1_off(BITS) + slot] = f32_to_e4m3(s1);
+      reinterpret_cast<uint16_t*>(&sm.rec[z_off(BITS)])[slot] = f32_to_f16_bits(z);
       if (dbg.aux) { float* o = dbg.aux + tile_idx * 384; o[tok_own] = s1; o[256 + tok_own] = z; }
     }
     if (tid < 128) {
@@ -420,8 +422,8 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       }
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      if (BITS == 2) *reinterpret_cast<uint16_t*>(&sm.rec[code_off(c0 + k, 2 * (2 * warp + lj))]) = (uint16_t)w[k];
-      else *reinterpret_cast<uint32_t*>(&sm.rec[code_off(c0 + k, 4 * (2 * warp + lj))]) = w[k];
+      if (BITS == 2) *reinterpret_cast<uint16_t*>(&sm.rec[code_off(2, c0 + k, 2 * (2 * warp + lj))]) = (uint16_t)w[k];
+      else *reinterpret_cast<uint32_t*>(&sm.rec[code_off(4, c0 + k, 4 * (2 * warp + lj))]) = w[k];
     }
   }
   if (dbg.k_best && tid == 0) dbg.k_best[tile_idx] = k_best;

@@ -109,37 +109,81 @@ def test_pack_unpack_round_trip_and_formats(kv, bits, kind):
     assert np.array_equal(zz.astype(np.float64), O.round_fp16(z.astype(np.float64)))
     info = kv.layout(p)
     stored = rec[info.s1_off:info.s1_off + 128]
+    e = np.arange(128)
     if kind == 0:
-        # K records keep s1 (and z) in the K-position order of their channel (csrc/kvarn_common.cuh)
-        e = np.arange(128)
-        kpos = ((e & ~15) | ((e & 3) << 2) | ((e >> 2) & 3)) if bits == 2 else ((e & ~7) | ((e & 1) << 2) | ((e >> 1) & 3))
-        assert sorted(kpos.tolist()) == list(range(128))
-        stored = stored[4 * (kpos & 31) + (kpos >> 5)]   # lane-contiguous order of the B-operand builder
+        # K records keep s1 (and z), per channel, in the order of the B-operand builder (include/kvarn.h)
+        stored = stored[_kaux_of_elem(bits, e)]
+    else:
+        # V records keep s1 (and z), per token, at the MMA row slot of the token
+        stored = stored[_slot_of_token(bits, e)]
     assert np.array_equal(stored, O.fp8_e4m3_bits(O.round_fp8_e4m3(s1.astype(np.float64))))
     # saturation
     rec = kv.pack_record(p, kind, codes, np.full(128, 1e6, np.float32), s2, z)
     assert np.all(kv.unpack_record(p, kind, rec)[1] == 448.0)
 
 
+def _kstep_kpos(bits, e):
+    # include/kvarn.h "record layout": k-step and position of row element e in the contraction
+    if bits == 2:
+        return e & 3, 16 * (e >> 6) + 4 * ((e >> 4) & 3) + ((e >> 2) & 3)
+    return 2 * (e >> 6) + (e & 1), 16 * ((e >> 5) & 1) + 4 * ((e >> 3) & 3) + ((e >> 1) & 3)
+
+
+def _kaux_of_elem(bits, e):
+    ks, kp = _kstep_kpos(bits, e)
+    return 4 * (8 * ks + (kp >> 2)) + (kp & 3)
+
+
+def _slot_of_token(bits, tau):
+    # row slot 32*warp + 16*mtile + 8*rho + g with warp = k-step, (half, t') = g, b = 2*mtile + rho
+    ks, kp = _kstep_kpos(bits, tau)
+    b, tp, half = kp & 3, (kp >> 2) & 3, kp >> 4
+    return 32 * ks + 16 * (b >> 1) + 8 * (b & 1) + 4 * half + tp
+
+
+def _code_off(bits, slot, byte_in_row):
+    wi, bb = byte_in_row >> 2, byte_in_row & 3
+    w, mt, rho, g = slot >> 5, (slot >> 4) & 1, (slot >> 3) & 1, slot & 7
+    t, q = wi & 3, wi >> 2
+    if bits == 2:
+        return w * 1024 + mt * 512 + (4 * g + t) * 16 + rho * 8 + q * 4 + bb
+    return w * 2048 + mt * 1024 + rho * 512 + (4 * g + t) * 16 + q * 4 + bb
+
+
+def test_layout_maps_are_bijections():
+    for bits in (2, 4):
+        e = np.arange(128)
+        assert sorted(_kaux_of_elem(bits, e).tolist()) == list(range(128))
+        assert sorted(_slot_of_token(bits, e).tolist()) == list(range(128))
+        rb = 128 * bits // 8
+        offs = sorted(_code_off(bits, s, b) for s in range(128) for b in range(rb))
+        assert offs == list(range(128 * rb))
+
+
 def test_code_row_layout(kv):
-    # include/kvarn.h: K rows are per token, V rows per channel, little-endian within
-    # a row (element e at bit bits*(e % (8/bits)) of byte e*bits/8); the 16-byte
-    # segment s of row r sits at byte s*2048 + r*16.
+    # include/kvarn.h: K rows are per token, V rows per channel, little-endian within a row (element e
+    # at bit bits*(e % (8/bits)) of byte e*bits/8); row slot / word placement as restated above.
     p = kv.default_params(2)
     codes = np.zeros((128, 128), np.uint8)
     codes[5, 9] = 3          # token 5, channel 9
-    codes[7, 100] = 2        # token 7, channel 100 -> byte 25 of its K row = segment 1, byte 9
+    codes[7, 100] = 2        # token 7, channel 100 -> byte 25 of its K row
     ones = np.ones(128, np.float32)
     rk = kv.pack_record(p, 0, codes, ones, ones, ones)
     rv = kv.pack_record(p, 1, codes, ones, ones, ones)
-    assert rk[0 * 2048 + 5 * 16 + 9 // 4] == 3 << (2 * (9 % 4))
-    assert rk[1 * 2048 + 7 * 16 + (100 // 4 - 16)] == 2 << (2 * (100 % 4))
+    assert rk[_code_off(2, int(_slot_of_token(2, 5)), 9 // 4)] == 3 << (2 * (9 % 4))
+    assert rk[_code_off(2, int(_slot_of_token(2, 7)), 100 // 4)] == 2 << (2 * (100 % 4))
     assert rk[:4096].sum() == (3 << 2) + (2 << 0)
-    assert rv[0 * 2048 + 9 * 16 + 5 // 4] == 3 << (2 * (5 % 4))
-    assert rv[0 * 2048 + 100 * 16 + 7 // 4] == 2 << (2 * (7 % 4))
+    assert rv[_code_off(2, 9, 5 // 4)] == 3 << (2 * (5 % 4))      # V rows: slot = channel
+    assert rv[_code_off(2, 100, 7 // 4)] == 2 << (2 * (7 % 4))
     p4 = kv.default_params(4)
     r4 = kv.pack_record(p4, 0, codes, ones, ones, ones)
-    assert r4[(100 // 2 // 16) * 2048 + 7 * 16 + (100 // 2) % 16] == 2 << (4 * (100 % 2))
+    assert r4[_code_off(4, int(_slot_of_token(4, 7)), 100 // 2)] == 2 << (4 * (100 % 2))
+    # a random record round-trips through the canonical view at both widths
+    rng = np.random.default_rng(3)
+    for bits, pp in ((2, p), (4, p4)):
+        c = rng.integers(0, 1 << bits, size=(128, 128)).astype(np.uint8)
+        for kind in (0, 1):
+            assert np.array_equal(kv.unpack_record(pp, kind, kv.pack_record(pp, kind, c, ones, ones, ones))[0], c)
 
 
 def test_missing_library_fails_loudly(tmp_path, monkeypatch):
