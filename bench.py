@@ -5,7 +5,8 @@ shaped decode layer: B=8, 32 q / 8 KV heads, head_dim 128, ctx 8192 = 64 chunks,
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
   write path  kvarn_quantize_chunk over the batch's 2 x 4096 K/V tiles (one launch)
-  read path   kvarn_decode_attention over a 64-chunk packed cache (2 launches)
+  read path   kvarn_decode_attention over a 64-chunk packed cache (one launch: the split
+              partials merge inside the kernel through DSMEM of a thread-block cluster)
 The bench cycles through L = 8 distinct "layers" (input + cache copies, 2.4 GB
 of inputs, 302 MB of records: far larger than the 126 MB L2); the read path of
 step i reads the cache written L/2 steps earlier, so neither kernel ever finds
@@ -14,8 +15,9 @@ stream inside the timed region.
 
   metric/value  2-bit decode-attention GB/s  (algorithmic bytes / decode time)
   also          quantize tokens/s, us/step, HBM / ALU roofline fractions,
-                the oracle timed on the host cores (cpu_baseline), and the same
-                step through the host-buffer C-ABI calls (e2e).
+                the oracle timed on the host cores (cpu_baseline), the same step through
+                the host-buffer C-ABI calls (e2e), and -- at N = 1 -- the long-context
+                (configs[4]-shaped) decode and the configs[3] quantizer sweep ("extras").
 
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample instead.
 Under torchrun (N > 1) every rank runs an independent replica of the workload
@@ -64,7 +66,7 @@ class ClockSampler:
              "clocks_event_reasons.sw_power_cap")
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(index)], stdout=subprocess.PIPE, text=True)
+                                          "-lms", "20", "-i", str(index)], stdout=subprocess.PIPE, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
         except Exception:
@@ -162,6 +164,19 @@ def run_reference(args, shape):
     print(json.dumps(line))
 
 
+def max_over_ranks(values, dist, device):
+    """MAX over ranks of a list of floats (device times): the slowest replica sets the job's time."""
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def replica_seed(base: int, layer: int, rank: int) -> int:
+    """Seed of layer `layer` of replica `rank`: every rank draws its own synthetic batch."""
+    return base + 100 * layer + 1000 * rank
+
+
 def workload_config(shape, layers):
     return {"workload": "BASELINE.json configs[1]: Llama-3.1-8B-shaped decode layer",
             "B": shape.B, "Hq": shape.Hq, "Hkv": shape.Hkv, "head_dim": D, "ctx": shape.ctx,
@@ -172,15 +187,84 @@ def workload_config(shape, layers):
             "parallelism": "replicas"}
 
 
+def _time_launches(fn, n, stream):
+    """median / min device time (ms) of n launches of fn(i), CUDA events on the launching stream"""
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+    for i in range(n):
+        evs[i][0].record(stream); fn(i); evs[i][1].record(stream)
+    torch.cuda.synchronize()
+    ts = sorted(a.elapsed_time(b) for a, b in evs)
+    return ts[len(ts) // 2], ts[0]
+
+
+def run_extras(kv, W, dev, hbm_peak):
+    """Long-context decode (configs[4] shape: B=64, 64 q / 8 KV heads, ctx 65536 + 64 residual tokens,
+    2-bit and 4-bit) and the configs[3] quantizer sweep (8 heads x 2^20 tokens, one launch, 2-bit and
+    4-bit).  Every launch reads far more than L2 holds (>= 2.4 GB), so launches are simply repeated."""
+    stream = torch.cuda.current_stream()
+    ex = {}
+    s4 = W.CONFIG4
+    for bits in (2, 4):
+        p = kv.default_params(bits)
+        rb = kv.record_bytes(p)
+        cache = kv.Cache(p, s4.B, s4.Hkv, s4.n_chunks, device=dev)
+        for b0 in range(0, s4.B, 4):   # fill 4 sequences at a time (1.1 GB of bf16 K/V each)
+            K, V = W.kv_tokens(4, s4.Hkv, s4.ctx, seed=s4.seed + b0, device=dev)
+            kv.prefill(p, cache.slice(b0, b0 + 4), K, V)
+            del K, V
+        q = W.queries(s4.B, s4.Hq, seed=s4.seed, device=dev)
+        ws = torch.empty((max(kv.decode_workspace_bytes(p, s4.B, s4.Hq, s4.Hkv, s4.n_chunks), 16),), dtype=torch.uint8, device=dev)
+        out = torch.empty((s4.B, s4.Hq, D), dtype=torch.float32, device=dev)
+        for _ in range(3):
+            kv.decode_attention(p, cache, q, out=out, ws=ws)
+        torch.cuda.synchronize()
+        med, mn = _time_launches(lambda i: kv.decode_attention(p, cache, q, out=out, ws=ws), 10, stream)
+        byts = cache.nbytes_read_by_decode(s4.ctx) + s4.B * s4.Hq * (D * 2 + D * 4)
+        ex[f"decode_cfg4_{bits}bit"] = {"us": med * 1e3, "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak,
+                                        "bytes": byts, "B": s4.B, "Hq": s4.Hq, "Hkv": s4.Hkv, "ctx": s4.ctx}
+        del cache, q, ws, out
+        torch.cuda.empty_cache()
+    n_tok = 1 << 20
+    K, V = W.quantizer_sweep_tiles(8, n_tok, seed=3, device=dev)
+    n_tiles = 8 * n_tok // G
+    Kt, Vt = K.view(n_tiles, G, D), V.view(n_tiles, G, D)
+    for bits in (2, 4):
+        p = kv.default_params(bits)
+        rb = kv.record_bytes(p)
+        kr = torch.empty((n_tiles, rb), dtype=torch.uint8, device=dev); vr = torch.empty_like(kr)
+        for _ in range(2):
+            kv.quantize_chunk(p, Kt, Vt, kr, vr)
+        torch.cuda.synchronize()
+        med, mn = _time_launches(lambda i: kv.quantize_chunk(p, Kt, Vt, kr, vr), 5, stream)
+        byts = 2 * n_tiles * (G * D * 2 + rb)
+        ex[f"quantize_cfg3_{bits}bit"] = {"ms": med, "tokens_per_s": n_tok / (med * 1e-3), "tiles_per_s": 2 * n_tiles / (med * 1e-3),
+                                          "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak,
+                                          "alu_frac": 2 * n_tiles * QUANT_FLOPS_PER_TILE / (med * 1e-3) / 1e12 / FP32_PEAK_TFLOPS_NOMINAL}
+        del kr, vr
+    return ex
+
+
+def stored_traffic():
+    """dram bytes per launch of the two kernels, from the committed ncu --set full capture."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    try:
+        return json.load(open(path))
+    except Exception:
+        return {}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--impl", default="kvarn", choices=["kvarn", "reference"])
     ap.add_argument("--layers", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--extras-only", action="store_true",
+                    help="run only the configs[4] decode / configs[3] quantizer measurements (profiling aid)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "kvarn" else args.warmup
 
@@ -205,6 +289,10 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     from paper_2606_03458_b200 import kvarn as kv
+    if args.extras_only:
+        if rank == 0:
+            print(json.dumps({"extras": run_extras(kv, W, dev, peaks()[0])}))
+        return
     p = kv.default_params(shape.bits)
     rb = kv.record_bytes(p)
     L = args.layers
@@ -214,9 +302,9 @@ def main():
     # ---- synthetic inputs, resident in HBM before the timed region -----------------
     Ks, Vs, caches, qs = [], [], [], []
     for l in range(L):
-        K, V = W.kv_tokens(shape.B, shape.Hkv, shape.ctx, seed=shape.seed + 100 * l + 1000 * rank, device=dev)
+        K, V = W.kv_tokens(shape.B, shape.Hkv, shape.ctx, seed=replica_seed(shape.seed, l, rank), device=dev)
         Ks.append(K.view(n_tiles, G, D)); Vs.append(V.view(n_tiles, G, D))
-        qs.append(W.queries(shape.B, shape.Hq, seed=shape.seed + 100 * l + 1000 * rank, device=dev))
+        qs.append(W.queries(shape.B, shape.Hq, seed=replica_seed(shape.seed, l, rank), device=dev))
         c = kv.Cache(p, shape.B, shape.Hkv, shape.n_chunks, device=dev)
         c.seq_lens.fill_(shape.ctx)
         caches.append(c)
@@ -255,10 +343,7 @@ def main():
     total_ms = t0.elapsed_time(t1)
     q_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
     d_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
-    times = torch.tensor([total_ms, q_ms, d_ms], dtype=torch.float64, device=dev)
-    if dist:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    total_ms, q_ms, d_ms = times.tolist()
+    total_ms, q_ms, d_ms = max_over_ranks([total_ms, q_ms, d_ms], dist, dev)
 
     # ---- algorithmic bytes --------------------------------------
     dec_bytes = BH * shape.n_chunks * 2 * rb + shape.B * shape.Hq * (D * 2 + D * 4)
@@ -290,9 +375,7 @@ def main():
         for _ in range(n_e2e): e2e_step()
         b.record(stream)
         torch.cuda.synchronize()
-        e_ms = torch.tensor([a.elapsed_time(b) / n_e2e], dtype=torch.float64, device=dev)
-        if dist: dist.all_reduce(e_ms, op=dist.ReduceOp.MAX)
-        e_ms = float(e_ms.item())
+        e_ms = max_over_ranks([a.elapsed_time(b) / n_e2e], dist, dev)[0]
         e2e = {"value": world * dec_bytes / (e_ms * 1e-3) / 1e9, "unit": "GB/s",
                "h2d_bytes_per_step": int(hk.numel() * 2 + hv.numel() * 2 + hq.numel() * 2),
                "d2h_bytes_per_step": int(hout.numel() * 4), "ms_per_step": e_ms,
@@ -318,12 +401,23 @@ def main():
                "quantize_tokens_per_s": n_t * G / tq / shape.Hkv,
                "gpu_over_cpu_decode": dec_gbs / (n_u * unit_bytes / td / 1e9)}
 
+    extras = None
+    if world == 1 and not args.no_extras:
+        for t in (Ks, Vs, caches, qs):
+            t.clear()
+        del ws, out
+        torch.cuda.empty_cache()
+        extras = run_extras(kv, W, dev, hbm_peak)
+
+    tr = stored_traffic()
     rl_quant = {"kernel": "quantize_kernel<2,bf16>", "bound": "alu", "achieved": q_tflops,
                 "peak": FP32_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s", "frac": q_tflops / FP32_PEAK_TFLOPS_NOMINAL,
-                "traffic": None, "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                "traffic": tr.get("quantize_kernel"), "algorithmic_bytes": q_bytes,
+                "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "hbm_achieved_GBps": q_gbs, "hbm_frac": q_gbs / hbm_peak, "ms": q_ms}
-    rl_dec = {"kernel": "decode_partial + decode_merge", "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak,
-              "unit": "GB/s", "frac": dec_gbs / hbm_peak, "traffic": None, "peak_source": peak_src,
+    rl_dec = {"kernel": "decode_kernel<2,4,bf16>", "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak,
+              "unit": "GB/s", "frac": dec_gbs / hbm_peak, "traffic": tr.get("decode_kernel"),
+              "algorithmic_bytes": dec_bytes, "peak_source": peak_src,
               "frac_of_nominal_8TBps": dec_gbs / 8000.0, "us": d_ms * 1e3}
     line = {
         "metric": "kvarn_2bit_decode_attn_GBps", "value": world * dec_gbs, "unit": "GB/s",
@@ -334,7 +428,8 @@ def main():
         "quantize_tokens_per_s": world * tok_s, "quantize_tiles_per_s": world * 2 * n_tiles / (q_ms * 1e-3),
         "roofline": rl_quant if q_ms > d_ms else rl_dec,
         "rooflines": {"quantize": rl_quant, "decode": rl_dec},
-        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": 3 * args.steps, "clocks": clocks,
+        "extras": extras,
+        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": 2 * args.steps, "clocks": clocks,
     }
     print(json.dumps(line))
     if dist: dist.destroy_process_group()

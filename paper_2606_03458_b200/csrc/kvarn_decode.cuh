@@ -58,7 +58,7 @@ struct DecodeArgs {
   void* out;
   float* ws;
   int B, Hkv, Hq, g, max_chunks, splits;
-  int cluster;    // CTAs per thread-block cluster along the split axis (1, 2, 4 or 8): merged through DSMEM
+  int cluster;    // CTAs per thread-block cluster along the split axis (1..16): merged through DSMEM
   int nclus;      // clusters per (sequence, KV head); splits = cluster * nclus; nclus > 1 -> workspace merge
   float q_scale;  // sm_scale * log2(e)
   int rotate_k, rotate_v, out_dtype;
@@ -656,8 +656,8 @@ __global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_kernel(const Deco
   int hbase = 0, hstride = 1;
   if (CS > 1) {
     const int crank = (int)cluster_ctarank();
-    float* land = reinterpret_cast<float*>(&sm.rec[0][0][0]);   // [<= 15][WS_STRIDE]
-    static_assert(sizeof(sm.rec) >= 15 * WS_STRIDE * sizeof(float), "landing area");
+    float* land = reinterpret_cast<float*>(&sm.rec[0][0][0]);   // [<= 16][WS_STRIDE]
+    static_assert(sizeof(sm.rec) >= 16 * WS_STRIDE * sizeof(float), "landing area");
     cluster_sync_all();
     const uint32_t land_addr = smem_u32(land);
 #pragma unroll

@@ -183,6 +183,20 @@ class Cache:
                               self.seq_lens.data_ptr(), self.ticket.data_ptr(),
                               self.decode_ticket.data_ptr(), B, Hkv, max_chunks, 0)
 
+    def slice(self, b0: int, b1: int) -> "Cache":
+        """A cache over sequences b0..b1-1 that shares this cache's buffers (views, no copy):
+        lets a large cache be filled or read a few sequences at a time."""
+        c = Cache.__new__(Cache)
+        c.B, c.Hkv, c.max_chunks, c.rb = b1 - b0, self.Hkv, self.max_chunks, self.rb
+        c.k_records, c.v_records = self.k_records[b0:b1], self.v_records[b0:b1]
+        c.k_resid, c.v_resid = self.k_resid[b0:b1], self.v_resid[b0:b1]
+        c.seq_lens, c.ticket = self.seq_lens[b0:b1], self.ticket[b0:b1]
+        c.decode_ticket = self.decode_ticket[b0 * self.Hkv:b1 * self.Hkv]
+        c.desc = CacheDesc(c.k_records.data_ptr(), c.v_records.data_ptr(), c.k_resid.data_ptr(),
+                           c.v_resid.data_ptr(), c.seq_lens.data_ptr(), c.ticket.data_ptr(),
+                           c.decode_ticket.data_ptr(), c.B, c.Hkv, c.max_chunks, 0)
+        return c
+
     def nbytes_read_by_decode(self, ctx: int) -> int:
         """Algorithmic bytes one decode step reads for context length ctx."""
         n_chunks, r = ctx // CHUNK, ctx % CHUNK

@@ -226,3 +226,59 @@ def test_append_capacity_guard(kv):
     torch.cuda.synchronize()
     assert cache.seq_lens.tolist() == [255] and torch.equal(cache.k_records, before)
     assert int(cache.ticket.sum()) == 0
+
+
+@pytest.mark.parametrize("Hq,splits", [(8, 3), (8, 5), (8, 7), (8, 8), (8, 16), (8, 21), (64, 2), (64, 3),
+                                       (64, 5), (64, 6), (64, 7), (64, 8), (64, 24)])
+def test_split_merge_paths_vs_oracle(kv, Hq, splits):
+    # every merge route of D7: one cluster of 2..8 CTAs (DSMEM reduce-scatter by head, g = 1 and
+    # g = 8 so that a rank owns 0, 1 or several heads), and several clusters through the workspace
+    n_tok = 128 * 26 + 77
+    K, V = W.kv_tokens(2, 8, n_tok, seed=63, device="cuda")
+    q = W.queries(2, Hq, seed=63, device="cuda")
+    p = kv.default_params(2, splits=splits)
+    cache = _build_cache(kv, p, K, V)
+    out = kv.decode_attention(p, cache, q)
+    _check_all_units(kv, p, cache, q, out, n_tok, units={(0, 0), (1, 3), (1, 7)})
+    assert int(cache.decode_ticket.abs().sum()) == 0
+    # a second call on the same cache (tickets self-reset) gives the same bits
+    assert torch.equal(out, kv.decode_attention(p, cache, q))
+
+
+def test_config2_shape_incremental_decode(kv):
+    # configs[2] (Qwen3-4B-shaped: B=16, 32 q / 8 KV heads) around the first append boundaries:
+    # prefill 512 tokens, then append + decode per step; oracle on sampled units at the context
+    # lengths SURVEY 8(d) names (639, 640, 641) -- the later growth to 32768 repeats these steps
+    s = W.CONFIG2
+    start, stop = 512, 642
+    K, V = W.kv_tokens(s.B, s.Hkv, stop, seed=s.seed, device="cuda")
+    q = W.queries(s.B, s.Hq, seed=s.seed, device="cuda")
+    p = kv.default_params(2)
+    cache = kv.Cache(p, s.B, s.Hkv, 8, device="cuda")
+    kv.prefill(p, cache, K[:, :, :start].contiguous(), V[:, :, :start].contiguous())
+    out = kv.decode_attention(p, cache, q)
+    _check_all_units(kv, p, cache, q, out, start, units={(0, 0), (15, 7)})
+    for t in range(start, stop):
+        kv.append(p, cache, K[:, :, t].contiguous(), V[:, :, t].contiguous())
+        out = kv.decode_attention(p, cache, q)
+        if t + 1 in (513, 639, 640, 641):
+            assert cache.seq_lens.tolist() == [t + 1] * s.B
+            _check_all_units(kv, p, cache, q, out, t + 1, units={(0, 0), (7, 3), (15, 7)})
+
+
+@pytest.mark.parametrize("bits", [2, 4])
+def test_config4_shape_sampled_units(kv, bits):
+    # configs[4] at full size (B=64, 64 q / 8 KV heads, ctx 65536 + 64-token bf16 residual), in the
+    # launch configuration bench.py's extras time; oracle on sampled (sequence, KV head) units
+    s = W.CONFIG4
+    p = kv.default_params(bits)
+    cache = kv.Cache(p, s.B, s.Hkv, s.n_chunks, device="cuda")
+    for b0 in range(0, s.B, 4):
+        K, V = W.kv_tokens(4, s.Hkv, s.ctx, seed=s.seed + b0, device="cuda")
+        kv.prefill(p, cache.slice(b0, b0 + 4), K, V)
+        del K, V
+    assert cache.seq_lens.tolist() == [s.ctx] * s.B
+    q = W.queries(s.B, s.Hq, seed=s.seed, device="cuda")
+    out = kv.decode_attention(p, cache, q)
+    assert torch.isfinite(out).all()
+    _check_all_units(kv, p, cache, q, out, s.ctx, units={(0, 0), (37, 5), (63, 7)})
