@@ -27,7 +27,8 @@ struct QuantArgs {
 
 template <int BITS, typename InT>
 __global__ void __launch_bounds__(256, 2) quantize_kernel(const QuantArgs A) {
-  __shared__ QuantSmem<BITS> sm;
+  extern __shared__ __align__(16) uint8_t quant_smem_raw[];
+  QuantSmem<BITS>& sm = *reinterpret_cast<QuantSmem<BITS>*>(quant_smem_raw);
   const int kind = A.kind_base + blockIdx.y;
   const long long tile = blockIdx.x;
   const long long outer = tile / A.n_inner, inner = tile - outer * A.n_inner;
@@ -61,7 +62,8 @@ struct AppendArgs {
 // the device from seq_lens (no host round trip).
 template <int BITS, typename InT>
 __global__ void __launch_bounds__(256, 2) append_kernel(const AppendArgs A) {
-  __shared__ QuantSmem<BITS> sm;
+  extern __shared__ __align__(16) uint8_t quant_smem_raw[];
+  QuantSmem<BITS>& sm = *reinterpret_cast<QuantSmem<BITS>*>(quant_smem_raw);
   const int kind = blockIdx.y, bh = blockIdx.x, b = bh / A.Hkv;
   const int tid = threadIdx.x;
   const int len = A.seq_lens[b];
@@ -136,16 +138,27 @@ static VarnConsts varn_consts(const kvarn_params* p) {
 
 static int last_cuda() { return cudaGetLastError() == cudaSuccess ? KVARN_OK : KVARN_CUDA; }
 
+// QuantSmem exceeds the 48 KB static limit (it keeps the per-iterate statistics of Alg. 1): dynamic, opt-in
+template <int BITS, auto KERN, typename Args>
+static void launch_quant_smem(dim3 grid, const Args& A, cudaStream_t st) {
+  static bool configured = false;   // per kernel (KERN is a template argument); benign race (idempotent call)
+  if (!configured) {
+    cudaFuncSetAttribute(KERN, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(QuantSmem<BITS>));
+    configured = true;
+  }
+  KERN<<<grid, dim3(256), sizeof(QuantSmem<BITS>), st>>>(A);
+}
+
 static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kinds, cudaStream_t st) {
   if (A.n_tiles == 0) return KVARN_OK;
-  dim3 grid((unsigned)A.n_tiles, (unsigned)n_kinds), block(256);
+  dim3 grid((unsigned)A.n_tiles, (unsigned)n_kinds);
   const bool f32 = p->in_dtype == KVARN_F32;
   if (p->bits == 2) {
-    if (f32) quantize_kernel<2, float><<<grid, block, 0, st>>>(A);
-    else quantize_kernel<2, __nv_bfloat16><<<grid, block, 0, st>>>(A);
+    if (f32) launch_quant_smem<2, quantize_kernel<2, float>>(grid, A, st);
+    else launch_quant_smem<2, quantize_kernel<2, __nv_bfloat16>>(grid, A, st);
   } else {
-    if (f32) quantize_kernel<4, float><<<grid, block, 0, st>>>(A);
-    else quantize_kernel<4, __nv_bfloat16><<<grid, block, 0, st>>>(A);
+    if (f32) launch_quant_smem<4, quantize_kernel<4, float>>(grid, A, st);
+    else launch_quant_smem<4, quantize_kernel<4, __nv_bfloat16>>(grid, A, st);
   }
   return last_cuda();
 }
@@ -369,15 +382,15 @@ int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_
   A.seq_lens = cache->seq_lens; A.ticket = cache->ticket;
   A.B = cache->B; A.Hkv = cache->Hkv; A.max_chunks = cache->max_chunks;
   A.rotate[0] = p->rotate_k; A.rotate[1] = p->rotate_v; A.vc = varn_consts(p);
-  dim3 grid((unsigned)(cache->B * cache->Hkv), 2), block(256);
+  dim3 grid((unsigned)(cache->B * cache->Hkv), 2);
   cudaStream_t s = (cudaStream_t)stream;
   const bool f32 = p->in_dtype == KVARN_F32;
   if (p->bits == 2) {
-    if (f32) append_kernel<2, float><<<grid, block, 0, s>>>(A);
-    else append_kernel<2, __nv_bfloat16><<<grid, block, 0, s>>>(A);
+    if (f32) launch_quant_smem<2, append_kernel<2, float>>(grid, A, s);
+    else launch_quant_smem<2, append_kernel<2, __nv_bfloat16>>(grid, A, s);
   } else {
-    if (f32) append_kernel<4, float><<<grid, block, 0, s>>>(A);
-    else append_kernel<4, __nv_bfloat16><<<grid, block, 0, s>>>(A);
+    if (f32) launch_quant_smem<4, append_kernel<4, float>>(grid, A, s);
+    else launch_quant_smem<4, append_kernel<4, __nv_bfloat16>>(grid, A, s);
   }
   return last_cuda();
 }

@@ -38,13 +38,20 @@ struct QuantDebug {
 
 template <int BITS>
 struct QuantSmem {
-  float part[8][2][128];  // cross-warp partials (row sums / min-max)
+  alignas(16) float part[8][2][128];  // cross-warp partials (row sums / min-max)
   float a[128];           // 1 / S_r  (per channel)
   float b[128];           // 1 / S_c  (per token)
-  float cv[128];          // raw column (token) variances of the current C
-  float rv[2][128];       // row (channel) variances of C after the row update
-  float Sc[128], Sr[128]; // best scales
-  float inv_s[128], z[128];
+  // per iterate k = 0..iters: column / row variances of C_k and the log-scales that produced it;
+  // the best iterate (Alg. 1 lines 7, 18) is selected once, after the loop
+  float cvh[KVARN_MAX_ITERS + 1][128];
+  float rvh[KVARN_MAX_ITERS + 1][128];
+  float Lch[KVARN_MAX_ITERS + 1][128];
+  float Lrh[KVARN_MAX_ITERS + 1][128];
+  float imb[KVARN_MAX_ITERS + 1];
+  alignas(16) float Sc[128];   // best scales
+  alignas(16) float Sr[128];
+  alignas(16) float inv_s[128];
+  alignas(16) float z[128];
   alignas(16) uint8_t rec[record_bytes(BITS)];
 };
 
@@ -89,6 +96,8 @@ __device__ __forceinline__ float xreduce16(float (&v)[16], int li, Op op) {
   }
   return v[0];
 }
+
+constexpr float RTN_MAGIC = 12582912.0f;   // 1.5 * 2^23: (t + MAGIC) - MAGIC = rint(t), ties to even, for |t| < 2^22
 
 struct OpAdd { __device__ float operator()(float a, float b) const { return a + b; } };
 struct OpMin { __device__ float operator()(float a, float b) const { return fminf(a, b); } };
@@ -147,10 +156,8 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
 #pragma unroll
   for (int i = 0; i < 8; ++i) b[i] = 1.f;
 
-  float Lc = 0.f, Lc_prev = 0.f, Lc_best = 0.f, b_own = 1.f;  // log column scale of tok_own
-  float Lr = 0.f, Lr_best = 0.f, a_own = 1.f;    // log row scale of channel tid (tid < 128)
-  float I_best = 0.f;
-  int k_best = 0;
+  float Lc = 0.f, b_own = 1.f;  // log column scale of tok_own
+  float Lr = 0.f, a_own = 1.f;  // log row scale of channel tid (tid < 128)
 
   // row half-step, part 1: per-channel sums of (b_t T) and (b_t T)^2 over this
   // warp's 16 tokens -> sm.part[warp][stat][channel]
@@ -208,9 +215,9 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
   };
 
   // Imb(C) (DESIGN R1) from the 128 column and 128 row variances in shared memory
-  auto imbalance = [&](int rv_buf) -> float {
-    const float4 c4 = reinterpret_cast<const float4*>(sm.cv)[lane];
-    const float4 r4 = reinterpret_cast<const float4*>(sm.rv[rv_buf])[lane];
+  auto imbalance = [&](int k) -> float {
+    const float4 c4 = reinterpret_cast<const float4*>(sm.cvh[k])[lane];
+    const float4 r4 = reinterpret_cast<const float4*>(sm.rvh[k])[lane];
     float mx = fmaxf(fmaxf(fmaxf(c4.x, c4.y), fmaxf(c4.z, c4.w)), fmaxf(fmaxf(r4.x, r4.y), fmaxf(r4.z, r4.w)));
     float mn = fminf(fminf(fminf(c4.x, c4.y), fminf(c4.z, c4.w)), fminf(fminf(r4.x, r4.y), fminf(r4.z, r4.w)));
     mx = warp_max(mx);
@@ -221,7 +228,7 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
   // pass 0: row variances of the initial C = T (needed by I_best <- Imb(C), line 7)
   row_partials();
   __syncthreads();
-  if (tid < 128) sm.rv[0][tid] = row_variance_own();
+  if (tid < 128) { sm.rvh[0][tid] = row_variance_own(); sm.Lrh[0][tid] = 0.f; }
   __syncthreads();
 
   for (int k = 1; k <= vc.iters + 1; ++k) {
@@ -249,8 +256,7 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       const float s1t = (li & 8) ? other : mine, s2t = (li & 8) ? mine : other;
       const float mean = s1t * inv_n;
       const float var = fmaxf(fmaf(-mean, mean, s2t * inv_n), 0.f) * (b_own * b_own);
-      Lc_prev = Lc;
-      if (li < 8) sm.cv[tok_own] = var;
+      if (li < 8) { sm.cvh[k - 1][tok_own] = var; sm.Lch[k - 1][tok_own] = Lc; }
       if (update) {
         const float vcl = fminf(fmaxf(var, vc.var_min), vc.var_max);
         Lc = fminf(fmaxf(Lc + 0.5f * logf(vcl), vc.log_lo), vc.log_hi);
@@ -263,14 +269,6 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     // ---- row half-step (lines 13-15) --------------------------------------------
     if (update) row_partials();
     __syncthreads();
-    // I_{k-1} = Imb(C_{k-1}) is now complete: keep the iterate if it is not worse
-    {
-      const float imb = imbalance((k - 1) & 1);
-      if (dbg.imb && tid == 0) dbg.imb[tile_idx * (KVARN_MAX_ITERS + 1) + (k - 1)] = imb;
-      if (k == 1 || imb <= I_best) {  // line 7 / line 18
-        I_best = imb; k_best = k - 1; Lc_best = Lc_prev; Lr_best = Lr;
-      }
-    }
     if (update) {
       if (tid < 128) {
         const float var = row_variance_own();
@@ -278,7 +276,8 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
         const float Lr_new = fminf(fmaxf(Lr + 0.5f * logf(vcl), vc.log_lo), vc.log_hi);
         const float a_new = expf(-Lr_new);
         const float ratio = a_new / a_own;
-        sm.rv[k & 1][tid] = var * ratio * ratio;  // row variance after rescaling the row
+        sm.rvh[k][tid] = var * ratio * ratio;  // row variance after rescaling the row
+        sm.Lrh[k][tid] = Lr_new;
         sm.a[tid] = a_new;
         Lr = Lr_new; a_own = a_new;
       }
@@ -287,9 +286,27 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     }
   }
 
+  // ---- best iterate (lines 7, 18): I_k = Imb(C_k), keep the last k with I_k <= min of the earlier ones
+  __syncthreads();
+  for (int k = warp; k <= vc.iters; k += 8) {
+    const float imb = imbalance(k);
+    if (lane == 0) {
+      sm.imb[k] = imb;
+      if (dbg.imb) dbg.imb[tile_idx * (KVARN_MAX_ITERS + 1) + k] = imb;
+    }
+  }
+  __syncthreads();
+  int k_best = 0;
+  {
+    float I_best = sm.imb[0];
+    for (int k = 1; k <= vc.iters; ++k) {
+      const float imb = sm.imb[k];
+      if (imb <= I_best) { I_best = imb; k_best = k; }
+    }
+  }
   // ---- best scales (line 24): T_bal = T / S_c* / S_r* ----------------------------
-  if (li < 8) { sm.Sc[tok_own] = expf(Lc_best); sm.b[tok_own] = expf(-Lc_best); }
-  if (tid < 128) { sm.Sr[tid] = expf(Lr_best); sm.a[tid] = expf(-Lr_best); }
+  if (li < 8) { const float L = sm.Lch[k_best][tok_own]; sm.Sc[tok_own] = expf(L); sm.b[tok_own] = expf(-L); }
+  if (tid < 128) { const float L = sm.Lrh[k_best][tid]; sm.Sr[tid] = expf(L); sm.a[tid] = expf(-L); }
   __syncthreads();
   reload_a();
   reload_b();
@@ -352,20 +369,38 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     inv_s[4] = i1.x; inv_s[5] = i1.y; inv_s[6] = i1.z; inv_s[7] = i1.w;
     zz[0] = z0.x; zz[1] = z0.y; zz[2] = z0.z; zz[3] = z0.w;
     zz[4] = z1.x; zz[5] = z1.y; zz[6] = z1.z; zz[7] = z1.w;
-    // codes: row per token, channel c at bit BITS*(c%..) -- natural little-endian order
+    // codes: row per token, channel c at bit BITS*(c%..) -- natural little-endian order.
+    // code = rint(x / s - z) by the magic-number add (RNE, like rintf); x lies inside [mn, mx] of its
+    // group, so x / s - z is within rounding error of [0, LV] and needs no clamp.  The 8 codes of a
+    // thread are packed by exact float accumulation sum code_j 2^(BITS j) (< 2^16 per accumulator).
+    float2 is2[4], nz2[4];
+#pragma unroll
+    for (int kp = 0; kp < 4; ++kp) { is2[kp] = f2(inv_s[2 * kp], inv_s[2 * kp + 1]); nz2[kp] = f2(-zz[2 * kp], -zz[2 * kp + 1]); }
+    const float2 magic = f2(RTN_MAGIC, RTN_MAGIC), nmagic = f2(-RTN_MAGIC, -RTN_MAGIC);
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-      uint32_t w = 0;
-#pragma unroll
-      for (int kp = 0; kp < 4; ++kp) {
-        float q0 = fminf(fmaxf(rintf(fmaf(x[i][kp].x, inv_s[2 * kp], -zz[2 * kp])), 0.f), (float)LV);
-        float q1 = fminf(fmaxf(rintf(fmaf(x[i][kp].y, inv_s[2 * kp + 1], -zz[2 * kp + 1])), 0.f), (float)LV);
-        w |= ((uint32_t)q0) << (BITS * 2 * kp);
-        w |= ((uint32_t)q1) << (BITS * (2 * kp + 1));
-      }
       const int slot = slot_of_token(BITS, t0 + i);
-      if (BITS == 2) *reinterpret_cast<uint16_t*>(&sm.rec[code_off(2, slot, 2 * li)]) = (uint16_t)w;
-      else *reinterpret_cast<uint32_t*>(&sm.rec[code_off(4, slot, 4 * li)]) = w;
+      if (BITS == 2) {
+        float2 acc = f2(0.f, 0.f);
+#pragma unroll
+        for (int kp = 0; kp < 4; ++kp) {
+          const float2 q = add2(add2(fma2(x[i][kp], is2[kp], nz2[kp]), magic), nmagic);
+          acc = fma2(q, f2((float)(1 << (4 * kp)), (float)(4 << (4 * kp))), acc);
+        }
+        *reinterpret_cast<uint16_t*>(&sm.rec[code_off(2, slot, 2 * li)]) = (uint16_t)__float2uint_rn(acc.x + acc.y);
+      } else {
+        float2 lo = f2(0.f, 0.f), hi = f2(0.f, 0.f);
+#pragma unroll
+        for (int kp = 0; kp < 2; ++kp) {
+          const float2 q0 = add2(add2(fma2(x[i][kp], is2[kp], nz2[kp]), magic), nmagic);
+          const float2 q1 = add2(add2(fma2(x[i][kp + 2], is2[kp + 2], nz2[kp + 2]), magic), nmagic);
+          const float2 wgt = f2((float)(1 << (8 * kp)), (float)(16 << (8 * kp)));
+          lo = fma2(q0, wgt, lo);
+          hi = fma2(q1, wgt, hi);
+        }
+        *reinterpret_cast<uint32_t*>(&sm.rec[code_off(4, slot, 4 * li)]) =
+            __float2uint_rn(lo.x + lo.y) | (__float2uint_rn(hi.x + hi.y) << 16);
+      }
     }
   } else {
     // group = token over the 128 channels: min / max inside the half-warp
@@ -407,23 +442,34 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     inv_s[4] = i1.x; inv_s[5] = i1.y; inv_s[6] = i1.z; inv_s[7] = i1.w;
     zz[0] = z0.x; zz[1] = z0.y; zz[2] = z0.z; zz[3] = z0.w;
     zz[4] = z1.x; zz[5] = z1.y; zz[6] = z1.z; zz[7] = z1.w;
-    // codes: row per CHANNEL, token t at bit BITS*(t%..) of the row
-    uint32_t w[8];
+    // codes: row per CHANNEL, token t at bit BITS*(t%..) of the row (rounding and packing as for K)
+    const float2 magic = f2(RTN_MAGIC, RTN_MAGIC), nmagic = f2(-RTN_MAGIC, -RTN_MAGIC);
+    float2 lo[4], hi[4];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) w[k] = 0;
+    for (int kp = 0; kp < 4; ++kp) { lo[kp] = f2(0.f, 0.f); hi[kp] = f2(0.f, 0.f); }
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < 8; ++i) {
+      const float2 is2 = f2(inv_s[i], inv_s[i]), nz2 = f2(-zz[i], -zz[i]);
+      const float wv = BITS == 2 ? (float)(1 << (2 * i)) : (float)(1 << (4 * (i & 3)));
+      const float2 wgt = f2(wv, wv);
 #pragma unroll
       for (int kp = 0; kp < 4; ++kp) {
-        float q0 = fminf(fmaxf(rintf(fmaf(x[i][kp].x, inv_s[i], -zz[i])), 0.f), (float)LV);
-        float q1 = fminf(fmaxf(rintf(fmaf(x[i][kp].y, inv_s[i], -zz[i])), 0.f), (float)LV);
-        w[2 * kp] |= ((uint32_t)q0) << (BITS * i);
-        w[2 * kp + 1] |= ((uint32_t)q1) << (BITS * i);
+        const float2 q = add2(add2(fma2(x[i][kp], is2, nz2), magic), nmagic);
+        if (BITS == 2 || i < 4) lo[kp] = fma2(q, wgt, lo[kp]);
+        else hi[kp] = fma2(q, wgt, hi[kp]);
       }
+    }
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      if (BITS == 2) *reinterpret_cast<uint16_t*>(&sm.rec[code_off(2, c0 + k, 2 * (2 * warp + lj))]) = (uint16_t)w[k];
-      else *reinterpret_cast<uint32_t*>(&sm.rec[code_off(4, c0 + k, 4 * (2 * warp + lj))]) = w[k];
+    for (int kp = 0; kp < 4; ++kp) {
+      if (BITS == 2) {
+        *reinterpret_cast<uint16_t*>(&sm.rec[code_off(2, c0 + 2 * kp, 2 * (2 * warp + lj))]) = (uint16_t)__float2uint_rn(lo[kp].x);
+        *reinterpret_cast<uint16_t*>(&sm.rec[code_off(2, c0 + 2 * kp + 1, 2 * (2 * warp + lj))]) = (uint16_t)__float2uint_rn(lo[kp].y);
+      } else {
+        *reinterpret_cast<uint32_t*>(&sm.rec[code_off(4, c0 + 2 * kp, 4 * (2 * warp + lj))]) =
+            __float2uint_rn(lo[kp].x) | (__float2uint_rn(hi[kp].x) << 16);
+        *reinterpret_cast<uint32_t*>(&sm.rec[code_off(4, c0 + 2 * kp + 1, 4 * (2 * warp + lj))]) =
+            __float2uint_rn(lo[kp].y) | (__float2uint_rn(hi[kp].y) << 16);
+      }
     }
   }
   if (dbg.k_best && tid == 0) dbg.k_best[tile_idx] = k_best;
