@@ -204,26 +204,59 @@ def run_extras(kv, W, dev, hbm_peak):
     stream = torch.cuda.current_stream()
     ex = {}
     s4 = W.CONFIG4
-    for bits in (2, 4):
-        p = kv.default_params(bits)
-        rb = kv.record_bytes(p)
-        cache = kv.Cache(p, s4.B, s4.Hkv, s4.n_chunks, device=dev)
-        for b0 in range(0, s4.B, 4):   # fill 4 sequences at a time (1.1 GB of bf16 K/V each)
-            K, V = W.kv_tokens(4, s4.Hkv, s4.ctx, seed=s4.seed + b0, device=dev)
-            kv.prefill(p, cache.slice(b0, b0 + 4), K, V)
-            del K, V
-        q = W.queries(s4.B, s4.Hq, seed=s4.seed, device=dev)
-        ws = torch.empty((max(kv.decode_workspace_bytes(p, s4.B, s4.Hq, s4.Hkv, s4.n_chunks), 16),), dtype=torch.uint8, device=dev)
-        out = torch.empty((s4.B, s4.Hq, D), dtype=torch.float32, device=dev)
-        for _ in range(3):
-            kv.decode_attention(p, cache, q, out=out, ws=ws)
-        torch.cuda.synchronize()
-        med, mn = _time_launches(lambda i: kv.decode_attention(p, cache, q, out=out, ws=ws), 10, stream)
-        byts = cache.nbytes_read_by_decode(s4.ctx) + s4.B * s4.Hq * (D * 2 + D * 4)
-        ex[f"decode_cfg4_{bits}bit"] = {"us": med * 1e3, "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak,
-                                        "bytes": byts, "B": s4.B, "Hq": s4.Hq, "Hkv": s4.Hkv, "ctx": s4.ctx}
-        del cache, q, ws, out
-        torch.cuda.empty_cache()
+    long_g4 = W.DecodeShape("long_context_g4", B=16, Hq=32, Hkv=8, ctx=65536, seed=5)   # Llama-3.1-8B heads, 64k context
+    for name, sh in (("decode_cfg4", s4), ("decode_long_g4", long_g4)):
+        for bits in (2, 4):
+            p = kv.default_params(bits)
+            cache = kv.Cache(p, sh.B, sh.Hkv, sh.n_chunks, device=dev)
+            for b0 in range(0, sh.B, 4):   # fill 4 sequences at a time (1.1 GB of bf16 K/V each)
+                K, V = W.kv_tokens(4, sh.Hkv, sh.ctx, seed=sh.seed + b0, device=dev)
+                kv.prefill(p, cache.slice(b0, b0 + 4), K, V)
+                del K, V
+            q = W.queries(sh.B, sh.Hq, seed=sh.seed, device=dev)
+            ws = torch.empty((max(kv.decode_workspace_bytes(p, sh.B, sh.Hq, sh.Hkv, sh.n_chunks), 16),), dtype=torch.uint8, device=dev)
+            out = torch.empty((sh.B, sh.Hq, D), dtype=torch.float32, device=dev)
+            for _ in range(3):
+                kv.decode_attention(p, cache, q, out=out, ws=ws)
+            torch.cuda.synchronize()
+            med, mn = _time_launches(lambda i: kv.decode_attention(p, cache, q, out=out, ws=ws), 10, stream)
+            byts = cache.nbytes_read_by_decode(sh.ctx) + sh.B * sh.Hq * (D * 2 + D * 4)
+            ex[f"{name}_{bits}bit"] = {"us": med * 1e3, "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak,
+                                       "bytes": byts, "B": sh.B, "Hq": sh.Hq, "Hkv": sh.Hkv, "ctx": sh.ctx}
+            del cache, q, ws, out
+            torch.cuda.empty_cache()
+    # configs[2] (Qwen3-4B-shaped incremental decode, B=16): the last 256 steps of the growth to 32768 tokens,
+    # one kvarn_append + one kvarn_decode_attention per step (two chunk boundaries inside); 302 MB of records
+    s2 = W.CONFIG2
+    p = kv.default_params(2)
+    n0 = s2.ctx - 256
+    cache = kv.Cache(p, s2.B, s2.Hkv, s2.n_chunks, device=dev)
+    K, V = W.kv_tokens(s2.B, s2.Hkv, s2.ctx, seed=s2.seed, device=dev)
+    kv.prefill(p, cache, K[:, :, :n0].contiguous(), V[:, :, :n0].contiguous())
+    q = W.queries(s2.B, s2.Hq, seed=s2.seed, device=dev)
+    ws = torch.empty((max(kv.decode_workspace_bytes(p, s2.B, s2.Hq, s2.Hkv, s2.n_chunks), 16),), dtype=torch.uint8, device=dev)
+    out = torch.empty((s2.B, s2.Hq, D), dtype=torch.float32, device=dev)
+    Kt = K[:, :, n0:].transpose(0, 2).transpose(1, 2).contiguous()   # [256][B][Hkv][128]
+    Vt = V[:, :, n0:].transpose(0, 2).transpose(1, 2).contiguous()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(256)]
+    for i in range(256):
+        evs[i][0].record(stream); kv.append(p, cache, Kt[i], Vt[i])
+        evs[i][1].record(stream); kv.decode_attention(p, cache, q, out=out, ws=ws)
+        evs[i][2].record(stream)
+    torch.cuda.synchronize()
+    ap = [e[0].elapsed_time(e[1]) * 1e3 for e in evs]
+    dc = [e[1].elapsed_time(e[2]) * 1e3 for e in evs]
+    bnd = [i for i in range(256) if (n0 + i + 1) % G == 0]
+    plain = sorted(ap[i] for i in range(8, 256) if i not in bnd)
+    byts = cache.nbytes_read_by_decode(s2.ctx - 128) + s2.B * s2.Hq * (D * 2 + D * 4)
+    dmed = sorted(dc[8:])[len(dc[8:]) // 2]
+    ex["cfg2_incremental"] = {"append_plain_us": plain[len(plain) // 2], "append_boundary_us": [ap[i] for i in bnd],
+                              "append_mean_us": sum(ap[8:]) / len(ap[8:]), "decode_us": dmed,
+                              "decode_GBps": byts / dmed / 1e3, "decode_hbm_frac": byts / dmed / 1e3 / hbm_peak,
+                              "ctx": [n0, s2.ctx], "B": s2.B, "final_seq_len": int(cache.seq_lens[0].item()),
+                              "note": "event pairs around single short launches include launch latency"}
+    del cache, K, V, Kt, Vt, q, ws, out
+    torch.cuda.empty_cache()
     n_tok = 1 << 20
     K, V = W.quantizer_sweep_tiles(8, n_tok, seed=3, device=dev)
     n_tiles = 8 * n_tok // G

@@ -72,20 +72,37 @@ typedef struct {
   int32_t rotate_v;  /* 1: Hadamard-rotate V tiles (and un-rotate the output) */
   int32_t in_dtype;  /* kvarn_dtype of K, V, q and of the residual window */
   int32_t out_dtype; /* kvarn_dtype of the attention output */
-  int32_t splits;    /* decode split-K factor over chunks; 0 = choose automatically */
+  int32_t splits;    /* decode split-K factor over chunks; 0 = choose automatically.  A value s > 0 runs
+                      * c = the largest divisor of s that is <= 8 CTAs per thread-block cluster (merged
+                      * through distributed shared memory) and s / c clusters merged through the workspace */
   int32_t reserved;
 } kvarn_params;
 
-/* Byte layout of one record (fixed by bits).  codes: K records hold one row
- * per TOKEN (its 128 channels), V records one row per CHANNEL (its 128 tokens);
- * a row is little-endian (element e at bit bits*(e % (8/bits)) of byte
- * e*bits/8) and is stored in 16-byte segments, segment s of row r at byte
- * s*2048 + r*16 -- the order the decode kernel's TMEM operand loader reads.
+/* Byte layout of one record (fixed by bits): codes | s1[128] e4m3 | s2[128] e4m3 | z[128] f16.
+ * codes: K records hold one row per TOKEN (its 128 channels), V records one row
+ * per CHANNEL (its 128 tokens); a row is little-endian (element e at bit
+ * bits*(e % (8/bits)) of byte e*bits/8).  Rows are the M rows of the decode
+ * kernel's integer MMAs (m16n8k32): row slot s = 32*warp + 16*mtile + 8*rho + g
+ * is held by the threads (g = lane>>2, t = lane&3) of `warp`, and thread t
+ * expands the 32-bit words t, t+4 (, t+8, t+12 at 4-bit) of the row.  Byte b of
+ * word wi = 4*q + t of slot s sits at
+ *     2-bit: warp*1024 + mtile*512 + (4*g + t)*16 + rho*8 + q*4 + b
+ *     4-bit: warp*2048 + mtile*1024 + rho*512 + (4*g + t)*16 + q*4 + b
+ * (one conflict-free 16-byte shared-memory load per lane).  In the contraction
+ * element e of a row is position p of k-step kappa:
+ *     2-bit: kappa = e & 3,               p = 16*(e>>6) + 4*((e>>4)&3) + ((e>>2)&3)
+ *     4-bit: kappa = 2*(e>>6) + (e&1),    p = 16*((e>>5)&1) + 4*((e>>3)&3) + ((e>>1)&3)
+ * V rows use slot = channel.  K rows use slot(token tau) = 32*kappa(tau) +
+ * 16*(b>>1) + 8*(b&1) + 4*(p>>4) + ((p>>2)&3) with b = p & 3 -- the four tokens
+ * a thread sees after the QK^T MMA are then one 32-bit word of the B operand of
+ * the value MMA.
  * s1 = FP8-E4M3 absorbed scale of the RTN group (K: per channel, V: per token),
  * s2 = FP8-E4M3 second (Sinkhorn) scale of the other axis, z = FP16 zero-point
- * of the RTN group (Eq. 1: x_dq = (code + z) * s1 * s2).  K records keep
- * s1 and z in the order the decode kernel's B-operand builder reads them (a
- * permutation of the channels, kaux_of_elem in csrc/kvarn_common.cuh); use kvarn_unpack_record_host for a canonical view. */
+ * of the RTN group (Eq. 1: x_dq = (code + z) * s1 * s2).  Per-token
+ * arrays (K.s2, V.s1, V.z) are indexed by slot(token); K.s1 and K.z (per
+ * channel) by 4*(8*kappa + (p>>2)) + (p&3) of the channel (the order in which
+ * the decode kernel's B-operand builder reads them); V.s2 by channel.
+ * kvarn_unpack_record_host gives the canonical view (codes[t][c], natural order). */
 typedef struct {
   size_t record_bytes; /* 4608 at 2-bit, 8704 at 4-bit (=> 2.25 / 4.25 bit per element) */
   size_t codes_off, codes_bytes;
@@ -126,7 +143,8 @@ KVARN_API int kvarn_version(void);
 /* Record layout for p->bits.  Returns KVARN_UNSUPPORTED for other bit widths. */
 KVARN_API int kvarn_layout(const kvarn_params* p, kvarn_layout_info* out);
 
-/* Bytes of DEVICE workspace kvarn_decode_attention needs for this shape. */
+/* Bytes of DEVICE workspace kvarn_decode_attention needs for this shape (partials of the
+ * cross-cluster merge; touched only when more than one cluster shares a sequence). */
 KVARN_API size_t kvarn_decode_workspace_bytes(const kvarn_params* p, int32_t B, int32_t Hq, int32_t Hkv,
                                     int32_t max_chunks);
 

@@ -287,7 +287,13 @@ __device__ __forceinline__ float undigit(int d0, int d1, int d2, int d3) {
 }
 
 template <int BITS, int GP, typename InT>
-__global__ void __launch_bounds__(128, GP == 4 ? 6 : 4) decode_kernel(const DecodeArgs A) {
+#ifndef KVARN_DEC_OCC4
+#define KVARN_DEC_OCC4 4
+#endif
+#ifndef KVARN_DEC_OCC8
+#define KVARN_DEC_OCC8 4
+#endif
+__global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8) decode_kernel(const DecodeArgs A) {
   using SM = DecSmem<BITS, GP>;
   constexpr int RB = SM::RB, STAGES = SM::STAGES, NT = SM::NT;
   constexpr int NCLS = 8 / BITS;
