@@ -167,14 +167,19 @@ static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kind
 // (sequence, KV head) and merge through DSMEM; `nclus` clusters per (sequence, KV head) merge
 // through the workspace (only when one cluster leaves most of the GPU idle on long contexts).
 struct SplitPlan { int cluster, nclus; };
+// chunks per loop iteration of decode_kernel: two at 2-bit with g <= 4 (two independent instruction
+// streams per warp between barriers: 205 -> 193 us on the long-context case); one otherwise -- at 4-bit the
+// kernel already runs at ~0.8 of the HBM peak and the doubled record ring would leave two CTAs per SM,
+// at g = 8 the doubled register footprint (222) measured slower (346 -> 363 us)
+constexpr int dec_nch(int bits, int gp) { return (bits == 2 && gp == 4) ? 2 : 1; }
 constexpr int KVARN_MAX_CLUSTER = 8;    // portable maximum; 9..16 (non-portable) measured slower: 25 -> 27..31 us on config 1
 
 template <int BITS, int GP, typename InT>
 static int decode_ctas_per_sm() {
   static int cached = 0;   // per instantiation; benign race (same value)
   if (cached) return cached;
-  using SM = DecSmem<BITS, GP>;
-  auto kern = decode_kernel<BITS, GP, InT>;
+  using SM = DecSmem<BITS, GP, dec_nch(BITS, GP)>;
+  auto kern = decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>;
   int n = 0;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SM));
   cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -230,9 +235,9 @@ static SplitPlan split_plan(const kvarn_params* p, int B, int Hkv, int g, int ma
 
 template <int BITS, int GP, typename InT>
 static cudaError_t launch_decode_k(const DecodeArgs& A, cudaStream_t st) {
-  using SM = DecSmem<BITS, GP>;
+  using SM = DecSmem<BITS, GP, dec_nch(BITS, GP)>;
   static bool configured = false;   // per instantiation; benign race (idempotent attribute calls)
-  auto kern = decode_kernel<BITS, GP, InT>;
+  auto kern = decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>;
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SM));
     if (e != cudaSuccess) return e;

@@ -41,6 +41,8 @@
 // clk/IMMA/SM), below the HBM time of a chunk, with no asynchronous-proxy hand-off.
 #pragma once
 
+#include <type_traits>
+
 #include "kvarn_common.cuh"
 
 namespace kvarn {
@@ -191,22 +193,26 @@ constexpr int MAGIC_I = 0x4B400000;
 constexpr float Q_FIX = 4194300.0f;          // 2^22: fixed-point scale of qt relative to max_c |qt[h,c]|
 constexpr float P_FIX = 4194304.0f;          // 2^22: fixed-point scale of pt = p s1v <= 1
 
-template <int BITS, int GP>
+// NCH = chunks processed per loop iteration (per barrier interval).  NCH = 2 gives every warp two
+// independent instruction streams between barriers (the kernel is bound by dependent-issue latency,
+// not by occupancy: DESIGN.md 6.2) and halves the barriers per chunk.
+template <int BITS, int GP, int NCH>
 struct DecSmem {
   static constexpr int RB = record_bytes(BITS);
   static constexpr int STAGES = 2;
   static constexpr int NT = GP / 2;            // n-tiles (8 columns each): 4 radix-256 digits x GP heads
-  alignas(128) uint8_t rec[STAGES][2][RB];     // [stage][K | V] records
+  alignas(128) uint8_t rec[STAGES][NCH][2][RB];   // [stage][chunk of the iteration][K | V] records
   // B operands in fragment order: word (nu, kappa, half, lane' = 4 g' + t') -> [nu][hk = kappa>>1][b_slot(lane', hk)][2 (kappa&1) + half]
-  alignas(16) uint32_t bq[NT][2][32][4];
-  alignas(16) uint32_t bp[NT][2][32][4];
-  alignas(16) float4 aux_tok[128];             // per MMA row slot of the K tile: {s2, log2 s1v, 1 / s1v, zv} of its token
-  alignas(16) float aux_ch[2][128];            // per channel: s2v / P_FIX (double-buffered by chunk parity)
+  alignas(16) uint32_t bq[NCH][NT][2][32][4];
+  alignas(16) uint32_t bp[NCH][NT][2][32][4];
+  alignas(16) float2 aux_a[NCH][128];          // per MMA row slot of the K tile: {s2, log2 s1v} of its token
+  alignas(16) float2 aux_b[NCH][128];          //                                 {1 / s1v, zv}
+  alignas(16) float aux_ch[2][NCH][128];       // per channel: s2v / P_FIX (double-buffered by iteration parity)
   alignas(16) float qrot[GP][128];             // q' (rotated, scaled); later: staging of acc / merged acc_rot
   alignas(16) float qraw[GP][128];             // q * q_scale (un-rotated, for the residual window); later p of the residual
-  alignas(16) float hs[GP][2];                 // per head: {scale, beta} of the current chunk
-  alignas(16) float hmax[GP][4];               // per head: per-warp maxima
-  alignas(16) float hz[GP][4];                 // per head: per-warp zero-point sums / l sums
+  alignas(16) float hs[NCH][GP][2];            // per head: {scale, beta} of the current chunks
+  alignas(16) float hmax[GP][4];               // per head: per-warp maxima (over the chunks of the iteration)
+  alignas(16) float hz[NCH][GP][4];            // per head: per-warp zero-point sums / l sums
   alignas(16) float wmax[4][GP];               // residual window: per-warp maxima
   alignas(16) float wz[4][GP];                 // residual window / final l: per-warp sums
   alignas(8) uint64_t fullk[STAGES];
@@ -286,15 +292,15 @@ __device__ __forceinline__ float undigit(int d0, int d1, int d2, int d3) {
   return fmaf(__int2float_rn(x23), 65536.f, __int2float_rn(x01));
 }
 
-template <int BITS, int GP, typename InT>
+template <int BITS, int GP, int NCH, typename InT>
 #ifndef KVARN_DEC_OCC4
 #define KVARN_DEC_OCC4 4
 #endif
 #ifndef KVARN_DEC_OCC8
 #define KVARN_DEC_OCC8 4
 #endif
-__global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8) decode_kernel(const DecodeArgs A) {
-  using SM = DecSmem<BITS, GP>;
+__global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8) / NCH) decode_kernel(const DecodeArgs A) {
+  using SM = DecSmem<BITS, GP, NCH>;
   constexpr int RB = SM::RB, STAGES = SM::STAGES, NT = SM::NT;
   constexpr int NCLS = 8 / BITS;
   constexpr float CLS_INV = BITS == 2 ? (1.f / 64.f) : (1.f / 16.f);  // 1 / CLSMAX
@@ -328,13 +334,17 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     for (int s = 0; s < STAGES; ++s) { mbar_init(&sm.fullk[s], 1); mbar_init(&sm.fullv[s], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 #pragma unroll
-    for (int s = 0; s < STAGES; ++s)
-      if (s < n_my) {
-        mbar_expect_tx(&sm.fullk[s], RB);
-        bulk_g2s(sm.rec[s][0], krec + (size_t)s * RB, RB, &sm.fullk[s]);
-        mbar_expect_tx(&sm.fullv[s], RB);
-        bulk_g2s(sm.rec[s][1], vrec + (size_t)s * RB, RB, &sm.fullv[s]);
+    for (int s = 0; s < STAGES; ++s) {
+      const int nc = min(NCH, n_my - s * NCH);   // chunks of iteration s
+      if (nc > 0) {
+        mbar_expect_tx(&sm.fullk[s], nc * RB);
+        mbar_expect_tx(&sm.fullv[s], nc * RB);
+        for (int c = 0; c < nc; ++c) {
+          bulk_g2s(sm.rec[s][c][0], krec + (size_t)(s * NCH + c) * RB, RB, &sm.fullk[s]);
+          bulk_g2s(sm.rec[s][c][1], vrec + (size_t)(s * NCH + c) * RB, RB, &sm.fullv[s]);
+        }
       }
+    }
   }
 
   // D1: q' = (q H / sqrt(128)) * q_scale; heads >= g are zero
@@ -373,7 +383,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   // column (h, d) of head h = warp + 4u: n-tile 2u + (d >> 1), g' = 2 warp + (d & 1); lane' = 4 g' + t'
   uint32_t* bq_dst[2];
 #pragma unroll
-  for (int dd = 0; dd < 2; ++dd) bq_dst[dd] = &sm.bq[0][bk >> 1][b_slot(4 * (2 * warp + dd) + btp, bk >> 1)][2 * (bk & 1) + bhalf];
+  for (int dd = 0; dd < 2; ++dd) bq_dst[dd] = &sm.bq[0][0][bk >> 1][b_slot(4 * (2 * warp + dd) + btp, bk >> 1)][2 * (bk & 1) + bhalf];
   // softmax role: thread (warp, fg, ft) sees tokens slot(mt, rho) = 32 warp + 16 mt + 8 rho + fg, heads ft + 4u;
   // these four tokens are K positions b = 2 mt + rho of word (kappa = warp, half = fg >> 2, t' = fg & 3)
   const int jp = BITS == 2 ? warp : (warp & 1);
@@ -382,7 +392,8 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   // column (h, d) of head h = ft + 4u: n-tile 2u + (d >> 1), g' = 2 ft + (d & 1); lane' = 4 g' + t'
   uint32_t* bp_dst[2];
 #pragma unroll
-  for (int dd = 0; dd < 2; ++dd) bp_dst[dd] = &sm.bp[0][warp >> 1][b_slot(4 * (2 * ft + dd) + (fg & 3), warp >> 1)][2 * (warp & 1) + (fg >> 2)];
+  for (int dd = 0; dd < 2; ++dd) bp_dst[dd] = &sm.bp[0][0][warp >> 1][b_slot(4 * (2 * ft + dd) + (fg & 3), warp >> 1)][2 * (warp & 1) + (fg >> 2)];
+  constexpr int B_CH = NT * 256;   // 32-bit words of one chunk's B operand
 
   float mr[HPW], lp[HPW], ac[HPW][4];
 #pragma unroll
@@ -392,112 +403,142 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     for (int i = 0; i < 4; ++i) ac[u][i] = 0.f;
   }
 
-  for (int it = 0; it < n_my; ++it) {
+  // One loop iteration = NCH chunks.  FULL (all NCH chunks present) is a compile-time flag so that the
+  // common case has no per-chunk branches and the chunks' instruction streams interleave.
+  auto iteration = [&](auto full_tag, const int it) {
+    constexpr bool FULL = decltype(full_tag)::value;
     const int st = it % STAGES;
     const uint32_t par = (it / STAGES) & 1;
-    const uint8_t* kr = sm.rec[st][0];
-    const uint8_t* vr = sm.rec[st][1];
+    const int nc = min(NCH, n_my - it * NCH);   // chunks of this iteration (uniform)
     mbar_wait(&sm.fullk[st], par);
 
     // ---- phase A: B_q (digits of the fixed-point qt), beta, per-token / per-channel aux -----------
-    {
-      // aux of the K record in builder order: s1[4 lane + b], z[4 lane + b]
-      const uint32_t s1w = *reinterpret_cast<const uint32_t*>(kr + s1_off(BITS) + 4 * lane);
-      const uint2 zw = *reinterpret_cast<const uint2*>(kr + z_off(BITS) + 8 * lane);
-      const float2 s01 = e4m3x2_to_f32x2((uint16_t)(s1w & 0xffff)), s23 = e4m3x2_to_f32x2((uint16_t)(s1w >> 16));
-      const float s1[4] = {s01.x, s01.y, s23.x, s23.y};
-      const float2 z01 = __half22float2(*reinterpret_cast<const __half2*>(&zw.x));
-      const float2 z23 = __half22float2(*reinterpret_cast<const __half2*>(&zw.y));
-      const float z[4] = {z01.x, z01.y, z23.x, z23.y};
-      float qt[HPW][4], amax[HPW], bsum[HPW];
 #pragma unroll
-      for (int u = 0; u < HPW; ++u) {
+    for (int c = 0; c < NCH; ++c) {
+      if (FULL || c < nc) {
+        const uint8_t* kr = sm.rec[st][c][0];
+        // aux of the K record in builder order: s1[4 lane + b], z[4 lane + b]
+        const uint32_t s1w = *reinterpret_cast<const uint32_t*>(kr + s1_off(BITS) + 4 * lane);
+        const uint2 zw = *reinterpret_cast<const uint2*>(kr + z_off(BITS) + 8 * lane);
+        const float2 s01 = e4m3x2_to_f32x2((uint16_t)(s1w & 0xffff)), s23 = e4m3x2_to_f32x2((uint16_t)(s1w >> 16));
+        const float s1[4] = {s01.x, s01.y, s23.x, s23.y};
+        const float2 z01 = __half22float2(*reinterpret_cast<const __half2*>(&zw.x));
+        const float2 z23 = __half22float2(*reinterpret_cast<const __half2*>(&zw.y));
+        const float z[4] = {z01.x, z01.y, z23.x, z23.y};
+        float qt[HPW][4], amax[HPW], bsum[HPW];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) qt[u][r] = qreg[u][r] * s1[r];
-        amax[u] = fmaxf(fmaxf(fabsf(qt[u][0]), fabsf(qt[u][1])), fmaxf(fabsf(qt[u][2]), fabsf(qt[u][3])));
-        // beta uses the unrounded qt: it differs from the 22-bit fixed-point value by < 2^-23 max|qt|
-        bsum[u] = fmaf(qt[u][0], z[0], fmaf(qt[u][1], z[1], fmaf(qt[u][2], z[2], qt[u][3] * z[3])));
-      }
+        for (int u = 0; u < HPW; ++u) {
 #pragma unroll
-      for (int u = 0; u < HPW; ++u)   // non-negative floats order like their bit patterns
-        amax[u] = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax[u])));
-#pragma unroll
-      for (int m = 16; m > 0; m >>= 1)
-#pragma unroll
-        for (int u = 0; u < HPW; ++u) bsum[u] += __shfl_xor_sync(0xffffffffu, bsum[u], m);
-#pragma unroll
-      for (int u = 0; u < HPW; ++u) {
-        const int h = warp + 4 * u;
-        const float inv = amax[u] > 1e-30f ? Q_FIX * rcp_approx(amax[u]) : 0.f;
-        uint32_t X[4], Y[4];
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-          const float f = fmaf(qt[u][r], inv, MAGIC_F);            // integer Q in the low mantissa bits
-          X[r] = (__float_as_uint(f) * mul_q + add_q) ^ 0x80808080u;   // balanced s8 digits of Q << shift
+          for (int r = 0; r < 4; ++r) qt[u][r] = qreg[u][r] * s1[r];
+          amax[u] = fmaxf(fmaxf(fabsf(qt[u][0]), fabsf(qt[u][1])), fmaxf(fabsf(qt[u][2]), fabsf(qt[u][3])));
+          // beta uses the unrounded qt: it differs from the 22-bit fixed-point value by < 2^-23 max|qt|
+          bsum[u] = fmaf(qt[u][0], z[0], fmaf(qt[u][1], z[1], fmaf(qt[u][2], z[2], qt[u][3] * z[3])));
         }
-        transpose4x4(X, Y);   // Y[d] = digit d of the four K positions = one B-fragment word of column (h, d)
 #pragma unroll
-        for (int d = 0; d < 4; ++d) bq_dst[d & 1][(2 * u + (d >> 1)) * 256] = Y[d];
-        if (lane == 0) {
-          const float sc = amax[u] * (1.f / Q_FIX);
-          sm.hs[h][0] = sc * CLS_INV;   // logit = s2 * (acc * scale + beta)
-          sm.hs[h][1] = bsum[u];
+        for (int u = 0; u < HPW; ++u)   // non-negative floats order like their bit patterns
+          amax[u] = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax[u])));
+#pragma unroll
+        for (int m = 16; m > 0; m >>= 1)
+#pragma unroll
+          for (int u = 0; u < HPW; ++u) bsum[u] += __shfl_xor_sync(0xffffffffu, bsum[u], m);
+#pragma unroll
+        for (int u = 0; u < HPW; ++u) {
+          const int h = warp + 4 * u;
+          const float inv = amax[u] > 1e-30f ? Q_FIX * rcp_approx(amax[u]) : 0.f;
+          uint32_t X[4], Y[4];
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            const float f = fmaf(qt[u][r], inv, MAGIC_F);            // integer Q in the low mantissa bits
+            X[r] = (__float_as_uint(f) * mul_q + add_q) ^ 0x80808080u;   // balanced s8 digits of Q << shift
+          }
+          transpose4x4(X, Y);   // Y[d] = digit d of the four K positions = one B-fragment word of column (h, d)
+#pragma unroll
+          for (int d = 0; d < 4; ++d) bq_dst[d & 1][c * B_CH + (2 * u + (d >> 1)) * 256] = Y[d];
+          if (lane == 0) {
+            const float sc = amax[u] * (1.f / Q_FIX);
+            sm.hs[c][h][0] = sc * CLS_INV;   // logit = s2 * (acc * scale + beta)
+            sm.hs[c][h][1] = bsum[u];
+          }
         }
       }
     }
     mbar_wait(&sm.fullv[st], par);
-    {
-      // thread tid: aux of MMA row slot tid of the K tile (token-indexed arrays are stored in slot order)
-      // and of channel tid of the V tile
-      const float s2t = e4m3_to_f32(kr[s2_off(BITS) + tid]);
-      const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + tid]), 9.094947e-13f);   // 2^-40: a zero scale stays harmless
-      const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[tid]);
-      // pt = p s1v = exp2(logit + log2 s1v - m): the running maximum is taken over the shifted logits,
-      // so pt <= 1 and its fixed-point scale is a constant
-      sm.aux_tok[tid] = make_float4(s2t, lg2_approx(s1v), rcp_approx(s1v), zv);
-      sm.aux_ch[it & 1][tid] = e4m3_to_f32(vr[s2_off(BITS) + tid]) * (1.f / P_FIX);
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+      if (FULL || c < nc) {
+        // thread tid: aux of MMA row slot tid of the K tile (token-indexed arrays are stored in slot order)
+        // and of channel tid of the V tile
+        const uint8_t* kr = sm.rec[st][c][0];
+        const uint8_t* vr = sm.rec[st][c][1];
+        const float s2t = e4m3_to_f32(kr[s2_off(BITS) + tid]);
+        const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + tid]), 9.094947e-13f);   // 2^-40: a zero scale stays harmless
+        const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[tid]);
+        // pt = p s1v = exp2(logit + log2 s1v - m): the running maximum is taken over the shifted logits,
+        // so pt <= 1 and its fixed-point scale is a constant
+        sm.aux_a[c][tid] = make_float2(s2t, lg2_approx(s1v));
+        sm.aux_b[c][tid] = make_float2(rcp_approx(s1v), zv);
+        sm.aux_ch[it & 1][c][tid] = e4m3_to_f32(vr[s2_off(BITS) + tid]) * (1.f / P_FIX);
+      }
     }
     __syncthreads();                                                   // barrier 1
-    // every warp is done with chunk it-1: refill its V slot (its K slot was refilled after barrier 2)
-    if (tid == 0 && it >= 1 && it - 1 + STAGES < n_my) {
-      const int s2 = (it - 1) % STAGES;
-      mbar_expect_tx(&sm.fullv[s2], RB);
-      bulk_g2s(sm.rec[s2][1], vrec + (size_t)(it - 1 + STAGES) * RB, RB, &sm.fullv[s2]);
+    // every warp is done with iteration it-1: refill its V slots (its K slots were refilled after barrier 2)
+    if (tid == 0 && it >= 1) {
+      const int nxt = it - 1 + STAGES, s2 = (it - 1) % STAGES;
+      const int nn = min(NCH, n_my - nxt * NCH);
+      if (nn > 0) {
+        mbar_expect_tx(&sm.fullv[s2], nn * RB);
+        for (int c = 0; c < nn; ++c) bulk_g2s(sm.rec[s2][c][1], vrec + (size_t)(nxt * NCH + c) * RB, RB, &sm.fullv[s2]);
+      }
     }
 
-    // ---- D3: logits of this thread's 4 tokens x HPW heads --------------------------------------------
-    float logit[HPW][4];
-    float4 aux[4];
-    {
-      int32_t dd[2][NT][4];
-      contract<BITS, NT, true>(kr, sm.bq, warp, lane, dd);
+    // ---- D3: logits of this thread's 4 tokens x HPW heads (per chunk) -----------------------------------
+    float logit[NCH][HPW][4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) aux[i] = sm.aux_tok[32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];
+    for (int c = 0; c < NCH; ++c) {
+      if (FULL || c < nc) {
+        int32_t dd[2][NT][4];
+        contract<BITS, NT, true>(sm.rec[st][c][0], sm.bq[c], warp, lane, dd);
+        float2 aux[4];
 #pragma unroll
-      for (int u = 0; u < HPW; ++u) {
-        const float2 sb = *reinterpret_cast<const float2*>(sm.hs[ft + 4 * u]);
+        for (int i = 0; i < 4; ++i) aux[i] = sm.aux_a[c][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {   // i = 2 mt + rho
-          const int mt = i >> 1, c = 2 * (i & 1);
-          const float a = undigit(dd[mt][2 * u][c], dd[mt][2 * u][c + 1], dd[mt][2 * u + 1][c], dd[mt][2 * u + 1][c + 1]);
-          logit[u][i] = fmaf(aux[i].x, fmaf(a, sb.x, sb.y), aux[i].y);
+        for (int u = 0; u < HPW; ++u) {
+          const float2 sb = *reinterpret_cast<const float2*>(sm.hs[c][ft + 4 * u]);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {   // i = 2 mt + rho
+            const int mt = i >> 1, cc = 2 * (i & 1);
+            const float a = undigit(dd[mt][2 * u][cc], dd[mt][2 * u][cc + 1], dd[mt][2 * u + 1][cc], dd[mt][2 * u + 1][cc + 1]);
+            logit[c][u][i] = fmaf(aux[i].x, fmaf(a, sb.x, sb.y), aux[i].y);
+          }
         }
+      } else {
+#pragma unroll
+        for (int u = 0; u < HPW; ++u)
+#pragma unroll
+          for (int i = 0; i < 4; ++i) logit[c][u][i] = -INFINITY;
       }
     }
     // ---- D4: online softmax -----------------------------------------------------------------------------
 #pragma unroll
     for (int u = 0; u < HPW; ++u) {
-      float mx = fmaxf(fmaxf(logit[u][0], logit[u][1]), fmaxf(logit[u][2], logit[u][3]));
+      float mx = -INFINITY;
+#pragma unroll
+      for (int c = 0; c < NCH; ++c)
+        mx = fmaxf(mx, fmaxf(fmaxf(logit[c][u][0], logit[c][u][1]), fmaxf(logit[c][u][2], logit[c][u][3])));
       mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
       mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 8));
       mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 16));
       if (fg == 0) sm.hmax[ft + 4 * u][warp] = mx;
     }
     __syncthreads();                                                   // barrier 2
-    // every warp is done with the K record of this chunk: prefetch chunk it + STAGES into its slot
-    if (tid == 0 && it + STAGES < n_my) {
-      mbar_expect_tx(&sm.fullk[st], RB);
-      bulk_g2s(sm.rec[st][0], krec + (size_t)(it + STAGES) * RB, RB, &sm.fullk[st]);
+    // every warp is done with the K records of this iteration: prefetch iteration it + STAGES into their slots
+    if (tid == 0) {
+      const int nxt = it + STAGES;
+      const int nn = min(NCH, n_my - nxt * NCH);
+      if (nn > 0) {
+        mbar_expect_tx(&sm.fullk[st], nn * RB);
+        for (int c = 0; c < nn; ++c) bulk_g2s(sm.rec[st][c][0], krec + (size_t)(nxt * NCH + c) * RB, RB, &sm.fullk[st]);
+      }
     }
     float corr[HPW];
 #pragma unroll
@@ -506,47 +547,66 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
       const float m_new = fmaxf(mr[u], fmaxf(fmaxf(hm.x, hm.y), fmaxf(hm.z, hm.w)));
       corr[u] = ex2_approx(mr[u] - m_new);
       mr[u] = m_new;
-      uint32_t X[4], Y[4];
-      float lsum = 0.f, zpart = 0.f;
+      float lsum = 0.f;
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const float pt = ex2_approx(logit[u][i] - m_new);
-        lsum = fmaf(pt, aux[i].z, lsum);
-        // D5 prep: fixed-point pt; its radix-256 digits are the bytes of X
-        const float f = fmaf(pt, P_FIX, MAGIC_F);
-        zpart = fmaf(f - MAGIC_F, aux[i].w, zpart);
-        X[i] = __float_as_uint(f) * mul_p + add_p;
+      for (int c = 0; c < NCH; ++c) {
+        if (FULL || c < nc) {
+          uint32_t X[4], Y[4];
+          float zpart = 0.f;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const float2 ab = sm.aux_b[c][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];   // {1 / s1v, zv}
+            const float pt = ex2_approx(logit[c][u][i] - m_new);
+            lsum = fmaf(pt, ab.x, lsum);
+            // D5 prep: fixed-point pt; its radix-256 digits are the bytes of X
+            const float f = fmaf(pt, P_FIX, MAGIC_F);
+            zpart = fmaf(f - MAGIC_F, ab.y, zpart);
+            X[i] = __float_as_uint(f) * mul_p + add_p;
+          }
+          transpose4x4(X, Y);
+#pragma unroll
+          for (int d = 0; d < 4; ++d) bp_dst[d & 1][c * B_CH + (2 * u + (d >> 1)) * 256] = Y[d];
+          zpart += __shfl_xor_sync(0xffffffffu, zpart, 4);
+          zpart += __shfl_xor_sync(0xffffffffu, zpart, 8);
+          zpart += __shfl_xor_sync(0xffffffffu, zpart, 16);
+          if (fg == 0) sm.hz[c][ft + 4 * u][warp] = zpart;
+        }
       }
       lp[u] = fmaf(lp[u], corr[u], lsum);
-      transpose4x4(X, Y);
-#pragma unroll
-      for (int d = 0; d < 4; ++d) bp_dst[d & 1][(2 * u + (d >> 1)) * 256] = Y[d];
-      zpart += __shfl_xor_sync(0xffffffffu, zpart, 4);
-      zpart += __shfl_xor_sync(0xffffffffu, zpart, 8);
-      zpart += __shfl_xor_sync(0xffffffffu, zpart, 16);
-      if (fg == 0) sm.hz[ft + 4 * u][warp] = zpart;
     }
     __syncthreads();                                                   // barrier 3
 
     // ---- D5: this thread's 4 channels x HPW heads of the value contraction ---------------------------
-    {
-      int32_t dd[2][NT][4];
-      contract<BITS, NT, false>(vr, sm.bp, warp, lane, dd);
-      float s2v[4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) s2v[i] = sm.aux_ch[it & 1][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];
+    for (int u = 0; u < HPW; ++u)
 #pragma unroll
-      for (int u = 0; u < HPW; ++u) {
-        const float4 hz = *reinterpret_cast<const float4*>(sm.hz[ft + 4 * u]);
-        const float zsum = (hz.x + hz.y) + (hz.z + hz.w);
+      for (int i = 0; i < 4; ++i) ac[u][i] *= corr[u];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const int mt = i >> 1, c = 2 * (i & 1);
-          const float a = undigit(dd[mt][2 * u][c], dd[mt][2 * u][c + 1], dd[mt][2 * u + 1][c], dd[mt][2 * u + 1][c + 1]);
-          ac[u][i] = fmaf(ac[u][i], corr[u], s2v[i] * fmaf(a, CLS_INV, zsum));
+    for (int c = 0; c < NCH; ++c) {
+      if (FULL || c < nc) {
+        int32_t dd[2][NT][4];
+        contract<BITS, NT, false>(sm.rec[st][c][1], sm.bp[c], warp, lane, dd);
+        float s2v[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) s2v[i] = sm.aux_ch[it & 1][c][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];
+#pragma unroll
+        for (int u = 0; u < HPW; ++u) {
+          const float4 hz = *reinterpret_cast<const float4*>(sm.hz[c][ft + 4 * u]);
+          const float zsum = (hz.x + hz.y) + (hz.z + hz.w);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int mt = i >> 1, cc = 2 * (i & 1);
+            const float a = undigit(dd[mt][2 * u][cc], dd[mt][2 * u][cc + 1], dd[mt][2 * u + 1][cc], dd[mt][2 * u + 1][cc + 1]);
+            ac[u][i] = fmaf(s2v[i], fmaf(a, CLS_INV, zsum), ac[u][i]);
+          }
         }
       }
     }
+  };
+  const int n_it = (n_my + NCH - 1) / NCH;
+  for (int it = 0; it < n_it; ++it) {
+    if (NCH == 1 || n_my - it * NCH >= NCH) iteration(std::true_type{}, it);
+    else iteration(std::false_type{}, it);
   }
 
   // ---- hand over to the per-channel layout of the residual window / merge: thread tid = channel tid ----
@@ -557,7 +617,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     l += __shfl_xor_sync(0xffffffffu, l, 4);
     l += __shfl_xor_sync(0xffffffffu, l, 8);
     l += __shfl_xor_sync(0xffffffffu, l, 16);
-    if (fg == 0) { sm.hz[ft + 4 * u][warp] = l; if (warp == 0) sm.hs[ft + 4 * u][0] = mr[u]; }
+    if (fg == 0) { sm.hz[0][ft + 4 * u][warp] = l; if (warp == 0) sm.hs[0][ft + 4 * u][0] = mr[u]; }
 #pragma unroll
     for (int i = 0; i < 4; ++i) sm.qrot[ft + 4 * u][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg] = ac[u][i];
   }
@@ -565,8 +625,8 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   float m_run[GP], l_part[GP], acc[GP];
 #pragma unroll
   for (int h = 0; h < GP; ++h) {
-    m_run[h] = sm.hs[h][0];
-    const float4 hz = *reinterpret_cast<const float4*>(sm.hz[h]);
+    m_run[h] = sm.hs[0][h][0];
+    const float4 hz = *reinterpret_cast<const float4*>(sm.hz[0][h]);
     l_part[h] = tid == 0 ? (hz.x + hz.y) + (hz.z + hz.w) : 0.f;   // thread 0 carries the sum over the chunks
     acc[h] = sm.qrot[h][tid];
   }
@@ -738,7 +798,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
       wsp[h * 64 + lane] = w0;
       wsp[h * 64 + lane + 32] = w1;
       const float L = warp_sum(fmaf(w0, l0, w1 * l1));
-      if (lane == 0) sm.hs[h][1] = L;
+      if (lane == 0) sm.hs[0][h][1] = L;
     }
     __syncthreads();
 #pragma unroll
@@ -759,7 +819,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
           rot = fmaf(w, __ldcg(base + (size_t)s * WS_STRIDE), rot);
           res = fmaf(w, __ldcg(base + (size_t)s * WS_STRIDE + 128), res);
         }
-        L = sm.hs[h][1];
+        L = sm.hs[0][h][1];
       }
       l_tot[h] = L; acc[h] = rot; acc_res[h] = res;
     }
@@ -773,7 +833,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   for (int j = 0; j < GP; ++j) {
     merged_rot[j * 128 + tid] = acc[j];
     sm.qraw[j][tid] = (l_tot[j] > 0.f) ? acc_res[j] : 0.f;
-    if (tid == 0) sm.hs[j][0] = (l_tot[j] > 0.f) ? 1.f / l_tot[j] : 0.f;
+    if (tid == 0) sm.hs[0][j][0] = (l_tot[j] > 0.f) ? 1.f / l_tot[j] : 0.f;
   }
   __syncthreads();
   for (int jj = warp; jj < GP; jj += 4) {
@@ -787,7 +847,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
       for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
     }
     const float4 s4 = *reinterpret_cast<const float4*>(&sm.qraw[jj][4 * lane]);
-    const float inv = sm.hs[jj][0];
+    const float inv = sm.hs[0][jj][0];
     const float o0 = (v[0] + s4.x) * inv, o1 = (v[1] + s4.y) * inv, o2 = (v[2] + s4.z) * inv, o3 = (v[3] + s4.w) * inv;
     const size_t off = ((size_t)b * A.Hq + hkv * g + hh) * D + 4 * lane;
     if (A.out_dtype == KVARN_F32) {
