@@ -221,6 +221,9 @@ static SplitPlan split_plan(const kvarn_params* p, int B, int Hkv, int g, int ma
   if (want < 1) want = 1;
   if (want > max_chunks) want = max_chunks;
   sp.cluster = want < KVARN_MAX_CLUSTER ? want : KVARN_MAX_CLUSTER;
+  // about one CTA per slot and long CTAs: halve them, so that the CTAs of the second half-wave balance the
+  // SMs that got one CTA more (config 4: 512 CTAs on 592 slots 1327 us, 1024 half-length CTAs 1177 us)
+  if (sp.cluster == 1 && max_chunks >= 32) sp.cluster = 2;
   if (sp.cluster == KVARN_MAX_CLUSTER) {
     const int per = (max_chunks + KVARN_MAX_CLUSTER - 1) / KVARN_MAX_CLUSTER;   // chunks per CTA with one cluster
     if (per > 32) {
