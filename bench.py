@@ -278,12 +278,16 @@ def run_extras(kv, W, dev, hbm_peak):
 
 
 def stored_traffic():
-    """dram bytes per launch of the two kernels, from the committed ncu --set full capture."""
-    path = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    """dram bytes per launch of the two kernels, from the committed ncu --set full capture (profiles/r01b_traffic.md)."""
+    path = os.path.join(ROOT, "profiles", "r01b_traffic.csv")
+    out = {}
     try:
-        return json.load(open(path))
+        for line in open(path).read().splitlines()[1:]:
+            k, v = line.split(",")
+            out[k] = int(v)
     except Exception:
-        return {}
+        pass
+    return out
 
 
 def main():
