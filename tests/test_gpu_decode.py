@@ -282,3 +282,20 @@ def test_config4_shape_sampled_units(kv, bits):
     out = kv.decode_attention(p, cache, q)
     assert torch.isfinite(out).all()
     _check_all_units(kv, p, cache, q, out, s.ctx, units={(0, 0), (37, 5), (63, 7)})
+
+
+@pytest.mark.parametrize("bits,Hq,n_tok,splits", [(2, 32, 128 * 40 + 5, 0), (2, 64, 128 * 33, 6), (4, 32, 128 * 9 + 127, 0),
+                                                   (2, 8, 128 * 50, 24)])
+def test_decode_is_deterministic_over_repeats(kv, bits, Hq, n_tok, splits):
+    # compute-sanitizer is closed on this pool, so shared-memory / DSMEM hazards are hunted by repetition:
+    # the kernel has no float atomics, hence any bit that changes between identical launches is a race
+    K, V = W.kv_tokens(4, 8, n_tok, seed=71, device="cuda")
+    q = W.queries(4, Hq, seed=71, device="cuda")
+    p = kv.default_params(bits, splits=splits)
+    cache = _build_cache(kv, p, K, V)
+    ref = kv.decode_attention(p, cache, q).clone()
+    out = torch.empty_like(ref)
+    for _ in range(200):
+        kv.decode_attention(p, cache, q, out=out)
+        assert torch.equal(out, ref)
+    _check_all_units(kv, p, cache, q, ref, n_tok, units={(0, 0), (3, 7)})

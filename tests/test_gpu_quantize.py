@@ -143,3 +143,15 @@ def test_zero_tiles_is_a_noop(kv):
     E = torch.empty((0, 128, 128), device="cuda", dtype=torch.bfloat16)
     k_rec, v_rec = kv.quantize_chunk(p, E, E.clone())
     assert k_rec.shape == (0, 4608)
+
+
+def test_quantize_is_deterministic_over_repeats(kv):
+    # same reasoning as the decode repeat test: identical launches must give identical bytes
+    K, V = W.quantizer_sweep_tiles(8, 128 * 64, seed=5, device="cuda")
+    Kt, Vt = K.reshape(-1, 128, 128), V.reshape(-1, 128, 128)
+    for bits in (2, 4):
+        p = kv.default_params(bits)
+        k0, v0 = kv.quantize_chunk(p, Kt, Vt)
+        for _ in range(20):
+            k1, v1 = kv.quantize_chunk(p, Kt, Vt)
+            assert torch.equal(k0, k1) and torch.equal(v0, v1)
