@@ -225,6 +225,26 @@ def run_extras(kv, W, dev, hbm_peak):
                                        "bytes": byts, "B": sh.B, "Hq": sh.Hq, "Hkv": sh.Hkv, "ctx": sh.ctx}
             del cache, q, ws, out
             torch.cuda.empty_cache()
+    # the paper's three-region layout: S = 128 raw sink tokens in front of the quantised body
+    sh = W.DecodeShape("long_context_g4_sink128", B=16, Hq=32, Hkv=8, ctx=128 + 65536 + 64, seed=6)
+    p = kv.default_params(2)
+    cache = kv.Cache(p, sh.B, sh.Hkv, 512, device=dev, n_sink=128)
+    for b0 in range(0, sh.B, 4):
+        K, V = W.kv_tokens(4, sh.Hkv, sh.ctx, seed=sh.seed + b0, device=dev)
+        kv.prefill(p, cache.slice(b0, b0 + 4), K, V)
+        del K, V
+    q = W.queries(sh.B, sh.Hq, seed=sh.seed, device=dev)
+    ws = torch.empty((max(kv.decode_workspace_bytes(p, sh.B, sh.Hq, sh.Hkv, 512), 16),), dtype=torch.uint8, device=dev)
+    out = torch.empty((sh.B, sh.Hq, D), dtype=torch.float32, device=dev)
+    for _ in range(3):
+        kv.decode_attention(p, cache, q, out=out, ws=ws)
+    torch.cuda.synchronize()
+    med, mn = _time_launches(lambda i: kv.decode_attention(p, cache, q, out=out, ws=ws), 10, stream)
+    byts = cache.nbytes_read_by_decode(sh.ctx) + sh.B * sh.Hq * (D * 2 + D * 4)
+    ex["decode_long_g4_2bit_sink128"] = {"us": med * 1e3, "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak,
+                                         "bytes": byts, "B": sh.B, "Hq": sh.Hq, "Hkv": sh.Hkv, "ctx": sh.ctx, "n_sink": 128}
+    del cache, q, ws, out
+    torch.cuda.empty_cache()
     # configs[2] (Qwen3-4B-shaped incremental decode, B=16): the last 256 steps of the growth to 32768 tokens,
     # one kvarn_append + one kvarn_decode_attention per step (two chunk boundaries inside); 302 MB of records
     s2 = W.CONFIG2

@@ -109,8 +109,11 @@ typedef struct {
   size_t s1_off, s2_off, z_off; /* 128 x u8, 128 x u8, 128 x f16 */
 } kvarn_layout_info;
 
-/* The cache of one attention layer (quantised body of 128-token groups
- * followed by the trailing not-yet-quantised tokens).  All DEVICE pointers. */
+/* The cache of one attention layer in the paper's three-region layout: n_sink sink tokens
+ * kept in in_dtype ("S sink tokens in FP16", S = 128 or 32 in the paper; 0 = no sink region), the
+ * quantised body of 128-token groups, and the trailing not-yet-quantised tokens.  For a sequence of
+ * len tokens:  sink = min(len, n_sink),  chunks = max(len - n_sink, 0) / 128,
+ * residual = max(len - n_sink, 0) % 128.  All DEVICE pointers. */
 typedef struct {
   void* k_records;      /* [B][Hkv][max_chunks][record_bytes], 16-B aligned */
   void* v_records;      /* same shape */
@@ -122,7 +125,9 @@ typedef struct {
                            * merge), zero-initialised by the caller once; every call leaves it zero.
                            * Calls that share it must be ordered on one stream. */
   int32_t B, Hkv, max_chunks;
-  int32_t reserved;
+  int32_t n_sink;       /* S: tokens [0, S) of every sequence stay raw in k_sink / v_sink; 0..128 */
+  void* k_sink;         /* [B][Hkv][n_sink][128] in_dtype (may be NULL when n_sink = 0) */
+  void* v_sink;         /* same shape */
 } kvarn_cache;
 
 /* Optional per-tile debug outputs of the quantizer (all DEVICE, each nullable).
@@ -164,10 +169,11 @@ KVARN_API int kvarn_quantize_chunk(const kvarn_params* p, const void* k, const v
                          int64_t rec_stride, const kvarn_debug* dbg, void* stream);
 
 /*
- * kvarn_prefill -- bulk-load a cache: quantise the first floor(n_tok/128)
- * chunks of every (sequence, KV head) of k, v = [B][Hkv][n_tok][128] into the
- * cache's records, copy the remaining n_tok%128 tokens into the residual window
- * and set seq_lens[b] = n_tok.  Same kernel as kvarn_quantize_chunk.
+ * kvarn_prefill -- bulk-load a cache from k, v = [B][Hkv][n_tok][128]: copy the
+ * first min(n_tok, n_sink) tokens of every (sequence, KV head) into the sink
+ * region, quantise the following floor((n_tok - n_sink)/128) chunks into the
+ * cache's records, copy the remaining tokens into the residual window and set
+ * seq_lens[b] = n_tok.  Same kernel as kvarn_quantize_chunk.
  */
 KVARN_API int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, const void* k, const void* v,
                   int32_t n_tok, void* stream);
@@ -175,11 +181,12 @@ KVARN_API int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, con
 /*
  * kvarn_append -- on-the-fly compression during decoding (P:17, P:53, P:83,
  * P:350): append ONE new token per sequence.  k_new, v_new = [B][Hkv][128]
- * in_dtype (DEVICE).  The token goes to residual slot len%128; a residual that
- * thereby reaches 128 tokens is quantised at once into chunk slot len/128 (bit
+ * in_dtype (DEVICE).  While len < n_sink the token goes to sink slot len; afterwards
+ * (with l = len - n_sink) it goes to residual slot l%128; a residual that
+ * thereby reaches 128 tokens is quantised at once into chunk slot l/128 (bit
  * for bit what kvarn_quantize_chunk gives on those 128 tokens) and the residual
  * becomes empty.  seq_lens[b] is read and advanced ON DEVICE (no host round
- * trip).  A sequence already holding max_chunks*128 + 127 tokens is left
+ * trip).  A sequence already holding n_sink + max_chunks*128 + 127 tokens is left
  * unchanged (its token is dropped); the caller bounds lengths on the host.
  */
 KVARN_API int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_new,
@@ -189,7 +196,7 @@ KVARN_API int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, cons
  * kvarn_decode_attention -- out[b][h] = softmax(q[b][h] K^T * sm_scale) V over
  * all seq_lens[b] tokens of KV head h / (Hq/Hkv): the quantised chunks, read as
  * packed codes + scales + zero-points (Eq. 1 with the second scale fused,
- * P:45), then the raw residual window.  The Hadamard
+ * P:45), the raw sink tokens and the raw residual window.  The Hadamard
  * rotation and the per-channel scales are folded into q and the output.
  *   q    DEVICE [B][Hq][128] in_dtype          out  DEVICE [B][Hq][128] out_dtype
  *   ws   DEVICE scratch of >= kvarn_decode_workspace_bytes(...) bytes, 16-B aligned

@@ -29,6 +29,7 @@ imbalance ................ pinned to its stated formula only -- the body of
 rtn_quantize / dequant ... pinned (on-grid round trip, textbook min-max RTN)
 fp8 / fp16 rounding ...... pinned (torch.float8_e4m3fn, numpy.float16 casts)
 attention ................ pinned (brute-force loops, torch SDPA, invariances)
+cache_partition .......... pinned (brute-force token walk, P:350's S/G/R settings)
 codes / scales of a tile vs values printed by the paper ... **parity unpinned**:
                            the paper prints no intermediate value for any tile.
 """
@@ -364,6 +365,36 @@ def decode_attention(q: np.ndarray, k_tiles: list, v_tiles: list,
     Ks.append(np.asarray(k_resid, dtype=np.float64).reshape(-1, d))
     Vs.append(np.asarray(v_resid, dtype=np.float64).reshape(-1, d))
     return attention(q, np.concatenate(Ks, axis=0), np.concatenate(Vs, axis=0), sm_scale)
+
+
+# --------------------------------------------------------------------------
+# Three-region cache layout (App. D "Quantization")
+# --------------------------------------------------------------------------
+def cache_partition(n_tok: int, n_sink: int = 0, group: int = 128):
+    """(sink, chunks, residual) of a sequence of ``n_tok`` tokens: "S sink tokens in
+    FP16 ..., a 2-bit quantized body composed of groups of G tokens each, and R trailing tokens
+    in FP16 ... which have not yet accumulated enough context to form a full quantization group".
+    The first min(n_tok, S) tokens are the sink, every complete group of G after them is
+    quantised, the rest trail in FP16 (reading R11: quantised the moment a group is complete)."""
+    sink = min(n_tok, n_sink)
+    body = n_tok - sink
+    return sink, body // group, body % group
+
+
+def cache_attention(q: np.ndarray, K: np.ndarray, V: np.ndarray, n_sink: int = 0, bits: int = 2,
+                    sm_scale: float | None = None) -> np.ndarray:
+    """End-to-end definition for one KV head: partition the (n_tok, d) raw K, V by
+    ``cache_partition``, quantise the body chunk by chunk (steps 1-4), and attend over
+    [raw sink ; dequantised body ; raw residual] (steps 5-6)."""
+    K = np.asarray(K, dtype=np.float64); V = np.asarray(V, dtype=np.float64)
+    ns, nc, r = cache_partition(K.shape[0], n_sink)
+    kt, vt = [], []
+    for c in range(nc):
+        sl = slice(ns + 128 * c, ns + 128 * (c + 1))
+        tk, tv = quantize_tile(K[sl], "k", bits=bits), quantize_tile(V[sl], "v", bits=bits)
+        kt.append((tk.codes, tk.s1, tk.s2, tk.z)); vt.append((tv.codes, tv.s1, tv.s2, tv.z))
+    raw = np.r_[0:ns, ns + 128 * nc:K.shape[0]]
+    return decode_attention(q, kt, vt, K[raw], V[raw], sm_scale=sm_scale)
 
 
 # --------------------------------------------------------------------------

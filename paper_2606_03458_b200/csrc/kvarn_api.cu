@@ -14,6 +14,7 @@ struct QuantArgs {
   const void* in[2];
   uint8_t* rec[2];
   long long n_inner;
+  long long in_base;                                       // elements: first tile starts here (after the sink tokens)
   long long in_outer_stride, in_tile_stride, tok_stride;  // elements
   long long rec_outer_stride, rec_stride;                 // bytes
   long long n_tiles;
@@ -32,7 +33,7 @@ __global__ void __launch_bounds__(256, 2) quantize_kernel(const QuantArgs A) {
   const int kind = A.kind_base + blockIdx.y;
   const long long tile = blockIdx.x;
   const long long outer = tile / A.n_inner, inner = tile - outer * A.n_inner;
-  const InT* src = reinterpret_cast<const InT*>(A.in[kind]) + outer * A.in_outer_stride +
+  const InT* src = reinterpret_cast<const InT*>(A.in[kind]) + A.in_base + outer * A.in_outer_stride +
                    inner * A.in_tile_stride;
   uint8_t* dst = A.rec[kind] + outer * A.rec_outer_stride + inner * A.rec_stride;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -51,9 +52,10 @@ struct AppendArgs {
   uint8_t* rec[2];
   void* resid[2];
   const void* tok[2];
+  void* sink[2];
   int32_t* seq_lens;
   int32_t* ticket;
-  int B, Hkv, max_chunks;
+  int B, Hkv, max_chunks, n_sink;
   int rotate[2];
   VarnConsts vc;
 };
@@ -67,12 +69,17 @@ __global__ void __launch_bounds__(256, 2) append_kernel(const AppendArgs A) {
   const int kind = blockIdx.y, bh = blockIdx.x, b = bh / A.Hkv;
   const int tid = threadIdx.x;
   const int len = A.seq_lens[b];
-  const int r = len & 127, chunk = len >> 7;
-  const bool full = (r == 127);
-  const bool can_store = full ? (chunk < A.max_chunks) : (chunk <= A.max_chunks);
+  const bool to_sink = len < A.n_sink;                 // the three-region layout of P:350: sink | body | residual
+  const int l = to_sink ? 0 : len - A.n_sink;
+  const int r = l & 127, chunk = l >> 7;
+  const bool full = !to_sink && (r == 127);
+  const bool can_store = to_sink || (full ? (chunk < A.max_chunks) : (chunk <= A.max_chunks));
   InT* resid = reinterpret_cast<InT*>(A.resid[kind]) + (size_t)bh * G * D;
   const InT* tok = reinterpret_cast<const InT*>(A.tok[kind]) + (size_t)bh * D;
-  if (can_store && !full) {
+  if (to_sink) {
+    InT* sink = reinterpret_cast<InT*>(A.sink[kind]) + (size_t)bh * A.n_sink * D;
+    if (tid < D) sink[(size_t)len * D + tid] = tok[tid];
+  } else if (can_store && !full) {
     if (tid < D) resid[(size_t)r * D + tid] = tok[tid];
   } else if (can_store) {
     const int lane = tid & 31, warp = tid >> 5;
@@ -102,14 +109,22 @@ __global__ void __launch_bounds__(256, 2) append_kernel(const AppendArgs A) {
 struct TailArgs {
   const void* in[2];
   void* resid[2];
+  void* sink[2];
   int32_t* seq_lens;
-  int B, Hkv, n_tok, n_full;
+  int B, Hkv, n_tok, n_full, n_sink;
 };
+// raw regions of a bulk load: the first min(n_tok, n_sink) tokens -> sink, the tokens after the full chunks -> residual
 template <typename InT>
 __global__ void prefill_tail_kernel(const TailArgs A) {
   const int bh = blockIdx.x, kind = blockIdx.y;
-  const int r = A.n_tok - A.n_full * G;
-  const InT* src = reinterpret_cast<const InT*>(A.in[kind]) + ((size_t)bh * A.n_tok + (size_t)A.n_full * G) * D;
+  const int ns = min(A.n_tok, A.n_sink);
+  const int r = A.n_tok - ns - A.n_full * G;
+  const InT* base = reinterpret_cast<const InT*>(A.in[kind]) + (size_t)bh * A.n_tok * D;
+  if (ns > 0) {
+    InT* sdst = reinterpret_cast<InT*>(A.sink[kind]) + (size_t)bh * A.n_sink * D;
+    for (int i = threadIdx.x; i < ns * D; i += blockDim.x) sdst[i] = base[i];
+  }
+  const InT* src = base + ((size_t)ns + (size_t)A.n_full * G) * D;
   InT* dst = reinterpret_cast<InT*>(A.resid[kind]) + (size_t)bh * G * D;
   for (int i = threadIdx.x; i < r * D; i += blockDim.x) dst[i] = src[i];
   if (kind == 0 && threadIdx.x == 0 && (bh % A.Hkv) == 0) A.seq_lens[bh / A.Hkv] = A.n_tok;
@@ -294,7 +309,7 @@ const char* kvarn_status_string(int status) {
   }
 }
 
-int kvarn_version(void) { return 1; }
+int kvarn_version(void) { return 2; }
 
 int kvarn_layout(const kvarn_params* p, kvarn_layout_info* out) {
   if (!p || !out) return KVARN_INVALID_ARG;
@@ -341,6 +356,9 @@ int kvarn_quantize_chunk(const kvarn_params* p, const void* k, const void* v, in
 static int check_cache(const kvarn_cache* c) {
   if (!c || !c->k_records || !c->v_records || !c->k_resid || !c->v_resid || !c->seq_lens) return KVARN_INVALID_ARG;
   if (c->B <= 0 || c->Hkv <= 0 || c->max_chunks < 0) return KVARN_INVALID_ARG;
+  if (c->n_sink < 0 || c->n_sink > G) return KVARN_UNSUPPORTED;
+  if (c->n_sink > 0 && (!c->k_sink || !c->v_sink)) return KVARN_INVALID_ARG;
+  if (c->n_sink > 0 && (!aligned16(c->k_sink) || !aligned16(c->v_sink))) return KVARN_MISALIGNED;
   if (!aligned16(c->k_records) || !aligned16(c->v_records) || !aligned16(c->k_resid) || !aligned16(c->v_resid))
     return KVARN_MISALIGNED;
   return KVARN_OK;
@@ -353,7 +371,8 @@ int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, const void* k
   if ((st = check_cache(cache))) return st;
   if (n_tok < 0 || ((!k || !v) && n_tok > 0)) return KVARN_INVALID_ARG;
   if (!aligned16(k) || !aligned16(v)) return KVARN_MISALIGNED;
-  const int n_full = n_tok / G;
+  const int ns = n_tok < cache->n_sink ? n_tok : cache->n_sink;
+  const int n_full = (n_tok - ns) / G;
   if (n_full > cache->max_chunks) return KVARN_CAPACITY;
   const long long BH = (long long)cache->B * cache->Hkv;
   if (BH * n_full > 0x7fffffffLL) return KVARN_CAPACITY;
@@ -361,6 +380,7 @@ int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, const void* k
   QuantArgs A{};
   A.in[0] = k; A.in[1] = v; A.rec[0] = (uint8_t*)cache->k_records; A.rec[1] = (uint8_t*)cache->v_records;
   A.n_inner = n_full > 0 ? n_full : 1;
+  A.in_base = (long long)ns * D;
   A.in_outer_stride = (long long)n_tok * D; A.in_tile_stride = (long long)G * D; A.tok_stride = D;
   A.rec_outer_stride = (long long)cache->max_chunks * record_bytes(p->bits);
   A.rec_stride = record_bytes(p->bits);
@@ -369,6 +389,7 @@ int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, const void* k
   if ((st = launch_quantize(p, A, 2, s))) return st;
   TailArgs T{};
   T.in[0] = k; T.in[1] = v; T.resid[0] = cache->k_resid; T.resid[1] = cache->v_resid;
+  T.sink[0] = cache->k_sink; T.sink[1] = cache->v_sink; T.n_sink = cache->n_sink;
   T.seq_lens = cache->seq_lens; T.B = cache->B; T.Hkv = cache->Hkv; T.n_tok = n_tok; T.n_full = n_full;
   dim3 grid((unsigned)BH, 2);
   if (p->in_dtype == KVARN_F32) prefill_tail_kernel<float><<<grid, 256, 0, s>>>(T);
@@ -388,6 +409,7 @@ int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_
   A.resid[0] = cache->k_resid; A.resid[1] = cache->v_resid;
   A.tok[0] = k_new; A.tok[1] = v_new;
   A.seq_lens = cache->seq_lens; A.ticket = cache->ticket;
+  A.sink[0] = cache->k_sink; A.sink[1] = cache->v_sink; A.n_sink = cache->n_sink;
   A.B = cache->B; A.Hkv = cache->Hkv; A.max_chunks = cache->max_chunks;
   A.rotate[0] = p->rotate_k; A.rotate[1] = p->rotate_v; A.vc = varn_consts(p);
   dim3 grid((unsigned)(cache->B * cache->Hkv), 2);
@@ -418,6 +440,7 @@ int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, cons
   DecodeArgs A{};
   A.k_records = (const uint8_t*)cache->k_records; A.v_records = (const uint8_t*)cache->v_records;
   A.k_resid = cache->k_resid; A.v_resid = cache->v_resid; A.seq_lens = cache->seq_lens;
+  A.k_sink = cache->k_sink; A.v_sink = cache->v_sink; A.n_sink = cache->n_sink;
   A.ticket = cache->decode_ticket;
   A.q = q; A.out = out; A.ws = (float*)ws;
   A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;

@@ -54,6 +54,9 @@ struct DecodeArgs {
   const uint8_t* v_records;
   const void* k_resid;
   const void* v_resid;
+  const void* k_sink;   // [B][Hkv][n_sink][128] raw sink tokens, or null
+  const void* v_sink;
+  int n_sink;
   const int32_t* seq_lens;
   int32_t* ticket;  // [B*Hkv], zero between calls (self-resetting)
   const void* q;
@@ -317,13 +320,21 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
 
   // ---- chunk range of this split ----------------------------------------------------
   const int len = A.seq_lens[b];
-  int n_chunks = len >> 7;
+  const int n_sink_tok = min(len, A.n_sink);      // three-region layout: sink | quantised body | residual
+  const int body = len - n_sink_tok;
+  int n_chunks = body >> 7;
   if (n_chunks > A.max_chunks) n_chunks = A.max_chunks;
-  const int resid = len & 127;
-  const int per = (n_chunks + A.splits - 1) / A.splits;
-  const int c_begin = min(n_chunks, split * per), c_end = min(n_chunks, c_begin + per);
+  const int resid = body & 127;
+  // Balanced split: a raw window (512 B per token against 72 B) weighs like one chunk per 12 tokens (measured:
+  // 127 residual tokens cost a CTA about 10 chunks), so the splits that own the sink / residual window get
+  // correspondingly fewer chunks.  Virtual units: [sink | chunk 0 .. n_chunks-1 | residual].
+  const int w_sink = (n_sink_tok + 11) / 12, w_res = (resid + 11) / 12;
+  const int per = (n_chunks + w_sink + w_res + A.splits - 1) / A.splits;
+  const int c_begin = min(max(split * per - w_sink, 0), n_chunks);
+  const int c_end = min(max((split + 1) * per - w_sink, 0), n_chunks);
   const int n_my = c_end - c_begin;
   const bool do_resid = (split == A.splits - 1) && resid > 0;
+  const bool do_sink = (split == 0) && n_sink_tok > 0;
 
   const uint8_t* krec = A.k_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
   const uint8_t* vrec = A.v_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
@@ -631,29 +642,35 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
     acc[h] = sm.qrot[h][tid];
   }
 
-  // ---- D6: residual window (raw tokens, un-rotated space) -------------------------------------
+  // ---- D6: raw windows (sink tokens of split 0, residual window of the last split; un-rotated space) ----
   float acc_res[GP];
 #pragma unroll
   for (int h = 0; h < GP; ++h) acc_res[h] = 0.f;
-  if (do_resid) {
-    const InT* kres = reinterpret_cast<const InT*>(A.k_resid) + (size_t)bh * G * D;
-    const InT* vres = reinterpret_cast<const InT*>(A.v_resid) + (size_t)bh * G * D;
+  float* psm = &sm.qrot[0][0];   // [GP][128] probabilities of the window (q' and the staged acc are dead by now)
+  auto raw_window = [&](const InT* kraw, const InT* vraw, const int cnt) {   // cnt <= 128 tokens, thread = token
     float logit[GP];
 #pragma unroll
     for (int h = 0; h < GP; ++h) logit[h] = 0.f;
-    if (tid < resid) {
-      const InT* row = kres + (size_t)tid * D;
-      for (int c = 0; c < D; c += 8) {
-        float kv[8];
-        ld_in8(row + c, kv);
+    if (tid < cnt) {
+      const InT* row = kraw + (size_t)tid * D;
+      constexpr int CB = 64;   // channels per batch: all loads of a batch are in flight together
+#pragma unroll 1
+      for (int c0 = 0; c0 < D; c0 += CB) {
+        float kv[CB / 8][8];
 #pragma unroll
-        for (int h = 0; h < GP; ++h) {
-          const float4 q0 = *reinterpret_cast<const float4*>(&sm.qraw[h][c]);
-          const float4 q1 = *reinterpret_cast<const float4*>(&sm.qraw[h][c + 4]);
-          float s = logit[h];
-          s = fmaf(kv[0], q0.x, s); s = fmaf(kv[1], q0.y, s); s = fmaf(kv[2], q0.z, s); s = fmaf(kv[3], q0.w, s);
-          s = fmaf(kv[4], q1.x, s); s = fmaf(kv[5], q1.y, s); s = fmaf(kv[6], q1.z, s); s = fmaf(kv[7], q1.w, s);
-          logit[h] = s;
+        for (int j = 0; j < CB / 8; ++j) ld_in8(row + c0 + 8 * j, kv[j]);
+#pragma unroll
+        for (int j = 0; j < CB / 8; ++j) {
+          const int c = c0 + 8 * j;
+#pragma unroll
+          for (int h = 0; h < GP; ++h) {
+            const float4 q0 = *reinterpret_cast<const float4*>(&sm.qraw[h][c]);
+            const float4 q1 = *reinterpret_cast<const float4*>(&sm.qraw[h][c + 4]);
+            float s = logit[h];
+            s = fmaf(kv[j][0], q0.x, s); s = fmaf(kv[j][1], q0.y, s); s = fmaf(kv[j][2], q0.z, s); s = fmaf(kv[j][3], q0.w, s);
+            s = fmaf(kv[j][4], q1.x, s); s = fmaf(kv[j][5], q1.y, s); s = fmaf(kv[j][6], q1.z, s); s = fmaf(kv[j][7], q1.w, s);
+            logit[h] = s;
+          }
         }
       }
     } else {
@@ -667,7 +684,7 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
       const float r = warp_reduce_multi<GP>(v, lane, RMax());
       if ((lane & (32 / GP - 1)) == 0) sm.wmax[warp][red_index<GP>(lane)] = r;
     }
-    __syncthreads();   // also: every thread is done reading qraw as q
+    __syncthreads();   // also: the previous window's probabilities have been consumed
     float p[GP];
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
@@ -678,26 +695,37 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
       p[h] = exp2f(logit[h] - m_new);        // exp2(-inf) = 0 for masked tokens
       l_part[h] = fmaf(l_part[h], corr, p[h]);
       acc[h] *= corr;
+      acc_res[h] *= corr;
+      psm[h * 128 + tid] = p[h];
     }
     __syncthreads();
+    constexpr int TB = 32;   // tokens per batch of the value pass (32 loads in flight per thread)
+#pragma unroll 1
+    for (int tb = 0; tb < cnt; tb += TB) {
+      float vv[TB];
 #pragma unroll
-    for (int h = 0; h < GP; ++h) sm.qraw[h][tid] = p[h];
-    __syncthreads();
-    for (int t0 = 0; t0 < resid; t0 += 8) {
-      float vv[8];
+      for (int j = 0; j < TB; ++j) vv[j] = (tb + j < cnt) ? ld_in<InT>(vraw + (size_t)(tb + j) * D + tid) : 0.f;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) vv[j] = (t0 + j < resid) ? ld_in<InT>(vres + (size_t)(t0 + j) * D + tid) : 0.f;
+      for (int j8 = 0; j8 < TB; j8 += 8) {
 #pragma unroll
-      for (int h = 0; h < GP; ++h) {
-        const float4 p0 = *reinterpret_cast<const float4*>(&sm.qraw[h][t0]);
-        const float4 p1 = *reinterpret_cast<const float4*>(&sm.qraw[h][t0 + 4]);
-        float s = acc_res[h];
-        s = fmaf(p0.x, vv[0], s); s = fmaf(p0.y, vv[1], s); s = fmaf(p0.z, vv[2], s); s = fmaf(p0.w, vv[3], s);
-        s = fmaf(p1.x, vv[4], s); s = fmaf(p1.y, vv[5], s); s = fmaf(p1.z, vv[6], s); s = fmaf(p1.w, vv[7], s);
-        acc_res[h] = s;
+        for (int h = 0; h < GP; ++h) {
+          const float4 p0 = *reinterpret_cast<const float4*>(&psm[h * 128 + tb + j8]);
+          const float4 p1 = *reinterpret_cast<const float4*>(&psm[h * 128 + tb + j8 + 4]);
+          float s = acc_res[h];
+          s = fmaf(p0.x, vv[j8], s); s = fmaf(p0.y, vv[j8 + 1], s); s = fmaf(p0.z, vv[j8 + 2], s); s = fmaf(p0.w, vv[j8 + 3], s);
+          s = fmaf(p1.x, vv[j8 + 4], s); s = fmaf(p1.y, vv[j8 + 5], s); s = fmaf(p1.z, vv[j8 + 6], s); s = fmaf(p1.w, vv[j8 + 7], s);
+          acc_res[h] = s;
+        }
       }
     }
-  }
+    __syncthreads();   // psm and wmax are free again
+  };
+  if (do_sink)
+    raw_window(reinterpret_cast<const InT*>(A.k_sink) + (size_t)bh * A.n_sink * D,
+               reinterpret_cast<const InT*>(A.v_sink) + (size_t)bh * A.n_sink * D, n_sink_tok);
+  if (do_resid)
+    raw_window(reinterpret_cast<const InT*>(A.k_resid) + (size_t)bh * G * D,
+               reinterpret_cast<const InT*>(A.v_resid) + (size_t)bh * G * D, resid);
 
   // ---- l: reduce the per-thread partial sums ----------------------------------------------------
   __syncthreads();
@@ -733,11 +761,12 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
         const uint32_t dst = mapa_shared(land_addr + (uint32_t)(j * CS + crank) * (WS_STRIDE * 4), (uint32_t)d);
         if (tid == 0) { st_cluster_f32(dst, m_run[h]); st_cluster_f32(dst + 4, l_tot[h]); }
         st_cluster_f32(dst + 16 + 4 * tid, acc[h]);
-        if (do_resid) st_cluster_f32(dst + 16 + 512 + 4 * tid, acc_res[h]);
+        if (do_resid || do_sink) st_cluster_f32(dst + 16 + 512 + 4 * tid, acc_res[h]);
       }
     }
     cluster_sync_all();
     const bool res_here = resid > 0 && split / CS == NC - 1;   // this cluster's last rank ran the residual window
+    const bool sink_here = n_sink_tok > 0 && split / CS == 0;    // this cluster's rank 0 ran the sink window
 #pragma unroll
     for (int j = 0; j < GP; ++j) {
       const int h = crank + j * CS;
@@ -750,7 +779,7 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
           const float w = (sl[0] == -INFINITY) ? 0.f : ex2_approx(sl[0] - mj);
           lj = fmaf(w, sl[1], lj);
           aj = fmaf(w, sl[4 + tid], aj);
-          if (res_here && r == CS - 1) rj = w * sl[132 + tid];
+          if ((res_here && r == CS - 1) || (sink_here && r == 0)) rj = fmaf(w, sl[132 + tid], rj);
         }
       }
       m_run[j] = mj; l_tot[j] = lj; acc[j] = aj; acc_res[j] = rj;

@@ -45,7 +45,7 @@ class CacheDesc(C.Structure):
     _fields_ = [("k_records", C.c_void_p), ("v_records", C.c_void_p), ("k_resid", C.c_void_p),
                 ("v_resid", C.c_void_p), ("seq_lens", C.c_void_p), ("ticket", C.c_void_p),
                 ("decode_ticket", C.c_void_p), ("B", C.c_int32), ("Hkv", C.c_int32), ("max_chunks", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("n_sink", C.c_int32), ("k_sink", C.c_void_p), ("v_sink", C.c_void_p)]
 
 
 class DebugDesc(C.Structure):
@@ -168,9 +168,13 @@ class Cache:
     """Device buffers of one layer's KVarN cache + the POD descriptor."""
 
     def __init__(self, p: Params, B: int, Hkv: int, max_chunks: int, device="cuda",
-                 resid_dtype=torch.bfloat16):
+                 resid_dtype=torch.bfloat16, n_sink: int = 0):
+        """n_sink = S of the paper's three-region layout: the first S tokens of every sequence
+        stay raw (0 = no sink region; the paper uses 128, and 32 for IFEval)."""
         rb = record_bytes(p)
-        self.B, self.Hkv, self.max_chunks, self.rb = B, Hkv, max_chunks, rb
+        self.B, self.Hkv, self.max_chunks, self.rb, self.n_sink = B, Hkv, max_chunks, rb, n_sink
+        self.k_sink = torch.zeros((B, Hkv, max(n_sink, 1), HEAD_DIM), dtype=resid_dtype, device=device)
+        self.v_sink = torch.zeros_like(self.k_sink)
         self.k_records = torch.zeros((B, Hkv, max(max_chunks, 1), rb), dtype=torch.uint8, device=device)
         self.v_records = torch.zeros_like(self.k_records)
         self.k_resid = torch.zeros((B, Hkv, CHUNK, HEAD_DIM), dtype=resid_dtype, device=device)
@@ -181,27 +185,31 @@ class Cache:
         self.desc = CacheDesc(self.k_records.data_ptr(), self.v_records.data_ptr(),
                               self.k_resid.data_ptr(), self.v_resid.data_ptr(),
                               self.seq_lens.data_ptr(), self.ticket.data_ptr(),
-                              self.decode_ticket.data_ptr(), B, Hkv, max_chunks, 0)
+                              self.decode_ticket.data_ptr(), B, Hkv, max_chunks, n_sink,
+                              self.k_sink.data_ptr(), self.v_sink.data_ptr())
 
     def slice(self, b0: int, b1: int) -> "Cache":
         """A cache over sequences b0..b1-1 that shares this cache's buffers (views, no copy):
         lets a large cache be filled or read a few sequences at a time."""
         c = Cache.__new__(Cache)
-        c.B, c.Hkv, c.max_chunks, c.rb = b1 - b0, self.Hkv, self.max_chunks, self.rb
+        c.B, c.Hkv, c.max_chunks, c.rb, c.n_sink = b1 - b0, self.Hkv, self.max_chunks, self.rb, self.n_sink
+        c.k_sink, c.v_sink = self.k_sink[b0:b1], self.v_sink[b0:b1]
         c.k_records, c.v_records = self.k_records[b0:b1], self.v_records[b0:b1]
         c.k_resid, c.v_resid = self.k_resid[b0:b1], self.v_resid[b0:b1]
         c.seq_lens, c.ticket = self.seq_lens[b0:b1], self.ticket[b0:b1]
         c.decode_ticket = self.decode_ticket[b0 * self.Hkv:b1 * self.Hkv]
         c.desc = CacheDesc(c.k_records.data_ptr(), c.v_records.data_ptr(), c.k_resid.data_ptr(),
                            c.v_resid.data_ptr(), c.seq_lens.data_ptr(), c.ticket.data_ptr(),
-                           c.decode_ticket.data_ptr(), c.B, c.Hkv, c.max_chunks, 0)
+                           c.decode_ticket.data_ptr(), c.B, c.Hkv, c.max_chunks, c.n_sink,
+                           c.k_sink.data_ptr(), c.v_sink.data_ptr())
         return c
 
     def nbytes_read_by_decode(self, ctx: int) -> int:
         """Algorithmic bytes one decode step reads for context length ctx."""
-        n_chunks, r = ctx // CHUNK, ctx % CHUNK
+        ns = min(ctx, self.n_sink)
+        n_chunks, r = (ctx - ns) // CHUNK, (ctx - ns) % CHUNK
         es = self.k_resid.element_size()
-        return self.B * self.Hkv * (n_chunks * 2 * self.rb + r * 2 * HEAD_DIM * es)
+        return self.B * self.Hkv * (n_chunks * 2 * self.rb + (r + ns) * 2 * HEAD_DIM * es)
 
 
 def prefill(p: Params, cache: Cache, k: torch.Tensor, v: torch.Tensor, stream=None):

@@ -18,20 +18,20 @@ def kv():
     return kvarn
 
 
-def _build_cache(kv, p, K, V, max_chunks=None):
+def _build_cache(kv, p, K, V, max_chunks=None, n_sink=0):
     B, Hkv, n_tok, _ = K.shape
     mc = (n_tok // 128 + 1) if max_chunks is None else max_chunks
-    cache = kv.Cache(p, B, Hkv, mc, device=K.device, resid_dtype=K.dtype)
+    cache = kv.Cache(p, B, Hkv, mc, device=K.device, resid_dtype=K.dtype, n_sink=n_sink)
     kv.prefill(p, cache, K, V)
     return cache
 
 
 def _oracle_unit(kv, p, cache, b, h, g, q, n_tok, sm_scale=None):
-    n_chunks, r = n_tok // 128, n_tok % 128
+    ns, n_chunks, r = O.cache_partition(n_tok, cache.n_sink)
     kr = cache.k_records[b, h, :n_chunks].cpu().numpy()
     vr = cache.v_records[b, h, :n_chunks].cpu().numpy()
-    kres = P.tile_f64(cache.k_resid[b, h, :r])
-    vres = P.tile_f64(cache.v_resid[b, h, :r])
+    kres = np.concatenate([P.tile_f64(cache.k_sink[b, h, :ns]), P.tile_f64(cache.k_resid[b, h, :r])])
+    vres = np.concatenate([P.tile_f64(cache.v_sink[b, h, :ns]), P.tile_f64(cache.v_resid[b, h, :r])])
     qq = P.tile_f64(q[b, h * g:(h + 1) * g])
     return P.oracle_attention_from_records(kv, p, kr, vr, kres, vres, qq, sm_scale)
 
@@ -299,3 +299,68 @@ def test_decode_is_deterministic_over_repeats(kv, bits, Hq, n_tok, splits):
         kv.decode_attention(p, cache, q, out=out)
         assert torch.equal(out, ref)
     _check_all_units(kv, p, cache, q, ref, n_tok, units={(0, 0), (3, 7)})
+
+
+# ---------------------------------------------------------------- FP16 sink region
+@pytest.mark.parametrize("S,n_tok", [(128, 10), (128, 128), (128, 129), (128, 128 + 128 * 3 + 5), (32, 20),
+                                     (32, 32 + 128 * 5), (32, 32 + 128 * 9 + 127), (64, 64 + 128 * 30 + 1)])
+def test_sink_region_prefill_and_decode(kv, S, n_tok):
+    K, V = W.kv_tokens(3, 8, n_tok, seed=81, device="cuda")
+    q = W.queries(3, 32, seed=81, device="cuda")
+    p = kv.default_params(2)
+    cache = _build_cache(kv, p, K, V, n_sink=S)
+    ns, nc, r = O.cache_partition(n_tok, S)
+    assert cache.seq_lens.tolist() == [n_tok] * 3
+    # the sink and residual regions hold the caller's raw tokens, the records the chunks after the sink
+    assert torch.equal(cache.k_sink[:, :, :ns], K[:, :, :ns]) and torch.equal(cache.v_sink[:, :, :ns], V[:, :, :ns])
+    assert torch.equal(cache.k_resid[:, :, :r], K[:, :, n_tok - r:]) and torch.equal(cache.v_resid[:, :, :r], V[:, :, n_tok - r:])
+    if nc:
+        kr, vr = kv.quantize_chunk(p, K[:, :, ns:ns + 128 * nc].reshape(-1, 128, 128).contiguous(),
+                                   V[:, :, ns:ns + 128 * nc].reshape(-1, 128, 128).contiguous())
+        assert torch.equal(cache.k_records[:, :, :nc].reshape(-1, cache.rb), kr)
+        assert torch.equal(cache.v_records[:, :, :nc].reshape(-1, cache.rb), vr)
+    out = kv.decode_attention(p, cache, q)
+    _check_all_units(kv, p, cache, q, out, n_tok, units={(0, 0), (2, 7)})
+    # (no end-to-end gate against the oracle's own codes here: on this peaked synthetic data a one-ulp
+    # FP8 flip of a stored scale -- a legal tie, reading R17 -- moves the output by ~10 %; parity is the
+    # exact comparison of the stored regions above plus attention over the GPU's own records)
+
+
+@pytest.mark.parametrize("splits", [0, 3, 8, 16])
+def test_sink_region_with_every_merge_route(kv, splits):
+    n_tok = 128 + 128 * 20 + 77
+    K, V = W.kv_tokens(2, 8, n_tok, seed=83, device="cuda")
+    q = W.queries(2, 64, seed=83, device="cuda")
+    p = kv.default_params(2, splits=splits)
+    cache = _build_cache(kv, p, K, V, n_sink=128)
+    out = kv.decode_attention(p, cache, q)
+    _check_all_units(kv, p, cache, q, out, n_tok, units={(0, 0), (1, 5)})
+    assert torch.equal(out, kv.decode_attention(p, cache, q))
+
+
+def test_sink_region_append_matches_prefill(kv):
+    # grow from inside the sink region across its end and two chunk boundaries
+    B, Hkv, Hq, S = 2, 2, 8, 32
+    start, total = 20, 32 + 128 * 2 + 9
+    K, V = W.kv_tokens(B, Hkv, total, seed=85, device="cuda")
+    q = W.queries(B, Hq, seed=85, device="cuda")
+    p = kv.default_params(2)
+    mc = 3
+    inc = kv.Cache(p, B, Hkv, mc, device="cuda", n_sink=S)
+    kv.prefill(p, inc, K[:, :, :start].contiguous(), V[:, :, :start].contiguous())
+    for t in range(start, total):
+        kv.append(p, inc, K[:, :, t].contiguous(), V[:, :, t].contiguous())
+        n = t + 1
+        if n in (31, 32, 33, 32 + 127, 32 + 128, 32 + 129, 32 + 256, total):
+            assert inc.seq_lens.tolist() == [n] * B
+            ref = kv.Cache(p, B, Hkv, mc, device="cuda", n_sink=S)
+            kv.prefill(p, ref, K[:, :, :n].contiguous(), V[:, :, :n].contiguous())
+            ns, nc, r = O.cache_partition(n, S)
+            assert torch.equal(inc.k_sink[:, :, :ns], ref.k_sink[:, :, :ns]) and torch.equal(inc.v_sink[:, :, :ns], ref.v_sink[:, :, :ns])
+            assert torch.equal(inc.k_records[:, :, :nc], ref.k_records[:, :, :nc])
+            assert torch.equal(inc.v_records[:, :, :nc], ref.v_records[:, :, :nc])
+            assert torch.equal(inc.k_resid[:, :, :r], ref.k_resid[:, :, :r]) and torch.equal(inc.v_resid[:, :, :r], ref.v_resid[:, :, :r])
+            out = kv.decode_attention(p, inc, q)
+            assert torch.equal(out, kv.decode_attention(p, ref, q))
+            _check_all_units(kv, p, inc, q, out, n, units={(0, 0), (1, 1)})
+    assert int(inc.ticket.abs().sum()) == 0

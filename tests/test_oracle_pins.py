@@ -427,3 +427,36 @@ def test_folded_algebra_equals_plain_definition():
     a = pt @ tv.codes.astype(np.float64) + (pt * tv.z).sum()
     out = ((tv.s2 * a) @ H.T) / p.sum()
     assert np.allclose(out, ref, rtol=1e-11, atol=1e-13)
+
+
+# ---------------------------------------------------------------- three-region layout
+def test_cache_partition_brute_force_token_walk():
+    # walk the tokens one by one as P:350 describes the regions: the first S go to the sink, later ones
+    # trail in FP16 until G of them form a full group, which is then quantised
+    for S in (0, 32, 128):
+        sink = chunks = trail = 0
+        for n in range(0, 700):
+            assert O.cache_partition(n, S) == (sink, chunks, trail), (n, S)
+            if sink < S:
+                sink += 1
+            else:
+                trail += 1
+                if trail == 128:
+                    chunks, trail = chunks + 1, 0
+    assert O.cache_partition(128 + 3 * 128 + 5, 128) == (128, 3, 5)      # the paper's S = G = 128
+    assert O.cache_partition(32 + 128, 32) == (32, 1, 0)                 # IFEval setting S = 32
+    assert O.cache_partition(20, 32) == (20, 0, 0)
+
+
+def test_cache_attention_sink_tokens_are_exact():
+    # with every token inside the sink / residual regions nothing is quantised: the result is plain attention
+    rng = np.random.default_rng(5)
+    K, V, q = rng.standard_normal((150, 128)), rng.standard_normal((150, 128)), rng.standard_normal((2, 128))
+    assert np.allclose(O.cache_attention(q, K, V, n_sink=128), O.attention(q, K, V), atol=1e-13)
+    # a quantised body changes the result, and the sink region (a x10 first token kept exact) reduces the error
+    K2 = rng.standard_normal((128 + 256, 128)); K2[0] *= 10.0
+    V2 = rng.standard_normal((128 + 256, 128))
+    ref = O.attention(q, K2, V2)
+    e_sink = np.abs(O.cache_attention(q, K2, V2, n_sink=128) - ref).max()
+    e_none = np.abs(O.cache_attention(q, K2[:384], V2[:384], n_sink=0) - ref).max()
+    assert 0 < e_sink < e_none
