@@ -30,6 +30,8 @@ rtn_quantize / dequant ... pinned (on-grid round trip, textbook min-max RTN)
 fp8 / fp16 rounding ...... pinned (torch.float8_e4m3fn, numpy.float16 casts)
 attention ................ pinned (brute-force loops, torch SDPA, invariances)
 cache_partition .......... pinned (brute-force token walk, P:350's S/G/R settings)
+block_attention .......... pinned (brute-force loops, torch SDPA with a causal mask,
+                           n_q = 1 and last-query special cases)
 codes / scales of a tile vs values printed by the paper ... **parity unpinned**:
                            the paper prints no intermediate value for any tile.
 """
@@ -395,6 +397,39 @@ def cache_attention(q: np.ndarray, K: np.ndarray, V: np.ndarray, n_sink: int = 0
         kt.append((tk.codes, tk.s1, tk.s2, tk.z)); vt.append((tv.codes, tv.s1, tv.s2, tv.z))
     raw = np.r_[0:ns, ns + 128 * nc:K.shape[0]]
     return decode_attention(q, kt, vt, K[raw], V[raw], sm_scale=sm_scale)
+
+
+# --------------------------------------------------------------------------
+# Multi-token read path: a block of new tokens against the compressed cache
+# (Fig. 4 "pseudo-decode", Sec. 3.2)
+# --------------------------------------------------------------------------
+def block_attention(q_blk: np.ndarray, k_tiles: list, v_tiles: list,
+                    k_raw: np.ndarray, v_raw: np.ndarray,
+                    k_blk: np.ndarray, v_blk: np.ndarray,
+                    sm_scale: float | None = None) -> np.ndarray:
+    """Causal attention of a block of ``n_q`` new tokens for one KV head (Fig. 4: "We split
+    the sequence into blocks of size b. After every block, the freshly produced K, V are quantized
+    before being written back to the KV-cache. Subsequent blocks access a *quantized* cache").
+
+    Query i of the block sees every token of the cache -- dequantised chunks ``k_tiles`` /
+    ``v_tiles`` (stored aux, as in ``decode_attention``) and the raw sink / residual tokens
+    ``k_raw`` / ``v_raw`` (r, d) -- plus the block's own, not yet quantised tokens 0..i
+    (``k_blk`` / ``v_blk`` (n_q, d)).  Plain definition, one query token at a time.
+
+    q_blk: (n_q, g, d).  Returns (n_q, g, d) float64.
+    """
+    q_blk = np.asarray(q_blk, dtype=np.float64)
+    k_blk = np.asarray(k_blk, dtype=np.float64)
+    v_blk = np.asarray(v_blk, dtype=np.float64)
+    n_q, _, d = q_blk.shape
+    k_raw = np.asarray(k_raw, dtype=np.float64).reshape(-1, d)
+    v_raw = np.asarray(v_raw, dtype=np.float64).reshape(-1, d)
+    out = np.zeros_like(q_blk)
+    for i in range(n_q):
+        out[i] = decode_attention(q_blk[i], k_tiles, v_tiles,
+                                  np.concatenate([k_raw, k_blk[:i + 1]], axis=0),
+                                  np.concatenate([v_raw, v_blk[:i + 1]], axis=0), sm_scale=sm_scale)
+    return out
 
 
 # --------------------------------------------------------------------------

@@ -460,3 +460,68 @@ def test_cache_attention_sink_tokens_are_exact():
     e_sink = np.abs(O.cache_attention(q, K2, V2, n_sink=128) - ref).max()
     e_none = np.abs(O.cache_attention(q, K2[:384], V2[:384], n_sink=0) - ref).max()
     assert 0 < e_sink < e_none
+
+
+# ---- multi-token read path (Fig. 4): block_attention ----------------------------------------
+def _tiny_cache(rng, n_chunks, r):
+    kt, vt = [], []
+    for _ in range(n_chunks):
+        tk = O.quantize_tile(rng.standard_normal((128, 128)), "k")
+        tv = O.quantize_tile(rng.standard_normal((128, 128)), "v")
+        kt.append((tk.codes, tk.s1, tk.s2, tk.z)); vt.append((tv.codes, tv.s1, tv.s2, tv.z))
+    return kt, vt, rng.standard_normal((r, 128)), rng.standard_normal((r, 128))
+
+
+def test_block_attention_brute_force_loops():
+    """Pin: explicit Python loops over (query token, head, visible token) on a small case."""
+    rng = np.random.default_rng(21)
+    kt, vt, kr, vr = _tiny_cache(rng, 1, 3)
+    n_q, g = 4, 2
+    q = rng.standard_normal((n_q, g, 128)); kb = rng.standard_normal((n_q, 128)); vb = rng.standard_normal((n_q, 128))
+    out = O.block_attention(q, kt, vt, kr, vr, kb, vb)
+    Kc = np.concatenate([O.dequantize_tile(*kt[0], kind="k"), kr]); Vc = np.concatenate([O.dequantize_tile(*vt[0], kind="v"), vr])
+    for i in range(n_q):
+        for h in range(g):
+            keys = [Kc[t] for t in range(len(Kc))] + [kb[t] for t in range(i + 1)]
+            vals = [Vc[t] for t in range(len(Vc))] + [vb[t] for t in range(i + 1)]
+            lg = [sum(q[i, h, c] * k[c] for c in range(128)) / np.sqrt(128.0) for k in keys]
+            m = max(lg); w = [np.exp(x - m) for x in lg]; tot = sum(w)
+            ref = sum(wi * v for wi, v in zip(w, vals)) / tot
+            assert np.allclose(out[i, h], ref, rtol=1e-10, atol=1e-12)
+
+
+def test_block_attention_matches_torch_sdpa_causal_mask():
+    """Pin: with a raw-only cache the block path is ordinary causal attention with a prefix --
+    torch's scaled_dot_product_attention with an explicit boolean mask (library routine)."""
+    import torch
+    rng = np.random.default_rng(22)
+    r, n_q, g = 37, 9, 4
+    kr, vr = rng.standard_normal((r, 128)), rng.standard_normal((r, 128))
+    q = rng.standard_normal((n_q, g, 128)); kb = rng.standard_normal((n_q, 128)); vb = rng.standard_normal((n_q, 128))
+    out = O.block_attention(q, [], [], kr, vr, kb, vb)
+    K = torch.tensor(np.concatenate([kr, kb])); V = torch.tensor(np.concatenate([vr, vb]))
+    mask = torch.ones((n_q, r + n_q), dtype=torch.bool)
+    for i in range(n_q):
+        mask[i, r + i + 1:] = False
+    qt = torch.tensor(q).permute(1, 0, 2)   # (g, n_q, d)
+    ref = torch.nn.functional.scaled_dot_product_attention(qt, K[None].expand(g, -1, -1), V[None].expand(g, -1, -1),
+                                                           attn_mask=mask[None]).permute(1, 0, 2).numpy()
+    assert np.allclose(out, ref, rtol=1e-10, atol=1e-12)
+
+
+def test_block_attention_special_cases():
+    """n_q = 1 is decode attention with the new token appended to the raw window; the last query of a
+    block sees the whole block (no mask); an empty cache leaves query 0 with v_blk[0] exactly."""
+    rng = np.random.default_rng(23)
+    kt, vt, kr, vr = _tiny_cache(rng, 2, 5)
+    g = 4
+    q = rng.standard_normal((6, g, 128)); kb = rng.standard_normal((6, 128)); vb = rng.standard_normal((6, 128))
+    one = O.block_attention(q[:1], kt, vt, kr, vr, kb[:1], vb[:1])
+    assert np.allclose(one[0], O.decode_attention(q[0], kt, vt, np.r_[kr, kb[:1]], np.r_[vr, vb[:1]]), rtol=1e-12)
+    out = O.block_attention(q, kt, vt, kr, vr, kb, vb)
+    assert np.allclose(out[-1], O.decode_attention(q[-1], kt, vt, np.r_[kr, kb], np.r_[vr, vb]), rtol=1e-12)
+    assert np.allclose(out[0], one[0], rtol=1e-12)          # causal: later block tokens do not leak into query 0
+    kb2, vb2 = kb.copy(), vb.copy(); kb2[3:] += 100.0; vb2[3:] -= 50.0
+    assert np.allclose(O.block_attention(q, kt, vt, kr, vr, kb2, vb2)[:3], out[:3], rtol=1e-12)
+    empty = O.block_attention(q, [], [], np.zeros((0, 128)), np.zeros((0, 128)), kb, vb)
+    assert np.allclose(empty[0], np.broadcast_to(vb[0], (g, 128)), rtol=1e-12)
