@@ -207,6 +207,23 @@ KVARN_API int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* c
                            void* stream);
 
 /*
+ * kvarn_block_attention -- the multi-token read path (Fig. 4 "pseudo-decode", Sec. 3.2:
+ * "We split the sequence into blocks of size b.  After every block, the freshly produced K, V are
+ * quantized before being written back to the KV-cache.  Subsequent blocks access a quantized cache").
+ * A block of n_q new tokens per sequence (speculative / chunked decoding, 1 <= n_q <= 128) attends
+ *   - every token already in the cache (sink tokens, packed chunks, residual window: exactly what
+ *     kvarn_decode_attention reads, no dequantised copy), and
+ *   - causally, the block's own raw tokens: query i sees block tokens 0..i.
+ * The block is NOT in the cache yet; the caller appends it afterwards (kvarn_append per token).
+ *   q      DEVICE [B][n_q][Hq][128] in_dtype       out  DEVICE [B][n_q][Hq][128] out_dtype
+ *   k_blk, v_blk  DEVICE [B][Hkv][n_q][128] in_dtype (raw, un-rotated), 16-B aligned
+ * Hq/Hkv must be 1, 2, 4 or 8.  Needs no workspace (split-K merges inside a thread-block cluster).
+ */
+KVARN_API int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                          const void* k_blk, const void* v_blk, int32_t n_q, int32_t Hq,
+                          float sm_scale, void* out, void* stream);
+
+/*
  * Host-buffer forms (end-to-end measurement; HOST pointers in, HOST out).
  * They copy host->device into caller-provided DEVICE staging, run the device
  * call above and copy the result back, all enqueued on `stream`; the caller

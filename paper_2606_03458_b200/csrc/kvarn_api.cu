@@ -264,7 +264,7 @@ static cudaError_t launch_decode_k(const DecodeArgs& A, cudaStream_t st) {
     configured = true;
   }
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(A.B * A.Hkv, A.splits, 1);
+  cfg.gridDim = dim3(A.B * A.Hkv, A.splits, (A.n_q + A.tpc - 1) / A.tpc);
   cfg.blockDim = dim3(128, 1, 1);
   cfg.dynamicSmemBytes = sizeof(SM);
   cfg.stream = st;
@@ -277,7 +277,7 @@ static cudaError_t launch_decode_k(const DecodeArgs& A, cudaStream_t st) {
 
 template <int BITS, typename InT>
 static cudaError_t launch_decode(const DecodeArgs& A, cudaStream_t st) {
-  return A.g <= 4 ? launch_decode_k<BITS, 4, InT>(A, st) : launch_decode_k<BITS, 8, InT>(A, st);
+  return A.tpc * A.g <= 4 ? launch_decode_k<BITS, 4, InT>(A, st) : launch_decode_k<BITS, 8, InT>(A, st);
 }
 
 }  // namespace kvarn
@@ -446,6 +446,45 @@ int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, cons
   A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;
   const SplitPlan sp = split_plan(p, cache->B, cache->Hkv, g, cache->max_chunks);
   A.cluster = sp.cluster; A.nclus = sp.nclus; A.splits = sp.cluster * sp.nclus;
+  A.q_scale = sm_scale * 1.4426950408889634f;
+  A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
+  A.n_q = 1; A.tpc = 1; A.k_blk = nullptr; A.v_blk = nullptr;
+  cudaStream_t s = (cudaStream_t)stream;
+  const bool f32 = p->in_dtype == KVARN_F32;
+  cudaError_t e;
+  if (p->bits == 2) e = f32 ? launch_decode<2, float>(A, s) : launch_decode<2, __nv_bfloat16>(A, s);
+  else e = f32 ? launch_decode<4, float>(A, s) : launch_decode<4, __nv_bfloat16>(A, s);
+  return e == cudaSuccess ? KVARN_OK : KVARN_CUDA;
+}
+
+// Multi-token read path (Fig. 4): the same kernel, the (query token, head)
+// pairs that share a KV head are its MMA columns, 8 per CTA; blockIdx.z walks the block in groups of
+// tpc = 8 / g tokens.  Split-K only through one thread-block cluster (no workspace merge).
+int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                          const void* k_blk, const void* v_blk, int32_t n_q, int32_t Hq,
+                          float sm_scale, void* out, void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if ((st = check_cache(cache))) return st;
+  if (!q || !out || !k_blk || !v_blk || Hq <= 0 || (Hq % cache->Hkv) != 0 || n_q < 1) return KVARN_INVALID_ARG;
+  const int g = Hq / cache->Hkv;
+  if (g > 8 || (g & (g - 1)) || n_q > G) return KVARN_UNSUPPORTED;
+  if (!aligned16(q) || !aligned16(out) || !aligned16(k_blk) || !aligned16(v_blk)) return KVARN_MISALIGNED;
+  DecodeArgs A{};
+  A.k_records = (const uint8_t*)cache->k_records; A.v_records = (const uint8_t*)cache->v_records;
+  A.k_resid = cache->k_resid; A.v_resid = cache->v_resid; A.seq_lens = cache->seq_lens;
+  A.k_sink = cache->k_sink; A.v_sink = cache->v_sink; A.n_sink = cache->n_sink;
+  A.ticket = cache->decode_ticket;   // unused: nclus = 1
+  A.q = q; A.out = out; A.ws = nullptr;
+  A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;
+  A.n_q = n_q; A.k_blk = k_blk; A.v_blk = v_blk;
+  A.tpc = n_q * g <= 4 ? n_q : (8 / g < n_q ? 8 / g : n_q);
+  const int nz = (n_q + A.tpc - 1) / A.tpc;
+  int want = p->splits > 0 ? p->splits : decode_slots(p, A.tpc * g) / (cache->B * cache->Hkv * nz);
+  if (want > KVARN_MAX_CLUSTER) want = KVARN_MAX_CLUSTER;
+  if (want > cache->max_chunks) want = cache->max_chunks;
+  if (want < 1) want = 1;
+  A.cluster = want; A.nclus = 1; A.splits = want;
   A.q_scale = sm_scale * 1.4426950408889634f;
   A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
   cudaStream_t s = (cudaStream_t)stream;

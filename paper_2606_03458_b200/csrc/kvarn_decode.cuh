@@ -67,6 +67,13 @@ struct DecodeArgs {
   int nclus;      // clusters per (sequence, KV head); splits = cluster * nclus; nclus > 1 -> workspace merge
   float q_scale;  // sm_scale * log2(e)
   int rotate_k, rotate_v, out_dtype;
+  // multi-token read path (kvarn_block_attention, Fig. 4): n_q query tokens per sequence, q / out
+  // [B][n_q][Hq][128]; blockIdx.z picks `tpc` of them, whose tpc * g (token, head) pairs are the MMA
+  // columns of the CTA.  k_blk / v_blk [B][Hkv][n_q][128]: the block's own raw tokens, attended
+  // causally (query i sees block tokens 0..i).  Plain decode: n_q = tpc = 1, k_blk = null.
+  int n_q, tpc;
+  const void* k_blk;
+  const void* v_blk;
 };
 
 // ------------------------------------------------------------------ PTX wrappers
@@ -317,6 +324,11 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
   const int bh = blockIdx.x, b = bh / A.Hkv, hkv = bh - b * A.Hkv;
   const int split = blockIdx.y;
   const int g = A.g;
+  const int lg = A.tpc == 1 ? 31 : __ffs(g) - 1;   // several tokens per CTA: g is a power of two; one token: column = head
+  // columns of this CTA: j -> (query token tok0 + (j >> lg), head j mod 2^lg); plain decode: tok0 = 0, ncols = g
+  const int n_q = A.n_q, tok0 = (int)blockIdx.z * A.tpc;
+  const int ncols = min(A.tpc, n_q - tok0) * g;
+  auto qrow = [&](int j) -> size_t { return ((size_t)b * n_q + tok0 + (j >> lg)) * A.Hq + hkv * g + (j - ((j >> lg) << lg)); };
 
   // ---- chunk range of this split ----------------------------------------------------
   const int len = A.seq_lens[b];
@@ -328,13 +340,16 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
   // Balanced split: a raw window (512 B per token against 72 B) weighs like one chunk per 12 tokens (measured:
   // 127 residual tokens cost a CTA about 10 chunks), so the splits that own the sink / residual window get
   // correspondingly fewer chunks.  Virtual units: [sink | chunk 0 .. n_chunks-1 | residual].
-  const int w_sink = (n_sink_tok + 11) / 12, w_res = (resid + 11) / 12;
+  const bool has_blk = A.k_blk != nullptr;
+  const int blk_cnt = has_blk ? min(n_q, tok0 + A.tpc) : 0;   // block tokens visible to some column of this CTA
+  const int w_sink = (n_sink_tok + 11) / 12, w_res = (resid + blk_cnt + 11) / 12;
   const int per = (n_chunks + w_sink + w_res + A.splits - 1) / A.splits;
   const int c_begin = min(max(split * per - w_sink, 0), n_chunks);
   const int c_end = min(max((split + 1) * per - w_sink, 0), n_chunks);
   const int n_my = c_end - c_begin;
   const bool do_resid = (split == A.splits - 1) && resid > 0;
   const bool do_sink = (split == 0) && n_sink_tok > 0;
+  const bool do_blk = (split == A.splits - 1) && has_blk;
 
   const uint8_t* krec = A.k_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
   const uint8_t* vrec = A.v_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
@@ -361,8 +376,8 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
   // D1: q' = (q H / sqrt(128)) * q_scale; heads >= g are zero
   for (int hh = warp; hh < GP; hh += 4) {
     float v[4] = {0.f, 0.f, 0.f, 0.f};
-    if (hh < g) {
-      const InT* qp = reinterpret_cast<const InT*>(A.q) + ((size_t)b * A.Hq + hkv * g + hh) * D + 4 * lane;
+    if (hh < ncols) {
+      const InT* qp = reinterpret_cast<const InT*>(A.q) + qrow(hh) * D + 4 * lane;
 #pragma unroll
       for (int j = 0; j < 4; ++j) v[j] = ld_in<InT>(qp + j) * A.q_scale;
     }
@@ -647,7 +662,9 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
 #pragma unroll
   for (int h = 0; h < GP; ++h) acc_res[h] = 0.f;
   float* psm = &sm.qrot[0][0];   // [GP][128] probabilities of the window (q' and the staged acc are dead by now)
-  auto raw_window = [&](const InT* kraw, const InT* vraw, const int cnt) {   // cnt <= 128 tokens, thread = token
+  // vis0: token tid is visible to column h iff tid <= vis0 + (h >> lg) (causal block); NO_MASK for sink / residual
+  constexpr int NO_MASK = 1 << 20;
+  auto raw_window = [&](const InT* kraw, const InT* vraw, const int cnt, const int vis0) {   // cnt <= 128 tokens, thread = token
     float logit[GP];
 #pragma unroll
     for (int h = 0; h < GP; ++h) logit[h] = 0.f;
@@ -676,6 +693,10 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
     } else {
 #pragma unroll
       for (int h = 0; h < GP; ++h) logit[h] = -INFINITY;
+    }
+    if (vis0 != NO_MASK) {
+#pragma unroll
+      for (int h = 0; h < GP; ++h) if (tid > vis0 + (h >> lg)) logit[h] = -INFINITY;
     }
     {
       float v[GP];
@@ -722,10 +743,13 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
   };
   if (do_sink)
     raw_window(reinterpret_cast<const InT*>(A.k_sink) + (size_t)bh * A.n_sink * D,
-               reinterpret_cast<const InT*>(A.v_sink) + (size_t)bh * A.n_sink * D, n_sink_tok);
+               reinterpret_cast<const InT*>(A.v_sink) + (size_t)bh * A.n_sink * D, n_sink_tok, NO_MASK);
   if (do_resid)
     raw_window(reinterpret_cast<const InT*>(A.k_resid) + (size_t)bh * G * D,
-               reinterpret_cast<const InT*>(A.v_resid) + (size_t)bh * G * D, resid);
+               reinterpret_cast<const InT*>(A.v_resid) + (size_t)bh * G * D, resid, NO_MASK);
+  if (do_blk)
+    raw_window(reinterpret_cast<const InT*>(A.k_blk) + (size_t)bh * n_q * D,
+               reinterpret_cast<const InT*>(A.v_blk) + (size_t)bh * n_q * D, blk_cnt, tok0);
 
   // ---- l: reduce the per-thread partial sums ----------------------------------------------------
   __syncthreads();
@@ -756,22 +780,22 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
     const uint32_t land_addr = smem_u32(land);
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
-      if (h < g) {
+      if (h < ncols) {
         const int j = h / CS, d = h - j * CS;
         const uint32_t dst = mapa_shared(land_addr + (uint32_t)(j * CS + crank) * (WS_STRIDE * 4), (uint32_t)d);
         if (tid == 0) { st_cluster_f32(dst, m_run[h]); st_cluster_f32(dst + 4, l_tot[h]); }
         st_cluster_f32(dst + 16 + 4 * tid, acc[h]);
-        if (do_resid || do_sink) st_cluster_f32(dst + 16 + 512 + 4 * tid, acc_res[h]);
+        if (do_resid || do_sink || do_blk) st_cluster_f32(dst + 16 + 512 + 4 * tid, acc_res[h]);
       }
     }
     cluster_sync_all();
-    const bool res_here = resid > 0 && split / CS == NC - 1;   // this cluster's last rank ran the residual window
+    const bool res_here = (resid > 0 || has_blk) && split / CS == NC - 1;   // this cluster's last rank ran the residual window
     const bool sink_here = n_sink_tok > 0 && split / CS == 0;    // this cluster's rank 0 ran the sink window
 #pragma unroll
     for (int j = 0; j < GP; ++j) {
       const int h = crank + j * CS;
       float mj = -INFINITY, lj = 0.f, aj = 0.f, rj = 0.f;
-      if (h < g) {
+      if (h < ncols) {
         const float* slot0 = land + j * CS * WS_STRIDE;
         for (int r = 0; r < CS; ++r) mj = fmaxf(mj, slot0[r * WS_STRIDE]);
         for (int r = 0; r < CS; ++r) {
@@ -785,7 +809,7 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
       m_run[j] = mj; l_tot[j] = lj; acc[j] = aj; acc_res[j] = rj;
     }
     hbase = crank; hstride = CS;
-    if (hbase >= g) return;   // this rank owns no head
+    if (hbase >= ncols) return;   // this rank owns no column
   }
 
   // ---- D7b: several clusters per (sequence, KV head): partials -> workspace, last arriver merges ----
@@ -794,8 +818,8 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
 #pragma unroll
     for (int j = 0; j < GP; ++j) {
       const int h = hbase + hstride * j;
-      if (h < g) {
-        float* o = A.ws + (((size_t)b * A.Hq + hkv * g + h) * NC + cidx) * WS_STRIDE;
+      if (h < ncols) {
+        float* o = A.ws + (qrow(h) * NC + cidx) * WS_STRIDE;
         if (tid == 0) { o[0] = m_run[j]; o[1] = l_tot[j]; }
         o[4 + tid] = acc[j];
         o[132 + tid] = acc_res[j];
@@ -804,10 +828,11 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
     __threadfence();
     __syncthreads();
     if (tid == 0) {
-      const int n_writers = NC * min(CS, g);   // CTAs that own at least one head
-      const int old = atomicAdd(&A.ticket[bh], 1);
+      const int n_writers = NC * min(CS, ncols);   // CTAs that own at least one column
+      int* tk = &A.ticket[(size_t)blockIdx.z * gridDim.x + bh];
+      const int old = atomicAdd(tk, 1);
       const int last = (old == n_writers - 1);
-      if (last) A.ticket[bh] = 0;
+      if (last) *tk = 0;
       sm.last_flag = last;
     }
     __syncthreads();
@@ -815,8 +840,8 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
     __threadfence();
     // weights of the partials: warp w handles heads w, w+4; lane s handles partials s, s+32
     float* wsp = reinterpret_cast<float*>(sm.bq);   // [GP][64] weights (B_q is dead by now)
-    for (int h = warp; h < g; h += 4) {
-      const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * NC * WS_STRIDE;
+    for (int h = warp; h < ncols; h += 4) {
+      const float* base = A.ws + qrow(h) * NC * WS_STRIDE;
       const float m0 = lane < NC ? __ldcg(base + (size_t)lane * WS_STRIDE) : -INFINITY;
       const float m1 = lane + 32 < NC ? __ldcg(base + (size_t)(lane + 32) * WS_STRIDE) : -INFINITY;
       const float l0 = lane < NC ? __ldcg(base + (size_t)lane * WS_STRIDE + 1) : 0.f;
@@ -833,8 +858,8 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
       float rot = 0.f, res = 0.f, L = 0.f;
-      if (h < g) {
-        const float* base = A.ws + ((size_t)b * A.Hq + hkv * g + h) * NC * WS_STRIDE + 4 + tid;
+      if (h < ncols) {
+        const float* base = A.ws + qrow(h) * NC * WS_STRIDE + 4 + tid;
         int s = 0;
         for (; s + 4 <= NC; s += 4) {
           float r[4], e[4];
@@ -867,7 +892,7 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
   __syncthreads();
   for (int jj = warp; jj < GP; jj += 4) {
     const int hh = hbase + hstride * jj;
-    if (hh >= g) break;
+    if (hh >= ncols) break;
     float4 r4 = *reinterpret_cast<const float4*>(&merged_rot[jj * 128 + 4 * lane]);
     float v[4] = {r4.x, r4.y, r4.z, r4.w};
     if (A.rotate_v) {
@@ -878,7 +903,7 @@ __global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC
     const float4 s4 = *reinterpret_cast<const float4*>(&sm.qraw[jj][4 * lane]);
     const float inv = sm.hs[0][jj][0];
     const float o0 = (v[0] + s4.x) * inv, o1 = (v[1] + s4.y) * inv, o2 = (v[2] + s4.z) * inv, o3 = (v[3] + s4.w) * inv;
-    const size_t off = ((size_t)b * A.Hq + hkv * g + hh) * D + 4 * lane;
+    const size_t off = qrow(hh) * D + 4 * lane;
     if (A.out_dtype == KVARN_F32) {
       *reinterpret_cast<float4*>(reinterpret_cast<float*>(A.out) + off) = make_float4(o0, o1, o2, o3);
     } else {

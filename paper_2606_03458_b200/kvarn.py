@@ -66,6 +66,8 @@ EXPORTS = {
     "kvarn_append": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p, C.c_void_p]),
     "kvarn_decode_attention": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_int32,
                                          C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "kvarn_block_attention": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p,
+                                        C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_void_p]),
     "kvarn_quantize_chunk_host": (C.c_int, [C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int64] +
                                   [C.c_void_p] * 7),
     "kvarn_decode_attention_host": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_int32,
@@ -254,6 +256,27 @@ def decode_attention(p: Params, cache: Cache, q: torch.Tensor, sm_scale: float |
     st = lib.kvarn_decode_attention(C.byref(p), C.byref(cache.desc), _ptr(q), Hq, sm_scale, _ptr(out),
                                     _ptr(ws), ws.numel(), _stream(stream))
     _check(st, "kvarn_decode_attention")
+    return out
+
+
+def block_attention(p: Params, cache: Cache, q: torch.Tensor, k_blk: torch.Tensor, v_blk: torch.Tensor,
+                    sm_scale: float | None = None, out: torch.Tensor | None = None, stream=None):
+    """q: [B, n_q, Hq, 128]; k_blk, v_blk: [B, Hkv, n_q, 128] (the block's own raw tokens, not yet in
+    the cache) -> out [B, n_q, Hq, 128]: causal attention over [cache ; block] (Fig. 4)."""
+    assert q.is_cuda and q.is_contiguous() and q.shape[0] == cache.B and q.shape[3] == HEAD_DIM
+    n_q, Hq = q.shape[1], q.shape[2]
+    assert k_blk.is_contiguous() and v_blk.is_contiguous() and k_blk.shape == v_blk.shape
+    assert tuple(k_blk.shape) == (cache.B, cache.Hkv, n_q, HEAD_DIM) and k_blk.dtype == q.dtype
+    p.in_dtype = _dtype_code(q)
+    assert cache.k_resid.dtype == q.dtype
+    if sm_scale is None:
+        sm_scale = 1.0 / float(np.sqrt(HEAD_DIM))
+    if out is None:
+        out = torch.empty((cache.B, n_q, Hq, HEAD_DIM), device=q.device,
+                          dtype=torch.float32 if p.out_dtype == F32 else torch.bfloat16)
+    st = lib.kvarn_block_attention(C.byref(p), C.byref(cache.desc), _ptr(q), _ptr(k_blk), _ptr(v_blk), n_q, Hq,
+                                   sm_scale, _ptr(out), _stream(stream))
+    _check(st, "kvarn_block_attention")
     return out
 
 

@@ -1,0 +1,132 @@
+"""GPU parity: kvarn_block_attention (multi-token read path; Fig. 4) through the
+C ABI vs the oracle's plain-definition causal block attention over the same record bytes (R17)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import kvarn_oracle as O
+from paper_2606_03458_b200 import workloads as W
+import kvarn_parity as P
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def kv():
+    from paper_2606_03458_b200 import kvarn
+    return kvarn
+
+
+def _cache(kv, p, K, V, n_sink=0):
+    B, Hkv, n_tok, _ = K.shape
+    cache = kv.Cache(p, B, Hkv, n_tok // 128 + 1, device=K.device, resid_dtype=K.dtype, n_sink=n_sink)
+    if n_tok:
+        kv.prefill(p, cache, K, V)
+    return cache
+
+
+def _oracle_block(kv, p, cache, b, h, g, q, kb, vb, n_tok, sm_scale=None):
+    """oracle.block_attention on the GPU-produced record bytes of unit (b, h)."""
+    ns, n_chunks, r = O.cache_partition(n_tok, cache.n_sink)
+    kt = [kv.unpack_record(p, 0, rec) for rec in cache.k_records[b, h, :n_chunks].cpu().numpy()]
+    vt = [kv.unpack_record(p, 1, rec) for rec in cache.v_records[b, h, :n_chunks].cpu().numpy()]
+    f64 = lambda t: tuple(np.asarray(a, dtype=np.float64) if i else a for i, a in enumerate(t))
+    kt, vt = [f64(t) for t in kt], [f64(t) for t in vt]
+    kraw = np.concatenate([P.tile_f64(cache.k_sink[b, h, :ns]), P.tile_f64(cache.k_resid[b, h, :r])])
+    vraw = np.concatenate([P.tile_f64(cache.v_sink[b, h, :ns]), P.tile_f64(cache.v_resid[b, h, :r])])
+    qq = q[b, :, h * g:(h + 1) * g].to(torch.float64).cpu().numpy()          # (n_q, g, d)
+    return O.block_attention(qq, kt, vt, kraw, vraw, P.tile_f64(kb[b, h]), P.tile_f64(vb[b, h]), sm_scale=sm_scale)
+
+
+def _check(kv, p, cache, q, kb, vb, out, n_tok, units=None):
+    B, n_q, Hq, _ = q.shape
+    g = Hq // cache.Hkv
+    out = out.to(torch.float64).cpu().numpy()
+    worst = 0.0
+    for b in range(B):
+        for h in range(cache.Hkv):
+            if units is not None and (b, h) not in units:
+                continue
+            ref = _oracle_block(kv, p, cache, b, h, g, q, kb, vb, n_tok)
+            got = out[b, :, h * g:(h + 1) * g]
+            worst = max(worst, P.attn_rel_err(got.reshape(-1, 128), ref.reshape(-1, 128)))
+    assert worst <= P.ATTN_RTOL, worst
+    return worst
+
+
+def _inputs(B, Hq, Hkv, n_tok, n_q, seed, dtype=torch.bfloat16):
+    K, V = W.kv_tokens(B, Hkv, n_tok + n_q, seed=seed, device="cuda")
+    K, V = K.to(dtype), V.to(dtype)
+    q = torch.stack([W.queries(B, Hq, seed=seed * 131 + i, device="cuda") for i in range(n_q)], dim=1).to(dtype).contiguous()
+    return (K[:, :, :n_tok].contiguous(), V[:, :, :n_tok].contiguous(),
+            K[:, :, n_tok:].contiguous(), V[:, :, n_tok:].contiguous(), q)
+
+
+@pytest.mark.parametrize("bits", [2, 4])
+@pytest.mark.parametrize("Hq,Hkv,n_q", [(32, 8, 1), (32, 8, 2), (32, 8, 5), (8, 8, 8), (8, 8, 19), (16, 8, 7),
+                                         (64, 8, 3), (32, 8, 128)])
+def test_block_attention_vs_oracle(kv, bits, Hq, Hkv, n_q):
+    n_tok = 128 * 3 + 41
+    K, V, kb, vb, q = _inputs(2, Hq, Hkv, n_tok, n_q, seed=60 + n_q)
+    p = kv.default_params(bits)
+    cache = _cache(kv, p, K, V)
+    out = kv.block_attention(p, cache, q, kb, vb)
+    units = None if n_q <= 8 else {(0, 0), (1, Hkv - 1)}
+    _check(kv, p, cache, q, kb, vb, out, n_tok, units)
+
+
+@pytest.mark.parametrize("n_tok", [0, 1, 127, 128, 129, 256])
+def test_block_attention_ragged_and_empty_cache(kv, n_tok):
+    n_q = 6
+    K, V, kb, vb, q = _inputs(1, 16, 4, n_tok, n_q, seed=70 + n_tok)
+    p = kv.default_params(2)
+    cache = _cache(kv, p, K, V)
+    out = kv.block_attention(p, cache, q, kb, vb)
+    _check(kv, p, cache, q, kb, vb, out, n_tok)
+
+
+@pytest.mark.parametrize("splits", [1, 2, 5, 8])
+def test_block_attention_split_routes_and_sink(kv, splits):
+    n_tok, n_q = 32 + 128 * 9 + 100, 4
+    K, V, kb, vb, q = _inputs(2, 16, 4, n_tok, n_q, seed=80)
+    p = kv.default_params(2, splits=splits)
+    cache = _cache(kv, p, K, V, n_sink=32)
+    out = kv.block_attention(p, cache, q, kb, vb)
+    _check(kv, p, cache, q, kb, vb, out, n_tok)
+
+
+def test_block_of_one_equals_decode_after_append(kv):
+    """n_q = 1: attending [cache ; the new token] = kvarn_append then kvarn_decode_attention."""
+    n_tok = 128 * 4 + 17
+    K, V, kb, vb, q = _inputs(3, 32, 8, n_tok, 1, seed=90)
+    p = kv.default_params(2)
+    cache = _cache(kv, p, K, V)
+    out_blk = kv.block_attention(p, cache, q, kb, vb)
+    kv.append(p, cache, kb[:, :, 0].contiguous(), vb[:, :, 0].contiguous())
+    out_dec = kv.decode_attention(p, cache, q[:, 0].contiguous())
+    err = (out_blk[:, 0] - out_dec).abs().max().item() / out_dec.abs().max().item()
+    assert err <= 2e-4, err
+
+
+def test_block_attention_is_causal(kv):
+    """Changing block tokens j > i must leave the outputs of queries 0..i bit-identical."""
+    n_tok, n_q = 300, 8
+    K, V, kb, vb, q = _inputs(1, 16, 4, n_tok, n_q, seed=95)
+    p = kv.default_params(2)
+    cache = _cache(kv, p, K, V)
+    out = kv.block_attention(p, cache, q, kb, vb)
+    kb2, vb2 = kb.clone(), vb.clone()
+    kb2[:, :, 5:] *= 3.0
+    vb2[:, :, 5:] -= 7.0
+    out2 = kv.block_attention(p, cache, q, kb2, vb2)
+    assert torch.equal(out[:, :5], out2[:, :5])
+    assert not torch.equal(out[:, 5:], out2[:, 5:])
+
+
+def test_block_attention_rejects_bad_arguments(kv):
+    p = kv.default_params(2)
+    cache = kv.Cache(p, 1, 2, 2)
+    q = torch.zeros((1, 2, 6, 128), dtype=torch.bfloat16, device="cuda")      # g = 3: unsupported here
+    kb = torch.zeros((1, 2, 2, 128), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(kv.KvarnError, match="UNSUPPORTED"):
+        kv.block_attention(p, cache, q, kb, kb.clone())
