@@ -223,6 +223,21 @@ def run_extras(kv, W, dev, hbm_peak):
             byts = cache.nbytes_read_by_decode(sh.ctx) + sh.B * sh.Hq * (D * 2 + D * 4)
             ex[f"{name}_{bits}bit"] = {"us": med * 1e3, "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak,
                                        "bytes": byts, "B": sh.B, "Hq": sh.Hq, "Hkv": sh.Hkv, "ctx": sh.ctx}
+            if name == "decode_long_g4" and bits == 2:
+                # multi-token read path (Fig. 4): a block of n_q new tokens against the same cache
+                for n_q in (2, 8):
+                    qb = torch.stack([W.queries(sh.B, sh.Hq, seed=sh.seed + 100 + i, device=dev) for i in range(n_q)], dim=1).contiguous()
+                    kb, vb = W.kv_tokens(sh.B, sh.Hkv, n_q, seed=sh.seed + 200, device=dev, sink_first=False)
+                    ob = torch.empty((sh.B, n_q, sh.Hq, D), dtype=torch.float32, device=dev)
+                    for _ in range(3):
+                        kv.block_attention(p, cache, qb, kb, vb, out=ob)
+                    torch.cuda.synchronize()
+                    medb, _ = _time_launches(lambda i: kv.block_attention(p, cache, qb, kb, vb, out=ob), 10, stream)
+                    bb = cache.nbytes_read_by_decode(sh.ctx) + sh.B * n_q * (sh.Hq * (D * 2 + D * 4) + 2 * sh.Hkv * D * 2)
+                    ex[f"block_long_g4_2bit_nq{n_q}"] = {"us": medb * 1e3, "us_per_query_token": medb * 1e3 / n_q,
+                                                         "GBps": bb / medb / 1e6, "hbm_frac": bb / medb / 1e6 / hbm_peak,
+                                                         "bytes": bb, "n_q": n_q, "vs_single_token_decode": medb / med}
+                    del qb, kb, vb, ob
             del cache, q, ws, out
             torch.cuda.empty_cache()
     # the paper's three-region layout: S = 128 raw sink tokens in front of the quantised body
@@ -294,6 +309,21 @@ def run_extras(kv, W, dev, hbm_peak):
                                           "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak,
                                           "alu_frac": 2 * n_tiles * QUANT_FLOPS_PER_TILE / (med * 1e-3) / 1e12 / FP32_PEAK_TFLOPS_NOMINAL}
         del kr, vr
+    # the paper's own write-path measurement (Sec. 4.2): "8 iterations of variance-normalization in every
+    # attention layer in Qwen3-4B" for one 128-token chunk = 36 layers x 8 KV heads x {K, V} = 576 tiles, one launch.
+    # Paper: 1.9 ms on "a GPU with 500 TFLOP at fp16 and 1.8 TB/s" (normalisation only; ours is the whole record). Context only.
+    n_lat = 36 * 8
+    p = kv.default_params(2)
+    rb = kv.record_bytes(p)
+    kr = torch.empty((n_lat, rb), dtype=torch.uint8, device=dev); vr = torch.empty_like(kr)
+    srcs = [(Kt[i * n_lat:(i + 1) * n_lat], Vt[i * n_lat:(i + 1) * n_lat]) for i in range(64)]   # 64 distinct inputs (> L2 in total)
+    for i in range(3):
+        kv.quantize_chunk(p, srcs[i][0], srcs[i][1], kr, vr)
+    torch.cuda.synchronize()
+    med, mn = _time_launches(lambda i: kv.quantize_chunk(p, srcs[i % 64][0], srcs[i % 64][1], kr, vr), 64, stream)
+    ex["quantize_latency_qwen3_4b_chunk"] = {"us": med * 1e3, "min_us": mn * 1e3, "tiles": 2 * n_lat,
+                                             "paper_ms_other_hw": 1.9, "note": "576 tiles in one launch (2 waves of 296 resident CTAs); P:159"}
+    del kr, vr
     return ex
 
 
