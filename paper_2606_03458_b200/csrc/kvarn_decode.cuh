@@ -309,7 +309,9 @@ template <int BITS, int GP, int NCH, typename InT>
 #ifndef KVARN_DEC_OCC8
 #define KVARN_DEC_OCC8 4
 #endif
-__global__ void __launch_bounds__(128, (GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8) / NCH) decode_kernel(const DecodeArgs A) {
+// GP = 4: four resident CTAs per SM with either NCH (128 registers; the two-chunk variant's 55.6 KB of shared memory
+// fits four times in 228 KB) -- with three, the 64k-context case drops from 195 to 213 us
+__global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8 / NCH) decode_kernel(const DecodeArgs A) {
   using SM = DecSmem<BITS, GP, NCH>;
   constexpr int RB = SM::RB, STAGES = SM::STAGES, NT = SM::NT;
   constexpr int NCLS = 8 / BITS;
