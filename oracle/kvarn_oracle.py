@@ -277,14 +277,46 @@ class QuantTile:
     varn: VarNResult
 
 
+def rtn_quantize_stored(X: np.ndarray, bits: int, group_axis: int, absorbed: np.ndarray):
+    """RTN against the STORED parameters ("round-before", reading R9b; P:382 stores s1 as FP8 and z as FP16,
+    the paper does not say whether the codes are taken before or after that rounding).
+
+    Per group: mn, mx, s = (mx - mn) / Lv as in ``rtn_quantize``; the scale that will be stored is
+    s1 = fp8(s * absorbed) (``absorbed`` = the Sinkhorn scale constant along the group, R8), so the step the
+    dequantiser really applies, in units of X, is s' = s1 / absorbed; z = fp16(mn / s');
+    codes = clip(rint(x / s' - z), 0, Lv).  A group whose s1 rounds to zero keeps s' = s.
+    Returns (codes, s1 (stored), z (stored), s1_f = s * absorbed, z_f = mn / s')."""
+    X = np.asarray(X, dtype=np.float64)
+    Lv = (1 << bits) - 1
+    ab = np.expand_dims(np.asarray(absorbed, dtype=np.float64), group_axis)
+    mn = X.min(axis=group_axis, keepdims=True)
+    mx = X.max(axis=group_axis, keepdims=True)
+    rng = mx - mn
+    degenerate = rng < RTN_DEGENERATE
+    s = np.where(degenerate, 1.0, rng / Lv)
+    s1_f = s * ab
+    s1 = round_fp8_e4m3(s1_f)
+    s_used = np.where(s1 > 0, s1 / ab, s)
+    z_f = mn / s_used
+    z = round_fp16(z_f)
+    codes = np.clip(np.rint(X / s_used - z), 0, Lv)
+    codes = np.where(degenerate, 0.0, codes).astype(np.uint8)
+    sq = lambda a: np.squeeze(a, axis=group_axis)
+    return codes, sq(s1), sq(z), sq(s1_f), sq(z_f)
+
+
 def quantize_tile(X: np.ndarray, kind: str, bits: int = 2, iters: int = VARN_ITERS,
                   rotate_on: bool = True, at_k: int | None = None,
-                  c_min: float = VARN_C_MIN, c_max: float = VARN_C_MAX) -> QuantTile:
+                  c_min: float = VARN_C_MIN, c_max: float = VARN_C_MAX,
+                  aux_round: str = "after") -> QuantTile:
     """Hadamard -> VarN -> RTN -> aux rounding, for one tile X[t, c] (128 x 128).
 
     kind 'k': RTN groups are channels (each over the chunk's tokens);
     kind 'v': RTN groups are tokens (each over the channels).
     ``at_k`` forces the iterate used (reading R10); default = Alg. 1's choice.
+    ``aux_round``: "after" (default, reading R9: codes from the unrounded parameters, aux rounded for
+    storage afterwards) or "before" (R9b: the second scale is rounded to FP8 first, the tile is balanced
+    with the rounded value, and RTN runs against the stored s1 / z -- ``rtn_quantize_stored``).
     """
     assert kind in ("k", "v")
     X = np.asarray(X, dtype=np.float64)
@@ -298,6 +330,18 @@ def quantize_tile(X: np.ndarray, kind: str, bits: int = 2, iters: int = VARN_ITE
     else:
         T_bal, S_c, S_r = varn_at(T, vr, at_k)
         k = at_k
+    if aux_round == "before":
+        if kind == "k":      # second scale = S_c (per token), absorbed = S_r (per channel)
+            s2 = round_fp8_e4m3(S_c)
+            codes_ct, s1, z, s1_f, z_f = rtn_quantize_stored(T / s2[None, :] / S_r[:, None], bits, 1, S_r)
+            s2_f = S_c
+        else:                # second scale = S_r (per channel), absorbed = S_c (per token)
+            s2 = round_fp8_e4m3(S_r)
+            codes_ct, s1, z, s1_f, z_f = rtn_quantize_stored(T / S_c[None, :] / s2[:, None], bits, 0, S_c)
+            s2_f = S_r
+        return QuantTile(kind=kind, bits=bits, codes=np.ascontiguousarray(codes_ct.T), s1=s1, s2=s2, z=z,
+                         s1_f=s1_f, s2_f=s2_f, z_f=z_f, k_best=k, varn=vr)
+    assert aux_round == "after"
     # step 3: RTN on the balanced tile.  T_bal is [channel, token].
     if kind == "k":      # per channel: group runs along tokens (axis 1)
         codes_ct, s, z = rtn_quantize(T_bal, bits, group_axis=1)
