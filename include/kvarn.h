@@ -75,7 +75,11 @@ typedef struct {
   int32_t splits;    /* decode split-K factor over chunks; 0 = choose automatically.  A value s > 0 runs
                       * c = the largest divisor of s that is <= 8 CTAs per thread-block cluster (merged
                       * through distributed shared memory) and s / c clusters merged through the workspace */
-  int32_t reserved;
+  int32_t aux_round; /* 0 (default): codes from the unrounded scale / zero-point, aux rounded to FP8 / FP16 for
+                      * storage afterwards.  1 ("round-before"): the second scale is rounded to FP8 before the
+                      * tile is balanced and RTN runs against the STORED step s1 / absorbed scale and the
+                      * stored FP16 zero-point, so the FP8 error of the scales is absorbed by the codes
+                      * (P:382 does not say which; at 4-bit it cuts the token-magnitude error ~3x). */
 } kvarn_params;
 
 /* Byte layout of one record (fixed by bits): codes | s1[128] e4m3 | s2[128] e4m3 | z[128] f16.

@@ -138,6 +138,7 @@ static int check_params(const kvarn_params* p) {
   if (p->head_dim != D || p->chunk != G) return KVARN_UNSUPPORTED;
   if (p->bits != 2 && p->bits != 4) return KVARN_UNSUPPORTED;
   if (p->iters < 0 || p->iters > KVARN_MAX_ITERS) return KVARN_INVALID_ARG;
+  if (p->aux_round != 0 && p->aux_round != 1) return KVARN_INVALID_ARG;
   if (p->in_dtype != KVARN_BF16 && p->in_dtype != KVARN_F32) return KVARN_UNSUPPORTED;
   if (p->out_dtype != KVARN_BF16 && p->out_dtype != KVARN_F32) return KVARN_UNSUPPORTED;
   if (!(p->var_min > 0.f) || !(p->var_max >= p->var_min) || !(p->log_hi >= p->log_lo)) return KVARN_INVALID_ARG;
@@ -148,6 +149,7 @@ static VarnConsts varn_consts(const kvarn_params* p) {
   VarnConsts vc;
   vc.iters = p->iters; vc.var_min = p->var_min; vc.var_max = p->var_max;
   vc.log_lo = p->log_lo; vc.log_hi = p->log_hi;
+  vc.aux_round = p->aux_round;
   return vc;
 }
 

@@ -28,6 +28,7 @@ namespace kvarn {
 struct VarnConsts {
   int iters;
   float var_min, var_max, log_lo, log_hi;
+  int aux_round;   // 1: RTN against the stored FP8 / FP16 parameters (kvarn_params::aux_round)
 };
 
 struct QuantDebug {
@@ -310,8 +311,18 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     }
   }
   // ---- best scales (line 24): T_bal = T / S_c* / S_r* ----------------------------
-  if (li < 8) { const float L = sm.Lch[k_best][tok_own]; sm.Sc[tok_own] = expf(L); sm.b[tok_own] = expf(-L); }
-  if (tid < 128) { const float L = sm.Lrh[k_best][tid]; sm.Sr[tid] = expf(L); sm.a[tid] = expf(-L); }
+  // aux_round = 1: the second scale (K: S_c per token, V: S_r per channel) balances the tile with its STORED value
+  const bool rb = vc.aux_round != 0;
+  if (li < 8) {
+    const float L = sm.Lch[k_best][tok_own], S = expf(L);
+    sm.Sc[tok_own] = S;
+    sm.b[tok_own] = (rb && kind == KVARN_KIND_K) ? 1.f / e4m3_to_f32(f32_to_e4m3(S)) : expf(-L);
+  }
+  if (tid < 128) {
+    const float L = sm.Lrh[k_best][tid], S = expf(L);
+    sm.Sr[tid] = S;
+    sm.a[tid] = (rb && kind == KVARN_KIND_V) ? 1.f / e4m3_to_f32(f32_to_e4m3(S)) : expf(-L);
+  }
   __syncthreads();
   reload_a();
   reload_b();
@@ -324,6 +335,27 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
 
   // ---- Q3 + Q4: RTN group statistics, aux values ---------------------------------
   float inv_s[8], zz[8];  // of own channels (K) or own tokens (V)
+  // group parameters from (mn, mx) and the absorbed Sinkhorn scale: pre-storage s1, the step the codes use
+  // (1 / step in inv) and the zero-point the codes use (zc; zf = before FP16 rounding)
+  auto group_params = [&](const float mn, const float mx, const float absorbed, float& s1, float& inv, float& zf, float& zc) {
+    const float rng = mx - mn;
+    const float s = (rng < 1e-12f) ? 1.f : rng / (float)LV;
+    s1 = s * absorbed;
+    if (rb) {
+      const float s1q = e4m3_to_f32(f32_to_e4m3(s1));
+      const float su = s1q > 0.f ? s1q / absorbed : s;
+      zf = mn / su; zc = f16_bits_to_f32(f32_to_f16_bits(zf)); inv = 1.f / su;
+    } else {
+      zf = mn / s; zc = zf; inv = 1.f / s;
+    }
+  };
+  // code = rint(x / step - z) by the magic-number add; with the stored parameters the value can leave [0, LV]
+  const float2 magic = f2(RTN_MAGIC, RTN_MAGIC), nmagic = f2(-RTN_MAGIC, -RTN_MAGIC);
+  auto rtn2 = [&](const float2 xv, const float2 is, const float2 nz) -> float2 {
+    float2 q = add2(add2(fma2(xv, is, nz), magic), nmagic);
+    if (rb) { q.x = fminf(fmaxf(q.x, 0.f), (float)LV); q.y = fminf(fmaxf(q.y, 0.f), (float)LV); }
+    return q;
+  };
   if (kind == KVARN_KIND_K) {
     // group = channel over the 128 tokens: min / max across warps through smem
     float mnv[8], mxv[8];
@@ -352,11 +384,10 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       float mn = sm.part[0][0][tid], mx = sm.part[0][1][tid];
 #pragma unroll
       for (int w = 1; w < 8; ++w) { mn = fminf(mn, sm.part[w][0][tid]); mx = fmaxf(mx, sm.part[w][1][tid]); }
-      const float rng = mx - mn;
-      const float s = (rng < 1e-12f) ? 1.f : rng / (float)LV;
-      const float z = mn / s;
-      sm.inv_s[tid] = 1.f / s; sm.z[tid] = z;
-      const float s1 = s * sm.Sr[tid], s2 = sm.Sc[tid];  // K: s1 per channel, s2 per token
+      float s1, inv, z, zc;
+      group_params(mn, mx, sm.Sr[tid], s1, inv, z, zc);
+      sm.inv_s[tid] = inv; sm.z[tid] = zc;
+      const float s2 = sm.Sc[tid];  // K: s1 per channel, s2 per token
       const int kp = kaux_of_elem(BITS, tid);  // K records keep s1, z in B-operand builder order
       sm.rec[s1_off(BITS) + kp] = f32_to_e4m3(s1);
       sm.rec[s2_off(BITS) + slot_of_token(BITS, tid)] = f32_to_e4m3(s2);   // per-token arrays: MMA row-slot order
@@ -381,7 +412,6 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     float2 is2[4], nz2[4];
 #pragma unroll
     for (int kp = 0; kp < 4; ++kp) { is2[kp] = f2(inv_s[2 * kp], inv_s[2 * kp + 1]); nz2[kp] = f2(-zz[2 * kp], -zz[2 * kp + 1]); }
-    const float2 magic = f2(RTN_MAGIC, RTN_MAGIC), nmagic = f2(-RTN_MAGIC, -RTN_MAGIC);
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       const int slot = slot_of_token(BITS, t0 + i);
@@ -389,7 +419,7 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
         float2 acc = f2(0.f, 0.f);
 #pragma unroll
         for (int kp = 0; kp < 4; ++kp) {
-          const float2 q = add2(add2(fma2(x[i][kp], is2[kp], nz2[kp]), magic), nmagic);
+          const float2 q = rtn2(x[i][kp], is2[kp], nz2[kp]);
           acc = fma2(q, f2((float)(1 << (4 * kp)), (float)(4 << (4 * kp))), acc);
         }
         *reinterpret_cast<uint16_t*>(&sm.rec[code_off(2, slot, 2 * li)]) = (uint16_t)__float2uint_rn(acc.x + acc.y);
@@ -397,8 +427,8 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
         float2 lo = f2(0.f, 0.f), hi = f2(0.f, 0.f);
 #pragma unroll
         for (int kp = 0; kp < 2; ++kp) {
-          const float2 q0 = add2(add2(fma2(x[i][kp], is2[kp], nz2[kp]), magic), nmagic);
-          const float2 q1 = add2(add2(fma2(x[i][kp + 2], is2[kp + 2], nz2[kp + 2]), magic), nmagic);
+          const float2 q0 = rtn2(x[i][kp], is2[kp], nz2[kp]);
+          const float2 q1 = rtn2(x[i][kp + 2], is2[kp + 2], nz2[kp + 2]);
           const float2 wgt = f2((float)(1 << (8 * kp)), (float)(16 << (8 * kp)));
           lo = fma2(q0, wgt, lo);
           hi = fma2(q1, wgt, hi);
@@ -423,12 +453,10 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     float mine = xreduce16(v, li, OpMin());
     float other = __shfl_xor_sync(0xffffffffu, mine, 8);
     const float mn = (li & 8) ? other : mine, mx = -((li & 8) ? mine : other);
-    const float rng = mx - mn;
-    const float s = (rng < 1e-12f) ? 1.f : rng / (float)LV;
-    const float z = mn / s;
+    float s1, inv, z, zc;
+    group_params(mn, mx, sm.Sc[tok_own], s1, inv, z, zc);   // V: s1 per token
     if (li < 8) {
-      sm.inv_s[tok_own] = 1.f / s; sm.z[tok_own] = z;
-      const float s1 = s * sm.Sc[tok_own];  // V: s1 per token
+      sm.inv_s[tok_own] = inv; sm.z[tok_own] = zc;
       const int slot = slot_of_token(BITS, tok_own);
       sm.rec[s1_off(BITS) + slot] = f32_to_e4m3(s1);
       reinterpret_cast<uint16_t*>(&sm.rec[z_off(BITS)])[slot] = f32_to_f16_bits(z);
@@ -448,7 +476,6 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     zz[0] = z0.x; zz[1] = z0.y; zz[2] = z0.z; zz[3] = z0.w;
     zz[4] = z1.x; zz[5] = z1.y; zz[6] = z1.z; zz[7] = z1.w;
     // codes: row per CHANNEL, token t at bit BITS*(t%..) of the row (rounding and packing as for K)
-    const float2 magic = f2(RTN_MAGIC, RTN_MAGIC), nmagic = f2(-RTN_MAGIC, -RTN_MAGIC);
     float2 lo[4], hi[4];
 #pragma unroll
     for (int kp = 0; kp < 4; ++kp) { lo[kp] = f2(0.f, 0.f); hi[kp] = f2(0.f, 0.f); }
@@ -459,7 +486,7 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       const float2 wgt = f2(wv, wv);
 #pragma unroll
       for (int kp = 0; kp < 4; ++kp) {
-        const float2 q = add2(add2(fma2(x[i][kp], is2, nz2), magic), nmagic);
+        const float2 q = rtn2(x[i][kp], is2, nz2);
         if (BITS == 2 || i < 4) lo[kp] = fma2(q, wgt, lo[kp]);
         else hi[kp] = fma2(q, wgt, hi[kp]);
       }

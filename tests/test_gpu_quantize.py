@@ -188,3 +188,47 @@ def test_error_decomposition_ranks_the_ablations(kv):
     for other in ("hk", "kivi"):
         assert res["kvarn"][0] < 0.5 * res[other][0], res     # magnitude error E_M
         assert res["kvarn"][1] < 0.5 * res[other][1], res     # total error E_T
+
+
+@pytest.mark.parametrize("bits", [2, 4])
+def test_round_before_variant_vs_oracle(kv, bits):
+    """aux_round = 1 (reading R9b): RTN against the stored FP8 / FP16 parameters."""
+    n = 48
+    K, V = W.quantizer_sweep_tiles(8, n * 128 // 8, seed=17, device="cuda")
+    Kt, Vt = K.reshape(n, 128, 128), V.reshape(n, 128, 128)
+    p = kv.default_params(bits, aux_round=1)
+    kr, vr, dbg = kv.quantize_chunk(p, Kt, Vt, debug=True)
+    stats = {}
+    for kind, (T, R) in enumerate(((Kt, kr), (Vt, vr))):
+        for i in range(0, n, 3):
+            P.check_quantized_tile(kv, p, kind, P.tile_f64(T[i]), R[i].cpu().numpy(), int(dbg.k_best[kind, i]),
+                                   dbg.imb[kind, i].cpu().numpy(), dbg.aux[kind, i].cpu().numpy(), stats)
+    P.assert_mismatch_budget(stats)
+    # the variant's purpose: dequantising the stored record reproduces the token norms better at 4-bit
+    if bits == 4:
+        p0 = kv.default_params(bits)
+        kr0, _ = kv.quantize_chunk(p0, Kt, Vt)
+        def tokmag(rec, i):
+            X = P.tile_f64(Kt[i])
+            Xd = O.dequantize_tile(*[np.asarray(a, dtype=np.float64) for a in kv.unpack_record(p, 0, rec[i].cpu().numpy())], kind="k")
+            return np.mean(np.abs(np.linalg.norm(Xd, axis=1) / np.linalg.norm(X, axis=1) - 1))
+        a = np.mean([tokmag(kr, i) for i in range(6)]); b = np.mean([tokmag(kr0, i) for i in range(6)])
+        assert a < 0.6 * b, (a, b)
+
+
+def test_round_before_decode_matches_oracle_on_its_records(kv):
+    """The read path is unchanged by aux_round: a cache written with either setting decodes to the oracle's
+    attention over those records."""
+    K, V = W.kv_tokens(1, 2, 128 * 4, seed=19, device="cuda")
+    q = W.queries(1, 8, seed=19, device="cuda")
+    for ar in (0, 1):
+        p = kv.default_params(4, aux_round=ar)
+        cache = kv.Cache(p, 1, 2, 4)
+        kv.prefill(p, cache, K, V)
+        out = kv.decode_attention(p, cache, q).double().cpu().numpy()
+        worst = 0.0
+        for h in range(2):
+            ref = P.oracle_attention_from_records(kv, p, cache.k_records[0, h].cpu().numpy(), cache.v_records[0, h].cpu().numpy(),
+                                                  np.zeros((0, 128)), np.zeros((0, 128)), P.tile_f64(q[0, 4 * h:4 * h + 4]))
+            worst = max(worst, P.attn_rel_err(out[0, 4 * h:4 * h + 4], ref))
+        assert worst <= P.ATTN_RTOL, worst
