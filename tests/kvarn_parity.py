@@ -40,7 +40,9 @@ def check_quantized_tile(kv, p, kind: int, X: np.ndarray, rec: np.ndarray, k_gpu
     assert np.allclose(s1_f, ref.s1_f, rtol=SCALE_RTOL, atol=0), np.abs(s1_f / ref.s1_f - 1).max()
     assert np.allclose(s2_f, ref.s2_f, rtol=SCALE_RTOL, atol=0), np.abs(s2_f / ref.s2_f - 1).max()
     # z = mn / s is O(1..10) in code units; tolerance relative to the code range
-    assert np.allclose(z_f, ref.z_f, rtol=SCALE_RTOL, atol=SCALE_RTOL * (1 << p.bits)), np.abs(z_f - ref.z_f).max()
+    # (R9b: z = mn / stored step, so it is only comparable where the stored s1 agrees -- an FP8 tie moves it by 6 %)
+    zcmp = (s1 == ref.s1) if p.aux_round else np.ones(128, dtype=bool)
+    assert np.allclose(z_f[zcmp], ref.z_f[zcmp], rtol=SCALE_RTOL, atol=SCALE_RTOL * (1 << p.bits)), np.abs(z_f - ref.z_f)[zcmp].max()
     # (4) stored bytes = storage rounding of the kernel's own fp32 values
     st_mis = int((s1.astype(np.float64) != O.round_fp8_e4m3(s1_f)).sum()
                  + (s2.astype(np.float64) != O.round_fp8_e4m3(s2_f)).sum()
