@@ -32,6 +32,8 @@ attention ................ pinned (brute-force loops, torch SDPA, invariances)
 cache_partition .......... pinned (brute-force token walk, P:350's S/G/R settings)
 block_attention .......... pinned (brute-force loops, torch SDPA with a causal mask,
                            n_q = 1 and last-query special cases)
+rope_hadamard / absorb_hadamard ... pinned (complex-number form of RoPE, relative-position
+                           invariance, q.k and a W_O preserved by the rotations)
 codes / scales of a tile vs values printed by the paper ... **parity unpinned**:
                            the paper prints no intermediate value for any tile.
 """
@@ -474,6 +476,39 @@ def block_attention(q_blk: np.ndarray, k_tiles: list, v_tiles: list,
                                   np.concatenate([k_raw, k_blk[:i + 1]], axis=0),
                                   np.concatenate([v_raw, v_blk[:i + 1]], axis=0), sm_scale=sm_scale)
     return out
+
+
+# --------------------------------------------------------------------------
+# Hadamard arrangement around the attention layer (App. A, Fig. 7)
+# --------------------------------------------------------------------------
+def rope_rotate_half(x: np.ndarray, cos: np.ndarray, sin: np.ndarray) -> np.ndarray:
+    """Rotary embedding in the half-split convention of the Llama / Qwen models the paper evaluates:
+    channel c < d/2 is paired with c + d/2;  y[c] = x[c] cos[c] - x[c+d/2] sin[c],
+    y[c+d/2] = x[c+d/2] cos[c] + x[c] sin[c].  x: (..., d); cos, sin: (..., d/2) broadcastable.
+    The paper only says the online transforms come "after the RoPE-embedding"; the caller
+    supplies the cos / sin table, so no frequency base is fixed here."""
+    x = np.asarray(x, dtype=np.float64)
+    h = x.shape[-1] // 2
+    x1, x2 = x[..., :h], x[..., h:]
+    return np.concatenate([x1 * cos - x2 * sin, x2 * cos + x1 * sin], axis=-1)
+
+
+def rope_hadamard(x: np.ndarray, cos: np.ndarray, sin: np.ndarray) -> np.ndarray:
+    """The online transform of q and K ("two online transforms after the RoPE-embedding ...
+    head-wise"): y = RoPE(x) H / sqrt(d) per head.  x: (..., d)."""
+    return rotate(rope_rotate_half(x, cos, sin))
+
+
+def absorb_hadamard(W_V: np.ndarray, W_O: np.ndarray, d: int = HEAD_DIM):
+    """The two absorbed transforms ("merged with W_V and W_O respectively and do not need to be
+    computed during inference").  With v = x W_V (W_V: (d_model, Hkv d)) and out = a W_O
+    (W_O: (Hq d, d_model)), block-diagonal R = diag(H / sqrt(d)):  W_V' = W_V R,  W_O' = R^T W_O, so that
+    v' = v R per head is what gets quantised (rotate_v = 0 at run time) and a' W_O' = a W_O."""
+    W_V = np.asarray(W_V, dtype=np.float64); W_O = np.asarray(W_O, dtype=np.float64)
+    R = hadamard_matrix(d) / np.sqrt(d)
+    Wv = W_V.reshape(W_V.shape[0], -1, d) @ R
+    Wo = np.einsum("ij,hjm->him", R.T, W_O.reshape(-1, d, W_O.shape[1]))
+    return Wv.reshape(W_V.shape), Wo.reshape(W_O.shape)
 
 
 # --------------------------------------------------------------------------

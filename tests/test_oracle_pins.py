@@ -576,3 +576,51 @@ def test_round_before_lowers_the_4bit_error():
     for kind in "kv":
         assert tokmag(4, "before", kind) < 0.5 * tokmag(4, "after", kind)
         assert abs(tokmag(2, "before", kind) / tokmag(2, "after", kind) - 1) < 0.3
+
+
+# ---- Hadamard arrangement (App. A): online q / K transform after RoPE, absorbed W_V / W_O ----
+def _rope_table(pos, d=128, base=10000.0):
+    inv = base ** (-np.arange(0, d, 2) / d)
+    ang = np.asarray(pos, dtype=np.float64)[:, None] * inv[None, :]
+    return np.cos(ang), np.sin(ang)
+
+
+def test_rope_is_a_complex_rotation_and_relative():
+    """Pin: the half-split RoPE is multiplication of z_c = x[c] + i x[c + d/2] by e^{i angle_c} (textbook form),
+    preserves norms, and q(m) . k(n) depends only on m - n."""
+    rng = np.random.default_rng(41)
+    x = rng.standard_normal((5, 128)); pos = np.array([0, 1, 7, 100, 4095])
+    cos, sin = _rope_table(pos)
+    y = O.rope_rotate_half(x, cos, sin)
+    zc = (x[:, :64] + 1j * x[:, 64:]) * (cos + 1j * sin)
+    assert np.allclose(y[:, :64], zc.real, atol=1e-12) and np.allclose(y[:, 64:], zc.imag, atol=1e-12)
+    assert np.allclose(np.linalg.norm(y, axis=1), np.linalg.norm(x, axis=1))
+    q, k = rng.standard_normal(128), rng.standard_normal(128)
+    def dot(m, n):
+        cm, sm_ = _rope_table([m]); cn, sn = _rope_table([n])
+        return float(O.rope_rotate_half(q[None], cm, sm_)[0] @ O.rope_rotate_half(k[None], cn, sn)[0])
+    assert np.isclose(dot(10, 3), dot(1010, 1003)) and not np.isclose(dot(10, 3), dot(10, 4))
+
+
+def test_rope_hadamard_preserves_attention_logits():
+    rng = np.random.default_rng(42)
+    q, k = rng.standard_normal((3, 128)), rng.standard_normal((9, 128))
+    cq, sq = _rope_table([20, 21, 22]); ck, sk = _rope_table(np.arange(9))
+    plain = O.rope_rotate_half(q, cq, sq) @ O.rope_rotate_half(k, ck, sk).T
+    assert np.allclose(O.rope_hadamard(q, cq, sq) @ O.rope_hadamard(k, ck, sk).T, plain, atol=1e-10)
+
+
+def test_absorbed_hadamards_cancel():
+    """the transforms merged into W_V and W_O leave the layer's function unchanged:
+    softmax(.) (x W_V') W_O' = softmax(.) (x W_V) W_O for any attention weights (GQA: Hq = 2 Hkv here)."""
+    rng = np.random.default_rng(43)
+    dm, Hkv, Hq = 48, 2, 4
+    W_V, W_O = rng.standard_normal((dm, Hkv * 128)), rng.standard_normal((Hq * 128, dm))
+    Wv2, Wo2 = O.absorb_hadamard(W_V, W_O)
+    x = rng.standard_normal((7, dm)); P_ = rng.random((Hq, 7)); P_ /= P_.sum(1, keepdims=True)
+    def layer(Wv, Wo):
+        v = (x @ Wv).reshape(7, Hkv, 128)
+        a = np.concatenate([P_[h] @ v[:, h // 2] for h in range(Hq)])      # (Hq * 128,)
+        return a @ Wo
+    assert np.allclose(layer(Wv2, Wo2), layer(W_V, W_O), atol=1e-9)
+    assert np.allclose((x @ Wv2).reshape(7, Hkv, 128), O.rotate((x @ W_V).reshape(7, Hkv, 128)), atol=1e-10)
