@@ -328,8 +328,8 @@ def run_extras(kv, W, dev, hbm_peak):
 
 
 def stored_traffic():
-    """dram bytes per launch of the two kernels, from the committed ncu --set full capture (profiles/r01b_traffic.md)."""
-    path = os.path.join(ROOT, "profiles", "r01b_traffic.csv")
+    """dram bytes per launch of the two kernels, from the committed ncu --set full capture (profiles/r01c_traffic.md)."""
+    path = os.path.join(ROOT, "profiles", "r01c_traffic.csv")
     out = {}
     try:
         for line in open(path).read().splitlines()[1:]:
