@@ -323,7 +323,22 @@ def run_extras(kv, W, dev, hbm_peak):
     med, mn = _time_launches(lambda i: kv.quantize_chunk(p, srcs[i % 64][0], srcs[i % 64][1], kr, vr), 64, stream)
     ex["quantize_latency_qwen3_4b_chunk"] = {"us": med * 1e3, "min_us": mn * 1e3, "tiles": 2 * n_lat,
                                              "paper_ms_other_hw": 1.9, "note": "576 tiles in one launch (2 waves of 296 resident CTAs); P:159"}
-    del kr, vr
+    del kr, vr, Kt, Vt, K, V, srcs
+    torch.cuda.empty_cache()
+    # App. A online transform fused with RoPE: K of 2^18 tokens x 8 heads, bf16; streaming kernel
+    n_rt, h_rt = 1 << 18, 8
+    xk = torch.randn((n_rt, h_rt, D), device=dev, dtype=torch.bfloat16)
+    ang = torch.arange(n_rt, device=dev, dtype=torch.float32)[:, None] * (10000.0 ** (-torch.arange(0, D, 2, device=dev, dtype=torch.float32) / D))[None, :]
+    ct, st = torch.cos(ang).contiguous(), torch.sin(ang).contiguous()
+    yk = torch.empty_like(xk)
+    for _ in range(2):
+        kv.rope_hadamard(xk, ct, st, out=yk)
+    torch.cuda.synchronize()
+    med, mn = _time_launches(lambda i: kv.rope_hadamard(xk, ct, st, out=yk), 10, stream)
+    byts = 2 * xk.numel() * 2 + 2 * ct.numel() * 4
+    ex["rope_hadamard_bf16"] = {"ms": med, "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak, "bytes": byts,
+                                "n_tok": n_rt, "n_heads": h_rt}
+    del xk, yk, ct, st, ang
     return ex
 
 

@@ -228,6 +228,28 @@ KVARN_API int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* ca
                           float sm_scale, void* out, void* stream);
 
 /*
+ * The Hadamard arrangement around the attention layer (App. A: "two absorbed transforms (that are
+ * merged with W_V and W_O respectively ...) and two online transforms after the RoPE-embedding.  The two online
+ * transforms are head-wise").  With these a model can produce q, K and V already rotated and run the cache with
+ * rotate_k = rotate_v = 0.  All pointers DEVICE; in place (y == x, out == w) is allowed; dtype = kvarn_dtype.
+ *
+ * kvarn_rope_hadamard -- the online transform of q or K fused with the rotary embedding:
+ *   y[t][h][:] = RoPE(x[t][h][:]) H / sqrt(128),  x, y [n_tok][n_heads][128], 16-B aligned.
+ *   cos_tab, sin_tab: fp32 [n_tok][64] of the token's position, half-split convention (channel c < 64 pairs with
+ *   c + 64: y[c] = x[c] cos[c] - x[c+64] sin[c], y[c+64] = x[c+64] cos[c] + x[c] sin[c]); both null = no RoPE.
+ *   rotate = 0 applies the rotary embedding only.
+ * kvarn_hadamard_rows -- every 128-element group of a contiguous array rotated (x [n_groups][128]): the absorbed
+ *   transform of W_V stored [d_model][Hkv*128] (W_V' = W_V R), or a plain online rotation.
+ * kvarn_hadamard_row_groups -- W' = R^T W for row-major W [n_rows][n_cols], n_rows a multiple of 128: each group
+ *   of 128 consecutive rows is rotated down the columns: the absorbed transform of W_O stored [Hq*128][d_model].
+ */
+KVARN_API int kvarn_rope_hadamard(const void* x, const float* cos_tab, const float* sin_tab, void* y, int64_t n_tok,
+                        int32_t n_heads, int32_t dtype, int32_t rotate, void* stream);
+KVARN_API int kvarn_hadamard_rows(const void* x, void* y, int64_t n_groups, int32_t dtype, void* stream);
+KVARN_API int kvarn_hadamard_row_groups(const void* w, void* out, int64_t n_rows, int64_t n_cols, int32_t dtype,
+                              void* stream);
+
+/*
  * Host-buffer forms (end-to-end measurement; HOST pointers in, HOST out).
  * They copy host->device into caller-provided DEVICE staging, run the device
  * call above and copy the result back, all enqueued on `stream`; the caller

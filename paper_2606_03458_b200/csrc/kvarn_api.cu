@@ -5,6 +5,7 @@
 
 #include "kvarn_common.cuh"
 #include "kvarn_decode.cuh"
+#include "kvarn_rotate.cuh"
 #include "kvarn_quantize.cuh"
 
 namespace kvarn {
@@ -495,6 +496,40 @@ int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* cache, const
   if (p->bits == 2) e = f32 ? launch_decode<2, float>(A, s) : launch_decode<2, __nv_bfloat16>(A, s);
   else e = f32 ? launch_decode<4, float>(A, s) : launch_decode<4, __nv_bfloat16>(A, s);
   return e == cudaSuccess ? KVARN_OK : KVARN_CUDA;
+}
+
+int kvarn_rope_hadamard(const void* x, const float* cos_tab, const float* sin_tab, void* y, int64_t n_tok,
+                        int32_t n_heads, int32_t dtype, int32_t rotate, void* stream) {
+  if (n_tok == 0) return KVARN_OK;
+  if (!x || !y || n_tok < 0 || n_heads <= 0 || (!cos_tab) != (!sin_tab)) return KVARN_INVALID_ARG;
+  if (dtype != KVARN_BF16 && dtype != KVARN_F32) return KVARN_UNSUPPORTED;
+  if (!aligned16(x) || !aligned16(y) || !aligned16(cos_tab) || !aligned16(sin_tab)) return KVARN_MISALIGNED;
+  const long long n_groups = (long long)n_tok * n_heads;
+  if (n_groups == 0) return KVARN_OK;
+  const unsigned grid = (unsigned)((n_groups + 7) / 8);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (dtype == KVARN_F32)
+    rope_hadamard_kernel<float><<<grid, 256, 0, s>>>((const float*)x, cos_tab, sin_tab, (float*)y, n_groups, n_heads, rotate);
+  else
+    rope_hadamard_kernel<__nv_bfloat16><<<grid, 256, 0, s>>>((const __nv_bfloat16*)x, cos_tab, sin_tab, (__nv_bfloat16*)y,
+                                                          n_groups, n_heads, rotate);
+  return last_cuda();
+}
+
+int kvarn_hadamard_rows(const void* x, void* y, int64_t n_groups, int32_t dtype, void* stream) {
+  return kvarn_rope_hadamard(x, nullptr, nullptr, y, n_groups, 1, dtype, 1, stream);
+}
+
+int kvarn_hadamard_row_groups(const void* w, void* out, int64_t n_rows, int64_t n_cols, int32_t dtype, void* stream) {
+  if (!w || !out || n_rows < 0 || n_cols < 0 || (n_rows % G) != 0) return KVARN_INVALID_ARG;
+  if (dtype != KVARN_BF16 && dtype != KVARN_F32) return KVARN_UNSUPPORTED;
+  if (n_rows == 0 || n_cols == 0) return KVARN_OK;
+  if (n_rows / G > 65535) return KVARN_UNSUPPORTED;
+  const dim3 grid((unsigned)((n_cols + 31) / 32), (unsigned)(n_rows / G));
+  cudaStream_t s = (cudaStream_t)stream;
+  if (dtype == KVARN_F32) hadamard_row_groups_kernel<float><<<grid, 128, 0, s>>>((const float*)w, (float*)out, n_cols);
+  else hadamard_row_groups_kernel<__nv_bfloat16><<<grid, 128, 0, s>>>((const __nv_bfloat16*)w, (__nv_bfloat16*)out, n_cols);
+  return last_cuda();
 }
 
 int kvarn_quantize_chunk_host(const kvarn_params* p, const void* k_host, const void* v_host,

@@ -68,6 +68,10 @@ EXPORTS = {
                                          C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
     "kvarn_block_attention": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_void_p]),
+    "kvarn_rope_hadamard": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32,
+                                      C.c_int32, C.c_int32, C.c_void_p]),
+    "kvarn_hadamard_rows": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]),
+    "kvarn_hadamard_row_groups": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int32, C.c_void_p]),
     "kvarn_quantize_chunk_host": (C.c_int, [C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int64] +
                                   [C.c_void_p] * 7),
     "kvarn_decode_attention_host": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_int32,
@@ -277,6 +281,37 @@ def block_attention(p: Params, cache: Cache, q: torch.Tensor, k_blk: torch.Tenso
     st = lib.kvarn_block_attention(C.byref(p), C.byref(cache.desc), _ptr(q), _ptr(k_blk), _ptr(v_blk), n_q, Hq,
                                    sm_scale, _ptr(out), _stream(stream))
     _check(st, "kvarn_block_attention")
+    return out
+
+
+def rope_hadamard(x: torch.Tensor, cos: torch.Tensor | None = None, sin: torch.Tensor | None = None,
+                  rotate: bool = True, out: torch.Tensor | None = None, stream=None):
+    """x: [n_tok, n_heads, 128]; cos, sin: fp32 [n_tok, 64] or None -> RoPE(x) H / sqrt(128) (App. A, P:332)."""
+    assert x.is_cuda and x.is_contiguous() and x.dim() == 3 and x.shape[2] == HEAD_DIM
+    if cos is not None:
+        assert cos.dtype == torch.float32 and sin.dtype == torch.float32 and cos.is_contiguous() and sin.is_contiguous()
+        assert tuple(cos.shape) == (x.shape[0], HEAD_DIM // 2) and cos.shape == sin.shape
+    out = torch.empty_like(x) if out is None else out
+    _check(lib.kvarn_rope_hadamard(_ptr(x), _ptr(cos), _ptr(sin), _ptr(out), x.shape[0], x.shape[1], _dtype_code(x),
+                                   int(rotate), _stream(stream)), "kvarn_rope_hadamard")
+    return out
+
+
+def hadamard_rows(x: torch.Tensor, out: torch.Tensor | None = None, stream=None):
+    """Rotate every 128-element group of a contiguous tensor whose last dimension is a multiple of 128."""
+    assert x.is_cuda and x.is_contiguous() and x.shape[-1] % HEAD_DIM == 0
+    out = torch.empty_like(x) if out is None else out
+    _check(lib.kvarn_hadamard_rows(_ptr(x), _ptr(out), x.numel() // HEAD_DIM, _dtype_code(x), _stream(stream)),
+           "kvarn_hadamard_rows")
+    return out
+
+
+def hadamard_row_groups(w: torch.Tensor, out: torch.Tensor | None = None, stream=None):
+    """w: [n_rows, n_cols], n_rows % 128 == 0 -> blockdiag(H / sqrt(128)) w (the absorbed transform of W_O)."""
+    assert w.is_cuda and w.is_contiguous() and w.dim() == 2
+    out = torch.empty_like(w) if out is None else out
+    _check(lib.kvarn_hadamard_row_groups(_ptr(w), _ptr(out), w.shape[0], w.shape[1], _dtype_code(w), _stream(stream)),
+           "kvarn_hadamard_row_groups")
     return out
 
 
