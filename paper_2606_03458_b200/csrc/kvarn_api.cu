@@ -506,7 +506,7 @@ int kvarn_rope_hadamard(const void* x, const float* cos_tab, const float* sin_ta
   if (!aligned16(x) || !aligned16(y) || !aligned16(cos_tab) || !aligned16(sin_tab)) return KVARN_MISALIGNED;
   const long long n_groups = (long long)n_tok * n_heads;
   if (n_groups == 0) return KVARN_OK;
-  const unsigned grid = (unsigned)((n_groups + 7) / 8);
+  const unsigned grid = (unsigned)((n_groups + 8 * ROT_GPW - 1) / (8 * ROT_GPW));
   cudaStream_t s = (cudaStream_t)stream;
   if (dtype == KVARN_F32)
     rope_hadamard_kernel<float><<<grid, 256, 0, s>>>((const float*)x, cos_tab, sin_tab, (float*)y, n_groups, n_heads, rotate);

@@ -38,34 +38,47 @@ template <> __device__ __forceinline__ void st4<__nv_bfloat16>(__nv_bfloat16* p,
 // One warp per 128-element group (a head's slice of one row): y = RoPE(x) H / sqrt(128).
 // cos / sin: [n_tok][64] fp32 (half-split convention: channel c < 64 pairs with c + 64), or null = no RoPE.
 // rotate = 0 leaves out the Hadamard (plain RoPE).  Group index = tok * n_heads + head.
+constexpr int ROT_GPW = 4;   // groups per warp: all loads of a warp's groups are issued before the first butterfly
 template <typename T>
 __global__ void __launch_bounds__(256) rope_hadamard_kernel(const T* __restrict__ x, const float* __restrict__ cs,
                                                             const float* __restrict__ sn, T* __restrict__ y,
                                                             long long n_groups, int n_heads, int rotate) {
   const int lane = threadIdx.x & 31;
-  const long long grp = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
-  if (grp >= n_groups) return;
-  float v[4];
-  ld4<T>(x + grp * D + 4 * lane, v);
-  if (cs) {
-    const long long tok = grp / n_heads;
-    const int c = 4 * (lane & 15);
-    const float4 co = *reinterpret_cast<const float4*>(cs + tok * 64 + c);
-    const float4 si = *reinterpret_cast<const float4*>(sn + tok * 64 + c);
-    const float cc[4] = {co.x, co.y, co.z, co.w}, ss[4] = {si.x, si.y, si.z, si.w};
-    const float sg = lane < 16 ? -1.f : 1.f;   // y[c] = x[c] cos - x[c+64] sin;  y[c+64] = x[c+64] cos + x[c] sin
+  const long long g0 = ((long long)blockIdx.x * 8 + (threadIdx.x >> 5)) * ROT_GPW;
+  if (g0 >= n_groups) return;
+  const int c = 4 * (lane & 15);
+  float v[ROT_GPW][4], cc[ROT_GPW][4], ss[ROT_GPW][4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const float other = __shfl_xor_sync(0xffffffffu, v[j], 16);
-      v[j] = fmaf(v[j], cc[j], sg * other * ss[j]);
+  for (int u = 0; u < ROT_GPW; ++u) {
+    const long long grp = g0 + u;
+    if (grp < n_groups) {
+      ld4<T>(x + grp * D + 4 * lane, v[u]);
+      if (cs) {
+        const long long tok = grp / n_heads;
+        ld4<float>(cs + tok * 64 + c, cc[u]);
+        ld4<float>(sn + tok * 64 + c, ss[u]);
+      }
     }
   }
-  if (rotate) {
-    fwht128_lane4(v, lane);
+  const float sg = lane < 16 ? -1.f : 1.f;   // y[c] = x[c] cos - x[c+64] sin;  y[c+64] = x[c+64] cos + x[c] sin
 #pragma unroll
-    for (int j = 0; j < 4; ++j) v[j] *= HAD_NORM;
+  for (int u = 0; u < ROT_GPW; ++u) {
+    const long long grp = g0 + u;
+    if (grp >= n_groups) break;   // warp-uniform
+    if (cs) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const float other = __shfl_xor_sync(0xffffffffu, v[u][j], 16);
+        v[u][j] = fmaf(v[u][j], cc[u][j], sg * other * ss[u][j]);
+      }
+    }
+    if (rotate) {
+      fwht128_lane4(v[u], lane);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[u][j] *= HAD_NORM;
+    }
+    st4<T>(y + grp * D + 4 * lane, v[u]);
   }
-  st4<T>(y + grp * D + 4 * lane, v);
 }
 
 // W' = blockdiag(H / sqrt(128)) W for a row-major [n_rows][n_cols] matrix, n_rows a multiple of 128: every group
