@@ -312,7 +312,7 @@ const char* kvarn_status_string(int status) {
   }
 }
 
-int kvarn_version(void) { return 2; }
+int kvarn_version(void) { return 3; }
 
 int kvarn_layout(const kvarn_params* p, kvarn_layout_info* out) {
   if (!p || !out) return KVARN_INVALID_ARG;
