@@ -130,3 +130,29 @@ def test_block_attention_rejects_bad_arguments(kv):
     kb = torch.zeros((1, 2, 2, 128), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(kv.KvarnError, match="UNSUPPORTED"):
         kv.block_attention(p, cache, q, kb, kb.clone())
+
+
+def test_block_attention_fp32_inputs_bf16_output_and_custom_scale(kv):
+    n_tok, n_q = 128 * 2 + 9, 3
+    K, V, kb, vb, q = _inputs(1, 8, 2, n_tok, n_q, seed=97, dtype=torch.float32)
+    p = kv.default_params(4)
+    cache = _cache(kv, p, K, V)
+    out = kv.block_attention(p, cache, q, kb, vb, sm_scale=0.05)
+    p.out_dtype = kv.BF16
+    out_bf = kv.block_attention(p, cache, q, kb, vb, sm_scale=0.05)
+    assert out_bf.dtype == torch.bfloat16
+    assert (out_bf.float() - out).abs().max().item() <= 2 ** -7 * out.abs().max().item()
+    ref = _oracle_block(kv, p, cache, 0, 1, 4, q, kb, vb, n_tok, sm_scale=0.05)
+    got = out.double().cpu().numpy()[0, :, 4:8]
+    assert P.attn_rel_err(got.reshape(-1, 128), ref.reshape(-1, 128)) <= P.ATTN_RTOL
+
+
+def test_block_attention_is_deterministic_over_repeats(kv):
+    """Race hunt by repetition (compute-sanitizer is closed on this pool): 100 identical launches, bit-identical."""
+    n_tok, n_q = 128 * 6 + 70, 5
+    K, V, kb, vb, q = _inputs(2, 32, 8, n_tok, n_q, seed=98)
+    p = kv.default_params(2)
+    cache = _cache(kv, p, K, V, n_sink=32)
+    first = kv.block_attention(p, cache, q, kb, vb).clone()
+    for _ in range(100):
+        assert torch.equal(kv.block_attention(p, cache, q, kb, vb), first)
