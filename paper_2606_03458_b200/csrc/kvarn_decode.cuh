@@ -114,6 +114,8 @@ __device__ __forceinline__ uint32_t mapa_shared(uint32_t saddr, uint32_t cta_ran
 __device__ __forceinline__ void st_cluster_f32(uint32_t addr, float v) {
   asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
 }
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
@@ -639,6 +641,10 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
 
   // ---- hand over to the per-channel layout of the residual window / merge: thread tid = channel tid ----
   __syncthreads();
+  // every warp has left the main loop and no TMA fill is outstanding: this CTA's record ring is dead and may
+  // receive the peers' partials.  Arrive now, wait only right before the first DSMEM store (D7a), so the
+  // barrier latency hides behind the raw windows and the l reductions.
+  if (A.cluster > 1) cluster_arrive();
 #pragma unroll
   for (int u = 0; u < HPW; ++u) {
     float l = lp[u];
@@ -778,7 +784,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     const int crank = (int)cluster_ctarank();
     float* land = reinterpret_cast<float*>(&sm.rec[0][0][0]);   // [<= 16][WS_STRIDE]
     static_assert(sizeof(sm.rec) >= 16 * WS_STRIDE * sizeof(float), "landing area");
-    cluster_sync_all();
+    cluster_wait();
     const uint32_t land_addr = smem_u32(land);
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
