@@ -211,6 +211,24 @@ KVARN_API int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* c
                            void* stream);
 
 /*
+ * Context-parallel building block ("Splitting one sequence's chunks across GPUs needs exactly one
+ * exchange: all-gather (m, l, acc[128]) per q head and LSE-merge").  Each rank holds a cache over ITS part of every
+ * sequence and calls kvarn_decode_attention_partial, which is kvarn_decode_attention stopping before the
+ * normalisation: part[b][h] = { m, l, 0, 0, o[128] } (KVARN_PART_STRIDE = 132 fp32), with m a reference exponent
+ * in log2 units of the scaled logits (the kernel's running maximum, which includes the folded value scale; -inf for
+ * an empty part), l = sum_t 2^(logit_t - m), o = sum_t 2^(logit_t - m) v_t in the caller's (un-rotated) space.  After the ranks all-gather their `part` arrays into parts[n_parts][n_rows][132]
+ * (n_rows = B * Hq; one NCCL all-gather), kvarn_merge_partials computes
+ *   out[row] = sum_r 2^(m_r - m*) o_r / sum_r 2^(m_r - m*) l_r,   m* = max_r m_r   (zeros if every part is empty).
+ * All pointers DEVICE, 16-B aligned; ws as for kvarn_decode_attention.
+ */
+#define KVARN_PART_STRIDE 132
+KVARN_API int kvarn_decode_attention_partial(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                                   int32_t Hq, float sm_scale, float* part, void* ws, size_t ws_bytes,
+                                   void* stream);
+KVARN_API int kvarn_merge_partials(const float* parts, int32_t n_parts, int64_t n_rows, void* out, int32_t out_dtype,
+                         void* stream);
+
+/*
  * kvarn_block_attention -- the multi-token read path (Fig. 4 "pseudo-decode", Sec. 3.2:
  * "We split the sequence into blocks of size b.  After every block, the freshly produced K, V are
  * quantized before being written back to the KV-cache.  Subsequent blocks access a quantized cache").

@@ -428,9 +428,8 @@ int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_
   return last_cuda();
 }
 
-int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
-                           int32_t Hq, float sm_scale, void* out, void* ws, size_t ws_bytes,
-                           void* stream) {
+static int decode_impl(const kvarn_params* p, const kvarn_cache* cache, const void* q, int32_t Hq, float sm_scale,
+                       void* out, void* ws, size_t ws_bytes, void* stream, int partial) {
   int st = check_params(p);
   if (st) return st;
   if ((st = check_cache(cache))) return st;
@@ -451,13 +450,35 @@ int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, cons
   A.cluster = sp.cluster; A.nclus = sp.nclus; A.splits = sp.cluster * sp.nclus;
   A.q_scale = sm_scale * 1.4426950408889634f;
   A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
-  A.n_q = 1; A.tpc = 1; A.k_blk = nullptr; A.v_blk = nullptr;
+  A.n_q = 1; A.tpc = 1; A.k_blk = nullptr; A.v_blk = nullptr; A.partial = partial;
   cudaStream_t s = (cudaStream_t)stream;
   const bool f32 = p->in_dtype == KVARN_F32;
   cudaError_t e;
   if (p->bits == 2) e = f32 ? launch_decode<2, float>(A, s) : launch_decode<2, __nv_bfloat16>(A, s);
   else e = f32 ? launch_decode<4, float>(A, s) : launch_decode<4, __nv_bfloat16>(A, s);
   return e == cudaSuccess ? KVARN_OK : KVARN_CUDA;
+}
+
+int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                           int32_t Hq, float sm_scale, void* out, void* ws, size_t ws_bytes,
+                           void* stream) {
+  return decode_impl(p, cache, q, Hq, sm_scale, out, ws, ws_bytes, stream, 0);
+}
+
+int kvarn_decode_attention_partial(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                                   int32_t Hq, float sm_scale, float* part, void* ws, size_t ws_bytes,
+                                   void* stream) {
+  return decode_impl(p, cache, q, Hq, sm_scale, part, ws, ws_bytes, stream, 1);
+}
+
+int kvarn_merge_partials(const float* parts, int32_t n_parts, int64_t n_rows, void* out, int32_t out_dtype,
+                         void* stream) {
+  if (!parts || !out || n_parts < 1 || n_rows < 0) return KVARN_INVALID_ARG;
+  if (out_dtype != KVARN_BF16 && out_dtype != KVARN_F32) return KVARN_UNSUPPORTED;
+  if (!aligned16(parts) || !aligned16(out)) return KVARN_MISALIGNED;
+  if (n_rows == 0) return KVARN_OK;
+  merge_partials_kernel<<<(unsigned)n_rows, 128, 0, (cudaStream_t)stream>>>(parts, n_parts, n_rows, out, out_dtype);
+  return last_cuda();
 }
 
 // Multi-token read path (Fig. 4): the same kernel, the (query token, head)

@@ -48,6 +48,7 @@
 namespace kvarn {
 
 constexpr int WS_STRIDE = 260;  // floats per partial: m, l, pad, pad, acc_rot[128], acc_res[128]
+constexpr int PART_STRIDE = 132;  // floats per exported partial (kvarn_decode_attention_partial): m, l, pad, pad, o[128]
 
 struct DecodeArgs {
   const uint8_t* k_records;
@@ -74,6 +75,9 @@ struct DecodeArgs {
   int n_q, tpc;
   const void* k_blk;
   const void* v_blk;
+  // context-parallel building block: 1 = write the un-normalised partial {m, l, o[128]} of every (b, q head) to
+  // `out` ([B][Hq][PART_STRIDE] fp32) instead of the normalised output; merged across ranks by merge_partials_kernel
+  int partial;
 };
 
 // ------------------------------------------------------------------ PTX wrappers
@@ -860,7 +864,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
       wsp[h * 64 + lane] = w0;
       wsp[h * 64 + lane + 32] = w1;
       const float L = warp_sum(fmaf(w0, l0, w1 * l1));
-      if (lane == 0) sm.hs[0][h][1] = L;
+      if (lane == 0) { sm.hs[0][h][1] = L; sm.hs[0][h][0] = mstar; }
     }
     __syncthreads();
 #pragma unroll
@@ -882,6 +886,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
           res = fmaf(w, __ldcg(base + (size_t)s * WS_STRIDE + 128), res);
         }
         L = sm.hs[0][h][1];
+        m_run[h] = sm.hs[0][h][0];
       }
       l_tot[h] = L; acc[h] = rot; acc_res[h] = res;
     }
@@ -895,7 +900,11 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   for (int j = 0; j < GP; ++j) {
     merged_rot[j * 128 + tid] = acc[j];
     sm.qraw[j][tid] = (l_tot[j] > 0.f) ? acc_res[j] : 0.f;
-    if (tid == 0) sm.hs[0][j][0] = (l_tot[j] > 0.f) ? 1.f / l_tot[j] : 0.f;
+    if (tid == 0) {
+      sm.hs[0][j][0] = A.partial ? 1.f : ((l_tot[j] > 0.f) ? 1.f / l_tot[j] : 0.f);
+      sm.hs[0][j][1] = (l_tot[j] > 0.f) ? m_run[j] : -INFINITY;
+      sm.hz[0][j][0] = l_tot[j];
+    }
   }
   __syncthreads();
   for (int jj = warp; jj < GP; jj += 4) {
@@ -911,6 +920,12 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     const float4 s4 = *reinterpret_cast<const float4*>(&sm.qraw[jj][4 * lane]);
     const float inv = sm.hs[0][jj][0];
     const float o0 = (v[0] + s4.x) * inv, o1 = (v[1] + s4.y) * inv, o2 = (v[2] + s4.z) * inv, o3 = (v[3] + s4.w) * inv;
+    if (A.partial) {
+      float* prow = reinterpret_cast<float*>(A.out) + qrow(hh) * PART_STRIDE;
+      *reinterpret_cast<float4*>(prow + 4 + 4 * lane) = make_float4(o0, o1, o2, o3);
+      if (lane == 0) *reinterpret_cast<float4*>(prow) = make_float4(sm.hs[0][jj][1], sm.hz[0][jj][0], 0.f, 0.f);
+      continue;
+    }
     const size_t off = qrow(hh) * D + 4 * lane;
     if (A.out_dtype == KVARN_F32) {
       *reinterpret_cast<float4*>(reinterpret_cast<float*>(A.out) + off) = make_float4(o0, o1, o2, o3);
@@ -921,6 +936,26 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
       *reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(A.out) + off) = u;
     }
   }
+}
+
+// LSE merge of R partial sets (e.g. all-gathered from R context-parallel ranks): one CTA per
+// (b, q head) row, thread = channel.  parts [R][n_rows][PART_STRIDE]; m is in log2 units of the scaled logits.
+__global__ void __launch_bounds__(128) merge_partials_kernel(const float* __restrict__ parts, int R, long long n_rows,
+                                                             void* __restrict__ out, int out_dtype) {
+  const long long row = blockIdx.x;
+  const int tid = threadIdx.x;
+  float mstar = -INFINITY;
+  for (int r = 0; r < R; ++r) mstar = fmaxf(mstar, parts[((long long)r * n_rows + row) * PART_STRIDE]);
+  float L = 0.f, o = 0.f;
+  for (int r = 0; r < R; ++r) {
+    const float* pr = parts + ((long long)r * n_rows + row) * PART_STRIDE;
+    const float w = (pr[0] == -INFINITY) ? 0.f : exp2f(pr[0] - mstar);
+    L = fmaf(w, pr[1], L);
+    o = fmaf(w, pr[4 + tid], o);
+  }
+  const float res = L > 0.f ? o / L : 0.f;
+  if (out_dtype == KVARN_F32) reinterpret_cast<float*>(out)[row * D + tid] = res;
+  else reinterpret_cast<__nv_bfloat16*>(out)[row * D + tid] = __float2bfloat16_rn(res);
 }
 
 }  // namespace kvarn

@@ -72,6 +72,9 @@ EXPORTS = {
                                       C.c_int32, C.c_int32, C.c_void_p]),
     "kvarn_hadamard_rows": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]),
     "kvarn_hadamard_row_groups": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int32, C.c_void_p]),
+    "kvarn_decode_attention_partial": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_int32,
+                                                 C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "kvarn_merge_partials": (C.c_int, [C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_int32, C.c_void_p]),
     "kvarn_quantize_chunk_host": (C.c_int, [C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int64] +
                                   [C.c_void_p] * 7),
     "kvarn_decode_attention_host": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_int32,
@@ -261,6 +264,52 @@ def decode_attention(p: Params, cache: Cache, q: torch.Tensor, sm_scale: float |
                                     _ptr(ws), ws.numel(), _stream(stream))
     _check(st, "kvarn_decode_attention")
     return out
+
+
+PART_STRIDE = 132
+
+
+def decode_attention_partial(p: Params, cache: Cache, q: torch.Tensor, sm_scale: float | None = None,
+                             part: torch.Tensor | None = None, ws: torch.Tensor | None = None, stream=None):
+    """q: [B, Hq, 128] -> part [B, Hq, 132] fp32 = {m, l, 0, 0, o[128]}: this cache's un-normalised share of the
+    attention (context-parallel building block)."""
+    assert q.is_cuda and q.is_contiguous() and q.shape[0] == cache.B and q.shape[2] == HEAD_DIM
+    Hq = q.shape[1]
+    p.in_dtype = _dtype_code(q)
+    assert cache.k_resid.dtype == q.dtype
+    if sm_scale is None:
+        sm_scale = 1.0 / float(np.sqrt(HEAD_DIM))
+    if part is None:
+        part = torch.empty((cache.B, Hq, PART_STRIDE), device=q.device, dtype=torch.float32)
+    if ws is None:
+        ws = torch.empty((max(decode_workspace_bytes(p, cache.B, Hq, cache.Hkv, cache.max_chunks), 16),),
+                         dtype=torch.uint8, device=q.device)
+    st = lib.kvarn_decode_attention_partial(C.byref(p), C.byref(cache.desc), _ptr(q), Hq, sm_scale, _ptr(part),
+                                            _ptr(ws), ws.numel(), _stream(stream))
+    _check(st, "kvarn_decode_attention_partial")
+    return part
+
+
+def merge_partials(parts: torch.Tensor, out_dtype=torch.float32, out: torch.Tensor | None = None, stream=None):
+    """parts: [R, B, Hq, 132] fp32 (the ranks' partials, all-gathered) -> out [B, Hq, 128]."""
+    assert parts.is_cuda and parts.is_contiguous() and parts.dtype == torch.float32 and parts.shape[-1] == PART_STRIDE
+    R, B, Hq = parts.shape[:3]
+    if out is None:
+        out = torch.empty((B, Hq, HEAD_DIM), device=parts.device, dtype=out_dtype)
+    _check(lib.kvarn_merge_partials(_ptr(parts), R, B * Hq, _ptr(out), F32 if out.dtype == torch.float32 else BF16,
+                                    _stream(stream)), "kvarn_merge_partials")
+    return out
+
+
+def context_parallel_decode(p: Params, cache: Cache, q: torch.Tensor, group=None, sm_scale: float | None = None):
+    """One decode step with every sequence's tokens split across the ranks of `group` (each rank's `cache` holds its
+    share): local partial -> all_gather_into_tensor (NCCL over NVLink) -> LSE merge.  Every rank gets the output."""
+    import torch.distributed as dist
+    part = decode_attention_partial(p, cache, q, sm_scale=sm_scale)
+    world = dist.get_world_size(group)
+    parts = torch.empty((world,) + tuple(part.shape), device=part.device, dtype=torch.float32)
+    dist.all_gather_into_tensor(parts, part, group=group)
+    return merge_partials(parts, out_dtype=torch.float32 if p.out_dtype == F32 else torch.bfloat16)
 
 
 def block_attention(p: Params, cache: Cache, q: torch.Tensor, k_blk: torch.Tensor, v_blk: torch.Tensor,
