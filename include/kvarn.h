@@ -197,6 +197,18 @@ KVARN_API int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, cons
                  const void* v_new, void* stream);
 
 /*
+ * kvarn_append_block -- the same for a block of 1 <= n_new <= 128 tokens per sequence (the write half of a
+ * pseudo-decode step, Fig. 4: "After every block, the freshly produced K, V are quantized before being
+ * written back to the KV-cache"; kvarn_block_attention is the read half).  k_new, v_new = [B][Hkv][n_new][128]
+ * in_dtype (DEVICE).  Tokens fill the sink region first, then the residual window; the (at most one) chunk the
+ * window completes is quantised in the same launch, the remaining tokens start the next window.  The result is bit
+ * for bit what n_new calls of kvarn_append (or kvarn_prefill of the longer sequence) leave.  A block that does not fit
+ * (chunk slot >= max_chunks) leaves the sequence unchanged.
+ */
+KVARN_API int kvarn_append_block(const kvarn_params* p, const kvarn_cache* cache, const void* k_new,
+                       const void* v_new, int32_t n_new, void* stream);
+
+/*
  * kvarn_decode_attention -- out[b][h] = softmax(q[b][h] K^T * sm_scale) V over
  * all seq_lens[b] tokens of KV head h / (Hq/Hkv): the quantised chunks, read as
  * packed codes + scales + zero-points (Eq. 1 with the second scale fused,

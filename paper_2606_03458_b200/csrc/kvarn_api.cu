@@ -57,44 +57,56 @@ struct AppendArgs {
   int32_t* seq_lens;
   int32_t* ticket;
   int B, Hkv, max_chunks, n_sink;
+  int n_new;   // tokens appended per sequence (1..128); tok = [B][Hkv][n_new][128]
   int rotate[2];
   VarnConsts vc;
 };
 
-// One CTA per (sequence, KV head, kind).  The decision to quantise is taken on
-// the device from seq_lens (no host round trip).
+// One CTA per (sequence, KV head, kind) appends n_new <= 128 tokens (kvarn_append: 1).  The decision to quantise
+// is taken on the device from seq_lens (no host round trip).  Three-region layout of P:350: tokens go to
+// the sink while len < n_sink, then to the residual window; since the window holds < 128 tokens and n_new <= 128 at
+// most one chunk completes: it is quantised from [window rows ; new tokens] and the rest starts the next window.
 template <int BITS, typename InT>
 __global__ void __launch_bounds__(256, 2) append_kernel(const AppendArgs A) {
   extern __shared__ __align__(16) uint8_t quant_smem_raw[];
   QuantSmem<BITS>& sm = *reinterpret_cast<QuantSmem<BITS>*>(quant_smem_raw);
   const int kind = blockIdx.y, bh = blockIdx.x, b = bh / A.Hkv;
   const int tid = threadIdx.x;
+  const int n = A.n_new;
   const int len = A.seq_lens[b];
-  const bool to_sink = len < A.n_sink;                 // the three-region layout of P:350: sink | body | residual
-  const int l = to_sink ? 0 : len - A.n_sink;
-  const int r = l & 127, chunk = l >> 7;
-  const bool full = !to_sink && (r == 127);
-  const bool can_store = to_sink || (full ? (chunk < A.max_chunks) : (chunk <= A.max_chunks));
+  const int n_s = min(max(A.n_sink - len, 0), n);     // new tokens that still belong to the sink region
+  const int nb = n - n_s;                             // new tokens of the body
+  const int l0 = max(len - A.n_sink, 0);              // body tokens already stored
+  const int r0 = l0 & 127, chunk = l0 >> 7;
+  const bool full = nb > 0 && r0 + nb >= G;           // the window completes a chunk
+  const bool can_store = nb == 0 || (full ? (chunk < A.max_chunks) : (chunk <= A.max_chunks));
   InT* resid = reinterpret_cast<InT*>(A.resid[kind]) + (size_t)bh * G * D;
-  const InT* tok = reinterpret_cast<const InT*>(A.tok[kind]) + (size_t)bh * D;
-  if (to_sink) {
-    InT* sink = reinterpret_cast<InT*>(A.sink[kind]) + (size_t)bh * A.n_sink * D;
-    if (tid < D) sink[(size_t)len * D + tid] = tok[tid];
-  } else if (can_store && !full) {
-    if (tid < D) resid[(size_t)r * D + tid] = tok[tid];
-  } else if (can_store) {
-    const int lane = tid & 31, warp = tid >> 5;
-    const int c0 = 8 * (lane & 15), t0 = 16 * warp + 8 * (lane >> 4);
-    float2 x[8][4];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const int t = t0 + i;
-      const InT* row = (t == 127) ? tok : resid + (size_t)t * D;
-      load_row8<InT>(row + c0, x[i]);
+  const InT* tok = reinterpret_cast<const InT*>(A.tok[kind]) + (size_t)bh * n * D;
+  if (can_store) {
+    if (n_s > 0) {
+      InT* sink = reinterpret_cast<InT*>(A.sink[kind]) + ((size_t)bh * A.n_sink + len) * D;
+      for (int i = tid; i < n_s * D; i += 256) sink[i] = tok[i];
     }
-    uint8_t* dst = A.rec[kind] + ((size_t)bh * A.max_chunks + chunk) * record_bytes(BITS);
-    QuantDebug dbg{nullptr, nullptr, nullptr};
-    quantize_tile<BITS>(x, kind, A.rotate[kind] != 0, A.vc, dst, dbg, 0, sm);
+    const InT* btok = tok + (size_t)n_s * D;          // first body token of the block
+    if (!full) {
+      for (int i = tid; i < nb * D; i += 256) resid[(size_t)r0 * D + i] = btok[i];
+    } else {
+      const int lane = tid & 31, warp = tid >> 5;
+      const int c0 = 8 * (lane & 15), t0 = 16 * warp + 8 * (lane >> 4);
+      float2 x[8][4];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int t = t0 + i;
+        const InT* row = (t < r0) ? resid + (size_t)t * D : btok + (size_t)(t - r0) * D;
+        load_row8<InT>(row + c0, x[i]);
+      }
+      uint8_t* dst = A.rec[kind] + ((size_t)bh * A.max_chunks + chunk) * record_bytes(BITS);
+      QuantDebug dbg{nullptr, nullptr, nullptr};
+      quantize_tile<BITS>(x, kind, A.rotate[kind] != 0, A.vc, dst, dbg, 0, sm);   // (barriers inside: every row is loaded)
+      const int rem = r0 + nb - G;                    // tokens that start the next window
+      const InT* rtok = btok + (size_t)(G - r0) * D;
+      for (int i = tid; i < rem * D; i += 256) resid[i] = rtok[i];
+    }
   }
   __syncthreads();
   if (tid == 0) {
@@ -102,7 +114,7 @@ __global__ void __launch_bounds__(256, 2) append_kernel(const AppendArgs A) {
     const int old = atomicAdd(&A.ticket[b], 1);
     if (old == 2 * A.Hkv - 1) {  // last CTA of this sequence: every CTA has read seq_lens[b]
       A.ticket[b] = 0;
-      if (can_store) A.seq_lens[b] = len + 1;
+      if (can_store) A.seq_lens[b] = len + n;
     }
   }
 }
@@ -402,10 +414,16 @@ int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, const void* k
 
 int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_new,
                  const void* v_new, void* stream) {
+  return kvarn_append_block(p, cache, k_new, v_new, 1, stream);
+}
+
+int kvarn_append_block(const kvarn_params* p, const kvarn_cache* cache, const void* k_new,
+                       const void* v_new, int32_t n_new, void* stream) {
   int st = check_params(p);
   if (st) return st;
   if ((st = check_cache(cache))) return st;
-  if (!k_new || !v_new || !cache->ticket) return KVARN_INVALID_ARG;
+  if (!k_new || !v_new || !cache->ticket || n_new < 1) return KVARN_INVALID_ARG;
+  if (n_new > G) return KVARN_UNSUPPORTED;
   if (!aligned16(k_new) || !aligned16(v_new)) return KVARN_MISALIGNED;
   AppendArgs A{};
   A.rec[0] = (uint8_t*)cache->k_records; A.rec[1] = (uint8_t*)cache->v_records;
@@ -413,7 +431,7 @@ int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_
   A.tok[0] = k_new; A.tok[1] = v_new;
   A.seq_lens = cache->seq_lens; A.ticket = cache->ticket;
   A.sink[0] = cache->k_sink; A.sink[1] = cache->v_sink; A.n_sink = cache->n_sink;
-  A.B = cache->B; A.Hkv = cache->Hkv; A.max_chunks = cache->max_chunks;
+  A.B = cache->B; A.Hkv = cache->Hkv; A.max_chunks = cache->max_chunks; A.n_new = n_new;
   A.rotate[0] = p->rotate_k; A.rotate[1] = p->rotate_v; A.vc = varn_consts(p);
   dim3 grid((unsigned)(cache->B * cache->Hkv), 2);
   cudaStream_t s = (cudaStream_t)stream;

@@ -64,6 +64,8 @@ EXPORTS = {
     "kvarn_prefill": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p,
                                 C.c_int32, C.c_void_p]),
     "kvarn_append": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p, C.c_void_p]),
+    "kvarn_append_block": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p, C.c_int32,
+                                     C.c_void_p]),
     "kvarn_decode_attention": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_int32,
                                          C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
     "kvarn_block_attention": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p,
@@ -239,6 +241,16 @@ def append(p: Params, cache: Cache, k_new: torch.Tensor, v_new: torch.Tensor, st
     assert cache.k_resid.dtype == k_new.dtype
     _check(lib.kvarn_append(C.byref(p), C.byref(cache.desc), _ptr(k_new), _ptr(v_new),
                             _stream(stream)), "kvarn_append")
+
+
+def append_block(p: Params, cache: Cache, k_new: torch.Tensor, v_new: torch.Tensor, stream=None):
+    """k_new, v_new: [B, Hkv, n_new, 128], 1 <= n_new <= 128 new tokens per sequence (Fig. 4)."""
+    assert k_new.is_cuda and k_new.is_contiguous() and v_new.is_contiguous() and k_new.shape == v_new.shape
+    assert k_new.dim() == 4 and tuple(k_new.shape[:2]) == (cache.B, cache.Hkv) and k_new.shape[3] == HEAD_DIM
+    p.in_dtype = _dtype_code(k_new)
+    assert cache.k_resid.dtype == k_new.dtype
+    _check(lib.kvarn_append_block(C.byref(p), C.byref(cache.desc), _ptr(k_new), _ptr(v_new), k_new.shape[2],
+                                  _stream(stream)), "kvarn_append_block")
 
 
 def decode_workspace_bytes(p: Params, B: int, Hq: int, Hkv: int, max_chunks: int) -> int:

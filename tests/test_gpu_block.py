@@ -156,3 +156,52 @@ def test_block_attention_is_deterministic_over_repeats(kv):
     first = kv.block_attention(p, cache, q, kb, vb).clone()
     for _ in range(100):
         assert torch.equal(kv.block_attention(p, cache, q, kb, vb), first)
+
+
+@pytest.mark.parametrize("bits,n_sink", [(2, 0), (2, 32), (4, 128)])
+def test_append_block_matches_prefill_bit_for_bit(kv, bits, n_sink):
+    """Pseudo-decode write half (Fig. 4): prefill(L0) + append_block(n_1) + append_block(n_2) ... leaves exactly
+    the cache prefill(L0 + sum n_i) leaves -- records, sink, residual window and seq_lens."""
+    B, Hkv = 2, 4
+    blocks = [1, 5, 128, 37, 100, 128, 90, 3, 127, 64]
+    L0 = 20                                              # shorter than n_sink = 32 / 128: blocks straddle the sink boundary
+    total = L0 + sum(blocks)
+    K, V = W.kv_tokens(B, Hkv, total, seed=101, device="cuda")
+    p = kv.default_params(bits)
+    mc = total // 128 + 1
+    inc = kv.Cache(p, B, Hkv, mc, n_sink=n_sink)
+    kv.prefill(p, inc, K[:, :, :L0].contiguous(), V[:, :, :L0].contiguous())
+    pos = L0
+    for n in blocks:
+        kv.append_block(p, inc, K[:, :, pos:pos + n].contiguous(), V[:, :, pos:pos + n].contiguous())
+        pos += n
+        ref = kv.Cache(p, B, Hkv, mc, n_sink=n_sink)
+        kv.prefill(p, ref, K[:, :, :pos].contiguous(), V[:, :, :pos].contiguous())
+        ns, nc, r = O.cache_partition(pos, n_sink)
+        assert inc.seq_lens.tolist() == [pos] * B
+        assert torch.equal(inc.k_records[:, :, :nc], ref.k_records[:, :, :nc]) and torch.equal(inc.v_records[:, :, :nc], ref.v_records[:, :, :nc])
+        assert torch.equal(inc.k_resid[:, :, :r], ref.k_resid[:, :, :r]) and torch.equal(inc.v_resid[:, :, :r], ref.v_resid[:, :, :r])
+        assert torch.equal(inc.k_sink[:, :, :ns], ref.k_sink[:, :, :ns]) and torch.equal(inc.v_sink[:, :, :ns], ref.v_sink[:, :, :ns])
+
+
+def test_pseudo_decode_step_and_capacity_guard(kv):
+    """block attention over the cache, then the block is appended; the next single-token decode sees it.  A block that
+    would need a chunk slot beyond max_chunks leaves the sequence unchanged."""
+    B, Hq, Hkv, L0, n = 1, 16, 4, 128 * 2 + 100, 60
+    K, V, kb, vb, q = _inputs(B, Hq, Hkv, L0, n, seed=103)
+    p = kv.default_params(2)
+    cache = kv.Cache(p, B, Hkv, 3)
+    kv.prefill(p, cache, K, V)
+    out_blk = kv.block_attention(p, cache, q, kb, vb)
+    kv.append_block(p, cache, kb, vb)                    # 100 + 60 = 160: completes chunk 2, 32 tokens remain
+    assert cache.seq_lens.tolist() == [L0 + n]
+    out_dec = kv.decode_attention(p, cache, q[:, -1].contiguous())
+    assert torch.isfinite(out_blk).all()
+    full = kv.Cache(p, B, Hkv, 3); kv.prefill(p, full, torch.cat([K, kb], 2).contiguous(), torch.cat([V, vb], 2).contiguous())
+    assert torch.equal(out_dec, kv.decode_attention(p, full, q[:, -1].contiguous()))
+    big = torch.zeros((B, Hkv, 128, 128), dtype=torch.bfloat16, device="cuda")
+    kv.append_block(p, cache, big, big.clone())           # 32 + 128 -> would complete chunk 3 = max_chunks: dropped
+    assert cache.seq_lens.tolist() == [L0 + n]
+    with pytest.raises(kv.KvarnError, match="UNSUPPORTED"):
+        kv.append_block(p, cache, torch.zeros((B, Hkv, 129, 128), dtype=torch.bfloat16, device="cuda"),
+                        torch.zeros((B, Hkv, 129, 128), dtype=torch.bfloat16, device="cuda"))
