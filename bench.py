@@ -237,6 +237,11 @@ def run_extras(kv, W, dev, hbm_peak):
                     ex[f"block_long_g4_2bit_nq{n_q}"] = {"us": medb * 1e3, "us_per_query_token": medb * 1e3 / n_q,
                                                          "GBps": bb / medb / 1e6, "hbm_frac": bb / medb / 1e6 / hbm_peak,
                                                          "bytes": bb, "n_q": n_q, "vs_single_token_decode": medb / med}
+                    if n_q == 8:
+                        # write half of the pseudo-decode step: the block joins the cache (13 x 8 tokens fit the residual window)
+                        meda, _ = _time_launches(lambda i: kv.append_block(p, cache, kb, vb), 13, stream)
+                        ex["append_block_nq8"] = {"us": meda * 1e3, "n_q": 8, "B": sh.B, "Hkv": sh.Hkv,
+                                                  "note": "one launch for 8 tokens x 16 sequences; launch-latency-bound like kvarn_append"}
                     del qb, kb, vb, ob
             del cache, q, ws, out
             torch.cuda.empty_cache()
