@@ -395,6 +395,12 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
+    # libkvarn.so is built in-tree (git-ignored): local rank 0 builds it if missing or stale, the others wait
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        from paper_2606_03458_b200 import build as _build
+        _build.build()
+    if dist is not None:
+        dist.barrier()
     from paper_2606_03458_b200 import kvarn as kv
     if args.extras_only:
         if rank == 0:

@@ -12,6 +12,13 @@ for _p in (ROOT, HERE):
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    # libkvarn.so is built in-tree and git-ignored: build it when it is missing or older than its sources
+    # (nvcc cross-compiles sm_100a without a GPU).  No fallback: if this fails the binding raises on import.
+    try:
+        from paper_2606_03458_b200 import build as _build
+        _build.build()
+    except Exception as e:   # noqa: BLE001  (reported, then the tests that need the library fail loudly)
+        sys.stderr.write(f"[conftest] libkvarn.so build failed: {e}\n")
 
 
 def pytest_collection_modifyitems(config, items):
