@@ -308,6 +308,41 @@ __device__ __forceinline__ float undigit(int d0, int d1, int d2, int d3) {
   return fmaf(__int2float_rn(x23), 65536.f, __int2float_rn(x01));
 }
 
+// Columns of a CTA: j -> (query token tok0 + (j >> lg), head j mod 2^lg); plain decode: tok0 = 0, ncols = g, lg = 31
+// (column = head, any g).  Evaluated once before and once after the main loop -- the volatile read of %ctaid.z
+// keeps the two evaluations apart, so that none of this lives in registers through the loop (at g = 8 the loop is
+// register-bound: carrying these values cost 6 % more loop instructions).
+// Which (sequence, KV head, split) this CTA serves and the regions of its sequence (sink | body | residual);
+// like col_map, evaluated before and after the main loop from volatile reads so nothing is carried through it.
+struct Where { int bh, b, hkv, split, n_sink_tok, n_chunks, resid; };
+__device__ __forceinline__ Where where_am_i(const DecodeArgs& A) {
+  unsigned x, y;
+  asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(x));
+  asm volatile("mov.u32 %0, %%ctaid.y;" : "=r"(y));
+  Where w;
+  w.bh = (int)x; w.b = w.bh / A.Hkv; w.hkv = w.bh - w.b * A.Hkv; w.split = (int)y;
+  int len;
+  asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(len) : "l"(A.seq_lens + w.b));
+  w.n_sink_tok = min(len, A.n_sink);
+  const int body = len - w.n_sink_tok;
+  w.n_chunks = min(body >> 7, A.max_chunks);
+  w.resid = body & 127;
+  return w;
+}
+
+struct ColMap { int lg, tok0, ncols, n_q, blk_cnt; };
+__device__ __forceinline__ ColMap col_map(const DecodeArgs& A) {
+  unsigned z;
+  asm volatile("mov.u32 %0, %%ctaid.z;" : "=r"(z));
+  ColMap c;
+  c.lg = A.tpc == 1 ? 31 : __ffs(A.g) - 1;
+  c.n_q = A.n_q;
+  c.tok0 = (int)z * A.tpc;
+  c.ncols = min(A.tpc, c.n_q - c.tok0) * A.g;
+  c.blk_cnt = A.k_blk != nullptr ? min(c.n_q, c.tok0 + A.tpc) : 0;   // block tokens visible to some column of this CTA
+  return c;
+}
+
 template <int BITS, int GP, int NCH, typename InT>
 #ifndef KVARN_DEC_OCC4
 #define KVARN_DEC_OCC4 4
@@ -329,35 +364,23 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int fg = lane >> 2, ft = lane & 3;   // MMA fragment coordinates: row group g, thread-in-group t
-  const int bh = blockIdx.x, b = bh / A.Hkv, hkv = bh - b * A.Hkv;
-  const int split = blockIdx.y;
   const int g = A.g;
-  const int lg = A.tpc == 1 ? 31 : __ffs(g) - 1;   // several tokens per CTA: g is a power of two; one token: column = head
-  // columns of this CTA: j -> (query token tok0 + (j >> lg), head j mod 2^lg); plain decode: tok0 = 0, ncols = g
-  const int n_q = A.n_q, tok0 = (int)blockIdx.z * A.tpc;
-  const int ncols = min(A.tpc, n_q - tok0) * g;
-  auto qrow = [&](int j) -> size_t { return ((size_t)b * n_q + tok0 + (j >> lg)) * A.Hq + hkv * g + (j - ((j >> lg) << lg)); };
+  float mr[HPW], lp[HPW], ac[HPW][4];   // running maximum, partial l, partial accumulator of this thread's (heads, rows)
+  const Where w0 = where_am_i(A);
+  {   // ======== setup + main loop: everything declared here dies before the epilogue ========
+  const int bh = w0.bh, b = w0.b, hkv = w0.hkv, split = w0.split;
+  const ColMap cm0 = col_map(A);   // before the main loop: q rows of D1, block weight of the split plan
 
   // ---- chunk range of this split ----------------------------------------------------
-  const int len = A.seq_lens[b];
-  const int n_sink_tok = min(len, A.n_sink);      // three-region layout: sink | quantised body | residual
-  const int body = len - n_sink_tok;
-  int n_chunks = body >> 7;
-  if (n_chunks > A.max_chunks) n_chunks = A.max_chunks;
-  const int resid = body & 127;
+  const int n_sink_tok = w0.n_sink_tok, n_chunks = w0.n_chunks, resid = w0.resid;
   // Balanced split: a raw window (512 B per token against 72 B) weighs like one chunk per 12 tokens (measured:
   // 127 residual tokens cost a CTA about 10 chunks), so the splits that own the sink / residual window get
   // correspondingly fewer chunks.  Virtual units: [sink | chunk 0 .. n_chunks-1 | residual].
-  const bool has_blk = A.k_blk != nullptr;
-  const int blk_cnt = has_blk ? min(n_q, tok0 + A.tpc) : 0;   // block tokens visible to some column of this CTA
-  const int w_sink = (n_sink_tok + 11) / 12, w_res = (resid + blk_cnt + 11) / 12;
+  const int w_sink = (n_sink_tok + 11) / 12, w_res = (resid + cm0.blk_cnt + 11) / 12;
   const int per = (n_chunks + w_sink + w_res + A.splits - 1) / A.splits;
   const int c_begin = min(max(split * per - w_sink, 0), n_chunks);
   const int c_end = min(max((split + 1) * per - w_sink, 0), n_chunks);
   const int n_my = c_end - c_begin;
-  const bool do_resid = (split == A.splits - 1) && resid > 0;
-  const bool do_sink = (split == 0) && n_sink_tok > 0;
-  const bool do_blk = (split == A.splits - 1) && has_blk;
 
   const uint8_t* krec = A.k_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
   const uint8_t* vrec = A.v_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
@@ -384,8 +407,9 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   // D1: q' = (q H / sqrt(128)) * q_scale; heads >= g are zero
   for (int hh = warp; hh < GP; hh += 4) {
     float v[4] = {0.f, 0.f, 0.f, 0.f};
-    if (hh < ncols) {
-      const InT* qp = reinterpret_cast<const InT*>(A.q) + qrow(hh) * D + 4 * lane;
+    if (hh < cm0.ncols) {
+      const size_t row = ((size_t)b * cm0.n_q + cm0.tok0 + (hh >> cm0.lg)) * A.Hq + hkv * g + (hh - ((hh >> cm0.lg) << cm0.lg));
+      const InT* qp = reinterpret_cast<const InT*>(A.q) + row * D + 4 * lane;
 #pragma unroll
       for (int j = 0; j < 4; ++j) v[j] = ld_in<InT>(qp + j) * A.q_scale;
     }
@@ -429,7 +453,6 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   for (int dd = 0; dd < 2; ++dd) bp_dst[dd] = &sm.bp[0][0][warp >> 1][b_slot(4 * (2 * ft + dd) + (fg & 3), warp >> 1)][2 * (warp & 1) + (fg >> 2)];
   constexpr int B_CH = NT * 256;   // 32-bit words of one chunk's B operand
 
-  float mr[HPW], lp[HPW], ac[HPW][4];
 #pragma unroll
   for (int u = 0; u < HPW; ++u) {
     mr[u] = -INFINITY; lp[u] = 0.f;
@@ -642,9 +665,21 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     if (NCH == 1 || n_my - it * NCH >= NCH) iteration(std::true_type{}, it);
     else iteration(std::false_type{}, it);
   }
+  }   // ======== end of setup + main loop ========
 
   // ---- hand over to the per-channel layout of the residual window / merge: thread tid = channel tid ----
   __syncthreads();
+  // 4-bit: re-derive the CTA's coordinates instead of carrying them through the loop (g = 8: 369 -> 350 us on a
+  // 64k context); at 2-bit ptxas schedules the loop better with them live (195 vs 199 us at g = 4)
+  const Where w1 = BITS == 4 ? where_am_i(A) : w0;
+  const int bh = w1.bh, b = w1.b, hkv = w1.hkv, split = w1.split, n_sink_tok = w1.n_sink_tok, resid = w1.resid;
+  const bool do_resid = (split == A.splits - 1) && resid > 0;
+  const bool do_sink = (split == 0) && n_sink_tok > 0;
+  const ColMap cm = col_map(A);   // after the main loop (see col_map)
+  const int lg = cm.lg, tok0 = cm.tok0, ncols = cm.ncols, n_q = cm.n_q, blk_cnt = cm.blk_cnt;
+  const bool has_blk = A.k_blk != nullptr;
+  const bool do_blk = (split == A.splits - 1) && has_blk;
+  auto qrow = [&](int j) -> size_t { return ((size_t)b * n_q + tok0 + (j >> lg)) * A.Hq + hkv * g + (j - ((j >> lg) << lg)); };
   // every warp has left the main loop and no TMA fill is outstanding: this CTA's record ring is dead and may
   // receive the peers' partials.  Arrive now, wait only right before the first DSMEM store (D7a), so the
   // barrier latency hides behind the raw windows and the l reductions.
