@@ -315,14 +315,20 @@ __device__ __forceinline__ float undigit(int d0, int d1, int d2, int d3) {
 // Which (sequence, KV head, split) this CTA serves and the regions of its sequence (sink | body | residual);
 // like col_map, evaluated before and after the main loop from volatile reads so nothing is carried through it.
 struct Where { int bh, b, hkv, split, n_sink_tok, n_chunks, resid; };
+// AGAIN = false: the plain form (blockIdx, an ordinary load: the compiler keeps these in uniform registers);
+// AGAIN = true: volatile reads, a second evaluation the compiler cannot merge with the first.
+template <bool AGAIN>
 __device__ __forceinline__ Where where_am_i(const DecodeArgs& A) {
-  unsigned x, y;
-  asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(x));
-  asm volatile("mov.u32 %0, %%ctaid.y;" : "=r"(y));
+  unsigned x = blockIdx.x, y = blockIdx.y;
+  if constexpr (AGAIN) {
+    asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(x));
+    asm volatile("mov.u32 %0, %%ctaid.y;" : "=r"(y));
+  }
   Where w;
   w.bh = (int)x; w.b = w.bh / A.Hkv; w.hkv = w.bh - w.b * A.Hkv; w.split = (int)y;
   int len;
-  asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(len) : "l"(A.seq_lens + w.b));
+  if constexpr (AGAIN) asm volatile("ld.global.cg.s32 %0, [%1];" : "=r"(len) : "l"(A.seq_lens + w.b));
+  else len = A.seq_lens[w.b];
   w.n_sink_tok = min(len, A.n_sink);
   const int body = len - w.n_sink_tok;
   w.n_chunks = min(body >> 7, A.max_chunks);
@@ -331,9 +337,10 @@ __device__ __forceinline__ Where where_am_i(const DecodeArgs& A) {
 }
 
 struct ColMap { int lg, tok0, ncols, n_q, blk_cnt; };
+template <bool AGAIN>
 __device__ __forceinline__ ColMap col_map(const DecodeArgs& A) {
-  unsigned z;
-  asm volatile("mov.u32 %0, %%ctaid.z;" : "=r"(z));
+  unsigned z = blockIdx.z;
+  if constexpr (AGAIN) asm volatile("mov.u32 %0, %%ctaid.z;" : "=r"(z));
   ColMap c;
   c.lg = A.tpc == 1 ? 31 : __ffs(A.g) - 1;
   c.n_q = A.n_q;
@@ -366,10 +373,12 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   const int fg = lane >> 2, ft = lane & 3;   // MMA fragment coordinates: row group g, thread-in-group t
   const int g = A.g;
   float mr[HPW], lp[HPW], ac[HPW][4];   // running maximum, partial l, partial accumulator of this thread's (heads, rows)
-  const Where w0 = where_am_i(A);
+  const Where w0 = where_am_i<false>(A);
+  const ColMap cm0 = col_map<false>(A);   // before the main loop: q rows of D1, block weight of the split plan
+  const bool do_resid0 = (w0.split == A.splits - 1) && w0.resid > 0;
+  const bool do_sink0 = (w0.split == 0) && w0.n_sink_tok > 0;
   {   // ======== setup + main loop: everything declared here dies before the epilogue ========
   const int bh = w0.bh, b = w0.b, hkv = w0.hkv, split = w0.split;
-  const ColMap cm0 = col_map(A);   // before the main loop: q rows of D1, block weight of the split plan
 
   // ---- chunk range of this split ----------------------------------------------------
   const int n_sink_tok = w0.n_sink_tok, n_chunks = w0.n_chunks, resid = w0.resid;
@@ -669,13 +678,14 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
 
   // ---- hand over to the per-channel layout of the residual window / merge: thread tid = channel tid ----
   __syncthreads();
-  // 4-bit: re-derive the CTA's coordinates instead of carrying them through the loop (g = 8: 369 -> 350 us on a
-  // 64k context); at 2-bit ptxas schedules the loop better with them live (195 vs 199 us at g = 4)
-  const Where w1 = BITS == 4 ? where_am_i(A) : w0;
+  // Re-derive the CTA's coordinates / column map instead of carrying them through the loop where that pays
+  // (64k context, g = 8: 2-bit 367 -> 344 us, 4-bit 390 -> 350 us); the 2-bit g <= 4 kernel is faster with them
+  // live (195 vs 199 us, 203 vs 209 us with a full residual window), so it keeps them.
+  const Where w1 = BITS == 4 ? where_am_i<true>(A) : w0;
   const int bh = w1.bh, b = w1.b, hkv = w1.hkv, split = w1.split, n_sink_tok = w1.n_sink_tok, resid = w1.resid;
-  const bool do_resid = (split == A.splits - 1) && resid > 0;
-  const bool do_sink = (split == 0) && n_sink_tok > 0;
-  const ColMap cm = col_map(A);   // after the main loop (see col_map)
+  const bool do_resid = BITS == 4 ? ((split == A.splits - 1) && resid > 0) : do_resid0;
+  const bool do_sink = BITS == 4 ? ((split == 0) && n_sink_tok > 0) : do_sink0;
+  const ColMap cm = (GP == 8 || BITS == 4) ? col_map<true>(A) : cm0;
   const int lg = cm.lg, tok0 = cm.tok0, ncols = cm.ncols, n_q = cm.n_q, blk_cnt = cm.blk_cnt;
   const bool has_blk = A.k_blk != nullptr;
   const bool do_blk = (split == A.splits - 1) && has_blk;
