@@ -90,6 +90,39 @@ def test_status_strings_and_argument_validation_without_gpu(kv):
     assert need > 0 and need % 16 == 0
 
 
+def test_argument_validation_of_the_later_entry_points_without_gpu(kv):
+    """Every check below fails before any pointer is dereferenced or any kernel is launched."""
+    L = kv.lib
+    p = kv.default_params(2)
+    cache = kv.CacheDesc(0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000, 0x6800, 2, 8, 4, 0)
+    ptr = C.c_void_p
+    # kvarn_block_attention: n_q < 1, g = 3 (not a power of two), n_q > 128, null block, misaligned q
+    blk = lambda q, kb, vb, n_q, Hq: L.kvarn_block_attention(C.byref(p), C.byref(cache), q, kb, vb, n_q, Hq, 0.1, ptr(0x9000), None)
+    assert blk(ptr(0x7000), ptr(0x7100), ptr(0x7200), 0, 32) == -1
+    assert blk(ptr(0x7000), ptr(0x7100), ptr(0x7200), 4, 24) == -2
+    assert blk(ptr(0x7000), ptr(0x7100), ptr(0x7200), 129, 32) == -2
+    assert blk(ptr(0x7000), None, ptr(0x7200), 4, 32) == -1
+    assert blk(ptr(0x7004), ptr(0x7100), ptr(0x7200), 4, 32) == -3
+    # kvarn_append_block: n_new out of range
+    assert L.kvarn_append_block(C.byref(p), C.byref(cache), ptr(0x7000), ptr(0x7100), 0, None) == -1
+    assert L.kvarn_append_block(C.byref(p), C.byref(cache), ptr(0x7000), ptr(0x7100), 129, None) == -2
+    # aux_round must be 0 or 1
+    bad = kv.default_params(2, aux_round=2)
+    assert L.kvarn_append_block(C.byref(bad), C.byref(cache), ptr(0x7000), ptr(0x7100), 1, None) == -1
+    # kvarn_merge_partials
+    assert L.kvarn_merge_partials(ptr(0x7000), 0, 4, ptr(0x8000), kv.F32, None) == -1
+    assert L.kvarn_merge_partials(ptr(0x7000), 2, 4, ptr(0x8000), 7, None) == -2
+    assert L.kvarn_merge_partials(ptr(0x7004), 2, 4, ptr(0x8000), kv.F32, None) == -3
+    assert L.kvarn_merge_partials(ptr(0x7000), 2, 0, ptr(0x8000), kv.F32, None) == 0
+    # rotations: cos without sin, bad dtype, rows not a multiple of 128, empty inputs are no-ops
+    assert L.kvarn_rope_hadamard(ptr(0x7000), ptr(0x7100), None, ptr(0x8000), 4, 2, kv.F32, 1, None) == -1
+    assert L.kvarn_rope_hadamard(ptr(0x7000), None, None, ptr(0x8000), 4, 2, 5, 1, None) == -2
+    assert L.kvarn_rope_hadamard(None, None, None, None, 0, 2, kv.F32, 1, None) == 0
+    assert L.kvarn_hadamard_row_groups(ptr(0x7000), ptr(0x8000), 100, 8, kv.F32, None) == -1
+    assert L.kvarn_hadamard_row_groups(ptr(0x7000), ptr(0x8000), 0, 8, kv.F32, None) == 0
+    assert L.kvarn_version() >= 3
+
+
 @pytest.mark.parametrize("bits", [2, 4])
 @pytest.mark.parametrize("kind", [0, 1])
 def test_pack_unpack_round_trip_and_formats(kv, bits, kind):
