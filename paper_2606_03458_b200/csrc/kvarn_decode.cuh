@@ -705,12 +705,13 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     for (int i = 0; i < 4; ++i) sm.qrot[ft + 4 * u][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg] = ac[u][i];
   }
   __syncthreads();
-  float m_run[GP], l_part[GP], acc[GP];
+  float m_run[GP], l_part[GP], l_tot[GP], acc[GP];
 #pragma unroll
   for (int h = 0; h < GP; ++h) {
     m_run[h] = sm.hs[0][h][0];
     const float4 hz = *reinterpret_cast<const float4*>(sm.hz[0][h]);
-    l_part[h] = tid == 0 ? (hz.x + hz.y) + (hz.z + hz.w) : 0.f;   // thread 0 carries the sum over the chunks
+    l_tot[h] = (hz.x + hz.y) + (hz.z + hz.w);                     // l of the chunks (every thread has it)
+    l_part[h] = tid == 0 ? l_tot[h] : 0.f;                        // with raw windows: thread 0 carries it into the sum
     acc[h] = sm.qrot[h][tid];
   }
 
@@ -808,19 +809,20 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     raw_window(reinterpret_cast<const InT*>(A.k_blk) + (size_t)bh * n_q * D,
                reinterpret_cast<const InT*>(A.v_blk) + (size_t)bh * n_q * D, blk_cnt, tok0);
 
-  // ---- l: reduce the per-thread partial sums ----------------------------------------------------
-  __syncthreads();
-  {
-    float v[GP];
+  // ---- l: reduce the per-thread partial sums (only a CTA that ran a raw window has any beyond the chunks') ----
+  if (do_sink || do_resid || do_blk) {   // CTA-uniform
+    __syncthreads();
+    {
+      float v[GP];
 #pragma unroll
-    for (int h = 0; h < GP; ++h) v[h] = l_part[h];
-    const float r = warp_reduce_multi<GP>(v, lane, RAdd());
-    if ((lane & (32 / GP - 1)) == 0) sm.wz[warp][red_index<GP>(lane)] = r;
+      for (int h = 0; h < GP; ++h) v[h] = l_part[h];
+      const float r = warp_reduce_multi<GP>(v, lane, RAdd());
+      if ((lane & (32 / GP - 1)) == 0) sm.wz[warp][red_index<GP>(lane)] = r;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int h = 0; h < GP; ++h) l_tot[h] = (sm.wz[0][h] + sm.wz[1][h]) + (sm.wz[2][h] + sm.wz[3][h]);
   }
-  __syncthreads();
-  float l_tot[GP];
-#pragma unroll
-  for (int h = 0; h < GP; ++h) l_tot[h] = (sm.wz[0][h] + sm.wz[1][h]) + (sm.wz[2][h] + sm.wz[3][h]);
 
   // ---- D7a: in-cluster merge of the split partials through distributed shared memory ----------
   // Reduce-scatter by head: head h is merged by the CTA of cluster rank h % CS, which receives the
