@@ -12,6 +12,12 @@
  * softmax(q K^T * sm_scale) V over [dequantised chunks ; raw residual tokens]
  * without ever materialising a dequantised cache.
  *
+ * Entry points: kvarn_quantize_chunk / kvarn_prefill (bulk write path), kvarn_append / kvarn_append_block
+ * (on-the-fly compression while decoding), kvarn_decode_attention (read path), kvarn_block_attention (a block of
+ * new tokens against the cache, Fig. 4), kvarn_decode_attention_partial + kvarn_merge_partials (a sequence
+ * spread over several caches / GPUs), kvarn_rope_hadamard / kvarn_hadamard_rows / kvarn_hadamard_row_groups (the
+ * Hadamard arrangement of App. A), the *_host forms, layout queries and the record pack / unpack test hooks.
+ *
  * Conventions
  *   - "DEVICE" pointers are CUDA device memory owned by the caller; "HOST"
  *     pointers are ordinary (preferably pinned) host memory.  The library
