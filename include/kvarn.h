@@ -138,6 +138,12 @@ typedef struct {
   int32_t n_sink;       /* S: tokens [0, S) of every sequence stay raw in k_sink / v_sink; 0..128 */
   void* k_sink;         /* [B][Hkv][n_sink][128] in_dtype (may be NULL when n_sink = 0) */
   void* v_sink;         /* same shape */
+  /* Capacity of a sequence: n_sink + max_chunks*128 + 127 tokens.  Two optional guards of the append path: */
+  int32_t max_len_hint; /* HOST knowledge: an upper bound on max_b seq_lens[b] before the call (the caller counts the
+                         * tokens it appends); <= 0 = unknown.  When > 0, kvarn_append / kvarn_append_block return
+                         * KVARN_CAPACITY and enqueue nothing if max_len_hint + n_new exceeds the capacity. */
+  int32_t* overflow;    /* DEVICE, nullable: sticky counter, incremented once per (sequence, call) whose tokens did
+                         * not fit and were dropped (lengths the host cannot bound); never reset by the library. */
 } kvarn_cache;
 
 /* Optional per-tile debug outputs of the quantizer (all DEVICE, each nullable).
@@ -197,7 +203,9 @@ KVARN_API int kvarn_prefill(const kvarn_params* p, const kvarn_cache* cache, con
  * for bit what kvarn_quantize_chunk gives on those 128 tokens) and the residual
  * becomes empty.  seq_lens[b] is read and advanced ON DEVICE (no host round
  * trip).  A sequence already holding n_sink + max_chunks*128 + 127 tokens is left
- * unchanged (its token is dropped); the caller bounds lengths on the host.
+ * unchanged (its token is dropped): with cache->max_len_hint > 0 the call returns
+ * KVARN_CAPACITY instead of launching when the bound proves that a token cannot fit,
+ * and a drop the host could not foresee is counted in cache->overflow (if non-null).
  */
 KVARN_API int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, const void* k_new,
                  const void* v_new, void* stream);
@@ -209,7 +217,7 @@ KVARN_API int kvarn_append(const kvarn_params* p, const kvarn_cache* cache, cons
  * in_dtype (DEVICE).  Tokens fill the sink region first, then the residual window; the (at most one) chunk the
  * window completes is quantised in the same launch, the remaining tokens start the next window.  The result is bit
  * for bit what n_new calls of kvarn_append (or kvarn_prefill of the longer sequence) leave.  A block that does not fit
- * (chunk slot >= max_chunks) leaves the sequence unchanged.
+ * (chunk slot >= max_chunks) leaves the sequence unchanged (KVARN_CAPACITY / cache->overflow as for kvarn_append).
  */
 KVARN_API int kvarn_append_block(const kvarn_params* p, const kvarn_cache* cache, const void* k_new,
                        const void* v_new, int32_t n_new, void* stream);
@@ -223,6 +231,12 @@ KVARN_API int kvarn_append_block(const kvarn_params* p, const kvarn_cache* cache
  *   q    DEVICE [B][Hq][128] in_dtype          out  DEVICE [B][Hq][128] out_dtype
  *   ws   DEVICE scratch of >= kvarn_decode_workspace_bytes(...) bytes, 16-B aligned
  * A sequence of length 0 yields zeros.  Hq/Hkv must be in 1..8.
+ * Precision: fp32 accumulation; the folded query and the probabilities enter the tensor cores as 22-bit
+ * fixed-point numbers, the query relative to max_c |q~[h, c]| of its chunk, a probability relative to the largest
+ * probability of the tokens that share its loop iteration (<= 256 tokens at 2-bit, <= 128 at 4-bit).  A token is
+ * therefore rounded to zero only if it lies more than 2^-23 below one of its <= 255 neighbours -- a bound that does
+ * not grow with the context length; numerator and denominator of the softmax use the same rounded values.  Raw
+ * (sink / residual / block) tokens are handled in fp32.
  */
 KVARN_API int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
                            int32_t Hq, float sm_scale, void* out, void* ws, size_t ws_bytes,

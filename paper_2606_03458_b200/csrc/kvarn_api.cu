@@ -1,5 +1,6 @@
 // C-ABI entry points of libkvarn (include/kvarn.h): argument validation, kernel
 // launches on the caller's stream, host-side record pack/unpack test hooks.
+#include <atomic>
 #include <cstdio>
 #include <cstring>
 
@@ -56,6 +57,7 @@ struct AppendArgs {
   void* sink[2];
   int32_t* seq_lens;
   int32_t* ticket;
+  int32_t* overflow;   // nullable: sticky count of (sequence, call) pairs whose tokens were dropped
   int B, Hkv, max_chunks, n_sink;
   int n_new;   // tokens appended per sequence (1..128); tok = [B][Hkv][n_new][128]
   int rotate[2];
@@ -115,6 +117,7 @@ __global__ void __launch_bounds__(256, 2) append_kernel(const AppendArgs A) {
     if (old == 2 * A.Hkv - 1) {  // last CTA of this sequence: every CTA has read seq_lens[b]
       A.ticket[b] = 0;
       if (can_store) A.seq_lens[b] = len + n;
+      else if (A.overflow) atomicAdd(A.overflow, 1);
     }
   }
 }
@@ -168,15 +171,39 @@ static VarnConsts varn_consts(const kvarn_params* p) {
 
 static int last_cuda() { return cudaGetLastError() == cudaSuccess ? KVARN_OK : KVARN_CUDA; }
 
-// QuantSmem exceeds the 48 KB static limit (it keeps the per-iterate statistics of Alg. 1): dynamic, opt-in
-template <int BITS, auto KERN, typename Args>
-static void launch_quant_smem(dim3 grid, const Args& A, cudaStream_t st) {
-  static bool configured = false;   // per kernel (KERN is a template argument); benign race (idempotent call)
-  if (!configured) {
-    cudaFuncSetAttribute(KERN, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(QuantSmem<BITS>));
-    configured = true;
+// The device the launch goes to: CUDA launches on the CURRENT device (the caller's stream must belong to it).
+static int current_device() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return -1; }
+  return dev;
+}
+
+// Opt-in to more than 48 KB of dynamic shared memory (+ the shared-memory carve-out).  The attribute belongs to
+// the (kernel, device) pair, so it is applied once PER DEVICE: a bit mask indexed by the current device, one mask
+// per kernel (KERN is a template argument).  Atomic: two host threads may race here, the call is idempotent.
+constexpr int KVARN_MAX_DEVICES = 64;
+template <auto KERN>
+static cudaError_t ensure_smem_optin(int bytes, bool max_carveout) {
+  static std::atomic<uint64_t> done{0};
+  const int dev = current_device();
+  if (dev < 0) return cudaErrorNoDevice;
+  if (dev < KVARN_MAX_DEVICES && ((done.load(std::memory_order_acquire) >> dev) & 1)) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(KERN, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return e;
+  if (max_carveout) {
+    e = cudaFuncSetAttribute(KERN, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
   }
+  if (dev < KVARN_MAX_DEVICES) done.fetch_or(1ull << dev, std::memory_order_release);
+  return cudaSuccess;
+}
+
+// QuantSmem exceeds the 48 KB static limit: dynamic, opt-in
+template <int BITS, auto KERN, typename Args>
+static int launch_quant_smem(dim3 grid, const Args& A, cudaStream_t st) {
+  if (ensure_smem_optin<KERN>((int)sizeof(QuantSmem<BITS>), false) != cudaSuccess) { cudaGetLastError(); return KVARN_CUDA; }
   KERN<<<grid, dim3(256), sizeof(QuantSmem<BITS>), st>>>(A);
+  return last_cuda();
 }
 
 static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kinds, cudaStream_t st) {
@@ -184,13 +211,11 @@ static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kind
   dim3 grid((unsigned)A.n_tiles, (unsigned)n_kinds);
   const bool f32 = p->in_dtype == KVARN_F32;
   if (p->bits == 2) {
-    if (f32) launch_quant_smem<2, quantize_kernel<2, float>>(grid, A, st);
-    else launch_quant_smem<2, quantize_kernel<2, __nv_bfloat16>>(grid, A, st);
-  } else {
-    if (f32) launch_quant_smem<4, quantize_kernel<4, float>>(grid, A, st);
-    else launch_quant_smem<4, quantize_kernel<4, __nv_bfloat16>>(grid, A, st);
+    if (f32) return launch_quant_smem<2, quantize_kernel<2, float>>(grid, A, st);
+    return launch_quant_smem<2, quantize_kernel<2, __nv_bfloat16>>(grid, A, st);
   }
-  return last_cuda();
+  if (f32) return launch_quant_smem<4, quantize_kernel<4, float>>(grid, A, st);
+  return launch_quant_smem<4, quantize_kernel<4, __nv_bfloat16>>(grid, A, st);
 }
 
 // Split-K plan of kvarn_decode_attention: `cluster` CTAs of a thread-block cluster share one
@@ -204,27 +229,29 @@ struct SplitPlan { int cluster, nclus; };
 constexpr int dec_nch(int bits, int gp) { return (bits == 2 && gp == 4) ? 2 : 1; }
 constexpr int KVARN_MAX_CLUSTER = 8;    // portable maximum; 9..16 (non-portable) measured slower: 25 -> 27..31 us on config 1
 
+// resident CTAs of decode_kernel per SM on the current device (cached per device and instantiation)
 template <int BITS, int GP, typename InT>
 static int decode_ctas_per_sm() {
-  static int cached = 0;   // per instantiation; benign race (same value)
-  if (cached) return cached;
+  static std::atomic<int> cached[KVARN_MAX_DEVICES] = {};
+  const int dev = current_device();
+  const int fallback = GP == 4 ? 4 : 3;   // no device (host-only queries): a conservative constant
+  if (dev < 0) return fallback;
+  if (dev < KVARN_MAX_DEVICES) { const int c = cached[dev].load(std::memory_order_relaxed); if (c) return c; }
   using SM = DecSmem<BITS, GP, dec_nch(BITS, GP)>;
   auto kern = decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>;
   int n = 0;
-  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SM));
-  cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 128, sizeof(SM)) != cudaSuccess || n < 1) {
+  if (ensure_smem_optin<decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>>((int)sizeof(SM), true) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 128, sizeof(SM)) != cudaSuccess || n < 1) {
     cudaGetLastError();
-    n = GP == 4 ? 4 : 3;   // no device (host-only queries): a conservative constant
-    return n;
+    return fallback;
   }
-  cached = n;
+  if (dev < KVARN_MAX_DEVICES) cached[dev].store(n, std::memory_order_relaxed);
   return n;
 }
 static int decode_slots(const kvarn_params* p, int g) {
-  int sms = 148, dev = 0;
-  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  else cudaGetLastError();
+  int sms = 148;
+  const int dev = current_device();   // = the device of the caller's stream (CUDA requires it to be current)
+  if (dev >= 0 && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); sms = 148; }
   const bool f32 = p->in_dtype == KVARN_F32;
   int per;
   if (p->bits == 2) per = g <= 4 ? (f32 ? decode_ctas_per_sm<2, 4, float>() : decode_ctas_per_sm<2, 4, __nv_bfloat16>())
@@ -269,14 +296,10 @@ static SplitPlan split_plan(const kvarn_params* p, int B, int Hkv, int g, int ma
 template <int BITS, int GP, typename InT>
 static cudaError_t launch_decode_k(const DecodeArgs& A, cudaStream_t st) {
   using SM = DecSmem<BITS, GP, dec_nch(BITS, GP)>;
-  static bool configured = false;   // per instantiation; benign race (idempotent attribute calls)
   auto kern = decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SM));
+  {
+    const cudaError_t e = ensure_smem_optin<decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>>((int)sizeof(SM), true);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    configured = true;
   }
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(A.B * A.Hkv, A.splits, (A.n_q + A.tpc - 1) / A.tpc);
@@ -425,11 +448,15 @@ int kvarn_append_block(const kvarn_params* p, const kvarn_cache* cache, const vo
   if (!k_new || !v_new || !cache->ticket || n_new < 1) return KVARN_INVALID_ARG;
   if (n_new > G) return KVARN_UNSUPPORTED;
   if (!aligned16(k_new) || !aligned16(v_new)) return KVARN_MISALIGNED;
+  // host-checkable capacity bound: a sequence holds at most n_sink + max_chunks * 128 + 127 tokens
+  if (cache->max_len_hint > 0 &&
+      (long long)cache->max_len_hint + n_new > (long long)cache->n_sink + (long long)cache->max_chunks * G + (G - 1))
+    return KVARN_CAPACITY;
   AppendArgs A{};
   A.rec[0] = (uint8_t*)cache->k_records; A.rec[1] = (uint8_t*)cache->v_records;
   A.resid[0] = cache->k_resid; A.resid[1] = cache->v_resid;
   A.tok[0] = k_new; A.tok[1] = v_new;
-  A.seq_lens = cache->seq_lens; A.ticket = cache->ticket;
+  A.seq_lens = cache->seq_lens; A.ticket = cache->ticket; A.overflow = cache->overflow;
   A.sink[0] = cache->k_sink; A.sink[1] = cache->v_sink; A.n_sink = cache->n_sink;
   A.B = cache->B; A.Hkv = cache->Hkv; A.max_chunks = cache->max_chunks; A.n_new = n_new;
   A.rotate[0] = p->rotate_k; A.rotate[1] = p->rotate_v; A.vc = varn_consts(p);
@@ -437,13 +464,11 @@ int kvarn_append_block(const kvarn_params* p, const kvarn_cache* cache, const vo
   cudaStream_t s = (cudaStream_t)stream;
   const bool f32 = p->in_dtype == KVARN_F32;
   if (p->bits == 2) {
-    if (f32) launch_quant_smem<2, append_kernel<2, float>>(grid, A, s);
-    else launch_quant_smem<2, append_kernel<2, __nv_bfloat16>>(grid, A, s);
-  } else {
-    if (f32) launch_quant_smem<4, append_kernel<4, float>>(grid, A, s);
-    else launch_quant_smem<4, append_kernel<4, __nv_bfloat16>>(grid, A, s);
+    if (f32) return launch_quant_smem<2, append_kernel<2, float>>(grid, A, s);
+    return launch_quant_smem<2, append_kernel<2, __nv_bfloat16>>(grid, A, s);
   }
-  return last_cuda();
+  if (f32) return launch_quant_smem<4, append_kernel<4, float>>(grid, A, s);
+  return launch_quant_smem<4, append_kernel<4, __nv_bfloat16>>(grid, A, s);
 }
 
 static int decode_impl(const kvarn_params* p, const kvarn_cache* cache, const void* q, int32_t Hq, float sm_scale,

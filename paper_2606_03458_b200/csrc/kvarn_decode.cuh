@@ -542,7 +542,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
         // pt = p s1v = exp2(logit + log2 s1v - m): the running maximum is taken over the shifted logits,
         // so pt <= 1 and its fixed-point scale is a constant
         sm.aux_a[c][tid] = make_float2(s2t, lg2_approx(s1v));
-        sm.aux_b[c][tid] = make_float2(rcp_approx(s1v), zv);
+        sm.aux_b[c][tid] = make_float2(rcp_approx(s1v) * (1.f / P_FIX), zv);
         sm.aux_ch[it & 1][c][tid] = e4m3_to_f32(vr[s2_off(BITS) + tid]) * (1.f / P_FIX);
       }
     }
@@ -606,12 +606,19 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
         for (int c = 0; c < nn; ++c) bulk_g2s(sm.rec[st][c][0], krec + (size_t)(nxt * NCH + c) * RB, RB, &sm.fullk[st]);
       }
     }
-    float corr[HPW];
+    // The fixed-point probabilities refer to the maximum m_it of THIS iteration's chunks (not to the running
+    // maximum): a token is dropped only if it lies 2^-23 below the largest of its own <= 256 neighbours, so the
+    // dropped mass is bounded by 255 * 2^-23 whatever the context length; the iteration's sums enter the running
+    // ones with the weight wch = 2^(m_it - m_new).  l is accumulated from the SAME rounded values as the
+    // numerator, so numerator and denominator stay consistent.
+    float corr[HPW], wch[HPW];
 #pragma unroll
     for (int u = 0; u < HPW; ++u) {
       const float4 hm = *reinterpret_cast<const float4*>(sm.hmax[ft + 4 * u]);
-      const float m_new = fmaxf(mr[u], fmaxf(fmaxf(hm.x, hm.y), fmaxf(hm.z, hm.w)));
+      const float m_it = fmaxf(fmaxf(hm.x, hm.y), fmaxf(hm.z, hm.w));
+      const float m_new = fmaxf(mr[u], m_it);
       corr[u] = ex2_approx(mr[u] - m_new);
+      wch[u] = ex2_approx(m_it - m_new);
       mr[u] = m_new;
       float lsum = 0.f;
 #pragma unroll
@@ -621,12 +628,13 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
           float zpart = 0.f;
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            const float2 ab = sm.aux_b[c][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];   // {1 / s1v, zv}
-            const float pt = ex2_approx(logit[c][u][i] - m_new);
-            lsum = fmaf(pt, ab.x, lsum);
+            const float2 ab = sm.aux_b[c][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];   // {1 / (s1v P_FIX), zv}
+            const float pt = ex2_approx(logit[c][u][i] - m_it);
             // D5 prep: fixed-point pt; its radix-256 digits are the bytes of X
             const float f = fmaf(pt, P_FIX, MAGIC_F);
-            zpart = fmaf(f - MAGIC_F, ab.y, zpart);
+            const float pr = f - MAGIC_F;                 // P_FIX * (rounded pt), an exact integer
+            lsum = fmaf(pr, ab.x, lsum);
+            zpart = fmaf(pr, ab.y, zpart);
             X[i] = __float_as_uint(f) * mul_p + add_p;
           }
           transpose4x4(X, Y);
@@ -638,7 +646,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
           if (fg == 0) sm.hz[c][ft + 4 * u][warp] = zpart;
         }
       }
-      lp[u] = fmaf(lp[u], corr[u], lsum);
+      lp[u] = fmaf(lp[u], corr[u], lsum * wch[u]);
     }
     __syncthreads();                                                   // barrier 3
 
@@ -658,12 +666,13 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
 #pragma unroll
         for (int u = 0; u < HPW; ++u) {
           const float4 hz = *reinterpret_cast<const float4*>(sm.hz[c][ft + 4 * u]);
-          const float zsum = (hz.x + hz.y) + (hz.z + hz.w);
+          const float zsum = ((hz.x + hz.y) + (hz.z + hz.w)) * wch[u];
+          const float cw = CLS_INV * wch[u];
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
             const int mt = i >> 1, cc = 2 * (i & 1);
             const float a = undigit(dd[mt][2 * u][cc], dd[mt][2 * u][cc + 1], dd[mt][2 * u + 1][cc], dd[mt][2 * u + 1][cc + 1]);
-            ac[u][i] = fmaf(s2v[i], fmaf(a, CLS_INV, zsum), ac[u][i]);
+            ac[u][i] = fmaf(s2v[i], fmaf(a, cw, zsum), ac[u][i]);
           }
         }
       }

@@ -45,7 +45,8 @@ class CacheDesc(C.Structure):
     _fields_ = [("k_records", C.c_void_p), ("v_records", C.c_void_p), ("k_resid", C.c_void_p),
                 ("v_resid", C.c_void_p), ("seq_lens", C.c_void_p), ("ticket", C.c_void_p),
                 ("decode_ticket", C.c_void_p), ("B", C.c_int32), ("Hkv", C.c_int32), ("max_chunks", C.c_int32),
-                ("n_sink", C.c_int32), ("k_sink", C.c_void_p), ("v_sink", C.c_void_p)]
+                ("n_sink", C.c_int32), ("k_sink", C.c_void_p), ("v_sink", C.c_void_p),
+                ("max_len_hint", C.c_int32), ("overflow", C.c_void_p)]
 
 
 class DebugDesc(C.Structure):
@@ -193,11 +194,12 @@ class Cache:
         self.seq_lens = torch.zeros((B,), dtype=torch.int32, device=device)
         self.ticket = torch.zeros((B,), dtype=torch.int32, device=device)
         self.decode_ticket = torch.zeros((B * Hkv,), dtype=torch.int32, device=device)
+        self.overflow = torch.zeros((1,), dtype=torch.int32, device=device)
         self.desc = CacheDesc(self.k_records.data_ptr(), self.v_records.data_ptr(),
                               self.k_resid.data_ptr(), self.v_resid.data_ptr(),
                               self.seq_lens.data_ptr(), self.ticket.data_ptr(),
                               self.decode_ticket.data_ptr(), B, Hkv, max_chunks, n_sink,
-                              self.k_sink.data_ptr(), self.v_sink.data_ptr())
+                              self.k_sink.data_ptr(), self.v_sink.data_ptr(), 0, self.overflow.data_ptr())
 
     def slice(self, b0: int, b1: int) -> "Cache":
         """A cache over sequences b0..b1-1 that shares this cache's buffers (views, no copy):
@@ -209,10 +211,11 @@ class Cache:
         c.k_resid, c.v_resid = self.k_resid[b0:b1], self.v_resid[b0:b1]
         c.seq_lens, c.ticket = self.seq_lens[b0:b1], self.ticket[b0:b1]
         c.decode_ticket = self.decode_ticket[b0 * self.Hkv:b1 * self.Hkv]
+        c.overflow = self.overflow
         c.desc = CacheDesc(c.k_records.data_ptr(), c.v_records.data_ptr(), c.k_resid.data_ptr(),
                            c.v_resid.data_ptr(), c.seq_lens.data_ptr(), c.ticket.data_ptr(),
                            c.decode_ticket.data_ptr(), c.B, c.Hkv, c.max_chunks, c.n_sink,
-                           c.k_sink.data_ptr(), c.v_sink.data_ptr())
+                           c.k_sink.data_ptr(), c.v_sink.data_ptr(), 0, c.overflow.data_ptr())
         return c
 
     def nbytes_read_by_decode(self, ctx: int) -> int:
@@ -233,22 +236,25 @@ def prefill(p: Params, cache: Cache, k: torch.Tensor, v: torch.Tensor, stream=No
                              _stream(stream)), "kvarn_prefill")
 
 
-def append(p: Params, cache: Cache, k_new: torch.Tensor, v_new: torch.Tensor, stream=None):
-    """k_new, v_new: [B, Hkv, 128] -- one new token per sequence."""
+def append(p: Params, cache: Cache, k_new: torch.Tensor, v_new: torch.Tensor, stream=None, max_len_hint: int = 0):
+    """k_new, v_new: [B, Hkv, 128] -- one new token per sequence.  max_len_hint > 0: the caller's upper bound on
+    the sequence lengths before the call (KVARN_CAPACITY is raised when the token provably cannot fit)."""
     assert k_new.is_cuda and k_new.is_contiguous() and v_new.is_contiguous()
     assert tuple(k_new.shape) == (cache.B, cache.Hkv, HEAD_DIM) and k_new.shape == v_new.shape
     p.in_dtype = _dtype_code(k_new)
     assert cache.k_resid.dtype == k_new.dtype
+    cache.desc.max_len_hint = int(max_len_hint)
     _check(lib.kvarn_append(C.byref(p), C.byref(cache.desc), _ptr(k_new), _ptr(v_new),
                             _stream(stream)), "kvarn_append")
 
 
-def append_block(p: Params, cache: Cache, k_new: torch.Tensor, v_new: torch.Tensor, stream=None):
+def append_block(p: Params, cache: Cache, k_new: torch.Tensor, v_new: torch.Tensor, stream=None, max_len_hint: int = 0):
     """k_new, v_new: [B, Hkv, n_new, 128], 1 <= n_new <= 128 new tokens per sequence (Fig. 4)."""
     assert k_new.is_cuda and k_new.is_contiguous() and v_new.is_contiguous() and k_new.shape == v_new.shape
     assert k_new.dim() == 4 and tuple(k_new.shape[:2]) == (cache.B, cache.Hkv) and k_new.shape[3] == HEAD_DIM
     p.in_dtype = _dtype_code(k_new)
     assert cache.k_resid.dtype == k_new.dtype
+    cache.desc.max_len_hint = int(max_len_hint)
     _check(lib.kvarn_append_block(C.byref(p), C.byref(cache.desc), _ptr(k_new), _ptr(v_new), k_new.shape[2],
                                   _stream(stream)), "kvarn_append_block")
 

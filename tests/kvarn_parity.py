@@ -5,10 +5,12 @@ from __future__ import annotations
 import numpy as np
 import torch
 
+from oracle import fanout
 from oracle import kvarn_oracle as O
 
 # Tolerances (BASELINE.json north_star)
 CODE_MISMATCH_FRAC = 1e-4     # codes bit-exact except fp32 rounding ties, each off by one level
+AUX_MISMATCH_FRAC = 1e-4      # stored FP8 / FP16 values vs the oracle's: rounding ties only, same budget
 SCALE_RTOL = 1e-5             # pre-storage scales and zero-points vs the oracle at the kernel's k
 IMB_ACCEPT = 1e-5             # reading R10: any iterate within this of the best imbalance is valid
 ATTN_RTOL = 2e-3              # per (b, q head): max|out - ref| / max|ref|
@@ -18,60 +20,85 @@ def tile_f64(x: torch.Tensor) -> np.ndarray:
     return x.detach().to(torch.float64).cpu().numpy()
 
 
-def check_quantized_tile(kv, p, kind: int, X: np.ndarray, rec: np.ndarray, k_gpu: int,
-                         imb_gpu: np.ndarray, aux_gpu: np.ndarray, stats: dict):
-    """Compare one GPU record (+ debug outputs) against the oracle on tile X[t, c]."""
-    kname = "k" if kind == 0 else "v"
-    mode = "before" if p.aux_round else "after"      # reading R9 / R9b
+def _tile_job(p, kind: int, X: np.ndarray, k_gpu: int):
+    """Arguments of oracle.fanout's 'quantize' worker for one tile."""
+    X = np.asarray(X)
+    if X.dtype != np.float32:      # inputs are bf16 or fp32 values: float32 holds them exactly (and pickles at half the size)
+        assert np.array_equal(X.astype(np.float32).astype(X.dtype), X)
+        X = X.astype(np.float32)
+    return (X, "k" if kind == 0 else "v", int(p.bits), int(p.iters),
+            bool(p.rotate_k if kind == 0 else p.rotate_v), "before" if p.aux_round else "after", int(k_gpu))
+
+
+def compare_quantized_tile(kv, p, kind: int, rec: np.ndarray, k_gpu: int, imb_gpu: np.ndarray,
+                           aux_gpu: np.ndarray, ref: dict, stats: dict):
+    """One GPU record (+ debug outputs) against the oracle's result `ref` (oracle.fanout 'quantize' worker:
+    the free-running trajectory I and the tile quantised at the kernel's iterate k_gpu)."""
     codes, s1, s2, z = kv.unpack_record(p, kind, rec)
-    ref_free = O.quantize_tile(X, kname, bits=p.bits, iters=p.iters, aux_round=mode,
-                               rotate_on=bool(p.rotate_k if kind == 0 else p.rotate_v))
-    I = np.array(ref_free.varn.I)
+    I = ref["I"]
     # (1) the iterate kept by the kernel is a valid choice of Alg. 1 line 18 (R10)
     assert 0 <= k_gpu <= p.iters
     assert I[k_gpu] <= I.min() * (1 + IMB_ACCEPT), (k_gpu, I)
-    # (2) imbalance trajectory
+    # (2) imbalance trajectory: a ratio of two variances, each a function of scales that agree to SCALE_RTOL
+    #     (squared: 2 x) -> 4 x SCALE_RTOL
     n = p.iters + 1
-    assert np.allclose(imb_gpu[:n], I[:n], rtol=2e-4), (imb_gpu[:n], I[:n])
+    assert np.allclose(imb_gpu[:n], I[:n], rtol=4 * SCALE_RTOL), (imb_gpu[:n], I[:n])
     # (3) pre-storage scales / zero-points at the kernel's k
-    ref = O.quantize_tile(X, kname, bits=p.bits, iters=p.iters, at_k=k_gpu, aux_round=mode,
-                          rotate_on=bool(p.rotate_k if kind == 0 else p.rotate_v))
     s1_f, s2_f, z_f = aux_gpu[0].astype(np.float64), aux_gpu[1].astype(np.float64), aux_gpu[2].astype(np.float64)
-    assert np.allclose(s1_f, ref.s1_f, rtol=SCALE_RTOL, atol=0), np.abs(s1_f / ref.s1_f - 1).max()
-    assert np.allclose(s2_f, ref.s2_f, rtol=SCALE_RTOL, atol=0), np.abs(s2_f / ref.s2_f - 1).max()
+    assert np.allclose(s1_f, ref["s1_f"], rtol=SCALE_RTOL, atol=0), np.abs(s1_f / ref["s1_f"] - 1).max()
+    assert np.allclose(s2_f, ref["s2_f"], rtol=SCALE_RTOL, atol=0), np.abs(s2_f / ref["s2_f"] - 1).max()
     # z = mn / s is O(1..10) in code units; tolerance relative to the code range
     # (R9b: z = mn / stored step, so it is only comparable where the stored s1 agrees -- an FP8 tie moves it by 6 %)
-    zcmp = (s1 == ref.s1) if p.aux_round else np.ones(128, dtype=bool)
-    assert np.allclose(z_f[zcmp], ref.z_f[zcmp], rtol=SCALE_RTOL, atol=SCALE_RTOL * (1 << p.bits)), np.abs(z_f - ref.z_f)[zcmp].max()
+    zcmp = (s1 == ref["s1"]) if p.aux_round else np.ones(128, dtype=bool)
+    assert np.allclose(z_f[zcmp], ref["z_f"][zcmp], rtol=SCALE_RTOL, atol=SCALE_RTOL * (1 << p.bits)), \
+        np.abs(z_f - ref["z_f"])[zcmp].max()
     # (4) stored bytes = storage rounding of the kernel's own fp32 values
     st_mis = int((s1.astype(np.float64) != O.round_fp8_e4m3(s1_f)).sum()
                  + (s2.astype(np.float64) != O.round_fp8_e4m3(s2_f)).sum()
                  + (z.astype(np.float64) != O.round_fp16(z_f)).sum())
     assert st_mis == 0
     # ... and equal the oracle's stored values except at rounding ties
-    aux_mis = int((s1 != ref.s1).sum() + (s2 != ref.s2).sum() + (z != ref.z).sum())
+    fp8_mis = int((s1 != ref["s1"]).sum() + (s2 != ref["s2"]).sum())
+    z_mis = int((z != ref["z"]).sum())
     # (5) codes
-    diff = codes.astype(np.int32) - ref.codes.astype(np.int32)
+    diff = codes.astype(np.int32) - ref["codes"].astype(np.int32)
     if p.aux_round:
         # R9b: the codes are taken against the STORED parameters, so a group whose stored s1 / z (or an
         # element whose stored second scale) differs from the oracle's by a rounding tie is not comparable
-        # element by element; those ties are already counted in aux_mis against the aux budget
-        grp_ok, oth_ok = (s1 == ref.s1) & (z == ref.z), (s2 == ref.s2)
+        # element by element; those ties are already counted against the aux budget
+        grp_ok, oth_ok = (s1 == ref["s1"]) & (z == ref["z"]), (s2 == ref["s2"])
         ok = (oth_ok[:, None] & grp_ok[None, :]) if kind == 0 else (grp_ok[:, None] & oth_ok[None, :])   # [t, c]
         diff = np.where(ok, diff, 0)
     assert np.abs(diff).max() <= 1
-    stats["codes"] = stats.get("codes", 0) + diff.size
-    stats["code_mismatch"] = stats.get("code_mismatch", 0) + int((diff != 0).sum())
-    stats["aux"] = stats.get("aux", 0) + 384
-    stats["aux_mismatch"] = stats.get("aux_mismatch", 0) + aux_mis
+    for key, val in (("tiles", 1), ("codes", diff.size), ("code_mismatch", int((diff != 0).sum())), ("aux", 384),
+                     ("aux_mismatch", fp8_mis + z_mis), ("fp8_mismatch", fp8_mis), ("z_mismatch", z_mis),
+                     ("k_differs", int(k_gpu != ref["k_free"]))):
+        stats[key] = stats.get(key, 0) + val
     return codes, s1, s2, z
 
 
+def check_quantized_tile(kv, p, kind: int, X: np.ndarray, rec: np.ndarray, k_gpu: int,
+                         imb_gpu: np.ndarray, aux_gpu: np.ndarray, stats: dict):
+    """Compare one GPU record (+ debug outputs) against the oracle on tile X[t, c]."""
+    ref = fanout.WORKERS["quantize"](_tile_job(p, kind, X, k_gpu))
+    return compare_quantized_tile(kv, p, kind, rec, k_gpu, imb_gpu, aux_gpu, ref, stats)
+
+
+def check_quantized_tiles(kv, p, kind: int, Xs, recs, k_gpus, imbs, auxs, stats: dict, procs=None):
+    """The same for many tiles, the oracle fanned out over the host cores (oracle/fanout.py)."""
+    refs = fanout.pmap("quantize", [_tile_job(p, kind, X, k) for X, k in zip(Xs, k_gpus)], procs)
+    for rec, k, imb, aux, ref in zip(recs, k_gpus, imbs, auxs, refs):
+        compare_quantized_tile(kv, p, kind, rec, int(k), imb, aux, ref, stats)
+
+
 def assert_mismatch_budget(stats: dict):
+    """north_star: at most 1e-4 of the codes differ (each by one level).  Stored aux values:
+    the same 1e-4 budget; a test over fewer than 10^4 stored values is allowed ONE tie (a budget below one
+    value would turn every legal tie into a failure): DESIGN.md "Tolerances" derives the expected rate
+    (dominated by the FP16 zero-points) and tests/test_gpu_parity_full.py measures it over > 5000 tiles."""
     frac = stats["code_mismatch"] / max(stats["codes"], 1)
     assert frac <= CODE_MISMATCH_FRAC, f"code mismatch fraction {frac:.2e}"
-    # stored aux values differ from the oracle's only at FP8/FP16 rounding ties
-    assert stats["aux_mismatch"] <= max(2, 2e-3 * stats["aux"]), stats
+    assert stats["aux_mismatch"] <= max(1, int(np.ceil(AUX_MISMATCH_FRAC * stats["aux"]))), stats
 
 
 def oracle_attention_from_records(kv, p, k_recs, v_recs, k_resid, v_resid, q, sm_scale=None):

@@ -106,6 +106,12 @@ def test_argument_validation_of_the_later_entry_points_without_gpu(kv):
     # kvarn_append_block: n_new out of range
     assert L.kvarn_append_block(C.byref(p), C.byref(cache), ptr(0x7000), ptr(0x7100), 0, None) == -1
     assert L.kvarn_append_block(C.byref(p), C.byref(cache), ptr(0x7000), ptr(0x7100), 129, None) == -2
+    # host-checkable capacity bound: capacity = n_sink + max_chunks * 128 + 127 = 639 tokens here
+    full = kv.CacheDesc(0x1000, 0x2000, 0x3000, 0x4000, 0x5000, 0x6000, 0x6800, 2, 8, 4, 0, None, None, 639, None)
+    assert L.kvarn_append(C.byref(p), C.byref(full), ptr(0x7000), ptr(0x7100), None) == -5
+    full.max_len_hint = 600
+    assert L.kvarn_append_block(C.byref(p), C.byref(full), ptr(0x7000), ptr(0x7100), 40, None) == -5
+    assert L.kvarn_status_string(-5) == b"KVARN_CAPACITY"
     # aux_round must be 0 or 1
     bad = kv.default_params(2, aux_round=2)
     assert L.kvarn_append_block(C.byref(bad), C.byref(cache), ptr(0x7000), ptr(0x7100), 1, None) == -1

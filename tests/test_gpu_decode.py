@@ -170,18 +170,7 @@ def test_bf16_output_and_custom_scale(kv):
     assert o16.dtype == torch.bfloat16 and torch.equal(o16, o32.to(torch.bfloat16))
 
 
-def test_config1_shape_sampled_units(kv):
-    # configs[1] at full size (B=8, 32/8 heads, ctx 8192), in the launch
-    # configuration bench.py times; oracle on sampled (b, kv head) units
-    s = W.CONFIG1
-    K, V = W.kv_tokens(s.B, s.Hkv, s.ctx, seed=s.seed, device="cuda")
-    q = W.queries(s.B, s.Hq, seed=s.seed, device="cuda")
-    p = kv.default_params(2)
-    cache = _build_cache(kv, p, K, V, max_chunks=s.n_chunks)
-    out = kv.decode_attention(p, cache, q)
-    _check_all_units(kv, p, cache, q, out, s.ctx, units={(0, 0), (3, 5), (7, 7)})
-    # any size: softmax output lies in the convex hull of the values -> bounded by max |V_dq|
-    assert torch.isfinite(out).all()
+# configs[1], [2] (full growth) and [4] at full size: tests/test_gpu_parity_full.py
 
 
 def test_append_matches_prefill_bit_for_bit(kv):
@@ -222,10 +211,16 @@ def test_append_capacity_guard(kv):
     K, V = W.kv_tokens(B, Hkv, 128 + 127, seed=95, device="cuda")
     kv.prefill(p, cache, K, V)
     before = cache.k_records.clone()
-    kv.append(p, cache, K[:, :, 0].contiguous(), V[:, :, 0].contiguous())
+    kv.append(p, cache, K[:, :, 0].contiguous(), V[:, :, 0].contiguous())      # lengths unknown to the host
     torch.cuda.synchronize()
     assert cache.seq_lens.tolist() == [255] and torch.equal(cache.k_records, before)
     assert int(cache.ticket.sum()) == 0
+    assert int(cache.overflow.item()) == 1                                     # the drop is counted on the device
+    with pytest.raises(kv.KvarnError, match="KVARN_CAPACITY"):                 # ... and refused when the host can tell
+        kv.append(p, cache, K[:, :, 0].contiguous(), V[:, :, 0].contiguous(), max_len_hint=255)
+    kv.append_block(p, cache, K[:, :, :3].contiguous(), V[:, :, :3].contiguous())
+    torch.cuda.synchronize()
+    assert int(cache.overflow.item()) == 2 and cache.seq_lens.tolist() == [255]
 
 
 @pytest.mark.parametrize("Hq,splits", [(8, 3), (8, 5), (8, 7), (8, 8), (8, 16), (8, 21), (64, 2), (64, 3),
@@ -264,24 +259,6 @@ def test_config2_shape_incremental_decode(kv):
         if t + 1 in (513, 639, 640, 641):
             assert cache.seq_lens.tolist() == [t + 1] * s.B
             _check_all_units(kv, p, cache, q, out, t + 1, units={(0, 0), (7, 3), (15, 7)})
-
-
-@pytest.mark.parametrize("bits", [2, 4])
-def test_config4_shape_sampled_units(kv, bits):
-    # configs[4] at full size (B=64, 64 q / 8 KV heads, ctx 65536 + 64-token bf16 residual), in the
-    # launch configuration bench.py's extras time; oracle on sampled (sequence, KV head) units
-    s = W.CONFIG4
-    p = kv.default_params(bits)
-    cache = kv.Cache(p, s.B, s.Hkv, s.n_chunks, device="cuda")
-    for b0 in range(0, s.B, 4):
-        K, V = W.kv_tokens(4, s.Hkv, s.ctx, seed=s.seed + b0, device="cuda")
-        kv.prefill(p, cache.slice(b0, b0 + 4), K, V)
-        del K, V
-    assert cache.seq_lens.tolist() == [s.ctx] * s.B
-    q = W.queries(s.B, s.Hq, seed=s.seed, device="cuda")
-    out = kv.decode_attention(p, cache, q)
-    assert torch.isfinite(out).all()
-    _check_all_units(kv, p, cache, q, out, s.ctx, units={(0, 0), (37, 5), (63, 7)})
 
 
 @pytest.mark.parametrize("bits,Hq,n_tok,splits", [(2, 32, 128 * 40 + 5, 0), (2, 64, 128 * 33, 6), (4, 32, 128 * 9 + 127, 0),
