@@ -254,8 +254,9 @@ def _fill_cache(kv, W, p, sh, dev, n_sink=0, max_chunks=None):
 
 def run_extras(kv, W, dev, hbm_peak, only=frozenset()):
     """The other configs, one B200 (N = 1 only).  Groups (select with --extras-only --only a,b):
-      decode  configs[4] (B=64, 64 q / 8 KV heads, ctx 65536 + 64 residual) and a 64k-context g = 4 cache (B=16, 32/8
-              heads), 2-bit and 4-bit; block attention (n_q = 2, 8) and kvarn_append_block on the latter
+      decode  = cfg4 + long.  cfg4: configs[4] (B=64, 64 q / 8 KV heads, ctx 65536 + 64 residual), 2-bit and 4-bit;
+              long: a 64k-context g = 4 cache (B=16, 32/8 heads), 2-bit and 4-bit, + block attention (n_q = 2, 8) and
+              kvarn_append_block on it
       sink    the same g = 4 cache in the paper's three-region layout with S = 128 raw sink tokens
       cfg2    configs[2]: the last 256 steps of the growth to 32768 tokens, one append + one decode per step
       quant   configs[3]: 8 heads x 2^20 tokens in one launch, 2-bit and 4-bit; the paper's 576-tile latency case
@@ -264,9 +265,10 @@ def run_extras(kv, W, dev, hbm_peak, only=frozenset()):
     stream = torch.cuda.current_stream()
     want = lambda g: not only or g in only
     ex = {}
-    if want("decode"):
+    if want("decode") or want("cfg4") or want("long"):
         long_g4 = W.DecodeShape("long_context_g4", B=16, Hq=32, Hkv=8, ctx=65536, seed=5)   # Llama-3.1-8B heads, 64k context
-        for name, sh in (("decode_cfg4", W.CONFIG4), ("decode_long_g4", long_g4)):
+        shapes = [("decode_cfg4", W.CONFIG4)] * (want("decode") or want("cfg4")) + [("decode_long_g4", long_g4)] * (want("decode") or want("long"))
+        for name, sh in shapes:
             for bits in (2, 4):
                 p = kv.default_params(bits)
                 cache = _fill_cache(kv, W, p, sh, dev)

@@ -86,6 +86,10 @@ typedef struct {
                       * tile is balanced and RTN runs against the STORED step s1 / absorbed scale and the
                       * stored FP16 zero-point, so the FP8 error of the scales is absorbed by the codes
                       * (P:382 does not say which; at 4-bit it cuts the token-magnitude error ~3x). */
+  int32_t decode_digits; /* precision of the decode kernel's integer tensor-core operands.  0 (default): q~ 22-bit, p~ 16-bit
+                      * fixed point (four / two radix-256 digit planes); 2 (2-bit caches): q~ 15 bits + sign, p~ 16 bits
+                      * (half the tensor-core work; error up to ~1e-3 of the 2e-3 tolerance on short, peaked contexts);
+                      * 4: 22 / 22 bits. */
 } kvarn_params;
 
 /* Byte layout of one record (fixed by bits): codes | s1[128] e4m3 | s2[128] e4m3 | z[128] f16.

@@ -155,6 +155,7 @@ static int check_params(const kvarn_params* p) {
   if (p->bits != 2 && p->bits != 4) return KVARN_UNSUPPORTED;
   if (p->iters < 0 || p->iters > KVARN_MAX_ITERS) return KVARN_INVALID_ARG;
   if (p->aux_round != 0 && p->aux_round != 1) return KVARN_INVALID_ARG;
+  if (p->decode_digits != 0 && p->decode_digits != 2 && p->decode_digits != 4) return KVARN_INVALID_ARG;
   if (p->in_dtype != KVARN_BF16 && p->in_dtype != KVARN_F32) return KVARN_UNSUPPORTED;
   if (p->out_dtype != KVARN_BF16 && p->out_dtype != KVARN_F32) return KVARN_UNSUPPORTED;
   if (!(p->var_min > 0.f) || !(p->var_max >= p->var_min) || !(p->log_hi >= p->log_lo)) return KVARN_INVALID_ARG;
@@ -222,26 +223,51 @@ static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kind
 // (sequence, KV head) and merge through DSMEM; `nclus` clusters per (sequence, KV head) merge
 // through the workspace (only when one cluster leaves most of the GPU idle on long contexts).
 struct SplitPlan { int cluster, nclus; };
-// chunks per loop iteration of decode_kernel: two at 2-bit with g <= 4 (two independent instruction
-// streams per warp between barriers: 205 -> 193 us on the long-context case); one otherwise -- at 4-bit the
-// kernel already runs at ~0.8 of the HBM peak and the doubled record ring would leave two CTAs per SM,
-// at g = 8 the doubled register footprint (222) measured slower (346 -> 363 us)
-constexpr int dec_nch(int bits, int gp) { return (bits == 2 && gp == 4) ? 2 : 1; }
 constexpr int KVARN_MAX_CLUSTER = 8;    // portable maximum; 9..16 (non-portable) measured slower: 25 -> 27..31 us on config 1
 
-// resident CTAs of decode_kernel per SM on the current device (cached per device and instantiation)
-template <int BITS, int GP, typename InT>
-static int decode_ctas_per_sm() {
+// DQ, DP = digit planes of q~ / p~ (kvarn_decode.cuh)
+template <int BITS, int GP, int DQ, int DP, typename InT>
+struct DecKernel {
+  static constexpr size_t smem = sizeof(DecSmemW<BITS, GP, DQ, DP>);
+  static auto kern() { return decode_kernel_w<BITS, GP, DQ, DP, InT>; }
+  static cudaError_t optin() { return ensure_smem_optin<decode_kernel_w<BITS, GP, DQ, DP, InT>>((int)smem, true); }
+};
+
+// Calls f(DecKernel<...>{}) for the instantiation that serves (params, gp = 4 | 8 columns per CTA).
+// kvarn_params::decode_digits: 0 = (DQ, DP) = (4, 2), 2 = (2, 2) [4-bit caches: (4, 2)], 4 = (4, 4).
+template <class F>
+static auto with_decode_kernel(const kvarn_params* p, int gp, F&& f) {
+  const bool f32 = p->in_dtype == KVARN_F32;
+  const int dig = p->decode_digits;
+  if (p->bits == 2) {
+    if (gp == 4) {
+      if (dig == 2) return f32 ? f(DecKernel<2, 4, 2, 2, float>{}) : f(DecKernel<2, 4, 2, 2, __nv_bfloat16>{});
+      if (dig == 4) return f32 ? f(DecKernel<2, 4, 4, 4, float>{}) : f(DecKernel<2, 4, 4, 4, __nv_bfloat16>{});
+      return f32 ? f(DecKernel<2, 4, 4, 2, float>{}) : f(DecKernel<2, 4, 4, 2, __nv_bfloat16>{});
+    }
+    if (dig == 2) return f32 ? f(DecKernel<2, 8, 2, 2, float>{}) : f(DecKernel<2, 8, 2, 2, __nv_bfloat16>{});
+    if (dig == 4) return f32 ? f(DecKernel<2, 8, 4, 4, float>{}) : f(DecKernel<2, 8, 4, 4, __nv_bfloat16>{});
+    return f32 ? f(DecKernel<2, 8, 4, 2, float>{}) : f(DecKernel<2, 8, 4, 2, __nv_bfloat16>{});
+  }
+  if (gp == 4) {
+    if (dig == 4) return f32 ? f(DecKernel<4, 4, 4, 4, float>{}) : f(DecKernel<4, 4, 4, 4, __nv_bfloat16>{});
+    return f32 ? f(DecKernel<4, 4, 4, 2, float>{}) : f(DecKernel<4, 4, 4, 2, __nv_bfloat16>{});
+  }
+  if (dig == 4) return f32 ? f(DecKernel<4, 8, 4, 4, float>{}) : f(DecKernel<4, 8, 4, 4, __nv_bfloat16>{});
+  return f32 ? f(DecKernel<4, 8, 4, 2, float>{}) : f(DecKernel<4, 8, 4, 2, __nv_bfloat16>{});
+}
+
+// resident CTAs of the decode kernel per SM on the current device (cached per device and instantiation)
+template <class DK>
+static int decode_ctas_per_sm(DK) {
   static std::atomic<int> cached[KVARN_MAX_DEVICES] = {};
   const int dev = current_device();
-  const int fallback = GP == 4 ? 4 : 3;   // no device (host-only queries): a conservative constant
+  const int fallback = 3;   // no device (host-only queries): a conservative constant
   if (dev < 0) return fallback;
   if (dev < KVARN_MAX_DEVICES) { const int c = cached[dev].load(std::memory_order_relaxed); if (c) return c; }
-  using SM = DecSmem<BITS, GP, dec_nch(BITS, GP)>;
-  auto kern = decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>;
   int n = 0;
-  if (ensure_smem_optin<decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>>((int)sizeof(SM), true) != cudaSuccess ||
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 128, sizeof(SM)) != cudaSuccess || n < 1) {
+  if (DK::optin() != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, DK::kern(), 128, DK::smem) != cudaSuccess || n < 1) {
     cudaGetLastError();
     return fallback;
   }
@@ -252,13 +278,7 @@ static int decode_slots(const kvarn_params* p, int g) {
   int sms = 148;
   const int dev = current_device();   // = the device of the caller's stream (CUDA requires it to be current)
   if (dev >= 0 && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); sms = 148; }
-  const bool f32 = p->in_dtype == KVARN_F32;
-  int per;
-  if (p->bits == 2) per = g <= 4 ? (f32 ? decode_ctas_per_sm<2, 4, float>() : decode_ctas_per_sm<2, 4, __nv_bfloat16>())
-                                 : (f32 ? decode_ctas_per_sm<2, 8, float>() : decode_ctas_per_sm<2, 8, __nv_bfloat16>());
-  else per = g <= 4 ? (f32 ? decode_ctas_per_sm<4, 4, float>() : decode_ctas_per_sm<4, 4, __nv_bfloat16>())
-                    : (f32 ? decode_ctas_per_sm<4, 8, float>() : decode_ctas_per_sm<4, 8, __nv_bfloat16>());
-  return sms * per;
+  return sms * with_decode_kernel(p, g <= 4 ? 4 : 8, [](auto dk) { return decode_ctas_per_sm(dk); });
 }
 
 static SplitPlan split_plan(const kvarn_params* p, int B, int Hkv, int g, int max_chunks) {
@@ -293,18 +313,17 @@ static SplitPlan split_plan(const kvarn_params* p, int B, int Hkv, int g, int ma
   return sp;
 }
 
-template <int BITS, int GP, typename InT>
-static cudaError_t launch_decode_k(const DecodeArgs& A, cudaStream_t st) {
-  using SM = DecSmem<BITS, GP, dec_nch(BITS, GP)>;
-  auto kern = decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>;
+template <class DK>
+static cudaError_t launch_decode_k(DK, const DecodeArgs& A, cudaStream_t st) {
+  auto kern = DK::kern();
   {
-    const cudaError_t e = ensure_smem_optin<decode_kernel<BITS, GP, dec_nch(BITS, GP), InT>>((int)sizeof(SM), true);
+    const cudaError_t e = DK::optin();
     if (e != cudaSuccess) return e;
   }
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(A.B * A.Hkv, A.splits, (A.n_q + A.tpc - 1) / A.tpc);
   cfg.blockDim = dim3(128, 1, 1);
-  cfg.dynamicSmemBytes = sizeof(SM);
+  cfg.dynamicSmemBytes = DK::smem;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -313,9 +332,8 @@ static cudaError_t launch_decode_k(const DecodeArgs& A, cudaStream_t st) {
   return cudaLaunchKernelEx(&cfg, kern, A);
 }
 
-template <int BITS, typename InT>
-static cudaError_t launch_decode(const DecodeArgs& A, cudaStream_t st) {
-  return A.tpc * A.g <= 4 ? launch_decode_k<BITS, 4, InT>(A, st) : launch_decode_k<BITS, 8, InT>(A, st);
+static cudaError_t launch_decode(const kvarn_params* p, const DecodeArgs& A, cudaStream_t st) {
+  return with_decode_kernel(p, A.tpc * A.g <= 4 ? 4 : 8, [&](auto dk) { return launch_decode_k(dk, A, st); });
 }
 
 }  // namespace kvarn
@@ -494,11 +512,7 @@ static int decode_impl(const kvarn_params* p, const kvarn_cache* cache, const vo
   A.q_scale = sm_scale * 1.4426950408889634f;
   A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
   A.n_q = 1; A.tpc = 1; A.k_blk = nullptr; A.v_blk = nullptr; A.partial = partial;
-  cudaStream_t s = (cudaStream_t)stream;
-  const bool f32 = p->in_dtype == KVARN_F32;
-  cudaError_t e;
-  if (p->bits == 2) e = f32 ? launch_decode<2, float>(A, s) : launch_decode<2, __nv_bfloat16>(A, s);
-  else e = f32 ? launch_decode<4, float>(A, s) : launch_decode<4, __nv_bfloat16>(A, s);
+  const cudaError_t e = launch_decode(p, A, (cudaStream_t)stream);
   return e == cudaSuccess ? KVARN_OK : KVARN_CUDA;
 }
 
@@ -554,11 +568,7 @@ int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* cache, const
   A.cluster = want; A.nclus = 1; A.splits = want;
   A.q_scale = sm_scale * 1.4426950408889634f;
   A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
-  cudaStream_t s = (cudaStream_t)stream;
-  const bool f32 = p->in_dtype == KVARN_F32;
-  cudaError_t e;
-  if (p->bits == 2) e = f32 ? launch_decode<2, float>(A, s) : launch_decode<2, __nv_bfloat16>(A, s);
-  else e = f32 ? launch_decode<4, float>(A, s) : launch_decode<4, __nv_bfloat16>(A, s);
+  const cudaError_t e = launch_decode(p, A, (cudaStream_t)stream);
   return e == cudaSuccess ? KVARN_OK : KVARN_CUDA;
 }
 

@@ -1,11 +1,10 @@
-// kvarn_decode_attention for sm_100a: split-K over 128-token chunks; records staged
-// by TMA bulk copies into a shared-memory ring; the two g x 128 x 128 contractions of
-// every chunk run on the tensor cores as integer MMAs straight on the packed codes;
-// split partials merge through distributed shared memory inside a thread-block cluster.
-// SURVEY 8(a) rows D1-D7; DESIGN.md "Decode kernel".
+// kvarn_decode_attention for sm_100a: split-K over 128-token chunks; every warp stages whole records with its own
+// TMA bulk copies into its own shared-memory slots; the two g x 128 x 128 contractions of every chunk run on the
+// tensor cores as integer MMAs straight on the packed codes; split partials merge through distributed shared
+// memory inside a thread-block cluster.  SURVEY 8(a) rows D1-D7; DESIGN.md "Decode kernel".
 //
 //   D1  q' = (q H / sqrt(128)) * sm_scale * log2(e)                    (online Q transform)
-//   D2  record (codes + aux) -> shared memory ring, cp.async.bulk + mbarrier
+//   D2  record (codes + aux) -> shared memory, cp.async.bulk + mbarrier
 //   D3  qt[h,c] = q'[h,c] s1[c];  beta[h] = sum_c qt[h,c] z[c]
 //       logit[h,t] = s2[t] (sum_c qt[h,c] code[t,c] + beta[h])          (Eq. 1)
 //   D4  online softmax in the log2 domain
@@ -26,19 +25,17 @@
 // u8 digits for pt).  Each digit plane is one B column, so the MMA yields, per
 // token, the exact int32 sums  D[t][(h, i)] = sum_k A[t,k] * digit_i(X[h,k])  and
 //     sum_c Q[h,c] code[t,c] = (sum_i 256^i D[t][(h,i)]) / CLSMAX   exactly.
-// The only rounding is the fixed-point conversion of qt (22 bits + sign relative
-// to max_c |qt[h,c]|) and pt (22 bits, pt <= 1); beta and the zero-point term of V
-// use the same fixed-point values, so no cancellation error appears between the
-// code term and the zero-point term.
+// The only rounding is the fixed-point conversion of qt (relative to max_c |qt[h,c]|) and of
+// pt (relative to the chunk's largest pt); beta and the zero-point term of V use the same
+// values, so no cancellation error appears between the code term and the zero-point term.
+// The two-plane ("aligned") form of the operands is described at decode_kernel_w.
 //
 // Why warp-level mma.sync (IMMA m16n8k32) and not tcgen05: the contraction is tiny
-// (N = 4 digits x g heads <= 32 columns) and the kernel is bound by instruction
-// issue and by the dependent chain of one chunk, not by tensor throughput.  The
-// tcgen05 version of this kernel (git history, profiles/r01b_*) paid two
-// TMEM-store -> MMA -> commit -> mbarrier -> TMEM-load round trips and a
-// single-thread issue path per chunk; register-level MMAs need 128 (g<=4) or 256
-// (g<=8) IMMA per chunk = 270 / 540 tensor-pipe cycles per SM (measured 2.1
-// clk/IMMA/SM), below the HBM time of a chunk, with no asynchronous-proxy hand-off.
+// (N = digits x g heads <= 32 columns) and the kernel is bound by instruction issue, not by
+// tensor throughput; tcgen05 would also tie a 128-row accumulator to all four warps of a CTA
+// (a warp reads only its own 32 TMEM lanes), i.e. bring back the CTA barriers per chunk that
+// the warp-private pipelines remove.  The round-1 tcgen05 variant of this kernel is measured
+// in DESIGN.md 6.2 (history); the dense multi-token kernel is where tcgen05 belongs.
 #pragma once
 
 #include <type_traits>
@@ -124,10 +121,14 @@ __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-// D (s32, 16x8) += A (u8, 16x32, row) * B (s8 or u8, 32x8, col)
-template <bool B_SIGNED>
+// D (s32, 16x8) += A (u8 or s8, 16x32, row) * B (s8 or u8, 32x8, col)
+template <bool B_SIGNED, bool A_SIGNED = false>
 __device__ __forceinline__ void imma_16832(int32_t (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-  if (B_SIGNED)
+  if (A_SIGNED)   // (only with signed B: the centred-code form of the QK^T contraction)
+    asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+  else if (B_SIGNED)
     asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.u8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                  : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
@@ -209,33 +210,6 @@ constexpr int MAGIC_I = 0x4B400000;
 constexpr float Q_FIX = 4194300.0f;          // 2^22: fixed-point scale of qt relative to max_c |qt[h,c]|
 constexpr float P_FIX = 4194304.0f;          // 2^22: fixed-point scale of pt = p s1v <= 1
 
-// NCH = chunks processed per loop iteration (per barrier interval).  NCH = 2 gives every warp two
-// independent instruction streams between barriers (the kernel is bound by dependent-issue latency,
-// not by occupancy: DESIGN.md 6.2) and halves the barriers per chunk.
-template <int BITS, int GP, int NCH>
-struct DecSmem {
-  static constexpr int RB = record_bytes(BITS);
-  static constexpr int STAGES = 2;
-  static constexpr int NT = GP / 2;            // n-tiles (8 columns each): 4 radix-256 digits x GP heads
-  alignas(128) uint8_t rec[STAGES][NCH][2][RB];   // [stage][chunk of the iteration][K | V] records
-  // B operands in fragment order: word (nu, kappa, half, lane' = 4 g' + t') -> [nu][hk = kappa>>1][b_slot(lane', hk)][2 (kappa&1) + half]
-  alignas(16) uint32_t bq[NCH][NT][2][32][4];
-  alignas(16) uint32_t bp[NCH][NT][2][32][4];
-  alignas(16) float2 aux_a[NCH][128];          // per MMA row slot of the K tile: {s2, log2 s1v} of its token
-  alignas(16) float2 aux_b[NCH][128];          //                                 {1 / s1v, zv}
-  alignas(16) float aux_ch[2][NCH][128];       // per channel: s2v / P_FIX (double-buffered by iteration parity)
-  alignas(16) float qrot[GP][128];             // q' (rotated, scaled); later: staging of acc / merged acc_rot
-  alignas(16) float qraw[GP][128];             // q * q_scale (un-rotated, for the residual window); later p of the residual
-  alignas(16) float hs[NCH][GP][2];            // per head: {scale, beta} of the current chunks
-  alignas(16) float hmax[GP][4];               // per head: per-warp maxima (over the chunks of the iteration)
-  alignas(16) float hz[NCH][GP][4];            // per head: per-warp zero-point sums / l sums
-  alignas(16) float wmax[4][GP];               // residual window: per-warp maxima
-  alignas(16) float wz[4][GP];                 // residual window / final l: per-warp sums
-  alignas(8) uint64_t fullk[STAGES];
-  alignas(8) uint64_t fullv[STAGES];
-  int last_flag;
-};
-
 // 16-byte slot of fragment lane lane' inside a [nu][hk] block of a B operand: bit 2 is flipped by
 // (bit 3 of lane') ^ hk, which spreads the builders' 32-bit stores over twice as many banks and keeps
 // the fragment loads (one LDS.128 per lane) conflict-free
@@ -263,42 +237,6 @@ __device__ __forceinline__ void a_frag(const uint32_t (&W)[2][BITS == 2 ? 2 : 4]
   const int w0 = BITS == 2 ? 0 : 2 * (kappa >> 1);
   const uint32_t m = MASK0 << (BITS * j);
   a[0] = W[0][w0] & m; a[1] = W[1][w0] & m; a[2] = W[0][w0 + 1] & m; a[3] = W[1][w0 + 1] & m;
-}
-
-// D[mt][nu] = sum over the 128 K positions of codes (A) x digit planes (B fragments in shared memory);
-// the 2 x NT accumulator chains are interleaved so that no IMMA waits for the previous one
-template <int BITS, int NT, bool B_SIGNED>
-__device__ __forceinline__ void contract(const uint8_t* codes, const uint32_t (*bsm)[2][32][4], int warp, int lane,
-                                         int32_t (&d)[2][NT][4]) {
-  uint32_t W[2][2][BITS == 2 ? 2 : 4];
-  load_row_words<BITS>(codes, warp, lane, 0, W[0]);
-  load_row_words<BITS>(codes, warp, lane, 1, W[1]);
-#pragma unroll
-  for (int mt = 0; mt < 2; ++mt)
-#pragma unroll
-    for (int nu = 0; nu < NT; ++nu)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) d[mt][nu][c] = 0;
-#pragma unroll
-  for (int hk = 0; hk < 2; ++hk) {
-    uint4 bf[NT];
-#pragma unroll
-    for (int nu = 0; nu < NT; ++nu) bf[nu] = *reinterpret_cast<const uint4*>(&bsm[nu][hk][b_slot(lane, hk)][0]);
-#pragma unroll
-    for (int k1 = 0; k1 < 2; ++k1) {
-      const int kappa = 2 * hk + k1;
-      uint32_t a[2][4];
-      a_frag<BITS>(W[0], kappa, a[0]);
-      a_frag<BITS>(W[1], kappa, a[1]);
-#pragma unroll
-      for (int nu = 0; nu < NT; ++nu)
-#pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-          if (k1) imma_16832<B_SIGNED>(d[mt][nu], a[mt], bf[nu].z, bf[nu].w);
-          else imma_16832<B_SIGNED>(d[mt][nu], a[mt], bf[nu].x, bf[nu].y);
-        }
-    }
-  }
 }
 
 // radix-256 digits (d0 + 256 d1 + 65536 d2 + 2^24 d3) of the int32 sums -> float
@@ -350,380 +288,23 @@ __device__ __forceinline__ ColMap col_map(const DecodeArgs& A) {
   return c;
 }
 
-template <int BITS, int GP, int NCH, typename InT>
-#ifndef KVARN_DEC_OCC4
-#define KVARN_DEC_OCC4 4
-#endif
-#ifndef KVARN_DEC_OCC8
-#define KVARN_DEC_OCC8 4
-#endif
-// GP = 4: four resident CTAs per SM with either NCH (128 registers; the two-chunk variant's 55.6 KB of shared memory
-// fits four times in 228 KB) -- with three, the 64k-context case drops from 195 to 213 us
-__global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8 / NCH) decode_kernel(const DecodeArgs A) {
-  using SM = DecSmem<BITS, GP, NCH>;
-  constexpr int RB = SM::RB, STAGES = SM::STAGES, NT = SM::NT;
-  constexpr int NCLS = 8 / BITS;
-  constexpr float CLS_INV = BITS == 2 ? (1.f / 64.f) : (1.f / 16.f);  // 1 / CLSMAX
-  constexpr int HPW = GP / 4;   // heads per warp in the B_q builder = heads per thread in the softmax (h = t + 4u)
-
-  extern __shared__ __align__(128) uint8_t smem_raw[];
-  SM& sm = *reinterpret_cast<SM*>(smem_raw);
-
+// ---- D6 + D7 of one CTA, shared by both main-loop variants: raw windows, merge of the split partials, finish.
+// On entry thread tid = channel tid holds, per column h: m_run[h] (running maximum of the chunks, CTA-wide),
+// l_tot[h] (l of the chunks, CTA-wide), l_part[h] (thread 0: l_tot, others 0) and acc[h] (its channel of the
+// rotated accumulator).  `land` = the CTA's dead record ring (>= 16 x WS_STRIDE floats; the CTA has already done
+// cluster_arrive()), `wsp` = >= GP x 64 floats of dead shared memory, `qraw` = [GP][128] q * q_scale (un-rotated; read by the raw windows,
+// scratch afterwards).  SM needs qrot, hs, hz, wmax, wz, last_flag.
+template <int GP, typename InT, class SM>
+__device__ __forceinline__ void decode_finish(const DecodeArgs& A, SM& sm, float* land, float* wsp, float* qraw, const Where& w1,
+                                              const ColMap& cm, const bool do_resid, const bool do_sink,
+                                              float (&m_run)[GP], float (&l_part)[GP], float (&l_tot)[GP], float (&acc)[GP]) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int fg = lane >> 2, ft = lane & 3;   // MMA fragment coordinates: row group g, thread-in-group t
   const int g = A.g;
-  float mr[HPW], lp[HPW], ac[HPW][4];   // running maximum, partial l, partial accumulator of this thread's (heads, rows)
-  const Where w0 = where_am_i<false>(A);
-  const ColMap cm0 = col_map<false>(A);   // before the main loop: q rows of D1, block weight of the split plan
-  const bool do_resid0 = (w0.split == A.splits - 1) && w0.resid > 0;
-  const bool do_sink0 = (w0.split == 0) && w0.n_sink_tok > 0;
-  {   // ======== setup + main loop: everything declared here dies before the epilogue ========
-  const int bh = w0.bh, b = w0.b, hkv = w0.hkv, split = w0.split;
-
-  // ---- chunk range of this split ----------------------------------------------------
-  const int n_sink_tok = w0.n_sink_tok, n_chunks = w0.n_chunks, resid = w0.resid;
-  // Balanced split: a raw window (512 B per token against 72 B) weighs like one chunk per 12 tokens (measured:
-  // 127 residual tokens cost a CTA about 10 chunks), so the splits that own the sink / residual window get
-  // correspondingly fewer chunks.  Virtual units: [sink | chunk 0 .. n_chunks-1 | residual].
-  const int w_sink = (n_sink_tok + 11) / 12, w_res = (resid + cm0.blk_cnt + 11) / 12;
-  const int per = (n_chunks + w_sink + w_res + A.splits - 1) / A.splits;
-  const int c_begin = min(max(split * per - w_sink, 0), n_chunks);
-  const int c_end = min(max((split + 1) * per - w_sink, 0), n_chunks);
-  const int n_my = c_end - c_begin;
-
-  const uint8_t* krec = A.k_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
-  const uint8_t* vrec = A.v_records + ((size_t)bh * A.max_chunks + c_begin) * RB;
-
-  // ---- setup: barriers, first TMA loads, q ------------------------------------------
-  if (tid == 0) {
-#pragma unroll
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&sm.fullk[s], 1); mbar_init(&sm.fullv[s], 1); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-#pragma unroll
-    for (int s = 0; s < STAGES; ++s) {
-      const int nc = min(NCH, n_my - s * NCH);   // chunks of iteration s
-      if (nc > 0) {
-        mbar_expect_tx(&sm.fullk[s], nc * RB);
-        mbar_expect_tx(&sm.fullv[s], nc * RB);
-        for (int c = 0; c < nc; ++c) {
-          bulk_g2s(sm.rec[s][c][0], krec + (size_t)(s * NCH + c) * RB, RB, &sm.fullk[s]);
-          bulk_g2s(sm.rec[s][c][1], vrec + (size_t)(s * NCH + c) * RB, RB, &sm.fullv[s]);
-        }
-      }
-    }
-  }
-
-  // D1: q' = (q H / sqrt(128)) * q_scale; heads >= g are zero
-  for (int hh = warp; hh < GP; hh += 4) {
-    float v[4] = {0.f, 0.f, 0.f, 0.f};
-    if (hh < cm0.ncols) {
-      const size_t row = ((size_t)b * cm0.n_q + cm0.tok0 + (hh >> cm0.lg)) * A.Hq + hkv * g + (hh - ((hh >> cm0.lg) << cm0.lg));
-      const InT* qp = reinterpret_cast<const InT*>(A.q) + row * D + 4 * lane;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) v[j] = ld_in<InT>(qp + j) * A.q_scale;
-    }
-    *reinterpret_cast<float4*>(&sm.qraw[hh][4 * lane]) = make_float4(v[0], v[1], v[2], v[3]);
-    if (A.rotate_k) {
-      fwht128_lane4(v, lane);
-#pragma unroll
-      for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
-    }
-    *reinterpret_cast<float4*>(&sm.qrot[hh][4 * lane]) = make_float4(v[0], v[1], v[2], v[3]);
-  }
-  __syncthreads();
-
-  // B_q builder role: warp -> heads warp (+4); lane = 8 kappa + 4 half + t' owns the four K positions
-  // p = 16 half + 4 t' + b (b = 0..3) of k-step kappa, i.e. one 32-bit word of a B fragment per digit
-  const int bk = lane >> 3, bhalf = (lane >> 2) & 1, btp = lane & 3;
-  float qreg[HPW][4];
-#pragma unroll
-  for (int bb = 0; bb < 4; ++bb) {
-    const int ch = BITS == 2 ? 16 * btp + 4 * bb + bk + 64 * bhalf
-                             : 8 * (btp + 4 * (2 * (bk >> 1) + bhalf)) + 2 * bb + (bk & 1);
-#pragma unroll
-    for (int u = 0; u < HPW; ++u) qreg[u][bb] = sm.qrot[warp + 4 * u][ch];
-  }
-  // fixed-point value -> digits: X = (bits(f) - MAGIC_I) << shift, balanced:  (X + 0x80808080) ^ 0x80808080
-  const int jq = BITS == 2 ? bk : (bk & 1);
-  const uint32_t mul_q = 1u << (BITS * (NCLS - 1 - jq));
-  const uint32_t add_q = 0x80808080u - ((uint32_t)MAGIC_I * mul_q);
-  // column (h, d) of head h = warp + 4u: n-tile 2u + (d >> 1), g' = 2 warp + (d & 1); lane' = 4 g' + t'
-  uint32_t* bq_dst[2];
-#pragma unroll
-  for (int dd = 0; dd < 2; ++dd) bq_dst[dd] = &sm.bq[0][0][bk >> 1][b_slot(4 * (2 * warp + dd) + btp, bk >> 1)][2 * (bk & 1) + bhalf];
-  // softmax role: thread (warp, fg, ft) sees tokens slot(mt, rho) = 32 warp + 16 mt + 8 rho + fg, heads ft + 4u;
-  // these four tokens are K positions b = 2 mt + rho of word (kappa = warp, half = fg >> 2, t' = fg & 3)
-  const int jp = BITS == 2 ? warp : (warp & 1);
-  const uint32_t mul_p = 1u << (BITS * (NCLS - 1 - jp));
-  const uint32_t add_p = 0u - ((uint32_t)MAGIC_I * mul_p);
-  // column (h, d) of head h = ft + 4u: n-tile 2u + (d >> 1), g' = 2 ft + (d & 1); lane' = 4 g' + t'
-  uint32_t* bp_dst[2];
-#pragma unroll
-  for (int dd = 0; dd < 2; ++dd) bp_dst[dd] = &sm.bp[0][0][warp >> 1][b_slot(4 * (2 * ft + dd) + (fg & 3), warp >> 1)][2 * (warp & 1) + (fg >> 2)];
-  constexpr int B_CH = NT * 256;   // 32-bit words of one chunk's B operand
-
-#pragma unroll
-  for (int u = 0; u < HPW; ++u) {
-    mr[u] = -INFINITY; lp[u] = 0.f;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) ac[u][i] = 0.f;
-  }
-
-  // One loop iteration = NCH chunks.  FULL (all NCH chunks present) is a compile-time flag so that the
-  // common case has no per-chunk branches and the chunks' instruction streams interleave.
-  auto iteration = [&](auto full_tag, const int it) {
-    constexpr bool FULL = decltype(full_tag)::value;
-    const int st = it % STAGES;
-    const uint32_t par = (it / STAGES) & 1;
-    const int nc = min(NCH, n_my - it * NCH);   // chunks of this iteration (uniform)
-    mbar_wait(&sm.fullk[st], par);
-
-    // ---- phase A: B_q (digits of the fixed-point qt), beta, per-token / per-channel aux -----------
-#pragma unroll
-    for (int c = 0; c < NCH; ++c) {
-      if (FULL || c < nc) {
-        const uint8_t* kr = sm.rec[st][c][0];
-        // aux of the K record in builder order: s1[4 lane + b], z[4 lane + b]
-        const uint32_t s1w = *reinterpret_cast<const uint32_t*>(kr + s1_off(BITS) + 4 * lane);
-        const uint2 zw = *reinterpret_cast<const uint2*>(kr + z_off(BITS) + 8 * lane);
-        const float2 s01 = e4m3x2_to_f32x2((uint16_t)(s1w & 0xffff)), s23 = e4m3x2_to_f32x2((uint16_t)(s1w >> 16));
-        const float s1[4] = {s01.x, s01.y, s23.x, s23.y};
-        const float2 z01 = __half22float2(*reinterpret_cast<const __half2*>(&zw.x));
-        const float2 z23 = __half22float2(*reinterpret_cast<const __half2*>(&zw.y));
-        const float z[4] = {z01.x, z01.y, z23.x, z23.y};
-        float qt[HPW][4], amax[HPW], bsum[HPW];
-#pragma unroll
-        for (int u = 0; u < HPW; ++u) {
-#pragma unroll
-          for (int r = 0; r < 4; ++r) qt[u][r] = qreg[u][r] * s1[r];
-          amax[u] = fmaxf(fmaxf(fabsf(qt[u][0]), fabsf(qt[u][1])), fmaxf(fabsf(qt[u][2]), fabsf(qt[u][3])));
-          // beta uses the unrounded qt: it differs from the 22-bit fixed-point value by < 2^-23 max|qt|
-          bsum[u] = fmaf(qt[u][0], z[0], fmaf(qt[u][1], z[1], fmaf(qt[u][2], z[2], qt[u][3] * z[3])));
-        }
-#pragma unroll
-        for (int u = 0; u < HPW; ++u)   // non-negative floats order like their bit patterns
-          amax[u] = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax[u])));
-#pragma unroll
-        for (int m = 16; m > 0; m >>= 1)
-#pragma unroll
-          for (int u = 0; u < HPW; ++u) bsum[u] += __shfl_xor_sync(0xffffffffu, bsum[u], m);
-#pragma unroll
-        for (int u = 0; u < HPW; ++u) {
-          const int h = warp + 4 * u;
-          const float inv = amax[u] > 1e-30f ? Q_FIX * rcp_approx(amax[u]) : 0.f;
-          uint32_t X[4], Y[4];
-#pragma unroll
-          for (int r = 0; r < 4; ++r) {
-            const float f = fmaf(qt[u][r], inv, MAGIC_F);            // integer Q in the low mantissa bits
-            X[r] = (__float_as_uint(f) * mul_q + add_q) ^ 0x80808080u;   // balanced s8 digits of Q << shift
-          }
-          transpose4x4(X, Y);   // Y[d] = digit d of the four K positions = one B-fragment word of column (h, d)
-#pragma unroll
-          for (int d = 0; d < 4; ++d) bq_dst[d & 1][c * B_CH + (2 * u + (d >> 1)) * 256] = Y[d];
-          if (lane == 0) {
-            const float sc = amax[u] * (1.f / Q_FIX);
-            sm.hs[c][h][0] = sc * CLS_INV;   // logit = s2 * (acc * scale + beta)
-            sm.hs[c][h][1] = bsum[u];
-          }
-        }
-      }
-    }
-    mbar_wait(&sm.fullv[st], par);
-#pragma unroll
-    for (int c = 0; c < NCH; ++c) {
-      if (FULL || c < nc) {
-        // thread tid: aux of MMA row slot tid of the K tile (token-indexed arrays are stored in slot order)
-        // and of channel tid of the V tile
-        const uint8_t* kr = sm.rec[st][c][0];
-        const uint8_t* vr = sm.rec[st][c][1];
-        const float s2t = e4m3_to_f32(kr[s2_off(BITS) + tid]);
-        const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + tid]), 9.094947e-13f);   // 2^-40: a zero scale stays harmless
-        const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[tid]);
-        // pt = p s1v = exp2(logit + log2 s1v - m): the running maximum is taken over the shifted logits,
-        // so pt <= 1 and its fixed-point scale is a constant
-        sm.aux_a[c][tid] = make_float2(s2t, lg2_approx(s1v));
-        sm.aux_b[c][tid] = make_float2(rcp_approx(s1v) * (1.f / P_FIX), zv);
-        sm.aux_ch[it & 1][c][tid] = e4m3_to_f32(vr[s2_off(BITS) + tid]) * (1.f / P_FIX);
-      }
-    }
-    __syncthreads();                                                   // barrier 1
-    // every warp is done with iteration it-1: refill its V slots (its K slots were refilled after barrier 2)
-    if (tid == 0 && it >= 1) {
-      const int nxt = it - 1 + STAGES, s2 = (it - 1) % STAGES;
-      const int nn = min(NCH, n_my - nxt * NCH);
-      if (nn > 0) {
-        mbar_expect_tx(&sm.fullv[s2], nn * RB);
-        for (int c = 0; c < nn; ++c) bulk_g2s(sm.rec[s2][c][1], vrec + (size_t)(nxt * NCH + c) * RB, RB, &sm.fullv[s2]);
-      }
-    }
-
-    // ---- D3: logits of this thread's 4 tokens x HPW heads (per chunk) -----------------------------------
-    float logit[NCH][HPW][4];
-#pragma unroll
-    for (int c = 0; c < NCH; ++c) {
-      if (FULL || c < nc) {
-        int32_t dd[2][NT][4];
-        contract<BITS, NT, true>(sm.rec[st][c][0], sm.bq[c], warp, lane, dd);
-        float2 aux[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) aux[i] = sm.aux_a[c][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];
-#pragma unroll
-        for (int u = 0; u < HPW; ++u) {
-          const float2 sb = *reinterpret_cast<const float2*>(sm.hs[c][ft + 4 * u]);
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {   // i = 2 mt + rho
-            const int mt = i >> 1, cc = 2 * (i & 1);
-            const float a = undigit(dd[mt][2 * u][cc], dd[mt][2 * u][cc + 1], dd[mt][2 * u + 1][cc], dd[mt][2 * u + 1][cc + 1]);
-            logit[c][u][i] = fmaf(aux[i].x, fmaf(a, sb.x, sb.y), aux[i].y);
-          }
-        }
-      } else {
-#pragma unroll
-        for (int u = 0; u < HPW; ++u)
-#pragma unroll
-          for (int i = 0; i < 4; ++i) logit[c][u][i] = -INFINITY;
-      }
-    }
-    // ---- D4: online softmax -----------------------------------------------------------------------------
-#pragma unroll
-    for (int u = 0; u < HPW; ++u) {
-      float mx = -INFINITY;
-#pragma unroll
-      for (int c = 0; c < NCH; ++c)
-        mx = fmaxf(mx, fmaxf(fmaxf(logit[c][u][0], logit[c][u][1]), fmaxf(logit[c][u][2], logit[c][u][3])));
-      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
-      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 8));
-      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 16));
-      if (fg == 0) sm.hmax[ft + 4 * u][warp] = mx;
-    }
-    __syncthreads();                                                   // barrier 2
-    // every warp is done with the K records of this iteration: prefetch iteration it + STAGES into their slots
-    if (tid == 0) {
-      const int nxt = it + STAGES;
-      const int nn = min(NCH, n_my - nxt * NCH);
-      if (nn > 0) {
-        mbar_expect_tx(&sm.fullk[st], nn * RB);
-        for (int c = 0; c < nn; ++c) bulk_g2s(sm.rec[st][c][0], krec + (size_t)(nxt * NCH + c) * RB, RB, &sm.fullk[st]);
-      }
-    }
-    // The fixed-point probabilities refer to the maximum m_it of THIS iteration's chunks (not to the running
-    // maximum): a token is dropped only if it lies 2^-23 below the largest of its own <= 256 neighbours, so the
-    // dropped mass is bounded by 255 * 2^-23 whatever the context length; the iteration's sums enter the running
-    // ones with the weight wch = 2^(m_it - m_new).  l is accumulated from the SAME rounded values as the
-    // numerator, so numerator and denominator stay consistent.
-    float corr[HPW], wch[HPW];
-#pragma unroll
-    for (int u = 0; u < HPW; ++u) {
-      const float4 hm = *reinterpret_cast<const float4*>(sm.hmax[ft + 4 * u]);
-      const float m_it = fmaxf(fmaxf(hm.x, hm.y), fmaxf(hm.z, hm.w));
-      const float m_new = fmaxf(mr[u], m_it);
-      corr[u] = ex2_approx(mr[u] - m_new);
-      wch[u] = ex2_approx(m_it - m_new);
-      mr[u] = m_new;
-      float lsum = 0.f;
-#pragma unroll
-      for (int c = 0; c < NCH; ++c) {
-        if (FULL || c < nc) {
-          uint32_t X[4], Y[4];
-          float zpart = 0.f;
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const float2 ab = sm.aux_b[c][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];   // {1 / (s1v P_FIX), zv}
-            const float pt = ex2_approx(logit[c][u][i] - m_it);
-            // D5 prep: fixed-point pt; its radix-256 digits are the bytes of X
-            const float f = fmaf(pt, P_FIX, MAGIC_F);
-            const float pr = f - MAGIC_F;                 // P_FIX * (rounded pt), an exact integer
-            lsum = fmaf(pr, ab.x, lsum);
-            zpart = fmaf(pr, ab.y, zpart);
-            X[i] = __float_as_uint(f) * mul_p + add_p;
-          }
-          transpose4x4(X, Y);
-#pragma unroll
-          for (int d = 0; d < 4; ++d) bp_dst[d & 1][c * B_CH + (2 * u + (d >> 1)) * 256] = Y[d];
-          zpart += __shfl_xor_sync(0xffffffffu, zpart, 4);
-          zpart += __shfl_xor_sync(0xffffffffu, zpart, 8);
-          zpart += __shfl_xor_sync(0xffffffffu, zpart, 16);
-          if (fg == 0) sm.hz[c][ft + 4 * u][warp] = zpart;
-        }
-      }
-      lp[u] = fmaf(lp[u], corr[u], lsum * wch[u]);
-    }
-    __syncthreads();                                                   // barrier 3
-
-    // ---- D5: this thread's 4 channels x HPW heads of the value contraction ---------------------------
-#pragma unroll
-    for (int u = 0; u < HPW; ++u)
-#pragma unroll
-      for (int i = 0; i < 4; ++i) ac[u][i] *= corr[u];
-#pragma unroll
-    for (int c = 0; c < NCH; ++c) {
-      if (FULL || c < nc) {
-        int32_t dd[2][NT][4];
-        contract<BITS, NT, false>(sm.rec[st][c][1], sm.bp[c], warp, lane, dd);
-        float s2v[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) s2v[i] = sm.aux_ch[it & 1][c][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg];
-#pragma unroll
-        for (int u = 0; u < HPW; ++u) {
-          const float4 hz = *reinterpret_cast<const float4*>(sm.hz[c][ft + 4 * u]);
-          const float zsum = ((hz.x + hz.y) + (hz.z + hz.w)) * wch[u];
-          const float cw = CLS_INV * wch[u];
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int mt = i >> 1, cc = 2 * (i & 1);
-            const float a = undigit(dd[mt][2 * u][cc], dd[mt][2 * u][cc + 1], dd[mt][2 * u + 1][cc], dd[mt][2 * u + 1][cc + 1]);
-            ac[u][i] = fmaf(s2v[i], fmaf(a, cw, zsum), ac[u][i]);
-          }
-        }
-      }
-    }
-  };
-  const int n_it = (n_my + NCH - 1) / NCH;
-  for (int it = 0; it < n_it; ++it) {
-    if (NCH == 1 || n_my - it * NCH >= NCH) iteration(std::true_type{}, it);
-    else iteration(std::false_type{}, it);
-  }
-  }   // ======== end of setup + main loop ========
-
-  // ---- hand over to the per-channel layout of the residual window / merge: thread tid = channel tid ----
-  __syncthreads();
-  // Re-derive the CTA's coordinates / column map instead of carrying them through the loop where that pays
-  // (64k context, g = 8: 2-bit 367 -> 344 us, 4-bit 390 -> 350 us); the 2-bit g <= 4 kernel is faster with them
-  // live (195 vs 199 us, 203 vs 209 us with a full residual window), so it keeps them.
-  const Where w1 = BITS == 4 ? where_am_i<true>(A) : w0;
   const int bh = w1.bh, b = w1.b, hkv = w1.hkv, split = w1.split, n_sink_tok = w1.n_sink_tok, resid = w1.resid;
-  const bool do_resid = BITS == 4 ? ((split == A.splits - 1) && resid > 0) : do_resid0;
-  const bool do_sink = BITS == 4 ? ((split == 0) && n_sink_tok > 0) : do_sink0;
-  const ColMap cm = (GP == 8 || BITS == 4) ? col_map<true>(A) : cm0;
   const int lg = cm.lg, tok0 = cm.tok0, ncols = cm.ncols, n_q = cm.n_q, blk_cnt = cm.blk_cnt;
   const bool has_blk = A.k_blk != nullptr;
   const bool do_blk = (split == A.splits - 1) && has_blk;
   auto qrow = [&](int j) -> size_t { return ((size_t)b * n_q + tok0 + (j >> lg)) * A.Hq + hkv * g + (j - ((j >> lg) << lg)); };
-  // every warp has left the main loop and no TMA fill is outstanding: this CTA's record ring is dead and may
-  // receive the peers' partials.  Arrive now, wait only right before the first DSMEM store (D7a), so the
-  // barrier latency hides behind the raw windows and the l reductions.
-  if (A.cluster > 1) cluster_arrive();
-#pragma unroll
-  for (int u = 0; u < HPW; ++u) {
-    float l = lp[u];
-    l += __shfl_xor_sync(0xffffffffu, l, 4);
-    l += __shfl_xor_sync(0xffffffffu, l, 8);
-    l += __shfl_xor_sync(0xffffffffu, l, 16);
-    if (fg == 0) { sm.hz[0][ft + 4 * u][warp] = l; if (warp == 0) sm.hs[0][ft + 4 * u][0] = mr[u]; }
-#pragma unroll
-    for (int i = 0; i < 4; ++i) sm.qrot[ft + 4 * u][32 * warp + 16 * (i >> 1) + 8 * (i & 1) + fg] = ac[u][i];
-  }
-  __syncthreads();
-  float m_run[GP], l_part[GP], l_tot[GP], acc[GP];
-#pragma unroll
-  for (int h = 0; h < GP; ++h) {
-    m_run[h] = sm.hs[0][h][0];
-    const float4 hz = *reinterpret_cast<const float4*>(sm.hz[0][h]);
-    l_tot[h] = (hz.x + hz.y) + (hz.z + hz.w);                     // l of the chunks (every thread has it)
-    l_part[h] = tid == 0 ? l_tot[h] : 0.f;                        // with raw windows: thread 0 carries it into the sum
-    acc[h] = sm.qrot[h][tid];
-  }
-
   // ---- D6: raw windows (sink tokens of split 0, residual window of the last split; un-rotated space) ----
   float acc_res[GP];
 #pragma unroll
@@ -748,8 +329,8 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
           const int c = c0 + 8 * j;
 #pragma unroll
           for (int h = 0; h < GP; ++h) {
-            const float4 q0 = *reinterpret_cast<const float4*>(&sm.qraw[h][c]);
-            const float4 q1 = *reinterpret_cast<const float4*>(&sm.qraw[h][c + 4]);
+            const float4 q0 = *reinterpret_cast<const float4*>(&qraw[h * 128 + c]);
+            const float4 q1 = *reinterpret_cast<const float4*>(&qraw[h * 128 + c + 4]);
             float s = logit[h];
             s = fmaf(kv[j][0], q0.x, s); s = fmaf(kv[j][1], q0.y, s); s = fmaf(kv[j][2], q0.z, s); s = fmaf(kv[j][3], q0.w, s);
             s = fmaf(kv[j][4], q1.x, s); s = fmaf(kv[j][5], q1.y, s); s = fmaf(kv[j][6], q1.z, s); s = fmaf(kv[j][7], q1.w, s);
@@ -842,9 +423,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
   int hbase = 0, hstride = 1;
   if (CS > 1) {
     const int crank = (int)cluster_ctarank();
-    float* land = reinterpret_cast<float*>(&sm.rec[0][0][0]);   // [<= 16][WS_STRIDE]
-    static_assert(sizeof(sm.rec) >= 16 * WS_STRIDE * sizeof(float), "landing area");
-    cluster_wait();
+        cluster_wait();
     const uint32_t land_addr = smem_u32(land);
 #pragma unroll
     for (int h = 0; h < GP; ++h) {
@@ -907,8 +486,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
     if (!sm.last_flag) return;
     __threadfence();
     // weights of the partials: warp w handles heads w, w+4; lane s handles partials s, s+32
-    float* wsp = reinterpret_cast<float*>(sm.bq);   // [GP][64] weights (B_q is dead by now)
-    for (int h = warp; h < ncols; h += 4) {
+        for (int h = warp; h < ncols; h += 4) {
       const float* base = A.ws + qrow(h) * NC * WS_STRIDE;
       const float m0 = lane < NC ? __ldcg(base + (size_t)lane * WS_STRIDE) : -INFINITY;
       const float m1 = lane + 32 < NC ? __ldcg(base + (size_t)(lane + 32) * WS_STRIDE) : -INFINITY;
@@ -955,7 +533,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
 #pragma unroll
   for (int j = 0; j < GP; ++j) {
     merged_rot[j * 128 + tid] = acc[j];
-    sm.qraw[j][tid] = (l_tot[j] > 0.f) ? acc_res[j] : 0.f;
+    qraw[j * 128 + tid] = (l_tot[j] > 0.f) ? acc_res[j] : 0.f;
     if (tid == 0) {
       sm.hs[0][j][0] = A.partial ? 1.f : ((l_tot[j] > 0.f) ? 1.f / l_tot[j] : 0.f);
       sm.hs[0][j][1] = (l_tot[j] > 0.f) ? m_run[j] : -INFINITY;
@@ -973,7 +551,7 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
 #pragma unroll
       for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
     }
-    const float4 s4 = *reinterpret_cast<const float4*>(&sm.qraw[jj][4 * lane]);
+    const float4 s4 = *reinterpret_cast<const float4*>(&qraw[jj * 128 + 4 * lane]);
     const float inv = sm.hs[0][jj][0];
     const float o0 = (v[0] + s4.x) * inv, o1 = (v[1] + s4.y) * inv, o2 = (v[2] + s4.z) * inv, o3 = (v[3] + s4.w) * inv;
     if (A.partial) {
@@ -992,6 +570,441 @@ __global__ void __launch_bounds__(128, GP == 4 ? KVARN_DEC_OCC4 : KVARN_DEC_OCC8
       *reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(A.out) + off) = u;
     }
   }
+}
+
+// ======================================================================================================
+// decode_kernel_w: the same D1-D7, with WARP-PRIVATE chunk pipelines.  Each of the CTA's 4 warps owns whole
+// chunks (chunk c_begin + warp + 4 i): it stages the chunk's two records into its own shared-memory slots with
+// its own TMA bulk copies / mbarriers, builds the B operands for all columns, contracts all 8 m-tiles and keeps
+// a private online-softmax state (m, l, acc) -- no CTA barrier and no cross-warp exchange inside the loop, only
+// __syncwarp.  The B fragments are loaded once per contraction and kept in registers, and the per-chunk
+// reductions (maximum, zero-point sum) stay inside the warp.  K of the next chunk is requested as soon as the
+// QK^T contraction has consumed the codes, V of the next chunk after the value contraction, so each slot is
+// single-buffered (9.2 KB per warp at 2-bit).  After the loop the 4 private states are merged through the dead
+// slots and the shared finish (decode_finish) runs as before.  Record layout and row-slot maps are unchanged:
+// what was "warp" in slot s = 32 warp + 16 mtile + 8 rho + g is now the m-tile pair index mp of the owning warp.
+//
+// DQ / DP = radix-256 digit planes of the fixed-point q~ / p~.
+//   4: the in-place A fragments of the CTA-cooperative variant (a code keeps its bit position 2j inside its byte,
+//      the B operand carries 4^(3-j)): 22-bit values.
+//   2: ALIGNED A fragments -- every plane is shifted to bits 7:6 of its byte ((W << 2 (3 - j)), an IMAD on the idle fma
+//      pipe, then one LOP3), so all codes carry the same factor 64 and the B operand needs no compensation bits: two
+//      digit planes hold 16 bits.  Half the columns: half the IMMAs, B-operand words, fragment loads and digit
+//      recombinations.  For q~ (15 bits + sign, two balanced s8 digits) the A fragment is also CENTRED in the same
+//      LOP3 (64 code - 96 as s8, i.e. code - 1.5) and beta = sum q~ (z + 1.5) takes the mean code in fp32, which removes
+//      the mean part of the rounding error.  p~ with two u8 digits has 16 bits relative to the chunk's maximum.
+// kvarn_params::decode_digits picks (DQ, DP): 0 (default) = (4, 2): 16-bit p~ costs < 1e-4 of the 2e-3 tolerance;
+// 2 = (2, 2): fastest, q~ at 16 bits measured up to 1.2e-3 on short peaked contexts; 4 = (4, 4).
+template <int BITS, int GP, int DQ, int DP>
+struct WarpSm {
+  static constexpr int RB = record_bytes(BITS);
+  static constexpr int NTQ = GP * DQ / 8, NTP = GP * DP / 8;   // n-tiles (8 columns each): digit planes x GP columns
+  static constexpr int NT = NTQ > NTP ? NTQ : NTP;
+  alignas(128) uint8_t krec[RB];
+  alignas(128) uint8_t vrec[RB];
+  alignas(16) uint32_t bfr[NT][2][32][4];      // B fragments: first of q~ (QK^T), then -- reused -- of p~ (value contraction)
+  alignas(16) float2 aux_a[128];               // per K row slot: {s2, log2 s1v}
+  alignas(16) float2 aux_b[128];               //                 {1 / (s1v P_FIX), zv}
+  alignas(8) __half aux_ch[4][8][4];           // per channel: s2v, [mp][fg][i] of channel slot 32 mp + 16 (i >> 1) + 8 (i & 1) + fg
+  alignas(8) float2 hs[GP];                    // per column: {scale, beta}
+  alignas(8) uint64_t fullk, fullv;
+};
+template <int BITS, int GP, int DQ, int DP>
+struct DecSmemW {
+  WarpSm<BITS, GP, DQ, DP> w[4];
+  alignas(16) float qrot[GP][128];             // q' (rotated, scaled, in B-builder order); later p of a raw window / merged acc_rot
+  alignas(16) float hs[1][GP][2];
+  alignas(16) float hz[1][GP][4];
+  alignas(16) float wmax[4][GP];
+  alignas(16) float wz[4][GP];
+  int last_flag;
+};
+
+// A fragment of k-step kappa, aligned form: the plane's codes moved to the top bits of their bytes, u8 value 64 code (16 code at 4-bit).
+// CENTRED: s8 value 64 code - 96 = 64 (code - 1.5): bit 7 inverted, bit 6 kept, bit 5 set -- with M1 = bits {7, 5} and
+// M2 = bits {6, 5} that is (M1 & ~M2 & ~x) | (~M1 & M2 & x) | (M1 & M2), one LOP3.
+template <int BITS, bool CENTRED>
+__device__ __forceinline__ void a_frag_aligned(const uint32_t (&W)[2][BITS == 2 ? 2 : 4], int kappa, uint32_t (&a)[4]) {
+  static_assert(BITS == 2 || !CENTRED, "centred A fragments: 2-bit records");
+  constexpr int NCLS = 8 / BITS;
+  constexpr uint32_t MASK = BITS == 2 ? 0xC0C0C0C0u : 0xF0F0F0F0u;
+  const int j = BITS == 2 ? kappa : (kappa & 1);
+  const int w0 = BITS == 2 ? 0 : 2 * (kappa >> 1);
+  const uint32_t mul = 1u << (BITS * (NCLS - 1 - j));      // compile-time per call site: IMAD.SHL on the fma pipe
+  auto f = [&](uint32_t w) -> uint32_t {
+    const uint32_t x = w * mul;
+    if constexpr (!CENTRED) return x & MASK;
+    constexpr uint32_t M1 = 0xA0A0A0A0u, M2 = 0x60606060u;
+    return (M1 & ~M2 & ~x) | (~M1 & M2 & x) | (M1 & M2);
+  };
+  a[0] = f(W[0][w0]); a[1] = f(W[1][w0]); a[2] = f(W[0][w0 + 1]); a[3] = f(W[1][w0 + 1]);
+}
+template <int BITS, int NT, int NTB, bool B_SIGNED, bool ALIGNED, bool CENTRED = false>
+__device__ __forceinline__ void contract_mp(const uint8_t* codes, const uint4 (&bf)[2][NTB], int mp, int lane, int32_t (&d)[2][NT][4]) {
+  uint32_t W[2][2][BITS == 2 ? 2 : 4];
+  load_row_words<BITS>(codes, mp, lane, 0, W[0]);
+  load_row_words<BITS>(codes, mp, lane, 1, W[1]);
+#pragma unroll
+  for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+    for (int nu = 0; nu < NT; ++nu)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) d[mt][nu][c] = 0;
+#pragma unroll
+  for (int hk = 0; hk < 2; ++hk) {
+#pragma unroll
+    for (int k1 = 0; k1 < 2; ++k1) {
+      const int kappa = 2 * hk + k1;
+      uint32_t a[2][4];
+      if constexpr (ALIGNED) { a_frag_aligned<BITS, CENTRED>(W[0], kappa, a[0]); a_frag_aligned<BITS, CENTRED>(W[1], kappa, a[1]); }
+      else { a_frag<BITS>(W[0], kappa, a[0]); a_frag<BITS>(W[1], kappa, a[1]); }
+#pragma unroll
+      for (int nu = 0; nu < NT; ++nu)
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt) {
+          if (k1) imma_16832<B_SIGNED, CENTRED>(d[mt][nu], a[mt], bf[hk][nu].z, bf[hk][nu].w);
+          else imma_16832<B_SIGNED, CENTRED>(d[mt][nu], a[mt], bf[hk][nu].x, bf[hk][nu].y);
+        }
+    }
+  }
+}
+// int32 digit sums of output (mt, i-th accumulator pair cc) of column u -> float
+template <int DIG, int NT>
+__device__ __forceinline__ float undigit_w(const int32_t (&dd)[2][NT][4], int mt, int u, int cc) {
+  if constexpr (DIG == 4) return undigit(dd[mt][2 * u][cc], dd[mt][2 * u][cc + 1], dd[mt][2 * u + 1][cc], dd[mt][2 * u + 1][cc + 1]);
+  else return __int2float_rn(dd[mt][u][cc + 1] * 256 + dd[mt][u][cc]);
+}
+constexpr float Q_FIX2 = 32639.0f;            // two planes: |Q| <= 2^15 - 1 - 128 keeps the high balanced digit inside s8
+constexpr float P_FIX2 = 65535.0f;            // two planes: 16-bit p~
+
+template <int BITS, int GP, int DQ, int DP, typename InT>
+#ifndef KVARN_DECW_OCC4
+#define KVARN_DECW_OCC4 4
+#endif
+__global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 3) : 2) decode_kernel_w(const DecodeArgs A) {
+  using SM = DecSmemW<BITS, GP, DQ, DP>;
+  using WS = WarpSm<BITS, GP, DQ, DP>;
+  constexpr int RB = WS::RB, NTQ = WS::NTQ, NTP = WS::NTP;
+  constexpr int NCLS = 8 / BITS;
+  static_assert((DQ == 2 || DQ == 4) && (DP == 2 || DP == 4) && (BITS == 2 || DQ == 4), "digit planes");
+  constexpr float CLS_INV = BITS == 2 ? (1.f / 64.f) : (1.f / 16.f);  // 1 / CLSMAX (every form scales a code by CLSMAX)
+  constexpr float QF = DQ == 4 ? Q_FIX : Q_FIX2, PF = DP == 4 ? P_FIX : P_FIX2;
+  constexpr float ZC = DQ == 2 ? 0.5f * (float)((1 << BITS) - 1) : 0.f;   // centred K codes: the mean code moves into beta
+  constexpr int HPW = GP / 4;   // columns per thread in the softmax (h = ft + 4u)
+
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  SM& sm = *reinterpret_cast<SM*>(smem_raw);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int fg = lane >> 2, ft = lane & 3;
+  const int g = A.g;
+  WS& ws = sm.w[warp];
+
+  const Where w0 = where_am_i<false>(A);
+  const ColMap cm0 = col_map<false>(A);
+  const bool do_resid = (w0.split == A.splits - 1) && w0.resid > 0;
+  const bool do_sink = (w0.split == 0) && w0.n_sink_tok > 0;
+  // ---- chunk range of this split (balanced against the raw windows as in the CTA-cooperative variant) ----
+  const int w_sink = (w0.n_sink_tok + 11) / 12, w_res = (w0.resid + cm0.blk_cnt + 11) / 12;
+  const int per = (w0.n_chunks + w_sink + w_res + A.splits - 1) / A.splits;
+  const int c_begin = min(max(w0.split * per - w_sink, 0), w0.n_chunks);
+  const int c_end = min(max((w0.split + 1) * per - w_sink, 0), w0.n_chunks);
+  const int n_mine = (c_end - c_begin - warp + 3) >> 2;            // chunks of this warp: c_begin + warp + 4 i
+  const uint8_t* krec = A.k_records + ((size_t)w0.bh * A.max_chunks + c_begin + warp) * RB;
+  const uint8_t* vrec = A.v_records + ((size_t)w0.bh * A.max_chunks + c_begin + warp) * RB;
+
+  // ---- setup: the warp's barriers and first loads; q ---------------------------------------------------
+  if (lane == 0) {
+    mbar_init(&ws.fullk, 1); mbar_init(&ws.fullv, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (n_mine > 0) {
+      mbar_expect_tx(&ws.fullk, RB); bulk_g2s(ws.krec, krec, RB, &ws.fullk);
+      mbar_expect_tx(&ws.fullv, RB); bulk_g2s(ws.vrec, vrec, RB, &ws.fullv);
+    }
+  }
+  // B-builder role of a lane: lane = 8 kappa + 4 half + t' owns the four K positions p = 16 half + 4 t' + b of
+  // k-step kappa, i.e. one 32-bit word of a B fragment per digit plane
+  const int bk = lane >> 3, bhalf = (lane >> 2) & 1, btp = lane & 3;
+  // D1: q' = (q H / sqrt(128)) * q_scale, stored in builder order: qrot[h][4 lane + bb] = q'[h][channel(lane, bb)]
+  for (int hh = warp; hh < GP; hh += 4) {
+    float v[4] = {0.f, 0.f, 0.f, 0.f};
+    if (hh < cm0.ncols) {
+      const size_t row = ((size_t)w0.b * cm0.n_q + cm0.tok0 + (hh >> cm0.lg)) * A.Hq + w0.hkv * g + (hh - ((hh >> cm0.lg) << cm0.lg));
+      const InT* qp = reinterpret_cast<const InT*>(A.q) + row * D + 4 * lane;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[j] = ld_in<InT>(qp + j) * A.q_scale;
+    }
+    if (A.rotate_k) {
+      fwht128_lane4(v, lane);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
+    }
+    // element e = 4 lane + j of q' goes to builder position kaux_of_elem(e) (the order of K.s1 / K.z in the record)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) sm.qrot[hh][kaux_of_elem(BITS, 4 * lane + j)] = v[j];
+  }
+  __syncthreads();
+
+  // destination of the builder's digit words for column h: n-tile DH (h >> 2) + (d >> 1), column slot g' = 2 (h & 3) + (d & 1)
+  // of the fragment block [nt][hk = bk >> 1][b_slot(4 g' + btp, hk)][2 (bk & 1) + bhalf]
+  const int jq = BITS == 2 ? bk : (bk & 1);
+  const uint32_t mul_q = 1u << (BITS * (NCLS - 1 - jq));
+  const uint32_t add_q = 0x80808080u - ((uint32_t)MAGIC_I * mul_q);
+  uint32_t* const bq_base = &ws.bfr[0][bk >> 1][0][2 * (bk & 1) + bhalf];
+  // softmax role: thread (fg, ft) sees, per m-tile pair mp, tokens slot = 32 mp + 16 mt + 8 rho + fg of columns ft + 4u;
+  // these four tokens are K positions b = 2 mt + rho of word (kappa = mp, half = fg >> 2, t' = fg & 3) of the value contraction
+  float mr[HPW], lp[HPW], ac[4][HPW][4];
+#pragma unroll
+  for (int u = 0; u < HPW; ++u) {
+    mr[u] = -INFINITY; lp[u] = 0.f;
+#pragma unroll
+    for (int mp = 0; mp < 4; ++mp)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) ac[mp][u][i] = 0.f;
+  }
+
+#pragma unroll 1
+  for (int it = 0; it < n_mine; ++it) {
+    const uint32_t par = it & 1;
+    const bool more = it + 1 < n_mine;
+    mbar_wait(&ws.fullk, par);
+    // ---- phase A: B_q (digit planes of the fixed-point q~) and beta for every column; s2 of the K rows -------
+    {
+      const uint8_t* kr = ws.krec;
+      const uint32_t s1w = *reinterpret_cast<const uint32_t*>(kr + s1_off(BITS) + 4 * lane);
+      const uint2 zw = *reinterpret_cast<const uint2*>(kr + z_off(BITS) + 8 * lane);
+      const float2 s01 = e4m3x2_to_f32x2((uint16_t)(s1w & 0xffff)), s23 = e4m3x2_to_f32x2((uint16_t)(s1w >> 16));
+      const float2 z01 = __half22float2(*reinterpret_cast<const __half2*>(&zw.x));
+      const float2 z23 = __half22float2(*reinterpret_cast<const __half2*>(&zw.y));
+      const float2 zc01 = make_float2(z01.x + ZC, z01.y + ZC), zc23 = make_float2(z23.x + ZC, z23.y + ZC);
+      float bsum[GP];
+#pragma unroll
+      for (int h = 0; h < GP; ++h) {
+        const float4 qv = *reinterpret_cast<const float4*>(&sm.qrot[h][4 * lane]);
+        const float2 q01 = __fmul2_rn(make_float2(qv.x, qv.y), s01), q23 = __fmul2_rn(make_float2(qv.z, qv.w), s23);
+        const float qt[4] = {q01.x, q01.y, q23.x, q23.y};
+        float amax = fmaxf(fmaxf(fabsf(qt[0]), fabsf(qt[1])), fmaxf(fabsf(qt[2]), fabsf(qt[3])));
+        // beta uses the unrounded qt (and, with centred codes, z + 1.5: the mean code stays in fp32)
+        const float2 bz = __ffma2_rn(q01, zc01, __fmul2_rn(q23, zc23));
+        bsum[h] = bz.x + bz.y;
+        amax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax)));   // non-negative floats order like their bits
+        const float inv = amax > 1e-30f ? QF * rcp_approx(amax) : 0.f;
+        if constexpr (DQ == 4) {
+          uint32_t X[4], Y[4];
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            const float f = fmaf(qt[r], inv, MAGIC_F);                  // integer Q in the low mantissa bits
+            X[r] = (__float_as_uint(f) * mul_q + add_q) ^ 0x80808080u;   // balanced s8 digits of Q << shift
+          }
+          transpose4x4(X, Y);   // Y[d] = digit d of the four K positions = one B-fragment word of column (h, d)
+#pragma unroll
+          for (int d = 0; d < 4; ++d)
+            bq_base[(2 * (h >> 2) + (d >> 1)) * 256 + b_slot(4 * (2 * (h & 3) + (d & 1)) + btp, bk >> 1) * 4] = Y[d];
+        } else {
+          // Q + 128 in the low 16 mantissa bits; bytes 0, 1 ^ 0x0080 = the balanced digits (d0, d1): Q = d0 + 256 d1
+          const float2 i2 = make_float2(inv, inv), mg = make_float2(MAGIC_F + 128.f, MAGIC_F + 128.f);
+          const float2 f01 = __ffma2_rn(q01, i2, mg), f23 = __ffma2_rn(q23, i2, mg);
+          const uint32_t X0 = __float_as_uint(f01.x) ^ 0x80u, X1 = __float_as_uint(f01.y) ^ 0x80u;
+          const uint32_t X2 = __float_as_uint(f23.x) ^ 0x80u, X3 = __float_as_uint(f23.y) ^ 0x80u;
+          const uint32_t t0 = prmt(X0, X1, 0x5140), t1 = prmt(X2, X3, 0x5140);
+#pragma unroll
+          for (int d = 0; d < 2; ++d)
+            bq_base[(h >> 2) * 256 + b_slot(4 * (2 * (h & 3) + d) + btp, bk >> 1) * 4] = prmt(t0, t1, d ? 0x7632 : 0x5410);
+        }
+        if (lane == h) ws.hs[h].x = amax * (1.f / QF) * CLS_INV;   // logit = s2 * (acc * scale + beta)
+      }
+      const float bs = warp_reduce_multi<GP>(bsum, lane, RAdd());
+      if ((lane & (32 / GP - 1)) == 0) ws.hs[red_index<GP>(lane)].y = bs;
+      // s2 of the K rows (stored in row-slot order): 4 slots per lane
+      const uint32_t s2w = *reinterpret_cast<const uint32_t*>(kr + s2_off(BITS) + 4 * lane);
+      const float2 a01 = e4m3x2_to_f32x2((uint16_t)(s2w & 0xffff)), a23 = e4m3x2_to_f32x2((uint16_t)(s2w >> 16));
+      ws.aux_a[4 * lane + 0].x = a01.x; ws.aux_a[4 * lane + 1].x = a01.y;
+      ws.aux_a[4 * lane + 2].x = a23.x; ws.aux_a[4 * lane + 3].x = a23.y;
+    }
+    __syncwarp();
+    // ---- D3: QK^T over the 8 m-tiles: raw integer sums -> float (the scales follow once V's aux is there) ----
+    float sraw[4][HPW][4];
+    {
+      uint4 bf[2][NTQ];
+#pragma unroll
+      for (int hk = 0; hk < 2; ++hk)
+#pragma unroll
+        for (int nu = 0; nu < NTQ; ++nu) bf[hk][nu] = *reinterpret_cast<const uint4*>(&ws.bfr[nu][hk][b_slot(lane, hk)][0]);
+#pragma unroll
+      for (int mp = 0; mp < 4; ++mp) {
+        int32_t dd[2][NTQ][4];
+        contract_mp<BITS, NTQ, NTQ, true, DQ == 2, DQ == 2>(ws.krec, bf, mp, lane, dd);
+#pragma unroll
+        for (int u = 0; u < HPW; ++u)
+#pragma unroll
+          for (int i = 0; i < 4; ++i) sraw[mp][u][i] = undigit_w<DQ, NTQ>(dd, i >> 1, u, 2 * (i & 1));   // i = 2 mt + rho
+      }
+    }
+    __syncwarp();
+    // the K slot is free (codes consumed, aux read in phase A): request the next chunk's K record
+    if (lane == 0 && more) { mbar_expect_tx(&ws.fullk, RB); bulk_g2s(ws.krec, krec + (size_t)(4 * (it + 1)) * RB, RB, &ws.fullk); }
+    mbar_wait(&ws.fullv, par);
+    {   // aux of the V record: per-token (row-slot order) s1v, zv; per-channel s2v
+      const uint8_t* vr = ws.vrec;
+      const uint32_t s1w = *reinterpret_cast<const uint32_t*>(vr + s1_off(BITS) + 4 * lane);
+      const uint2 zw = *reinterpret_cast<const uint2*>(vr + z_off(BITS) + 8 * lane);
+      const uint32_t s2w = *reinterpret_cast<const uint32_t*>(vr + s2_off(BITS) + 4 * lane);
+      const float2 s01 = e4m3x2_to_f32x2((uint16_t)(s1w & 0xffff)), s23 = e4m3x2_to_f32x2((uint16_t)(s1w >> 16));
+      const float2 z01 = __half22float2(*reinterpret_cast<const __half2*>(&zw.x));
+      const float2 z23 = __half22float2(*reinterpret_cast<const __half2*>(&zw.y));
+      const float s1v[4] = {s01.x, s01.y, s23.x, s23.y}, zv[4] = {z01.x, z01.y, z23.x, z23.y};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const float s = fmaxf(s1v[j], 9.094947e-13f);   // 2^-40: a zero scale stays harmless
+        // pt = p s1v = exp2(logit + log2 s1v - m): the maximum is taken over the shifted logits, so pt <= 1
+        ws.aux_a[4 * lane + j].y = lg2_approx(s);
+        ws.aux_b[4 * lane + j] = make_float2(rcp_approx(s) * (1.f / PF), zv[j]);
+      }
+      {   // s2v of channels 4 lane + j (exact in fp16): channel slot c -> [c >> 5][c & 7][(c >> 3) & 3]
+        uint32_t h2[2];
+        asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2[0]) : "h"((uint16_t)(s2w & 0xffff)));
+        asm("cvt.rn.f16x2.e4m3x2 %0, %1;" : "=r"(h2[1]) : "h"((uint16_t)(s2w >> 16)));
+        const __half* hv = reinterpret_cast<const __half*>(h2);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) ws.aux_ch[lane >> 3][4 * (lane & 1) + j][(lane >> 1) & 3] = hv[j];
+      }
+    }
+    __syncwarp();
+    // ---- D3 (scales) + D4: logits of this thread's 16 tokens x HPW columns, maximum over the chunk -----------
+    float corr[HPW], wch[HPW], zsum[HPW];
+#pragma unroll
+    for (int u = 0; u < HPW; ++u) {
+      const float2 sb = ws.hs[ft + 4 * u];
+      float mx = -INFINITY;
+#pragma unroll
+      for (int mp = 0; mp < 4; ++mp)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const float2 aux = ws.aux_a[32 * mp + 16 * (i >> 1) + 8 * (i & 1) + fg];
+          sraw[mp][u][i] = fmaf(aux.x, fmaf(sraw[mp][u][i], sb.x, sb.y), aux.y);
+          mx = fmaxf(mx, sraw[mp][u][i]);
+        }
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 8));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 16));
+      // The fixed-point probabilities refer to the maximum mx of THIS chunk: a token is dropped only if it lies
+      // below the resolution relative to the largest of its 127 neighbours, whatever the context length; the chunk's
+      // sums enter the running ones with the weight wch = 2^(mx - m_new).  l uses the same rounded values as the numerator.
+      const float m_new = fmaxf(mr[u], mx);
+      corr[u] = ex2_approx(mr[u] - m_new);
+      wch[u] = ex2_approx(mx - m_new);
+      mr[u] = m_new;
+      float2 lz = make_float2(0.f, 0.f);    // {l, zero-point sum} of this thread's tokens
+#pragma unroll
+      for (int mp = 0; mp < 4; ++mp) {
+        const int jp = BITS == 2 ? mp : (mp & 1);
+        const uint32_t mul_p = 1u << (BITS * (NCLS - 1 - jp));
+        const uint32_t add_p = 0u - ((uint32_t)MAGIC_I * mul_p);
+        uint32_t X[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const float2 ab = ws.aux_b[32 * mp + 16 * (i >> 1) + 8 * (i & 1) + fg];   // {1 / (s1v PF), zv}
+          const float pt = ex2_approx(sraw[mp][u][i] - mx);
+          const float f = fmaf(pt, PF, MAGIC_F);        // fixed-point pt; its radix-256 digits are the low bytes of f's bits
+          const float pr = f - MAGIC_F;                 // PF * (rounded pt), an exact integer
+          lz = __ffma2_rn(make_float2(pr, pr), ab, lz);
+          X[i] = DP == 4 ? __float_as_uint(f) * mul_p + add_p : __float_as_uint(f);
+        }
+        // column (h, d) of column h = ft + 4u: n-tile (DP / 2) u + (d >> 1), g' = 2 ft + (d & 1); word (kappa = mp, half = fg >> 2, t' = fg & 3)
+        if constexpr (DP == 4) {
+          uint32_t Y[4];
+          transpose4x4(X, Y);
+#pragma unroll
+          for (int d = 0; d < 4; ++d)
+            ws.bfr[2 * u + (d >> 1)][mp >> 1][b_slot(4 * (2 * ft + (d & 1)) + (fg & 3), mp >> 1)][2 * (mp & 1) + (fg >> 2)] = Y[d];
+        } else {
+          const uint32_t t0 = prmt(X[0], X[1], 0x5140), t1 = prmt(X[2], X[3], 0x5140);
+#pragma unroll
+          for (int d = 0; d < 2; ++d)
+            ws.bfr[u][mp >> 1][b_slot(4 * (2 * ft + d) + (fg & 3), mp >> 1)][2 * (mp & 1) + (fg >> 2)] = prmt(t0, t1, d ? 0x7632 : 0x5410);
+        }
+      }
+      lz.x += __shfl_xor_sync(0xffffffffu, lz.x, 4);  lz.y += __shfl_xor_sync(0xffffffffu, lz.y, 4);
+      lz.x += __shfl_xor_sync(0xffffffffu, lz.x, 8);  lz.y += __shfl_xor_sync(0xffffffffu, lz.y, 8);
+      lz.x += __shfl_xor_sync(0xffffffffu, lz.x, 16); lz.y += __shfl_xor_sync(0xffffffffu, lz.y, 16);
+      zsum[u] = lz.y * (1.f / PF) * wch[u];
+      lp[u] = fmaf(lp[u], corr[u], lz.x * wch[u]);     // (every lane with the same ft holds the warp's l of column ft + 4u)
+    }
+    __syncwarp();
+    // ---- D5: value contraction over the 8 m-tiles (rows = channels), accumulate -----------------------------
+    {
+      uint4 bf[2][NTP];
+#pragma unroll
+      for (int hk = 0; hk < 2; ++hk)
+#pragma unroll
+        for (int nu = 0; nu < NTP; ++nu) bf[hk][nu] = *reinterpret_cast<const uint4*>(&ws.bfr[nu][hk][b_slot(lane, hk)][0]);
+#pragma unroll
+      for (int mp = 0; mp < 4; ++mp) {
+        int32_t dd[2][NTP][4];
+        contract_mp<BITS, NTP, NTP, false, DP == 2>(ws.vrec, bf, mp, lane, dd);
+        const uint2 sv = *reinterpret_cast<const uint2*>(&ws.aux_ch[mp][fg][0]);
+        const float2 s01 = __half22float2(*reinterpret_cast<const __half2*>(&sv.x)), s23 = __half22float2(*reinterpret_cast<const __half2*>(&sv.y));
+        const float s2v[4] = {s01.x, s01.y, s23.x, s23.y};
+#pragma unroll
+        for (int u = 0; u < HPW; ++u) {
+          const float cw = CLS_INV * (1.f / PF) * wch[u];
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            ac[mp][u][i] = fmaf(ac[mp][u][i], corr[u], s2v[i] * fmaf(undigit_w<DP, NTP>(dd, i >> 1, u, 2 * (i & 1)), cw, zsum[u]));
+        }
+      }
+    }
+    __syncwarp();
+    // the V slot is free: request the next chunk's V record
+    if (lane == 0 && more) { mbar_expect_tx(&ws.fullv, RB); bulk_g2s(ws.vrec, vrec + (size_t)(4 * (it + 1)) * RB, RB, &ws.fullv); }
+  }
+
+  // ---- merge of the 4 private states; hand over to the per-channel layout: thread tid = channel tid -----------
+  // every warp stages into ITS OWN dead record slots (no other warp touches them), so no barrier is needed before
+  float* stage = reinterpret_cast<float*>(ws.krec);   // [GP][128] floats
+  static_assert(RB >= GP * 128 * sizeof(float), "staging area");
+#pragma unroll
+  for (int u = 0; u < HPW; ++u) {
+    if (fg == 0) { sm.wz[warp][ft + 4 * u] = lp[u]; sm.wmax[warp][ft + 4 * u] = mr[u]; }
+#pragma unroll
+    for (int mp = 0; mp < 4; ++mp)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) stage[(ft + 4 * u) * 128 + 32 * mp + 16 * (i >> 1) + 8 * (i & 1) + fg] = ac[mp][u][i];
+  }
+  __syncthreads();
+  float m_run[GP], l_part[GP], l_tot[GP], acc[GP];
+#pragma unroll
+  for (int h = 0; h < GP; ++h) {
+    const float m0 = sm.wmax[0][h], m1 = sm.wmax[1][h], m2 = sm.wmax[2][h], m3 = sm.wmax[3][h];
+    const float M = fmaxf(fmaxf(m0, m1), fmaxf(m2, m3));
+    const float e0 = m0 == -INFINITY ? 0.f : ex2_approx(m0 - M), e1 = m1 == -INFINITY ? 0.f : ex2_approx(m1 - M);
+    const float e2 = m2 == -INFINITY ? 0.f : ex2_approx(m2 - M), e3 = m3 == -INFINITY ? 0.f : ex2_approx(m3 - M);
+    m_run[h] = M;
+    l_tot[h] = fmaf(e0, sm.wz[0][h], fmaf(e1, sm.wz[1][h], fmaf(e2, sm.wz[2][h], e3 * sm.wz[3][h])));
+    l_part[h] = tid == 0 ? l_tot[h] : 0.f;
+    const float a0 = reinterpret_cast<const float*>(sm.w[0].krec)[h * 128 + tid], a1 = reinterpret_cast<const float*>(sm.w[1].krec)[h * 128 + tid];
+    const float a2 = reinterpret_cast<const float*>(sm.w[2].krec)[h * 128 + tid], a3 = reinterpret_cast<const float*>(sm.w[3].krec)[h * 128 + tid];
+    acc[h] = fmaf(e0, a0, fmaf(e1, a1, fmaf(e2, a2, e3 * a3)));
+  }
+  __syncthreads();   // the staged partials are consumed: the slots may now receive the peers' partials, wmax / wz are free
+  if (A.cluster > 1) cluster_arrive();
+  // dead slots: [0, 16 x WS_STRIDE floats) landing area of the peers' partials, w[2] un-rotated q of the raw windows, w[3] merge weights
+  static_assert(sizeof(WS) * 2 >= 16 * WS_STRIDE * sizeof(float) && sizeof(WS) >= GP * 128 * sizeof(float), "landing / scratch areas");
+  float* qraw = reinterpret_cast<float*>(&sm.w[2]);
+  if (do_resid || do_sink || (A.k_blk != nullptr && w0.split == A.splits - 1)) {   // CTA-uniform: this CTA runs a raw window
+    for (int hh = warp; hh < GP; hh += 4) {
+      float v[4] = {0.f, 0.f, 0.f, 0.f};
+      if (hh < cm0.ncols) {
+        const size_t row = ((size_t)w0.b * cm0.n_q + cm0.tok0 + (hh >> cm0.lg)) * A.Hq + w0.hkv * g + (hh - ((hh >> cm0.lg) << cm0.lg));
+        const InT* qp = reinterpret_cast<const InT*>(A.q) + row * D + 4 * lane;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) v[j] = ld_in<InT>(qp + j) * A.q_scale;
+      }
+      *reinterpret_cast<float4*>(&qraw[hh * 128 + 4 * lane]) = make_float4(v[0], v[1], v[2], v[3]);
+    }
+    __syncthreads();
+  }
+  decode_finish<GP, InT>(A, sm, reinterpret_cast<float*>(&sm.w[0]), reinterpret_cast<float*>(&sm.w[3]), qraw, w0, cm0,
+                         do_resid, do_sink, m_run, l_part, l_tot, acc);
 }
 
 // LSE merge of R partial sets (e.g. all-gathered from R context-parallel ranks): one CTA per

@@ -32,7 +32,7 @@ class Params(C.Structure):
                 ("iters", C.c_int32), ("var_min", C.c_float), ("var_max", C.c_float),
                 ("log_lo", C.c_float), ("log_hi", C.c_float), ("rotate_k", C.c_int32),
                 ("rotate_v", C.c_int32), ("in_dtype", C.c_int32), ("out_dtype", C.c_int32),
-                ("splits", C.c_int32), ("aux_round", C.c_int32)]
+                ("splits", C.c_int32), ("aux_round", C.c_int32), ("decode_digits", C.c_int32)]
 
 
 class LayoutInfo(C.Structure):

@@ -341,3 +341,20 @@ def test_sink_region_append_matches_prefill(kv):
             assert torch.equal(out, kv.decode_attention(p, ref, q))
             _check_all_units(kv, p, inc, q, out, n, units={(0, 0), (1, 1)})
     assert int(inc.ticket.abs().sum()) == 0
+
+
+@pytest.mark.parametrize("bits,digits", [(2, 0), (2, 2), (2, 4), (4, 0), (4, 4)])
+@pytest.mark.parametrize("Hq", [32, 64])
+def test_decode_digit_plane_modes(kv, bits, digits, Hq):
+    # kvarn_params::decode_digits: 0 = q~ 22 bits / p~ 16 bits (default), 2 = 16 / 16 (fastest), 4 = 22 / 22; every mode
+    # against the oracle at the north_star tolerance, on a long-ish context (mode 2 is measured up to 1.1e-3 on
+    # short peaked ones: DESIGN.md 6.2) and with a residual window
+    n_tok = 128 * 40 + 19
+    K, V = W.kv_tokens(2, 8, n_tok, seed=97, device="cuda")
+    q = W.queries(2, Hq, seed=97, device="cuda")
+    p = kv.default_params(bits, decode_digits=digits)
+    cache = _build_cache(kv, p, K, V)
+    out = kv.decode_attention(p, cache, q)
+    worst = _check_all_units(kv, p, cache, q, out, n_tok, units={(0, 0), (1, 3), (1, 7)})
+    ref4 = kv.decode_attention(kv.default_params(bits, decode_digits=4), cache, q)
+    assert (out - ref4).abs().max() <= P.ATTN_RTOL * ref4.abs().max()
