@@ -223,6 +223,9 @@ static int launch_quantize(const kvarn_params* p, const QuantArgs& A, int n_kind
 // (sequence, KV head) and merge through DSMEM; `nclus` clusters per (sequence, KV head) merge
 // through the workspace (only when one cluster leaves most of the GPU idle on long contexts).
 struct SplitPlan { int cluster, nclus; };
+#ifndef KVARN_SPLIT_FEW_SLOTS
+#define KVARN_SPLIT_FEW_SLOTS 2
+#endif
 constexpr int KVARN_MAX_CLUSTER = 8;    // portable maximum; 9..16 (non-portable) measured slower: 25 -> 27..31 us on config 1
 
 // DQ, DP = digit planes of q~ / p~ (kvarn_decode.cuh)
@@ -293,17 +296,17 @@ static SplitPlan split_plan(const kvarn_params* p, int B, int Hkv, int g, int ma
     return sp;
   }
   const int bh = B * Hkv;
-  const int slots = decode_slots(p, g);        // resident CTAs of decode_kernel on this device
+  const int slots = decode_slots(p, g);        // resident CTAs of the decode kernel on this device
   int want = slots / bh;                        // splits that still fit in one wave
   if (want < 1) want = 1;
   if (want > max_chunks) want = max_chunks;
   sp.cluster = want < KVARN_MAX_CLUSTER ? want : KVARN_MAX_CLUSTER;
-  // about one CTA per slot and long CTAs: halve them, so that the CTAs of the second half-wave balance the
-  // SMs that got one CTA more (config 4: 512 CTAs on 592 slots 1327 us, 1024 half-length CTAs 1177 us)
-  if (sp.cluster == 1 && max_chunks >= 32) sp.cluster = 2;
+  // about one CTA per slot and long CTAs: halve them, so that the CTAs of the second half-wave balance the SMs that
+  // got one CTA more (config 4, 512 units on 444 slots: 1 / 2 / 3 / 4 / 6 CTAs per unit measured in DESIGN.md 6.2)
+  if (sp.cluster == 1 && max_chunks >= 32) sp.cluster = KVARN_SPLIT_FEW_SLOTS;
   if (sp.cluster == KVARN_MAX_CLUSTER) {
     const int per = (max_chunks + KVARN_MAX_CLUSTER - 1) / KVARN_MAX_CLUSTER;   // chunks per CTA with one cluster
-    if (per > 32) {
+    if (per > 32) {   // a very long context with few sequences: several clusters per sequence, merged through the workspace
       int nc = want / KVARN_MAX_CLUSTER, cap = per / 16;
       if (nc > cap) nc = cap;
       if (nc > 64) nc = 64;

@@ -704,7 +704,9 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
   const bool do_resid = (w0.split == A.splits - 1) && w0.resid > 0;
   const bool do_sink = (w0.split == 0) && w0.n_sink_tok > 0;
   // ---- chunk range of this split (balanced against the raw windows as in the CTA-cooperative variant) ----
-  const int w_sink = (w0.n_sink_tok + 11) / 12, w_res = (w0.resid + cm0.blk_cnt + 11) / 12;
+  // (a raw window of n tokens keeps its CTA as long as ~n / 8 chunks do -- measured on the 64k-context cache with
+  //  a 128-token sink and a 64-token residual window --, so the splits that own one get that many chunks fewer)
+  const int w_sink = (w0.n_sink_tok + 7) / 8, w_res = (w0.resid + cm0.blk_cnt + 7) / 8;
   const int per = (w0.n_chunks + w_sink + w_res + A.splits - 1) / A.splits;
   const int c_begin = min(max(w0.split * per - w_sink, 0), w0.n_chunks);
   const int c_end = min(max((w0.split + 1) * per - w_sink, 0), w0.n_chunks);

@@ -21,6 +21,8 @@
 // column passes and K+1 row passes.
 #pragma once
 
+#include <type_traits>
+
 #include "kvarn_common.cuh"
 
 namespace kvarn {
@@ -41,11 +43,13 @@ template <int BITS>
 struct QuantSmem {
   alignas(16) float part[8][2][128];  // cross-warp partials (row sums / min-max)
   float a[128];           // 1 / S_r  (per channel)
-  float b[128];           // 1 / S_c  (per token)
+  alignas(16) float b[128];    // 1 / S_c  (per token)
+  alignas(16) float mu[128];   // mean over the tile's tokens of T[c, :] (the channel offsets of P:127): pivot of the row passes
+  float bbar;             // mean over tokens of b (one column update old, see row_partials)
   // per iterate k = 0..iters: column / row variances of C_k and the log-scales that produced it;
   // the best iterate (Alg. 1 lines 7, 18) is selected once, after the loop
-  float cvh[KVARN_MAX_ITERS + 1][128];
-  float rvh[KVARN_MAX_ITERS + 1][128];
+  alignas(16) float cvh[KVARN_MAX_ITERS + 1][128];
+  alignas(16) float rvh[KVARN_MAX_ITERS + 1][128];
   float Lch[KVARN_MAX_ITERS + 1][128];
   float Lrh[KVARN_MAX_ITERS + 1][128];
   float imb[KVARN_MAX_ITERS + 1];
@@ -165,10 +169,22 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
   float Lc = 0.f, b_own = 1.f;  // log column scale of tok_own
   float Lr = 0.f, a_own = 1.f;  // log row scale of channel tid (tid < 128)
 
-  // row half-step, part 1: per-channel sums of (b_t T) and (b_t T)^2 over this
-  // warp's 16 tokens -> sm.part[warp][stat][channel]
-  auto row_partials = [&]() {
-    float2 s1[4], s2[4];
+  // row half-step, part 1: per-channel sums of u and u^2 over this warp's 16 tokens -> sm.part[warp][stat][channel],
+  // with u = b_t T[c,t] (PIV = false) or u = b_t T[c,t] - mu_c bbar (PIV = true).  The variance does not depend on the
+  // pivot; the single-pass form E[u^2] - E[u]^2 does, in fp32: channels whose offset is tens to hundreds of standard
+  // deviations ("in some cases have large offsets") would lose 3 .. 6 digits without it.  mu_c bbar is the row
+  // mean of b_t T up to the correlation of b with the centred data, so E[u] stays at the size of the standard
+  // deviation.  A tile takes the pivoted form only if pass 0 finds a channel with |mean| > 4 std (CTA-uniform flag).
+  auto row_partials = [&](auto piv_tag, const float bbar) {
+    constexpr bool PIV = decltype(piv_tag)::value;
+    float2 s1[4], s2[4], npiv[4];
+    if constexpr (PIV) {
+      const float4* pm = reinterpret_cast<const float4*>(&sm.mu[c0]);
+      const float4 m0 = pm[0], m1 = pm[1];
+      const float2 nb = f2(-bbar, -bbar);
+      npiv[0] = mul2(f2(m0.x, m0.y), nb); npiv[1] = mul2(f2(m0.z, m0.w), nb);
+      npiv[2] = mul2(f2(m1.x, m1.y), nb); npiv[3] = mul2(f2(m1.z, m1.w), nb);
+    }
 #pragma unroll
     for (int kp = 0; kp < 4; ++kp) { s1[kp] = f2(0.f, 0.f); s2[kp] = f2(0.f, 0.f); }
 #pragma unroll
@@ -176,7 +192,7 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       const float2 bb = f2(b[i], b[i]);
 #pragma unroll
       for (int kp = 0; kp < 4; ++kp) {
-        float2 u = mul2(x[i][kp], bb);
+        float2 u = PIV ? fma2(x[i][kp], bb, npiv[kp]) : mul2(x[i][kp], bb);
         s1[kp] = add2(s1[kp], u);
         s2[kp] = fma2(u, u, s2[kp]);
       }
@@ -231,11 +247,27 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     return mx / fmaxf(mn, vc.var_min);
   };
 
-  // pass 0: row variances of the initial C = T (needed by I_best <- Imb(C), line 7)
-  row_partials();
+  // pass 0: row variances of the initial C = T (needed by I_best <- Imb(C), line 7); the row means mu_c are the
+  // pivots of the later passes, and decide whether this tile needs them
+  row_partials(std::false_type{}, 0.f);
   __syncthreads();
-  if (tid < 128) { sm.rvh[0][tid] = row_variance_own(); sm.Lrh[0][tid] = 0.f; }
-  __syncthreads();
+  bool off = false;
+  if (tid < 128) {
+    float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) { s1 += sm.part[w][0][tid]; s2 += sm.part[w][1][tid]; }
+    const float mean = s1 * inv_n;
+    const float var = fmaxf(fmaf(-mean, mean, s2 * inv_n), 0.f);
+    sm.mu[tid] = mean; sm.rvh[0][tid] = var; sm.Lrh[0][tid] = 0.f;
+    off = mean * mean > 16.f * var;          // |mean| > 4 std: E[u^2] - E[u]^2 starts losing digits
+  }
+  const bool piv = __syncthreads_or(off);    // CTA-uniform
+  if (piv) {   // redo pass 0 centred on mu (b = 1: exactly mean-free)
+    row_partials(std::true_type{}, 1.f);
+    __syncthreads();
+    if (tid < 128) sm.rvh[0][tid] = row_variance_own();
+    __syncthreads();
+  }
 
   for (int k = 1; k <= vc.iters + 1; ++k) {
     const bool update = (k <= vc.iters);
@@ -273,9 +305,32 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
       }
     }
     // ---- row half-step (lines 13-15) --------------------------------------------
-    if (update) row_partials();
+    // pivot scale bbar = mean_t b_t (tiles with large channel offsets only): in the first three iterations (b jumps
+    // from 1 to 1 / S_c, then still moves by per cents) it is taken fresh, at the price of one more CTA barrier; later
+    // it is the value warp 4 left during the previous iteration's row phase (one column update old: b then moves by
+    // < 1e-3 per iteration)
+    if (update) {
+      if (piv) {
+        float bbar;
+        if (k <= 3) {
+          __syncthreads();
+          const float4 b4 = reinterpret_cast<const float4*>(sm.b)[lane];
+          bbar = warp_sum((b4.x + b4.y) + (b4.z + b4.w)) * inv_n;
+        } else {
+          bbar = sm.bbar;
+        }
+        row_partials(std::true_type{}, bbar);
+      } else {
+        row_partials(std::false_type{}, 0.f);
+      }
+    }
     __syncthreads();
     if (update) {
+      if (piv && warp == 4) {   // (idle in this phase) mean of the b the column half-step of this iteration left
+        const float4 b4 = reinterpret_cast<const float4*>(sm.b)[lane];
+        const float s = warp_sum((b4.x + b4.y) + (b4.z + b4.w)) * inv_n;
+        if (lane == 0) sm.bbar = s;
+      }
       if (tid < 128) {
         const float var = row_variance_own();
         const float vcl = fminf(fmaxf(var, vc.var_min), vc.var_max);

@@ -31,26 +31,26 @@ def _tile_job(p, kind: int, X: np.ndarray, k_gpu: int):
 
 
 def compare_quantized_tile(kv, p, kind: int, rec: np.ndarray, k_gpu: int, imb_gpu: np.ndarray,
-                           aux_gpu: np.ndarray, ref: dict, stats: dict):
+                           aux_gpu: np.ndarray, ref: dict, stats: dict, tol: float = 1.0):
     """One GPU record (+ debug outputs) against the oracle's result `ref` (oracle.fanout 'quantize' worker:
     the free-running trajectory I and the tile quantised at the kernel's iterate k_gpu)."""
     codes, s1, s2, z = kv.unpack_record(p, kind, rec)
     I = ref["I"]
     # (1) the iterate kept by the kernel is a valid choice of Alg. 1 line 18 (R10)
     assert 0 <= k_gpu <= p.iters
-    assert I[k_gpu] <= I.min() * (1 + IMB_ACCEPT), (k_gpu, I)
+    assert I[k_gpu] <= I.min() * (1 + IMB_ACCEPT * tol), (k_gpu, I)
     # (2) imbalance trajectory: a ratio of two variances, each a function of scales that agree to SCALE_RTOL
     #     (squared: 2 x) -> 4 x SCALE_RTOL
     n = p.iters + 1
-    assert np.allclose(imb_gpu[:n], I[:n], rtol=4 * SCALE_RTOL), (imb_gpu[:n], I[:n])
+    assert np.allclose(imb_gpu[:n], I[:n], rtol=4 * SCALE_RTOL * tol), (imb_gpu[:n], I[:n])
     # (3) pre-storage scales / zero-points at the kernel's k
     s1_f, s2_f, z_f = aux_gpu[0].astype(np.float64), aux_gpu[1].astype(np.float64), aux_gpu[2].astype(np.float64)
-    assert np.allclose(s1_f, ref["s1_f"], rtol=SCALE_RTOL, atol=0), np.abs(s1_f / ref["s1_f"] - 1).max()
-    assert np.allclose(s2_f, ref["s2_f"], rtol=SCALE_RTOL, atol=0), np.abs(s2_f / ref["s2_f"] - 1).max()
+    assert np.allclose(s1_f, ref["s1_f"], rtol=SCALE_RTOL * tol, atol=0), np.abs(s1_f / ref["s1_f"] - 1).max()
+    assert np.allclose(s2_f, ref["s2_f"], rtol=SCALE_RTOL * tol, atol=0), np.abs(s2_f / ref["s2_f"] - 1).max()
     # z = mn / s is O(1..10) in code units; tolerance relative to the code range
     # (R9b: z = mn / stored step, so it is only comparable where the stored s1 agrees -- an FP8 tie moves it by 6 %)
     zcmp = (s1 == ref["s1"]) if p.aux_round else np.ones(128, dtype=bool)
-    assert np.allclose(z_f[zcmp], ref["z_f"][zcmp], rtol=SCALE_RTOL, atol=SCALE_RTOL * (1 << p.bits)), \
+    assert np.allclose(z_f[zcmp], ref["z_f"][zcmp], rtol=SCALE_RTOL * tol, atol=SCALE_RTOL * tol * (1 << p.bits)), \
         np.abs(z_f - ref["z_f"])[zcmp].max()
     # (4) stored bytes = storage rounding of the kernel's own fp32 values
     st_mis = int((s1.astype(np.float64) != O.round_fp8_e4m3(s1_f)).sum()
@@ -84,21 +84,22 @@ def check_quantized_tile(kv, p, kind: int, X: np.ndarray, rec: np.ndarray, k_gpu
     return compare_quantized_tile(kv, p, kind, rec, k_gpu, imb_gpu, aux_gpu, ref, stats)
 
 
-def check_quantized_tiles(kv, p, kind: int, Xs, recs, k_gpus, imbs, auxs, stats: dict, procs=None):
-    """The same for many tiles, the oracle fanned out over the host cores (oracle/fanout.py)."""
+def check_quantized_tiles(kv, p, kind: int, Xs, recs, k_gpus, imbs, auxs, stats: dict, procs=None, tol: float = 1.0):
+    """The same for many tiles, the oracle fanned out over the host cores (oracle/fanout.py).  tol > 1 widens the
+    floating-point tolerances (inputs whose own fp32 rounding exceeds them: see the caller)."""
     refs = fanout.pmap("quantize", [_tile_job(p, kind, X, k) for X, k in zip(Xs, k_gpus)], procs)
     for rec, k, imb, aux, ref in zip(recs, k_gpus, imbs, auxs, refs):
-        compare_quantized_tile(kv, p, kind, rec, int(k), imb, aux, ref, stats)
+        compare_quantized_tile(kv, p, kind, rec, int(k), imb, aux, ref, stats, tol)
 
 
-def assert_mismatch_budget(stats: dict):
+def assert_mismatch_budget(stats: dict, aux_frac: float = AUX_MISMATCH_FRAC, code_frac: float = CODE_MISMATCH_FRAC):
     """north_star: at most 1e-4 of the codes differ (each by one level).  Stored aux values:
     the same 1e-4 budget; a test over fewer than 10^4 stored values is allowed ONE tie (a budget below one
     value would turn every legal tie into a failure): DESIGN.md "Tolerances" derives the expected rate
     (dominated by the FP16 zero-points) and tests/test_gpu_parity_full.py measures it over > 5000 tiles."""
     frac = stats["code_mismatch"] / max(stats["codes"], 1)
-    assert frac <= CODE_MISMATCH_FRAC, f"code mismatch fraction {frac:.2e}"
-    assert stats["aux_mismatch"] <= max(1, int(np.ceil(AUX_MISMATCH_FRAC * stats["aux"]))), stats
+    assert frac <= code_frac, f"code mismatch fraction {frac:.2e}"
+    assert stats["aux_mismatch"] <= max(1, int(np.ceil(aux_frac * stats["aux"]))), stats
 
 
 def oracle_attention_from_records(kv, p, k_recs, v_recs, k_resid, v_resid, q, sm_scale=None):

@@ -206,7 +206,9 @@ def test_round_before_variant_vs_oracle(kv, bits):
         for i in range(0, n, 3):
             P.check_quantized_tile(kv, p, kind, P.tile_f64(T[i]), R[i].cpu().numpy(), int(dbg.k_best[kind, i]),
                                    dbg.imb[kind, i].cpu().numpy(), dbg.aux[kind, i].cpu().numpy(), stats)
-    P.assert_mismatch_budget(stats)
+    # R9b: z = fp16(mn / (fp8(s1) / absorbed)) -- a quotient of rounded quantities -- lands on an FP16 boundary more
+    # often than the plain z = mn / s: measured 3 of 6144 zero-points here, against 9e-5 per zero-point in the default mode
+    P.assert_mismatch_budget(stats, aux_frac=3e-4)
     # the variant's purpose: dequantising the stored record reproduces the token norms better at 4-bit
     if bits == 4:
         p0 = kv.default_params(bits)
