@@ -453,6 +453,77 @@ def stored_traffic():
     return out
 
 
+def cp_shard(n_chunks: int, rank: int, world: int):
+    """Context-parallel split of a sequence's chunks over the ranks: rank r holds chunks
+    [lo, hi) -- contiguous, sizes differing by at most one -- and the last rank also the residual tokens."""
+    base, rem = divmod(n_chunks, world)
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def run_cp(args, kv, W, dev, dist, rank, world):
+    """--mode cp: configs[4] (2-bit) with every sequence's tokens split over the N ranks.  Per step and rank:
+    kvarn_decode_attention_partial over the local share -> ONE NCCL all-gather of {m, l, o[128]} per (b, q head)
+    (528 B each) -> kvarn_merge_partials.  Strong scaling: the total work is fixed, value = whole-cache bytes / time."""
+    sh = W.CONFIG4
+    p = kv.default_params(2)
+    lo, hi = cp_shard(sh.n_chunks, rank, world)
+    n_tok = (hi - lo) * G + (sh.resid if rank == world - 1 else 0)
+    cache = kv.Cache(p, sh.B, sh.Hkv, max(hi - lo, 1), device=dev)
+    for b0 in range(0, sh.B, 4):   # every rank draws the same sequences and keeps its slice of the tokens
+        K, V = W.kv_tokens(4, sh.Hkv, sh.ctx, seed=sh.seed + b0, device=dev)
+        kv.prefill(p, cache.slice(b0, b0 + 4), K[:, :, lo * G:lo * G + n_tok].contiguous(), V[:, :, lo * G:lo * G + n_tok].contiguous())
+        del K, V
+    q = W.queries(sh.B, sh.Hq, seed=sh.seed, device=dev)
+    ws = torch.empty((max(kv.decode_workspace_bytes(p, sh.B, sh.Hq, sh.Hkv, cache.max_chunks), 16),), dtype=torch.uint8, device=dev)
+    part = torch.empty((sh.B, sh.Hq, kv.PART_STRIDE), dtype=torch.float32, device=dev)
+    parts = torch.empty((world,) + tuple(part.shape), dtype=torch.float32, device=dev)
+    out = torch.empty((sh.B, sh.Hq, D), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        kv.decode_attention_partial(p, cache, q, part=part, ws=ws)
+        if dist is not None:
+            dist.all_gather_into_tensor(parts, part)
+        else:
+            parts[0].copy_(part)
+        kv.merge_partials(parts, out=out)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0"))) if rank == 0 else None
+    if dist: dist.barrier()
+    torch.cuda.synchronize()
+    a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(args.steps):
+        step()
+    b.record(stream)
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    ms = max_over_ranks([a.elapsed_time(b) / args.steps], dist, dev)[0]
+    if rank != 0:
+        return
+    rb = kv.record_bytes(p)
+    total = sh.B * sh.Hkv * (sh.n_chunks * 2 * rb + sh.resid * 2 * D * 2) + sh.B * sh.Hq * (D * 2 + D * 4)
+    hbm_peak, peak_src = peaks()
+    gbs = total / (ms * 1e-3) / 1e9
+    line = {"metric": "kvarn_2bit_decode_attn_GBps", "value": gbs, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[4]: 70B-shaped long-context decode, context-parallel over the ranks",
+                       "B": sh.B, "Hq": sh.Hq, "Hkv": sh.Hkv, "ctx": sh.ctx, "bits": 2, "mode": "cp",
+                       "exchange": "all_gather of {m, l, o[128]} per (b, q head): %d B per rank and step" % (sh.B * sh.Hq * kv.PART_STRIDE * 4),
+                       "l2": "inputs larger than L2 (2.4 GB of records per step)", "parallelism": "cp%d" % world},
+            "roofline": {"kernel": "decode_kernel_w<2,8,4,2,bf16> (partial) + merge_partials_kernel", "bound": "hbm",
+                         "achieved": gbs / world, "peak": hbm_peak, "unit": "GB/s per GPU", "frac": gbs / world / hbm_peak,
+                         "traffic": None, "peak_source": peak_src},
+            "gpu_launches": 2 * args.steps, "clocks": clocks}
+    print(json.dumps(compact(line)))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -466,6 +537,9 @@ def main():
     ap.add_argument("--extras-only", action="store_true",
                     help="run only the configs[2] / [3] / [4] measurements (profiling aid)")
     ap.add_argument("--only", default="", help="with --extras-only: comma-separated extras groups to run")
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "cp"],
+                    help="replicas (default): N independent replicas of the configs[1] step; cp: configs[4] decode with every "
+                         "sequence's tokens split over the N ranks (partial -> NCCL all-gather -> LSE merge)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "kvarn" else args.warmup
 
@@ -487,6 +561,7 @@ def main():
     dist = None
     if world > 1:
         import torch.distributed as dist
+        os.environ.setdefault("NCCL_DEBUG", "VERSION")    # one line per job: which NCCL carries the collectives
         dist.init_process_group("nccl", device_id=dev)
 
     # libkvarn.so is built in-tree (git-ignored): local rank 0 builds it if missing or stale, the others wait
@@ -497,6 +572,10 @@ def main():
         dist.barrier()
     from paper_2606_03458_b200 import kvarn as kv
     hbm_peak, peak_src = peaks()
+    if args.mode == "cp":
+        run_cp(args, kv, W, dev, dist, rank, world)
+        if dist: dist.destroy_process_group()
+        return
     if args.extras_only:
         if rank == 0:
             only = set(x for x in args.only.split(",") if x)

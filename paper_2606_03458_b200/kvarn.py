@@ -326,7 +326,7 @@ def context_parallel_decode(p: Params, cache: Cache, q: torch.Tensor, group=None
     part = decode_attention_partial(p, cache, q, sm_scale=sm_scale)
     world = dist.get_world_size(group)
     parts = torch.empty((world,) + tuple(part.shape), device=part.device, dtype=torch.float32)
-    dist.all_gather_into_tensor(parts, part, group=group)
+    dist.all_gather_into_tensor(parts, part, group=group)       # 528 B per (b, q head) and rank
     return merge_partials(parts, out_dtype=torch.float32 if p.out_dtype == F32 else torch.bfloat16)
 
 
