@@ -269,83 +269,89 @@ __device__ void quantize_tile(float2 (&x)[8][4], const int kind, const bool rota
     __syncthreads();
   }
 
-  for (int k = 1; k <= vc.iters + 1; ++k) {
-    const bool update = (k <= vc.iters);
-    // ---- column half-step (lines 10-12): statistics of a_c T over channels ----
-    {
-      float v[16];
+  // The iterations, compiled twice: the plain form and the pivoted one (tiles with large channel offsets); a tile
+  // runs one of them, so the plain form carries none of the pivot's code in its loop.
+  auto varn_loop = [&](auto piv_tag) {
+    constexpr bool PIV = decltype(piv_tag)::value;
+    for (int k = 1; k <= vc.iters + 1; ++k) {
+      const bool update = (k <= vc.iters);
+      // ---- column half-step (lines 10-12): statistics of a_c T over channels ----
       {
-        float2 s1[8], s2[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) { s1[i] = f2(0.f, 0.f); s2[i] = f2(0.f, 0.f); }
-#pragma unroll
-        for (int i = 0; i < 8; ++i)
-#pragma unroll
-          for (int kp = 0; kp < 4; ++kp) {
-            float2 u = mul2(x[i][kp], a2[kp]);
-            s1[i] = add2(s1[i], u);
-            s2[i] = fma2(u, u, s2[i]);
-          }
-#pragma unroll
-        for (int i = 0; i < 8; ++i) { v[i] = s1[i].x + s1[i].y; v[8 + i] = s2[i].x + s2[i].y; }
-      }
-      float mine = xreduce16(v, li, OpAdd());
-      float other = __shfl_xor_sync(0xffffffffu, mine, 8);
-      const float s1t = (li & 8) ? other : mine, s2t = (li & 8) ? mine : other;
-      const float mean = s1t * inv_n;
-      const float var = fmaxf(fmaf(-mean, mean, s2t * inv_n), 0.f) * (b_own * b_own);
-      if (li < 8) { sm.cvh[k - 1][tok_own] = var; sm.Lch[k - 1][tok_own] = Lc; }
-      if (update) {
-        const float vcl = fminf(fmaxf(var, vc.var_min), vc.var_max);
-        Lc = fminf(fmaxf(fmaf(0.34657359027997264f, fast_log2(vcl), Lc), vc.log_lo), vc.log_hi);   // + 0.5 ln v
-        b_own = fast_exp2(-1.4426950408889634f * Lc);                                               // e^-Lc
-        if (li < 8) sm.b[tok_own] = b_own;
-        __syncwarp();
-        reload_b();
-      }
-    }
-    // ---- row half-step (lines 13-15) --------------------------------------------
-    // pivot scale bbar = mean_t b_t (tiles with large channel offsets only): in the first three iterations (b jumps
-    // from 1 to 1 / S_c, then still moves by per cents) it is taken fresh, at the price of one more CTA barrier; later
-    // it is the value warp 4 left during the previous iteration's row phase (one column update old: b then moves by
-    // < 1e-3 per iteration)
-    if (update) {
-      if (piv) {
-        float bbar;
-        if (k <= 3) {
-          __syncthreads();
-          const float4 b4 = reinterpret_cast<const float4*>(sm.b)[lane];
-          bbar = warp_sum((b4.x + b4.y) + (b4.z + b4.w)) * inv_n;
-        } else {
-          bbar = sm.bbar;
+        float v[16];
+        {
+          float2 s1[8], s2[8];
+  #pragma unroll
+          for (int i = 0; i < 8; ++i) { s1[i] = f2(0.f, 0.f); s2[i] = f2(0.f, 0.f); }
+  #pragma unroll
+          for (int i = 0; i < 8; ++i)
+  #pragma unroll
+            for (int kp = 0; kp < 4; ++kp) {
+              float2 u = mul2(x[i][kp], a2[kp]);
+              s1[i] = add2(s1[i], u);
+              s2[i] = fma2(u, u, s2[i]);
+            }
+  #pragma unroll
+          for (int i = 0; i < 8; ++i) { v[i] = s1[i].x + s1[i].y; v[8 + i] = s2[i].x + s2[i].y; }
         }
-        row_partials(std::true_type{}, bbar);
-      } else {
-        row_partials(std::false_type{}, 0.f);
+        float mine = xreduce16(v, li, OpAdd());
+        float other = __shfl_xor_sync(0xffffffffu, mine, 8);
+        const float s1t = (li & 8) ? other : mine, s2t = (li & 8) ? mine : other;
+        const float mean = s1t * inv_n;
+        const float var = fmaxf(fmaf(-mean, mean, s2t * inv_n), 0.f) * (b_own * b_own);
+        if (li < 8) { sm.cvh[k - 1][tok_own] = var; sm.Lch[k - 1][tok_own] = Lc; }
+        if (update) {
+          const float vcl = fminf(fmaxf(var, vc.var_min), vc.var_max);
+          Lc = fminf(fmaxf(fmaf(0.34657359027997264f, fast_log2(vcl), Lc), vc.log_lo), vc.log_hi);   // + 0.5 ln v
+          b_own = fast_exp2(-1.4426950408889634f * Lc);                                               // e^-Lc
+          if (li < 8) sm.b[tok_own] = b_own;
+          __syncwarp();
+          reload_b();
+        }
       }
-    }
-    __syncthreads();
-    if (update) {
-      if (piv && warp == 4) {   // (idle in this phase) mean of the b the column half-step of this iteration left
-        const float4 b4 = reinterpret_cast<const float4*>(sm.b)[lane];
-        const float s = warp_sum((b4.x + b4.y) + (b4.z + b4.w)) * inv_n;
-        if (lane == 0) sm.bbar = s;
-      }
-      if (tid < 128) {
-        const float var = row_variance_own();
-        const float vcl = fminf(fmaxf(var, vc.var_min), vc.var_max);
-        const float Lr_new = fminf(fmaxf(fmaf(0.34657359027997264f, fast_log2(vcl), Lr), vc.log_lo), vc.log_hi);
-        const float a_new = fast_exp2(-1.4426950408889634f * Lr_new);
-        const float ratio = a_new * fast_exp2(1.4426950408889634f * Lr);   // a_new / a_old
-        sm.rvh[k][tid] = var * ratio * ratio;  // row variance after rescaling the row
-        sm.Lrh[k][tid] = Lr_new;
-        sm.a[tid] = a_new;
-        Lr = Lr_new; a_own = a_new;
+      // ---- row half-step (lines 13-15) --------------------------------------------
+      // pivot scale bbar = mean_t b_t (tiles with large channel offsets only): in the first three iterations (b jumps
+      // from 1 to 1 / S_c, then still moves by per cents) it is taken fresh, at the price of one more CTA barrier; later
+      // it is the value warp 4 left during the previous iteration's row phase (one column update old: b then moves by
+      // < 1e-3 per iteration)
+      if (update) {
+        if constexpr (PIV) {
+          float bbar;
+          if (k <= 3) {
+            __syncthreads();
+            const float4 b4 = reinterpret_cast<const float4*>(sm.b)[lane];
+            bbar = warp_sum((b4.x + b4.y) + (b4.z + b4.w)) * inv_n;
+          } else {
+            bbar = sm.bbar;
+          }
+          row_partials(std::true_type{}, bbar);
+        } else {
+          row_partials(std::false_type{}, 0.f);
+        }
       }
       __syncthreads();
-      reload_a();
+      if (update) {
+        if (PIV && warp == 4) {   // (idle in this phase) mean of the b the column half-step of this iteration left
+          const float4 b4 = reinterpret_cast<const float4*>(sm.b)[lane];
+          const float s = warp_sum((b4.x + b4.y) + (b4.z + b4.w)) * inv_n;
+          if (lane == 0) sm.bbar = s;
+        }
+        if (tid < 128) {
+          const float var = row_variance_own();
+          const float vcl = fminf(fmaxf(var, vc.var_min), vc.var_max);
+          const float Lr_new = fminf(fmaxf(fmaf(0.34657359027997264f, fast_log2(vcl), Lr), vc.log_lo), vc.log_hi);
+          const float a_new = fast_exp2(-1.4426950408889634f * Lr_new);
+          const float ratio = a_new * fast_exp2(1.4426950408889634f * Lr);   // a_new / a_old
+          sm.rvh[k][tid] = var * ratio * ratio;  // row variance after rescaling the row
+          sm.Lrh[k][tid] = Lr_new;
+          sm.a[tid] = a_new;
+          Lr = Lr_new; a_own = a_new;
+        }
+        __syncthreads();
+        reload_a();
+      }
     }
-  }
+  };
+  if (piv) varn_loop(std::true_type{}); else varn_loop(std::false_type{});
 
   // ---- best iterate (lines 7, 18): I_k = Imb(C_k), keep the last k with I_k <= min of the earlier ones
   __syncthreads();
