@@ -335,7 +335,8 @@ static cudaError_t launch_decode_k(DK, const DecodeArgs& A, cudaStream_t st) {
   return cudaLaunchKernelEx(&cfg, kern, A);
 }
 
-static cudaError_t launch_decode(const kvarn_params* p, const DecodeArgs& A, cudaStream_t st) {
+static cudaError_t launch_decode(const kvarn_params* p, DecodeArgs& A, cudaStream_t st) {
+  A.shl_mul[0] = 4u; A.shl_mul[1] = 16u; A.shl_mul[2] = 64u;
   return with_decode_kernel(p, A.tpc * A.g <= 4 ? 4 : 8, [&](auto dk) { return launch_decode_k(dk, A, st); });
 }
 

@@ -75,6 +75,10 @@ struct DecodeArgs {
   // context-parallel building block: 1 = write the un-normalised partial {m, l, o[128]} of every (b, q head) to
   // `out` ([B][Hq][PART_STRIDE] fp32) instead of the normalised output; merged across ranks by merge_partials_kernel
   int partial;
+  // 4, 16, 64: the plane shifts of the aligned A fragments as MULTIPLIERS from the constant bank -- an integer
+  // multiply issues on the fma pipe, and only an operand ptxas cannot see through keeps it from becoming a shift
+  // on the alu pipe (the busiest unit of the 2-bit kernel)
+  uint32_t shl_mul[3];
 };
 
 // ------------------------------------------------------------------ PTX wrappers
@@ -624,15 +628,16 @@ struct DecSmemW {
 // CENTRED: s8 value 64 code - 96 = 64 (code - 1.5): bit 7 inverted, bit 6 kept, bit 5 set -- with M1 = bits {7, 5} and
 // M2 = bits {6, 5} that is (M1 & ~M2 & ~x) | (~M1 & M2 & x) | (M1 & M2), one LOP3.
 template <int BITS, bool CENTRED>
-__device__ __forceinline__ void a_frag_aligned(const uint32_t (&W)[2][BITS == 2 ? 2 : 4], int kappa, uint32_t (&a)[4]) {
+__device__ __forceinline__ void a_frag_aligned(const uint32_t (&W)[2][BITS == 2 ? 2 : 4], int kappa, uint32_t (&a)[4],
+                                               const uint32_t (&shl_mul)[3]) {
   static_assert(BITS == 2 || !CENTRED, "centred A fragments: 2-bit records");
   constexpr int NCLS = 8 / BITS;
   constexpr uint32_t MASK = BITS == 2 ? 0xC0C0C0C0u : 0xF0F0F0F0u;
   const int j = BITS == 2 ? kappa : (kappa & 1);
   const int w0 = BITS == 2 ? 0 : 2 * (kappa >> 1);
-  const uint32_t mul = 1u << (BITS * (NCLS - 1 - j));      // compile-time per call site: IMAD.SHL on the fma pipe
+  const int sh = BITS * (NCLS - 1 - j);      // compile-time per call site: 0, 2, 4 or 6
   auto f = [&](uint32_t w) -> uint32_t {
-    const uint32_t x = w * mul;
+    const uint32_t x = sh == 0 ? w : w * shl_mul[sh / 2 - 1];
     if constexpr (!CENTRED) return x & MASK;
     constexpr uint32_t M1 = 0xA0A0A0A0u, M2 = 0x60606060u;
     return (M1 & ~M2 & ~x) | (~M1 & M2 & x) | (M1 & M2);
@@ -640,7 +645,8 @@ __device__ __forceinline__ void a_frag_aligned(const uint32_t (&W)[2][BITS == 2 
   a[0] = f(W[0][w0]); a[1] = f(W[1][w0]); a[2] = f(W[0][w0 + 1]); a[3] = f(W[1][w0 + 1]);
 }
 template <int BITS, int NT, int NTB, bool B_SIGNED, bool ALIGNED, bool CENTRED = false>
-__device__ __forceinline__ void contract_mp(const uint8_t* codes, const uint4 (&bf)[2][NTB], int mp, int lane, int32_t (&d)[2][NT][4]) {
+__device__ __forceinline__ void contract_mp(const uint8_t* codes, const uint4 (&bf)[2][NTB], int mp, int lane, int32_t (&d)[2][NT][4],
+                                            const uint32_t (&shl_mul)[3]) {
   uint32_t W[2][2][BITS == 2 ? 2 : 4];
   load_row_words<BITS>(codes, mp, lane, 0, W[0]);
   load_row_words<BITS>(codes, mp, lane, 1, W[1]);
@@ -656,7 +662,7 @@ __device__ __forceinline__ void contract_mp(const uint8_t* codes, const uint4 (&
     for (int k1 = 0; k1 < 2; ++k1) {
       const int kappa = 2 * hk + k1;
       uint32_t a[2][4];
-      if constexpr (ALIGNED) { a_frag_aligned<BITS, CENTRED>(W[0], kappa, a[0]); a_frag_aligned<BITS, CENTRED>(W[1], kappa, a[1]); }
+      if constexpr (ALIGNED) { a_frag_aligned<BITS, CENTRED>(W[0], kappa, a[0], shl_mul); a_frag_aligned<BITS, CENTRED>(W[1], kappa, a[1], shl_mul); }
       else { a_frag<BITS>(W[0], kappa, a[0]); a_frag<BITS>(W[1], kappa, a[1]); }
 #pragma unroll
       for (int nu = 0; nu < NT; ++nu)
@@ -834,7 +840,7 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
 #pragma unroll
       for (int mp = 0; mp < 4; ++mp) {
         int32_t dd[2][NTQ][4];
-        contract_mp<BITS, NTQ, NTQ, true, DQ == 2, DQ == 2>(ws.krec, bf, mp, lane, dd);
+        contract_mp<BITS, NTQ, NTQ, true, DQ == 2, DQ == 2>(ws.krec, bf, mp, lane, dd, A.shl_mul);
 #pragma unroll
         for (int u = 0; u < HPW; ++u)
 #pragma unroll
@@ -942,7 +948,7 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
 #pragma unroll
       for (int mp = 0; mp < 4; ++mp) {
         int32_t dd[2][NTP][4];
-        contract_mp<BITS, NTP, NTP, false, DP == 2>(ws.vrec, bf, mp, lane, dd);
+        contract_mp<BITS, NTP, NTP, false, DP == 2>(ws.vrec, bf, mp, lane, dd, A.shl_mul);
         const uint2 sv = *reinterpret_cast<const uint2*>(&ws.aux_ch[mp][fg][0]);
         const float2 s01 = __half22float2(*reinterpret_cast<const __half2*>(&sv.x)), s23 = __half22float2(*reinterpret_cast<const __half2*>(&sv.y));
         const float s2v[4] = {s01.x, s01.y, s23.x, s23.y};
