@@ -286,6 +286,20 @@ KVARN_API int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* ca
                           float sm_scale, void* out, void* stream);
 
 /*
+ * kvarn_block_attention_dense -- the same operation and arguments as kvarn_block_attention, computed by a dense
+ * tensor-core kernel (tcgen05 + tensor memory): every chunk of the cache is expanded once into fp16 tiles
+ * (code x scale is exact in fp16) and the block's 128-row tiles of (query token, head) pairs run S = Q K^T and
+ * O += P V as M = 128 MMAs; the raw windows go through the decode kernel and the pieces are LSE-merged.  The right
+ * form for blocks with >= ~32 (token, head) rows per KV head (blocks of b tokens); kvarn_block_attention is the
+ * right one for a few speculative tokens.  ws: DEVICE scratch of >= kvarn_block_dense_workspace_bytes(...) bytes.
+ */
+KVARN_API size_t kvarn_block_dense_workspace_bytes(const kvarn_params* p, int32_t B, int32_t Hq, int32_t Hkv, int32_t n_q,
+                                         int32_t max_chunks);
+KVARN_API int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                                const void* k_blk, const void* v_blk, int32_t n_q, int32_t Hq,
+                                float sm_scale, void* out, void* ws, size_t ws_bytes, void* stream);
+
+/*
  * The Hadamard arrangement around the attention layer (App. A: "two absorbed transforms (that are
  * merged with W_V and W_O respectively ...) and two online transforms after the RoPE-embedding.  The two online
  * transforms are head-wise").  With these a model can produce q, K and V already rotated and run the cache with

@@ -6,6 +6,7 @@
 
 #include "kvarn_common.cuh"
 #include "kvarn_decode.cuh"
+#include "kvarn_block_dense.cuh"
 #include "kvarn_rotate.cuh"
 #include "kvarn_quantize.cuh"
 
@@ -574,6 +575,80 @@ int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* cache, const
   A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
   const cudaError_t e = launch_decode(p, A, (cudaStream_t)stream);
   return e == cudaSuccess ? KVARN_OK : KVARN_CUDA;
+}
+
+// Dense form of kvarn_block_attention for blocks with many query rows per KV head (tcgen05 + TMEM; kvarn_block_dense.cuh):
+// packed chunks by block_dense_kernel, raw windows by decode_kernel_w (skip_chunks), merged by merge_partials_kernel.
+static int dense_splits(int B, int Hkv, int n_tiles, int max_chunks) {
+  int sms = 148;
+  const int dev = current_device();
+  if (dev >= 0 && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); sms = 148; }
+  int s = sms / (B * Hkv * n_tiles);            // one CTA per SM (197 KB of shared memory, 512 TMEM columns)
+  if (s > max_chunks / 4) s = max_chunks / 4;   // at least 4 chunks per CTA
+  if (s > 32) s = 32;
+  return s < 1 ? 1 : s;
+}
+
+size_t kvarn_block_dense_workspace_bytes(const kvarn_params* p, int32_t B, int32_t Hq, int32_t Hkv, int32_t n_q,
+                                         int32_t max_chunks) {
+  if (!p || B <= 0 || Hq <= 0 || Hkv <= 0 || n_q <= 0 || (Hq % Hkv) != 0) return 0;
+  const int g = Hq / Hkv, n_tiles = (n_q * g + 127) / 128;
+  return (size_t)(dense_splits(B, Hkv, n_tiles, max_chunks) + 1) * B * n_q * Hq * PART_STRIDE * sizeof(float);
+}
+
+int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                                const void* k_blk, const void* v_blk, int32_t n_q, int32_t Hq,
+                                float sm_scale, void* out, void* ws, size_t ws_bytes, void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if ((st = check_cache(cache))) return st;
+  if (!q || !out || !k_blk || !v_blk || !ws || Hq <= 0 || (Hq % cache->Hkv) != 0 || n_q < 1) return KVARN_INVALID_ARG;
+  const int g = Hq / cache->Hkv;
+  if (g > 8 || (g & (g - 1)) || n_q > G) return KVARN_UNSUPPORTED;
+  if (!aligned16(q) || !aligned16(out) || !aligned16(k_blk) || !aligned16(v_blk) || !aligned16(ws)) return KVARN_MISALIGNED;
+  if (ws_bytes < kvarn_block_dense_workspace_bytes(p, cache->B, Hq, cache->Hkv, n_q, cache->max_chunks)) return KVARN_WORKSPACE_TOO_SMALL;
+  cudaStream_t s = (cudaStream_t)stream;
+  const bool f32 = p->in_dtype == KVARN_F32;
+  const long long n_rows = (long long)cache->B * n_q * Hq;
+  DenseArgs E{};
+  E.k_records = (const uint8_t*)cache->k_records; E.v_records = (const uint8_t*)cache->v_records; E.seq_lens = cache->seq_lens;
+  E.q = q; E.parts = (float*)ws;
+  E.B = cache->B; E.Hkv = cache->Hkv; E.Hq = Hq; E.g = g; E.max_chunks = cache->max_chunks; E.n_sink = cache->n_sink; E.n_q = n_q;
+  E.n_tiles = (n_q * g + 127) / 128;
+  E.splits = dense_splits(cache->B, cache->Hkv, E.n_tiles, cache->max_chunks);
+  E.q_scale = sm_scale * 1.4426950408889634f; E.rotate_k = p->rotate_k; E.rotate_v = p->rotate_v;
+  {
+    const dim3 grid((unsigned)(cache->B * cache->Hkv * E.n_tiles), (unsigned)E.splits);
+    cudaError_t e;
+    if (p->bits == 2) {
+      if (f32) { e = ensure_smem_optin<block_dense_kernel<2, float>>((int)sizeof(DenseSmem<2>), true);
+                 if (e == cudaSuccess) block_dense_kernel<2, float><<<grid, 128, sizeof(DenseSmem<2>), s>>>(E); }
+      else { e = ensure_smem_optin<block_dense_kernel<2, __nv_bfloat16>>((int)sizeof(DenseSmem<2>), true);
+             if (e == cudaSuccess) block_dense_kernel<2, __nv_bfloat16><<<grid, 128, sizeof(DenseSmem<2>), s>>>(E); }
+    } else {
+      if (f32) { e = ensure_smem_optin<block_dense_kernel<4, float>>((int)sizeof(DenseSmem<4>), true);
+                 if (e == cudaSuccess) block_dense_kernel<4, float><<<grid, 128, sizeof(DenseSmem<4>), s>>>(E); }
+      else { e = ensure_smem_optin<block_dense_kernel<4, __nv_bfloat16>>((int)sizeof(DenseSmem<4>), true);
+             if (e == cudaSuccess) block_dense_kernel<4, __nv_bfloat16><<<grid, 128, sizeof(DenseSmem<4>), s>>>(E); }
+    }
+    if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return KVARN_CUDA;
+  }
+  // raw windows (sink, residual, the block's own causal tokens): the decode kernel without its chunks, as one more partial
+  DecodeArgs A{};
+  A.k_records = E.k_records; A.v_records = E.v_records;
+  A.k_resid = cache->k_resid; A.v_resid = cache->v_resid; A.seq_lens = cache->seq_lens;
+  A.k_sink = cache->k_sink; A.v_sink = cache->v_sink; A.n_sink = cache->n_sink;
+  A.ticket = cache->decode_ticket;
+  A.q = q; A.out = (float*)ws + (size_t)E.splits * n_rows * PART_STRIDE; A.ws = nullptr;
+  A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;
+  A.n_q = n_q; A.k_blk = k_blk; A.v_blk = v_blk;
+  A.tpc = n_q * g <= 4 ? n_q : (8 / g < n_q ? 8 / g : n_q);
+  A.cluster = 1; A.nclus = 1; A.splits = 1;
+  A.q_scale = E.q_scale; A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = KVARN_F32;
+  A.partial = 1; A.skip_chunks = 1;
+  if (launch_decode(p, A, s) != cudaSuccess) return KVARN_CUDA;
+  merge_partials_kernel<<<(unsigned)n_rows, 128, 0, s>>>((const float*)ws, E.splits + 1, n_rows, out, p->out_dtype);
+  return last_cuda();
 }
 
 int kvarn_rope_hadamard(const void* x, const float* cos_tab, const float* sin_tab, void* y, int64_t n_tok,

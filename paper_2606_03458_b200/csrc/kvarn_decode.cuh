@@ -79,6 +79,8 @@ struct DecodeArgs {
   // multiply issues on the fma pipe, and only an operand ptxas cannot see through keeps it from becoming a shift
   // on the alu pipe (the busiest unit of the 2-bit kernel)
   uint32_t shl_mul[3];
+  // 1: leave the packed chunks to another kernel (block_dense_kernel) and run the raw windows only
+  int skip_chunks;
 };
 
 // ------------------------------------------------------------------ PTX wrappers
@@ -713,9 +715,10 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
   // (a raw window of n tokens keeps its CTA as long as ~n / 8 chunks do -- measured on the 64k-context cache with
   //  a 128-token sink and a 64-token residual window --, so the splits that own one get that many chunks fewer)
   const int w_sink = (w0.n_sink_tok + 7) / 8, w_res = (w0.resid + cm0.blk_cnt + 7) / 8;
-  const int per = (w0.n_chunks + w_sink + w_res + A.splits - 1) / A.splits;
-  const int c_begin = min(max(w0.split * per - w_sink, 0), w0.n_chunks);
-  const int c_end = min(max((w0.split + 1) * per - w_sink, 0), w0.n_chunks);
+  const int nch = A.skip_chunks ? 0 : w0.n_chunks;
+  const int per = (nch + w_sink + w_res + A.splits - 1) / A.splits;
+  const int c_begin = min(max(w0.split * per - w_sink, 0), nch);
+  const int c_end = min(max((w0.split + 1) * per - w_sink, 0), nch);
   const int n_mine = (c_end - c_begin - warp + 3) >> 2;            // chunks of this warp: c_begin + warp + 4 i
   const uint8_t* krec = A.k_records + ((size_t)w0.bh * A.max_chunks + c_begin + warp) * RB;
   const uint8_t* vrec = A.v_records + ((size_t)w0.bh * A.max_chunks + c_begin + warp) * RB;

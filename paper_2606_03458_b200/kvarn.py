@@ -71,6 +71,10 @@ EXPORTS = {
                                          C.c_float, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
     "kvarn_block_attention": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_void_p]),
+    "kvarn_block_dense_workspace_bytes": (C.c_size_t, [C.POINTER(Params), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32]),
+    "kvarn_block_attention_dense": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_void_p,
+                                              C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_void_p,
+                                              C.c_size_t, C.c_void_p]),
     "kvarn_rope_hadamard": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32,
                                       C.c_int32, C.c_int32, C.c_void_p]),
     "kvarn_hadamard_rows": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]),
@@ -331,7 +335,8 @@ def context_parallel_decode(p: Params, cache: Cache, q: torch.Tensor, group=None
 
 
 def block_attention(p: Params, cache: Cache, q: torch.Tensor, k_blk: torch.Tensor, v_blk: torch.Tensor,
-                    sm_scale: float | None = None, out: torch.Tensor | None = None, stream=None):
+                    sm_scale: float | None = None, out: torch.Tensor | None = None, stream=None,
+                    dense: bool = False, ws: torch.Tensor | None = None):
     """q: [B, n_q, Hq, 128]; k_blk, v_blk: [B, Hkv, n_q, 128] (the block's own raw tokens, not yet in
     the cache) -> out [B, n_q, Hq, 128]: causal attention over [cache ; block] (Fig. 4)."""
     assert q.is_cuda and q.is_contiguous() and q.shape[0] == cache.B and q.shape[3] == HEAD_DIM
@@ -345,6 +350,14 @@ def block_attention(p: Params, cache: Cache, q: torch.Tensor, k_blk: torch.Tenso
     if out is None:
         out = torch.empty((cache.B, n_q, Hq, HEAD_DIM), device=q.device,
                           dtype=torch.float32 if p.out_dtype == F32 else torch.bfloat16)
+    if dense:   # the tcgen05 form (kvarn_block_attention_dense): for blocks with many (token, head) rows per KV head
+        if ws is None:
+            need = int(lib.kvarn_block_dense_workspace_bytes(C.byref(p), cache.B, Hq, cache.Hkv, n_q, cache.max_chunks))
+            ws = torch.empty((max(need, 16),), dtype=torch.uint8, device=q.device)
+        st = lib.kvarn_block_attention_dense(C.byref(p), C.byref(cache.desc), _ptr(q), _ptr(k_blk), _ptr(v_blk), n_q, Hq,
+                                             sm_scale, _ptr(out), _ptr(ws), ws.numel(), _stream(stream))
+        _check(st, "kvarn_block_attention_dense")
+        return out
     st = lib.kvarn_block_attention(C.byref(p), C.byref(cache.desc), _ptr(q), _ptr(k_blk), _ptr(v_blk), n_q, Hq,
                                    sm_scale, _ptr(out), _stream(stream))
     _check(st, "kvarn_block_attention")

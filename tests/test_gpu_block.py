@@ -205,3 +205,30 @@ def test_pseudo_decode_step_and_capacity_guard(kv):
     with pytest.raises(kv.KvarnError, match="UNSUPPORTED"):
         kv.append_block(p, cache, torch.zeros((B, Hkv, 129, 128), dtype=torch.bfloat16, device="cuda"),
                         torch.zeros((B, Hkv, 129, 128), dtype=torch.bfloat16, device="cuda"))
+
+
+# ---------------------------------------------------------------- dense tcgen05 form (kvarn_block_attention_dense)
+@pytest.mark.parametrize("bits", [2, 4])
+@pytest.mark.parametrize("Hq,Hkv,n_q,n_tok,n_sink", [(32, 8, 128, 128 * 5 + 41, 0), (32, 8, 40, 128 * 9, 0), (64, 8, 16, 128 * 4 + 100, 0),
+                                                      (8, 8, 128, 128 * 3 + 7, 0), (32, 8, 33, 128 * 6 + 5, 32), (16, 8, 3, 128 * 2 + 1, 0),
+                                                      (32, 8, 8, 77, 0), (32, 8, 20, 0, 0)])
+def test_block_attention_dense_vs_oracle(kv, bits, Hq, Hkv, n_q, n_tok, n_sink):
+    # row tiles full and ragged (n_q g = 512, 160, 128, 128, 132, 6), several chunks per CTA, sink / residual / empty cache
+    K, V, kb, vb, q = _inputs(2, Hq, Hkv, n_tok, n_q, seed=160 + n_q)
+    p = kv.default_params(bits)
+    cache = _cache(kv, p, K, V, n_sink=n_sink)
+    out = kv.block_attention(p, cache, q, kb, vb, dense=True)
+    _check(kv, p, cache, q, kb, vb, out, n_tok, {(0, 0), (1, Hkv - 1)})
+    ref = kv.block_attention(p, cache, q, kb, vb)                      # the integer-MMA form
+    assert (out - ref).abs().max() <= P.ATTN_RTOL * ref.abs().max()
+    assert torch.equal(out, kv.block_attention(p, cache, q, kb, vb, dense=True))     # deterministic
+
+
+def test_block_attention_dense_long_context_and_splits(kv):
+    # one sequence, one KV head pair, 40 chunks: the chunk range is split over several CTAs whose partials are LSE-merged
+    n_tok, n_q = 128 * 40 + 9, 32
+    K, V, kb, vb, q = _inputs(1, 8, 2, n_tok, n_q, seed=171)
+    p = kv.default_params(2)
+    cache = _cache(kv, p, K, V)
+    out = kv.block_attention(p, cache, q, kb, vb, dense=True)
+    _check(kv, p, cache, q, kb, vb, out, n_tok)
