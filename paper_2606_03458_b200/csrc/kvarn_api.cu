@@ -622,14 +622,14 @@ int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache,
     cudaError_t e;
     if (p->bits == 2) {
       if (f32) { e = ensure_smem_optin<block_dense_kernel<2, float>>((int)sizeof(DenseSmem<2>), true);
-                 if (e == cudaSuccess) block_dense_kernel<2, float><<<grid, 128, sizeof(DenseSmem<2>), s>>>(E); }
+                 if (e == cudaSuccess) block_dense_kernel<2, float><<<grid, DENSE_THREADS, sizeof(DenseSmem<2>), s>>>(E); }
       else { e = ensure_smem_optin<block_dense_kernel<2, __nv_bfloat16>>((int)sizeof(DenseSmem<2>), true);
-             if (e == cudaSuccess) block_dense_kernel<2, __nv_bfloat16><<<grid, 128, sizeof(DenseSmem<2>), s>>>(E); }
+             if (e == cudaSuccess) block_dense_kernel<2, __nv_bfloat16><<<grid, DENSE_THREADS, sizeof(DenseSmem<2>), s>>>(E); }
     } else {
       if (f32) { e = ensure_smem_optin<block_dense_kernel<4, float>>((int)sizeof(DenseSmem<4>), true);
-                 if (e == cudaSuccess) block_dense_kernel<4, float><<<grid, 128, sizeof(DenseSmem<4>), s>>>(E); }
+                 if (e == cudaSuccess) block_dense_kernel<4, float><<<grid, DENSE_THREADS, sizeof(DenseSmem<4>), s>>>(E); }
       else { e = ensure_smem_optin<block_dense_kernel<4, __nv_bfloat16>>((int)sizeof(DenseSmem<4>), true);
-             if (e == cudaSuccess) block_dense_kernel<4, __nv_bfloat16><<<grid, 128, sizeof(DenseSmem<4>), s>>>(E); }
+             if (e == cudaSuccess) block_dense_kernel<4, __nv_bfloat16><<<grid, DENSE_THREADS, sizeof(DenseSmem<4>), s>>>(E); }
     }
     if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return KVARN_CUDA;
   }

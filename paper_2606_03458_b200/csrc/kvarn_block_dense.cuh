@@ -3,7 +3,10 @@
 // for blocks with many (query token, head) rows per KV head; the raw windows (sink, residual, the block's own causal
 // tokens) are left to decode_kernel_w (skip_chunks = 1, partial = 1) and everything is merged by merge_partials_kernel.
 //
-// One CTA = one (sequence, KV head), one tile of 128 query rows r = (token i, head h), one range of chunks.  Per chunk:
+// One CTA = one (sequence, KV head), one tile of 128 query rows r = (token i, head h), one range of chunks; 9 warps in
+// three roles that meet only through mbarriers: warps 4-7 expand the records (producers), one thread of warp 8 issues
+// the MMAs, warps 0-3 own the softmax (thread = query row = TMEM lane).  While the softmax warps work on chunk i the
+// producers already expand V of chunk i and K of chunk i + 1 and the tensor core runs QK^T of chunk i + 1.  Per chunk:
 //   K record --TMA--> shared memory --128 threads--> Kt = code x s1[c] as fp16 (EXACT: a 2-/4-bit code times an E4M3
 //     scale has <= 8 significant bits), K-major UMMA tile [token][channel], + two rows hi / lo of (s1 z)[c] for beta
 //   S[r][t] = sum_c (q'_hi + q'_lo)[r][c] Kt[t][c]          tcgen05.mma kind::f16, M = 128, N = 144, K = 128, twice (hi, lo)
@@ -94,10 +97,13 @@ struct DenseSmem {
   alignas(1024) uint8_t pt[128 * DN_KP * 2];       // rows: query rows; columns 0..127 p~ (rho order), 128, 129: hi / lo of zsum
   alignas(128) uint8_t rec[2][2][RB];              // [stage][K | V]
   alignas(16) __half2 s1h[64];                     // s1 of the K record as fp16 pairs in K-position order
-  alignas(16) float2 aux_a[128];                   // per token (rho order): {s2, log2 s1v}
-  alignas(16) float2 aux_b[128];                   //                        {1 / s1v, zv}
+  alignas(16) float2 aux_a[2][128];                // [chunk parity] per token (rho order): {s2, log2 s1v}
+  alignas(16) float2 aux_b[2][128];                //                                       {1 / s1v, zv}
+  alignas(16) float2 ml[128];                      // epilogue: {m, l} of the rows
   alignas(8) uint64_t full[2][2];                  // TMA arrival [stage][K | V]
-  alignas(8) uint64_t bar_s, bar_o;                // MMA completion: S ready, O accumulated
+  alignas(8) uint64_t bar_s, bar_o;                // MMA completion (tcgen05.commit): S ready, O accumulated
+  alignas(8) uint64_t kt_full, aux_full, vt_full;  // producers -> issuer / softmax warps (128 arrivals each)
+  alignas(8) uint64_t s_free, p_full;              // softmax warps -> issuer (128 arrivals each)
   uint32_t tmem_base;
 };
 
@@ -142,8 +148,15 @@ __device__ __forceinline__ void dequant_row(const uint32_t (&W)[4 * BITS], const
   }
 }
 
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void producer_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+
+constexpr int DENSE_THREADS = 288;
+
 template <int BITS, typename InT>
-__global__ void __launch_bounds__(128, 1) block_dense_kernel(const DenseArgs A) {
+__global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const DenseArgs A) {
   using SM = DenseSmem<BITS>;
   constexpr int RB = SM::RB;
   constexpr uint32_t TMEM_COLS = 512;           // S: columns [0, 144), O: columns [256, 384)
@@ -165,9 +178,11 @@ __global__ void __launch_bounds__(128, 1) block_dense_kernel(const DenseArgs A) 
   const uint8_t* vrec = A.v_records + ((size_t)unit * A.max_chunks + c_begin) * RB;
 
   // ---- setup: barriers, TMEM, first records, q ------------------------------------------------------------------
-  if (tid == 0) {
+  if (tid == 128) {
     for (int s = 0; s < 2; ++s) { mbar_init(&sm.full[s][0], 1); mbar_init(&sm.full[s][1], 1); }
     mbar_init(&sm.bar_s, 1); mbar_init(&sm.bar_o, 1);
+    mbar_init(&sm.kt_full, 128); mbar_init(&sm.aux_full, 128); mbar_init(&sm.vt_full, 128);
+    mbar_init(&sm.s_free, 128); mbar_init(&sm.p_full, 128);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     if (n_my > 0) {
       mbar_expect_tx(&sm.full[0][0], RB); bulk_g2s(sm.rec[0][0], krec, RB, &sm.full[0][0]);
@@ -179,11 +194,11 @@ __global__ void __launch_bounds__(128, 1) block_dense_kernel(const DenseArgs A) 
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   // zero the tiles once: rows / columns that are never rewritten (padding of N = 144 and K = 144) stay zero
-  for (int i = tid; i < (int)(sizeof(sm.kt) / 16); i += 128) reinterpret_cast<uint4*>(sm.kt)[i] = make_uint4(0, 0, 0, 0);
-  for (int i = tid; i < (int)(sizeof(sm.vt) / 16); i += 128) reinterpret_cast<uint4*>(sm.vt)[i] = make_uint4(0, 0, 0, 0);
-  for (int i = tid; i < (int)(sizeof(sm.pt) / 16); i += 128) reinterpret_cast<uint4*>(sm.pt)[i] = make_uint4(0, 0, 0, 0);
+  for (int i = tid; i < (int)(sizeof(sm.kt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.kt)[i] = make_uint4(0, 0, 0, 0);
+  for (int i = tid; i < (int)(sizeof(sm.vt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.vt)[i] = make_uint4(0, 0, 0, 0);
+  for (int i = tid; i < (int)(sizeof(sm.pt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.pt)[i] = make_uint4(0, 0, 0, 0);
   // q' = (q H / sqrt(128)) q_scale as two fp16 terms, columns in K-position order
-  for (int r = warp; r < 128; r += 4) {
+  for (int r = warp; r < 128; r += DENSE_THREADS / 32) {
     const int R = rt * 128 + r;
     float v[4] = {0.f, 0.f, 0.f, 0.f};
     if (R < n_rows) {
@@ -207,169 +222,194 @@ __global__ void __launch_bounds__(128, 1) block_dense_kernel(const DenseArgs A) 
       *reinterpret_cast<__half*>(sm.qlo + kmaj_off(r, kp, DN_KT)) = lo;
     }
   }
+  fence_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
-  const uint32_t t_row = tmem + ((uint32_t)(warp * 32) << 16);      // this warp's 32 TMEM lanes (lane = query row)
   constexpr uint32_t IDESC_S = umma_idesc_f16(128, DN_NS), IDESC_O = umma_idesc_f16(128, 128);
   constexpr uint32_t SBO_T = (DN_KT / 8) * 128, SBO_P = (DN_KP / 8) * 128;
-
-  // this thread's token (K rows, per-token aux) and channel (V rows)
-  const int tau = tid, rho_t = dense_kpos<BITS>(tau), slot_t = slot_of_token(BITS, tau);
-  float m_ref = -INFINITY, l_run = 0.f;         // reference exponent of the row (log2 units), running l
   constexpr float P_OFF = 8.f;                  // p~ = 2^(logit - max + 8): probabilities down to 2^-32 of the maximum survive fp16
+  float m_ref = -INFINITY, l_run = 0.f;         // softmax warps: reference exponent of the row (log2 units), running l
 
-  for (int it = 0; it < n_my; ++it) {
-    const int st = it & 1;
-    const uint32_t par_rec = (it >> 1) & 1, par_mma = it & 1;
-    if (tid == 0 && it + 1 < n_my) {            // next chunk's records into the other stage (its readers finished last iteration)
-      mbar_expect_tx(&sm.full[st ^ 1][0], RB); bulk_g2s(sm.rec[st ^ 1][0], krec + (size_t)(it + 1) * RB, RB, &sm.full[st ^ 1][0]);
-      mbar_expect_tx(&sm.full[st ^ 1][1], RB); bulk_g2s(sm.rec[st ^ 1][1], vrec + (size_t)(it + 1) * RB, RB, &sm.full[st ^ 1][1]);
+  if (warp >= 4 && warp < 8) {
+    // =============================== producers: thread = token (K rows, per-token aux) = channel (V rows) ==========
+    const int pt = tid - 128;
+    const int rho_t = dense_kpos<BITS>(pt), slot_t = slot_of_token(BITS, pt);
+    for (int it = 0; it < n_my; ++it) {
+      const int st = it & 1;
+      const uint32_t par_rec = (it >> 1) & 1, par_prev = (it & 1) ^ 1;
+      if (pt == 0 && it + 1 < n_my) {          // next chunk's records into the other stage (all producers left it: producer_sync below)
+        mbar_expect_tx(&sm.full[st ^ 1][0], RB); bulk_g2s(sm.rec[st ^ 1][0], krec + (size_t)(it + 1) * RB, RB, &sm.full[st ^ 1][0]);
+        mbar_expect_tx(&sm.full[st ^ 1][1], RB); bulk_g2s(sm.rec[st ^ 1][1], vrec + (size_t)(it + 1) * RB, RB, &sm.full[st ^ 1][1]);
+      }
+      mbar_wait(&sm.full[st][0], par_rec);
+      mbar_wait(&sm.full[st][1], par_rec);
+      const uint8_t* kr = sm.rec[st][0];
+      const uint8_t* vr = sm.rec[st][1];
+      if (it > 0) mbar_wait(&sm.bar_s, par_prev);       // QK^T of the previous chunk has consumed Kt
+      {
+        // thread = K position pt: channel c, s1 and z in the record's builder order
+        const int c = dense_elem_of_kpos<BITS>(pt), ka = kaux_of_elem(BITS, c);
+        const float s1 = e4m3_to_f32(kr[s1_off(BITS) + ka]);
+        const float z = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(kr + z_off(BITS))[ka]);
+        reinterpret_cast<__half*>(sm.s1h)[pt] = __float2half_rn(s1);                    // exact
+        const float sz = s1 * z;
+        const __half hi = __float2half_rn(sz), lo = __float2half_rn(sz - __half2float(hi));
+        *reinterpret_cast<__half*>(sm.kt + kmaj_off(128, pt, DN_KT)) = hi;
+        *reinterpret_cast<__half*>(sm.kt + kmaj_off(129, pt, DN_KT)) = lo;
+        // per-token aux of both records (parity-buffered: the softmax warps may still read the previous chunk's)
+        const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + slot_t]), 9.094947e-13f);
+        const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[slot_t]);
+        sm.aux_a[st][rho_t] = make_float2(e4m3_to_f32(kr[s2_off(BITS) + slot_t]), lg2_approx(s1v));
+        sm.aux_b[st][rho_t] = make_float2(rcp_approx(s1v), zv);
+      }
+      // (phase discipline: no barrier may complete a second time before every waiter of its previous phase has
+      //  looked -- the softmax warps pass their aux_full wait before they arrive on s_free)
+      if (it > 0) mbar_wait(&sm.s_free, par_prev);
+      mbar_arrive(&sm.aux_full);
+      producer_sync();                                   // s1h complete
+      {
+        uint32_t W[4 * BITS];
+        load_row_all<BITS>(kr, slot_t, W);
+        dequant_row<BITS, true>(W, sm.s1h, __half2(), sm.kt, rho_t, DN_KT);
+      }
+      fence_async_smem();
+      mbar_arrive(&sm.kt_full);
+      if (it > 0) mbar_wait(&sm.bar_o, par_prev);       // PV of the previous chunk has consumed Vt
+      {
+        const float s2v = e4m3_to_f32(vr[s2_off(BITS) + pt]);                            // thread = channel pt
+        const __half2 sc = __float2half2_rn(s2v);
+        uint32_t W[4 * BITS];
+        load_row_all<BITS>(vr, pt, W);
+        dequant_row<BITS, false>(W, nullptr, sc, sm.vt, pt, DN_KP);
+        *reinterpret_cast<__half2*>(sm.vt + kmaj_off(pt, 128, DN_KP)) = sc;               // K columns 128, 129: s2v (zero-point term)
+      }
+      fence_async_smem();
+      mbar_arrive(&sm.vt_full);
+      producer_sync();                                   // every producer has left rec[st] and s1h
     }
-    // ---- K: scale table, beta rows, per-token s2; then the tile ---------------------------------------------------
-    mbar_wait(&sm.full[st][0], par_rec);
-    const uint8_t* kr = sm.rec[st][0];
-    {
-      // thread = K position tid: channel c, s1 and z in the record's builder order
-      const int c = dense_elem_of_kpos<BITS>(tid), ka = kaux_of_elem(BITS, c);
-      const float s1 = e4m3_to_f32(kr[s1_off(BITS) + ka]);
-      const float z = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(kr + z_off(BITS))[ka]);
-      reinterpret_cast<__half*>(sm.s1h)[tid] = __float2half_rn(s1);                    // exact
-      const float sz = s1 * z;
-      const __half hi = __float2half_rn(sz), lo = __float2half_rn(sz - __half2float(hi));
-      *reinterpret_cast<__half*>(sm.kt + kmaj_off(128, tid, DN_KT)) = hi;
-      *reinterpret_cast<__half*>(sm.kt + kmaj_off(129, tid, DN_KT)) = lo;
-      sm.aux_a[rho_t].x = e4m3_to_f32(kr[s2_off(BITS) + slot_t]);
-    }
-    __syncthreads();
-    {
-      uint32_t W[4 * BITS];
-      load_row_all<BITS>(kr, slot_t, W);
-      dequant_row<BITS, true>(W, sm.s1h, __half2(), sm.kt, rho_t, DN_KT);
-    }
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    if (tid == 0) {
-      tc_fence_after();
+  } else if (warp == 8) {
+    // =============================== MMA issuer: one thread =========================================================
+    if (lane == 0) {
+      for (int it = 0; it < n_my; ++it) {
+        const uint32_t par = it & 1;
+        mbar_wait(&sm.kt_full, par);
+        if (it > 0) mbar_wait(&sm.s_free, par ^ 1);     // the softmax warps have read S of the previous chunk
+        tc_fence_after();
 #pragma unroll
-      for (int term = 0; term < 2; ++term)
+        for (int term = 0; term < 2; ++term)
 #pragma unroll
-        for (int ks = 0; ks < DN_KT / 16; ++ks)
-          umma_f16(tmem, umma_desc(smem_u32(term ? sm.qlo : sm.qhi) + ks * 256, 128, SBO_T),
-                   umma_desc(smem_u32(sm.kt) + ks * 256, 128, SBO_T), IDESC_S, (term | ks) != 0);
-      umma_commit(&sm.bar_s);
-    }
-    // ---- V: per-token aux, then the tile (after the previous chunk's PV MMA has released Vt / Pt) -------------------
-    if (it > 0) mbar_wait(&sm.bar_o, par_mma ^ 1);
-    tc_fence_after();
-    mbar_wait(&sm.full[st][1], par_rec);
-    const uint8_t* vr = sm.rec[st][1];
-    {
-      const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + slot_t]), 9.094947e-13f);
-      const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[slot_t]);
-      sm.aux_a[rho_t].y = lg2_approx(s1v);
-      sm.aux_b[rho_t] = make_float2(rcp_approx(s1v), zv);
-      const float s2v = e4m3_to_f32(vr[s2_off(BITS) + tid]);                             // thread = channel tid
-      const __half2 sc = __float2half2_rn(s2v);
-      uint32_t W[4 * BITS];
-      load_row_all<BITS>(vr, tid, W);
-      dequant_row<BITS, false>(W, nullptr, sc, sm.vt, tid, DN_KP);
-      *reinterpret_cast<__half2*>(sm.vt + kmaj_off(tid, 128, DN_KP)) = sc;                // K columns 128, 129: s2v (zero-point term)
-    }
-    __syncthreads();
-    // ---- softmax of row tid over the chunk's 128 tokens --------------------------------------------------------
-    mbar_wait(&sm.bar_s, par_mma);
-    tc_fence_after();
-    float beta;
-    {
-      uint32_t v[16];
-      tmem_ld16(t_row + 128, v);
-      beta = __uint_as_float(v[0]) + __uint_as_float(v[1]);
-    }
-    float mx = -INFINITY;
-#pragma unroll 1
-    for (int c0 = 0; c0 < 128; c0 += 16) {
-      uint32_t v[16];
-      tmem_ld16(t_row + c0, v);
+          for (int ks = 0; ks < DN_KT / 16; ++ks)
+            umma_f16(tmem, umma_desc(smem_u32(term ? sm.qlo : sm.qhi) + ks * 256, 128, SBO_T),
+                     umma_desc(smem_u32(sm.kt) + ks * 256, 128, SBO_T), IDESC_S, (term | ks) != 0);
+        umma_commit(&sm.bar_s);
+        mbar_wait(&sm.vt_full, par);
+        mbar_wait(&sm.p_full, par);
+        tc_fence_after();
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const float2 a = sm.aux_a[c0 + j];
-        mx = fmaxf(mx, fmaf(a.x, __uint_as_float(v[j]) + beta, a.y));
+        for (int ks = 0; ks < DN_KP / 16; ++ks)
+          umma_f16(tmem + O_COL, umma_desc(smem_u32(sm.pt) + ks * 256, 128, SBO_P), umma_desc(smem_u32(sm.vt) + ks * 256, 128, SBO_P),
+                   IDESC_O, (it | ks) != 0);
+        umma_commit(&sm.bar_o);
       }
     }
-    const float m_new = fmaxf(m_ref, mx - P_OFF);
-    const float f_old = ex2_approx(m_ref - m_new);          // 0 for the first chunk (m_ref = -inf)
-    if (__any_sync(0xffffffffu, m_new > m_ref) && it > 0) {  // some row of the warp rises: rescale the accumulator rows in TMEM
+  } else {
+    // =============================== softmax warps: thread = query row = TMEM lane =================================
+    const uint32_t t_row = tmem + ((uint32_t)(warp * 32) << 16);
+    uint8_t* prow = sm.pt + (tid >> 3) * SBO_P + (tid & 7) * 16;
+    for (int it = 0; it < n_my; ++it) {
+      const int st = it & 1;
+      const uint32_t par = it & 1;
+      mbar_wait(&sm.bar_s, par);
+      mbar_wait(&sm.aux_full, par);
+      tc_fence_after();
+      float v[128];
+      float beta;
+      {
+        uint32_t u[16];
+        tmem_ld16(t_row + 128, u);
+        beta = __uint_as_float(u[0]) + __uint_as_float(u[1]);
+#pragma unroll
+        for (int c0 = 0; c0 < 128; c0 += 16) {
+          tmem_ld16(t_row + c0, u);
+#pragma unroll
+          for (int j = 0; j < 16; ++j) v[c0 + j] = __uint_as_float(u[j]);
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(&sm.s_free);                           // S is in registers: the next QK^T may overwrite it
+      float mx = -INFINITY;
+#pragma unroll
+      for (int j = 0; j < 128; ++j) {
+        const float2 a = sm.aux_a[st][j];
+        v[j] = fmaf(a.x, v[j] + beta, a.y);
+        mx = fmaxf(mx, v[j]);
+      }
+      const float m_new = fmaxf(m_ref, mx - P_OFF);
+      const float f_old = ex2_approx(m_ref - m_new);     // 0 for the first chunk (m_ref = -inf)
+      if (it > 0) {
+        mbar_wait(&sm.bar_o, par ^ 1);                   // PV of the previous chunk is complete: Pt is free, O is consistent
+        tc_fence_after();
+        if (__any_sync(0xffffffffu, m_new > m_ref)) {    // some row of the warp rises: rescale the accumulator rows in TMEM
+#pragma unroll 1
+          for (int c0 = 0; c0 < 128; c0 += 16) {
+            uint32_t u[16];
+            tmem_ld16(t_row + O_COL + c0, u);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) u[j] = __float_as_uint(__uint_as_float(u[j]) * f_old);
+            tmem_st16(t_row + O_COL + c0, u);
+          }
+          asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        }
+      }
+      m_ref = m_new;
+      float lsum = 0.f, zsum = 0.f;
+#pragma unroll
+      for (int c0 = 0; c0 < 128; c0 += 8) {
+        uint32_t o[4];
+#pragma unroll
+        for (int j = 0; j < 8; j += 2) {
+          const float2 b0 = sm.aux_b[st][c0 + j], b1 = sm.aux_b[st][c0 + j + 1];
+          const float p0 = ex2_approx(v[c0 + j] - m_new), p1 = ex2_approx(v[c0 + j + 1] - m_new);
+          const __half2 ph = __floats2half2_rn(p0, p1);
+          const float2 pf = __half22float2(ph);                 // the rounded values: numerator and denominator agree
+          lsum = fmaf(pf.x, b0.x, fmaf(pf.y, b1.x, lsum));
+          zsum = fmaf(pf.x, b0.y, fmaf(pf.y, b1.y, zsum));
+          o[j >> 1] = *reinterpret_cast<const uint32_t*>(&ph);
+        }
+        *reinterpret_cast<uint4*>(prow + (c0 >> 3) * 128) = make_uint4(o[0], o[1], o[2], o[3]);
+      }
+      l_run = fmaf(l_run, f_old, lsum);
+      {
+        const __half zh = __float2half_rn(zsum), zl = __float2half_rn(zsum - __half2float(zh));
+        *reinterpret_cast<__half2*>(prow + 16 * 128) = __halves2half2(zh, zl);             // K columns 128, 129
+      }
+      fence_async_smem();
+      tc_fence_before();
+      mbar_arrive(&sm.p_full);
+    }
+    // ---- O rows -> shared memory (the q tiles are dead: every QK^T has completed) -------------------------------
+    float* stage = reinterpret_cast<float*>(sm.qhi);     // [128][128] fp32 = qhi + qlo
+    if (n_my > 0) {
+      mbar_wait(&sm.bar_o, (n_my - 1) & 1);
+      tc_fence_after();
 #pragma unroll 1
       for (int c0 = 0; c0 < 128; c0 += 16) {
-        uint32_t v[16];
-        tmem_ld16(t_row + O_COL + c0, v);
+        uint32_t u[16];
+        tmem_ld16(t_row + O_COL + c0, u);
 #pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) * f_old);
-        tmem_st16(t_row + O_COL + c0, v);
+        for (int j = 0; j < 16; j += 4)
+          *reinterpret_cast<uint4*>(&stage[tid * 128 + ((c0 + j) ^ ((tid & 7) << 2))]) = make_uint4(u[j], u[j + 1], u[j + 2], u[j + 3]);
       }
-      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
-    m_ref = m_new;
-    float lsum = 0.f, zsum = 0.f;
-    uint8_t* prow = sm.pt + (tid >> 3) * SBO_P + (tid & 7) * 16;
-#pragma unroll 1
-    for (int c0 = 0; c0 < 128; c0 += 16) {
-      uint32_t v[16], o[8];
-      tmem_ld16(t_row + c0, v);
-#pragma unroll
-      for (int j = 0; j < 16; j += 2) {
-        const float2 a0 = sm.aux_a[c0 + j], a1 = sm.aux_a[c0 + j + 1];
-        const float2 b0 = sm.aux_b[c0 + j], b1 = sm.aux_b[c0 + j + 1];
-        const float p0 = ex2_approx(fmaf(a0.x, __uint_as_float(v[j]) + beta, a0.y) - m_new);
-        const float p1 = ex2_approx(fmaf(a1.x, __uint_as_float(v[j + 1]) + beta, a1.y) - m_new);
-        const __half2 ph = __floats2half2_rn(p0, p1);
-        const float2 pf = __half22float2(ph);                 // the rounded values: numerator and denominator agree
-        lsum = fmaf(pf.x, b0.x, fmaf(pf.y, b1.x, lsum));
-        zsum = fmaf(pf.x, b0.y, fmaf(pf.y, b1.y, zsum));
-        o[j >> 1] = *reinterpret_cast<const uint32_t*>(&ph);
-      }
-      *reinterpret_cast<uint4*>(prow + (c0 >> 3) * 128) = make_uint4(o[0], o[1], o[2], o[3]);
-      *reinterpret_cast<uint4*>(prow + ((c0 >> 3) + 1) * 128) = make_uint4(o[4], o[5], o[6], o[7]);
-    }
-    l_run = fmaf(l_run, f_old, lsum);
-    {
-      const __half zh = __float2half_rn(zsum), zl = __float2half_rn(zsum - __half2float(zh));
-      *reinterpret_cast<__half2*>(prow + 16 * 128) = __halves2half2(zh, zl);             // K columns 128, 129
-    }
-    fence_async_smem();
+    sm.ml[tid] = make_float2(m_ref, l_run);
     tc_fence_before();
-    __syncthreads();
-    if (tid == 0) {
-      tc_fence_after();
-#pragma unroll
-      for (int ks = 0; ks < DN_KP / 16; ++ks)
-        umma_f16(tmem + O_COL, umma_desc(smem_u32(sm.pt) + ks * 256, 128, SBO_P), umma_desc(smem_u32(sm.vt) + ks * 256, 128, SBO_P),
-                 IDESC_O, (it | ks) != 0);
-      umma_commit(&sm.bar_o);
-    }
   }
-
-  // ---- epilogue: O rows -> shared memory, inverse Hadamard, partial {m, l, o[128]} per query row ------------------
-  float* stage = reinterpret_cast<float*>(sm.qhi);     // [128][128] fp32 = qhi + qlo (both dead)
-  if (n_my > 0) {
-    mbar_wait(&sm.bar_o, (n_my - 1) & 1);
-    tc_fence_after();
-#pragma unroll 1
-    for (int c0 = 0; c0 < 128; c0 += 16) {
-      uint32_t v[16];
-      tmem_ld16(t_row + O_COL + c0, v);
-#pragma unroll
-      for (int j = 0; j < 16; j += 4)
-        *reinterpret_cast<uint4*>(&stage[tid * 128 + ((c0 + j) ^ ((tid & 7) << 2))]) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
-    }
-  }
-  reinterpret_cast<float2*>(sm.aux_a)[tid] = make_float2(m_ref, l_run);
-  tc_fence_before();
   __syncthreads();
-  for (int r = warp; r < 128; r += 4) {
+  // ---- epilogue (all warps): inverse Hadamard, partial {m, l, o[128]} per query row -------------------------------
+  const float* stage = reinterpret_cast<const float*>(sm.qhi);
+  for (int r = warp; r < 128; r += DENSE_THREADS / 32) {
     const int R = rt * 128 + r;
     if (R >= n_rows) break;
     const int i = R / g, h = R - i * g;
@@ -387,7 +427,7 @@ __global__ void __launch_bounds__(128, 1) block_dense_kernel(const DenseArgs A) 
     }
     *reinterpret_cast<float4*>(prow + 4 + 4 * lane) = make_float4(v[0], v[1], v[2], v[3]);
     if (lane == 0) {
-      const float2 ml = reinterpret_cast<const float2*>(sm.aux_a)[r];
+      const float2 ml = sm.ml[r];
       *reinterpret_cast<float4*>(prow) = make_float4(n_my > 0 ? ml.x : -INFINITY, n_my > 0 ? ml.y : 0.f, 0.f, 0.f);
     }
   }
