@@ -593,7 +593,7 @@ size_t kvarn_block_dense_workspace_bytes(const kvarn_params* p, int32_t B, int32
                                          int32_t max_chunks) {
   if (!p || B <= 0 || Hq <= 0 || Hkv <= 0 || n_q <= 0 || (Hq % Hkv) != 0) return 0;
   const int g = Hq / Hkv, n_tiles = (n_q * g + 127) / 128;
-  return (size_t)(dense_splits(B, Hkv, n_tiles, max_chunks) + 1) * B * n_q * Hq * PART_STRIDE * sizeof(float);
+  return (size_t)(DENSE_SETS * dense_splits(B, Hkv, n_tiles, max_chunks) + 1) * B * n_q * Hq * PART_STRIDE * sizeof(float);
 }
 
 int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache, const void* q,
@@ -639,7 +639,7 @@ int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache,
   A.k_resid = cache->k_resid; A.v_resid = cache->v_resid; A.seq_lens = cache->seq_lens;
   A.k_sink = cache->k_sink; A.v_sink = cache->v_sink; A.n_sink = cache->n_sink;
   A.ticket = cache->decode_ticket;
-  A.q = q; A.out = (float*)ws + (size_t)E.splits * n_rows * PART_STRIDE; A.ws = nullptr;
+  A.q = q; A.out = (float*)ws + (size_t)(DENSE_SETS * E.splits) * n_rows * PART_STRIDE; A.ws = nullptr;
   A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;
   A.n_q = n_q; A.k_blk = k_blk; A.v_blk = v_blk;
   A.tpc = n_q * g <= 4 ? n_q : (8 / g < n_q ? 8 / g : n_q);
@@ -647,7 +647,7 @@ int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache,
   A.q_scale = E.q_scale; A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = KVARN_F32;
   A.partial = 1; A.skip_chunks = 1;
   if (launch_decode(p, A, s) != cudaSuccess) return KVARN_CUDA;
-  merge_partials_kernel<<<(unsigned)n_rows, 128, 0, s>>>((const float*)ws, E.splits + 1, n_rows, out, p->out_dtype);
+  merge_partials_kernel<<<(unsigned)n_rows, 128, 0, s>>>((const float*)ws, DENSE_SETS * E.splits + 1, n_rows, out, p->out_dtype);
   return last_cuda();
 }
 
