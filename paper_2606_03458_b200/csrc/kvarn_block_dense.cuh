@@ -88,19 +88,47 @@ template <int BITS> __host__ __device__ constexpr int dense_elem_of_kpos(int kp)
   return (kp / CPW) * CPW + ((kp % CPW) >> 1) + (kp & 1) * (CPW / 2);
 }
 
+// Kt and Vt are written by the producers with 16-byte stores from lanes that hold different 8-column units of
+// different rows.  Their core matrices are therefore spread with LBO = 144 B (K direction) and an odd number of
+// 16-byte groups per 8 rows (SBO): with the lane assignment of ProducerLane every quarter warp then stores to eight
+// different bank groups, and its record loads are one contiguous 128 B line per warp (no bank conflict on either side).
+constexpr int DN_LBO = 144;
+constexpr int DN_SBO_K = (16 * 9 + 1) * 16;      // 2320 B per 8 rows of Kt (16 units of 144 B + 16 B)
+constexpr int DN_SBO_V = (18 * 9 + 1) * 16;      // 2608 B per 8 rows of Vt (18 units + 16 B)
+__host__ __device__ constexpr int tile_off(int r, int k, int SBO) {
+  return (r >> 3) * SBO + (k >> 3) * DN_LBO + (r & 7) * 16 + (k & 7) * 2;
+}
+
+// inverse of slot_of_token
+__host__ __device__ constexpr int token_of_slot(int bits, int s) {
+  return bits == 2 ? (((s >> 5) & 3) | (((s >> 3) & 1) << 2) | (((s >> 4) & 1) << 3) | ((s & 3) << 4) | (((s >> 2) & 1) << 6))
+                   : (((s >> 5) & 1) | (((s >> 3) & 1) << 1) | (((s >> 4) & 1) << 2) | ((s & 3) << 3) | (((s >> 2) & 1) << 5) |
+                      (((s >> 6) & 1) << 6));
+}
+constexpr bool token_slot_roundtrip(int bits) {
+  for (int t = 0; t < 128; ++t)
+    if (token_of_slot(bits, slot_of_token(bits, t)) != t) return false;
+  return true;
+}
+static_assert(token_slot_roundtrip(2) && token_slot_roundtrip(4), "token_of_slot must invert slot_of_token");
+
 template <int BITS>
 struct DenseSmem {
   static constexpr int RB = record_bytes(BITS);
   alignas(1024) uint8_t qhi[128 * DN_KT * 2];      // q' (rotated, scaled), first fp16 term; later: staging of O (with qlo)
   alignas(1024) uint8_t qlo[128 * DN_KT * 2];      // second fp16 term
-  alignas(1024) uint8_t kt[DN_NS * DN_KT * 2];     // rows 0..127: token rho(t); 128, 129: hi / lo of s1 z; 130..143: zero
-  alignas(1024) uint8_t vt[128 * DN_KP * 2];       // rows: channels; columns 0..127 tokens (rho order), 128, 129: s2v, rest zero
+  alignas(1024) uint8_t kt[18 * DN_SBO_K];         // rows 0..127: token rho(t); 128, 129: hi / lo of s1 z; 130..143: zero
+  alignas(1024) uint8_t vt[16 * DN_SBO_V];         // rows: channels; columns 0..127 tokens (rho order), 128, 129: s2v, rest zero
   alignas(1024) uint8_t pt[2][128 * DN_KPH * 2];   // [token half] rows: query rows; columns 0..63 p~, 64, 65: hi / lo of zsum
   alignas(128) uint8_t rec_k[2][RB];               // [chunk parity]
   alignas(128) uint8_t rec_v[2][RB];
   alignas(16) __half2 s1h[64];                     // s1 of the K record as fp16 pairs in K-position order
-  alignas(16) float2 aux_a[2][128];                // [chunk parity] per token (rho order): {s2, log2 s1v}
-  alignas(16) float2 aux_b[2][128];                //                                       {1 / s1v, zv}
+  alignas(16) __half2 s1n[64];                     // the addends -dq_bias s1 of the same pairs
+  alignas(16) __half2 fh[2][64];                   // [chunk parity] f_t = s1v[t] 2^-E of the V record, pairs in K-position order
+  alignas(16) float2 aux_s2[2][64];                // [chunk parity] per token pair (rho order): s2 of the K record
+  alignas(16) float2 aux_zm[2][64];                //                                            f_t zv[t] of the V record
+  alignas(8) float2 e_chunk[2];                    // [chunk parity] {E, 2^-E}: E = largest binary exponent of the chunk's s1v
+  int e_warp[4];
   alignas(16) float2 ml[128];                      // epilogue: {m, l} of the rows
   alignas(8) uint64_t full_k[2], full_v[2];        // TMA arrival [chunk parity]
   alignas(8) uint64_t bar_s, bar_o[2];             // MMA completion (tcgen05.commit): S ready, O of a token half accumulated
@@ -109,45 +137,63 @@ struct DenseSmem {
   uint32_t tmem_base;
 };
 
-// the packed words of half `half` (K positions 64 half .. 64 half + 63) of the code row in slot `slot`
+// Producer thread (warp pw = 0..7, lane): pw = (w, mtile) of the record's slot numbering; the lane names
+// (g & 1, t, rho, word quarter) so that iteration i of a warp reads the 128 contiguous bytes
+// [w, mtile(, rho)] + 128 i of the code block.  The thread's word index `wi` is the same in every iteration: its
+// scales live in registers for the whole chunk.
 template <int BITS>
-__device__ __forceinline__ void load_row_half(const uint8_t* codes, int slot, int half, uint32_t (&W)[2 * BITS]) {
-  const int w = slot >> 5, mt = (slot >> 4) & 1, rho = (slot >> 3) & 1, g = slot & 7;
-#pragma unroll
-  for (int t = 0; t < 4; ++t) {
-    if constexpr (BITS == 2) {
-      W[t] = *reinterpret_cast<const uint32_t*>(codes + w * 1024 + mt * 512 + (4 * g + t) * 16 + rho * 8 + 4 * half);
-    } else {
-      const uint2 v = *reinterpret_cast<const uint2*>(codes + w * 2048 + mt * 1024 + rho * 512 + (4 * g + t) * 16 + 8 * half);
-      W[t] = v.x; W[4 + t] = v.y;
-    }
+struct ProducerLane {
+  int glo, t, rho, q;      // 2-bit: q = which half of the 8 words; 4-bit: q = which quarter of the 16 words, rho unused
+  __device__ __forceinline__ explicit ProducerLane(int lane) {
+    glo = lane >> 4; t = (lane >> 1) & 3;
+    if constexpr (BITS == 2) { rho = lane & 1; q = (lane >> 3) & 1; }
+    else { rho = 0; q = (lane & 1) | (((lane >> 3) & 1) << 1); }
   }
-}
+  __device__ __forceinline__ int wi() const { return 4 * q + t; }
+  static constexpr int ITERS = BITS == 2 ? 4 : 8;
+  // byte offset of the word inside the code block, slot of its row
+  __device__ __forceinline__ int word_off(int pw, int it) const {
+    const int w = pw >> 1, mt = pw & 1;
+    if constexpr (BITS == 2) return w * 1024 + mt * 512 + it * 128 + glo * 64 + t * 16 + rho * 8 + q * 4;
+    else return w * 2048 + mt * 1024 + (it >> 2) * 512 + (it & 3) * 128 + glo * 64 + t * 16 + q * 4;
+  }
+  __device__ __forceinline__ int slot(int pw, int it) const {
+    const int w = pw >> 1, mt = pw & 1;
+    if constexpr (BITS == 2) return w * 32 + mt * 16 + rho * 8 + 2 * it + glo;
+    else return w * 32 + mt * 16 + (it >> 2) * 8 + 2 * (it & 3) + glo;
+  }
+};
 
-// Half a code row (64 codes) -> 64 fp16 values code * scale in K-position order, written as 8 units of 16 bytes of
-// row `row` of a K-major tile with KT columns.  scale_tab: half2 per K-position pair (64 entries), or null: `sc` for all.
-template <int BITS, bool TAB>
-__device__ __forceinline__ void dequant_half(const uint32_t (&W)[2 * BITS], const __half2* scale_tab, __half2 sc,
-                                             uint8_t* tile, int row, int KT, int half) {
-  constexpr int CPW = 32 / BITS, PPW = CPW / 2;                 // codes, pairs per word
+// Expansion of a code pair without un-biasing: the two codes of pair j of a word (codes j and j + CPW / 2) are moved to
+// mantissa bits [p, p + BITS) of the two fp16 lanes, p = dq_p(j) >= 4, under the exponent of 2^(10 - p): the lanes then
+// hold 2^(10 - p) + code, and ONE fma gives code * s = (2^(10 - p) + code) * s - 2^(10 - p) s, exactly (the product is
+// exact inside the fma, the result has <= 8 significant bits, the addend is at most 64 * 448).  Three (2-bit) codes
+// share one shifted copy of the word.
+template <int BITS> __host__ __device__ constexpr int dq_p(int j) { return BITS == 2 ? 4 + 2 * (j % 3) : 4; }
+template <int BITS> __host__ __device__ constexpr float dq_bias(int j) { return (float)(1 << (10 - dq_p<BITS>(j))); }
+
+// One packed word (CPW codes = CPW consecutive K positions) of a row -> fp16 values, written as CPW / 8 units of
+// 16 bytes at `dst` (+ DN_LBO per unit).  K: value = code * s[j] via add[j] = -dq_bias s[j].  V: value =
+// (code * sc) * f[j]: both products exact (<= 8, then <= 11 significant bits).
+template <int BITS, bool IS_K>
+__device__ __forceinline__ void dequant_word(uint32_t W, const __half2 (&s)[16 / BITS], const __half2 (&add)[16 / BITS],
+                                             __half2 sc, const __half2 (&nsc)[3], uint8_t* dst) {
+  constexpr int PPW = 16 / BITS;
   constexpr uint32_t MASK = BITS == 2 ? 0x00030003u : 0x000F000Fu;
-  const __half2 k1024 = __floats2half2_rn(1024.f, 1024.f);
-  uint8_t* base = tile + (row >> 3) * ((KT >> 3) * 128) + (row & 7) * 16 + half * 1024;
-  if (TAB) scale_tab += 32 * half;
+  uint32_t o[PPW];
 #pragma unroll
-  for (int u = 0; u < 8; ++u) {                                  // unit u: K positions 64 half + 8u .. + 7 = 4 pairs
-    uint32_t o[4];
-#pragma unroll
-    for (int pp = 0; pp < 4; ++pp) {
-      const int pair = 4 * u + pp;                               // pair index inside the half
-      const int wi = pair / PPW, j = pair % PPW;
-      uint32_t h = ((W[wi] >> (BITS * j)) & MASK) | 0x64006400u; // fp16 1024 + code, twice
-      __half2 x = __hsub2(*reinterpret_cast<__half2*>(&h), k1024);
-      x = __hmul2(x, TAB ? scale_tab[pair] : sc);
-      o[pp] = *reinterpret_cast<uint32_t*>(&x);
-    }
-    *reinterpret_cast<uint4*>(base + u * 128) = make_uint4(o[0], o[1], o[2], o[3]);
+  for (int j = 0; j < PPW; ++j) {
+    const int p = dq_p<BITS>(j), delta = p - BITS * j;
+    const uint32_t Wg = delta >= 0 ? (W << delta) : (W >> (-delta));
+    uint32_t h = (Wg & (MASK << p)) | (((uint32_t)(25 - p) << 10) * 0x00010001u);
+    __half2 x;
+    if constexpr (IS_K) x = __hfma2(*reinterpret_cast<__half2*>(&h), s[j], add[j]);
+    else x = __hmul2(__hfma2(*reinterpret_cast<__half2*>(&h), sc, nsc[BITS == 2 ? j % 3 : 0]), s[j]);
+    o[j] = *reinterpret_cast<uint32_t*>(&x);
   }
+#pragma unroll
+  for (int u = 0; u < PPW / 4; ++u)
+    *reinterpret_cast<uint4*>(dst + u * DN_LBO) = make_uint4(o[4 * u], o[4 * u + 1], o[4 * u + 2], o[4 * u + 3]);
 }
 
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
@@ -161,6 +207,7 @@ __device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t& a, uint32_t& 
 
 
 
+
 constexpr int DENSE_THREADS = 544;          // warps 0-7 softmax, 8-15 producers, 16 MMA issuer
 constexpr int DENSE_SETS = 2;               // partial sets per CTA: one per token half (independent online softmax streams)
 
@@ -168,6 +215,7 @@ template <int BITS, typename InT>
 __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const DenseArgs A) {
   using SM = DenseSmem<BITS>;
   constexpr int RB = SM::RB;
+  constexpr int PPW = 16 / BITS, CPW = 32 / BITS;
   constexpr uint32_t TMEM_COLS = 512;           // S: columns [0, 144), O of token half h: columns [256 + 128 h, 384 + 128 h)
   constexpr uint32_t O_COL = 256;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -236,7 +284,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
   constexpr uint32_t IDESC_S = umma_idesc_f16(128, DN_NS), IDESC_O = umma_idesc_f16(128, 128);
-  constexpr uint32_t SBO_T = (DN_KT / 8) * 128, SBO_P = (DN_KP / 8) * 128, SBO_PH = (DN_KPH / 8) * 128;
+  constexpr uint32_t SBO_T = (DN_KT / 8) * 128, SBO_PH = (DN_KPH / 8) * 128;
   constexpr float P_OFF = 8.f;                  // p~ = 2^(logit - max + 8): probabilities down to 2^-32 of the maximum survive fp16
   float m_ref = -INFINITY, l_run = 0.f;         // softmax warps: reference exponent of the (row, token half), running l
 
@@ -244,10 +292,25 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   // barrier completes phase i + 1 before every waiter of phase i has looked (a parity wait cannot tell i from i + 2):
   // the waits marked (*) below are there for that reason alone.
   if (warp >= 8 && warp < 16) {
-    // =============================== producers: thread = (token | channel row, half of its codes) ====================
-    const int pt = tid - 256, row = pt & 127, half = pt >> 7;
-    const int rho_t = dense_kpos<BITS>(row), slot_t = slot_of_token(BITS, row);
-    // chunk c: per-channel and per-token aux, then Kt; afterwards the K record of chunk c + 2 is requested
+    // =============================== producers ======================================================================
+    const int pt = tid - 256, pw = warp - 8;
+    const ProducerLane<BITS> L(lane);
+    const int wi = L.wi();
+    // per-thread constants of the aux phase: threads 0..127 own S column / K position n = pt of the token axis,
+    // threads 128..255 own K position pt - 128 of the channel axis
+    const int n_ax = pt & 127;
+    const int tok = dense_elem_of_kpos<BITS>(n_ax), slot_tok = slot_of_token(BITS, tok);
+    const int ka = kaux_of_elem(BITS, dense_elem_of_kpos<BITS>(n_ax));
+    // tile rows of the thread's words: Kt row = S column of the slot's token, Vt row = slot (channel)
+    int krow_off[ProducerLane<BITS>::ITERS], vrow_off[ProducerLane<BITS>::ITERS];
+#pragma unroll
+    for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i) {
+      const int sl = L.slot(pw, i);
+      const int kr_ = dense_kpos<BITS>(token_of_slot(BITS, sl));
+      krow_off[i] = tile_off(kr_, 0, DN_SBO_K) + wi * (CPW / 8) * DN_LBO;
+      vrow_off[i] = tile_off(sl, 0, DN_SBO_V) + wi * (CPW / 8) * DN_LBO;
+    }
+    // chunk c: aux of both records, then Kt; afterwards the K record of chunk c + 2 is requested
     auto expand_k = [&](int c) {
       const int st = c & 1;
       const uint32_t par_rec = (c >> 1) & 1;
@@ -255,32 +318,57 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       mbar_wait(&sm.full_v[st], par_rec);
       const uint8_t* kr = sm.rec_k[st];
       const uint8_t* vr = sm.rec_v[st];
-      if (half == 0) {
-        // thread = K position `row`: channel c, s1 and z in the record's builder order
-        const int ch = dense_elem_of_kpos<BITS>(row), ka = kaux_of_elem(BITS, ch);
+      float s1v = 0.f;
+      if (pt < 128) {
+        // binary exponent of s1v[token]; E = the largest of the chunk (through e_warp)
+        s1v = e4m3_to_f32(vr[s1_off(BITS) + slot_tok]);
+        const int e = s1v > 0.f ? (int)((__float_as_uint(s1v) >> 23) & 0xFF) - 127 : -64;
+        const int em = __reduce_max_sync(0xffffffffu, e);
+        if (lane == 0) sm.e_warp[pw] = em;
+      } else {
+        // channel of K position n_ax: s1 and z in the record's builder order
         const float s1 = e4m3_to_f32(kr[s1_off(BITS) + ka]);
         const float z = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(kr + z_off(BITS))[ka]);
-        reinterpret_cast<__half*>(sm.s1h)[row] = __float2half_rn(s1);                    // exact
+        reinterpret_cast<__half*>(sm.s1h)[n_ax] = __float2half_rn(s1);                    // exact
+        reinterpret_cast<__half*>(sm.s1n)[n_ax] = __float2half_rn(-dq_bias<BITS>((n_ax >> 1) % PPW) * s1);
         const float sz = s1 * z;
         const __half hi = __float2half_rn(sz), lo = __float2half_rn(sz - __half2float(hi));
-        *reinterpret_cast<__half*>(sm.kt + kmaj_off(128, row, DN_KT)) = hi;
-        *reinterpret_cast<__half*>(sm.kt + kmaj_off(129, row, DN_KT)) = lo;
-      } else {
-        // per-token aux of both records (parity-buffered: the softmax warps still read the previous chunk's)
-        const float s1v = fmaxf(e4m3_to_f32(vr[s1_off(BITS) + slot_t]), 9.094947e-13f);
-        const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[slot_t]);
-        sm.aux_a[st][rho_t] = make_float2(e4m3_to_f32(kr[s2_off(BITS) + slot_t]), lg2_approx(s1v));
-        sm.aux_b[st][rho_t] = make_float2(rcp_approx(s1v), zv);
+        *reinterpret_cast<__half*>(sm.kt + tile_off(128, n_ax, DN_SBO_K)) = hi;
+        *reinterpret_cast<__half*>(sm.kt + tile_off(129, n_ax, DN_SBO_K)) = lo;
       }
-      producer_sync();                                   // s1h complete
+      producer_sync();                                   // s1h, s1n, e_warp complete
+      if (pt < 128) {
+        const int E = max(max(sm.e_warp[0], sm.e_warp[1]), max(sm.e_warp[2], sm.e_warp[3]));
+        const float two_mE = __uint_as_float((uint32_t)(127 - max(E, -64)) << 23);        // 2^-E
+        const float f = s1v * two_mE;                    // in [0, 2): the V tile carries s2v f, the logits carry E
+        const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[slot_tok]);
+        reinterpret_cast<__half*>(sm.fh[st])[n_ax] = __float2half_rn(f);
+        reinterpret_cast<float*>(&sm.aux_s2[st][n_ax >> 1])[n_ax & 1] = e4m3_to_f32(kr[s2_off(BITS) + slot_tok]);
+        reinterpret_cast<float*>(&sm.aux_zm[st][n_ax >> 1])[n_ax & 1] = f * zv;
+        if (pt == 0) sm.e_chunk[st] = make_float2((float)max(E, -64), two_mE);
+      }
       {
-        uint32_t W[2 * BITS];
-        load_row_half<BITS>(kr, slot_t, half, W);
-        dequant_half<BITS, true>(W, sm.s1h, __half2(), sm.kt, rho_t, DN_KT, half);
+        __half2 sK[PPW], aK[PPW];
+        const __half2 nsc0[3] = {__half2(), __half2(), __half2()};
+#pragma unroll
+        for (int j = 0; j < PPW; j += 4) {
+          const uint4 s4 = *reinterpret_cast<const uint4*>(&sm.s1h[wi * PPW + j]);
+          const uint4 a4 = *reinterpret_cast<const uint4*>(&sm.s1n[wi * PPW + j]);
+          sK[j] = *reinterpret_cast<const __half2*>(&s4.x); sK[j + 1] = *reinterpret_cast<const __half2*>(&s4.y);
+          sK[j + 2] = *reinterpret_cast<const __half2*>(&s4.z); sK[j + 3] = *reinterpret_cast<const __half2*>(&s4.w);
+          aK[j] = *reinterpret_cast<const __half2*>(&a4.x); aK[j + 1] = *reinterpret_cast<const __half2*>(&a4.y);
+          aK[j + 2] = *reinterpret_cast<const __half2*>(&a4.z); aK[j + 3] = *reinterpret_cast<const __half2*>(&a4.w);
+        }
+        uint32_t W[ProducerLane<BITS>::ITERS];
+#pragma unroll
+        for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i) W[i] = *reinterpret_cast<const uint32_t*>(kr + L.word_off(pw, i));
+#pragma unroll
+        for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i)
+          dequant_word<BITS, true>(W[i], sK, aK, __half2(), nsc0, sm.kt + krow_off[i]);
       }
       fence_async_smem();
       mbar_arrive(&sm.kt_full);
-      producer_sync();                                   // every producer has left rec_k[st] and s1h
+      producer_sync();                                   // every producer has left rec_k[st], s1h, s1n, e_warp
       if (pt == 0 && c + 2 < n_my) {
         mbar_expect_tx(&sm.full_k[st], RB); bulk_g2s(sm.rec_k[st], krec + (size_t)(c + 2) * RB, RB, &sm.full_k[st]);
       }
@@ -298,12 +386,26 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       mbar_wait(&sm.full_v[st], (it >> 1) & 1);
       {
         const uint8_t* vr = sm.rec_v[st];
-        const float s2v = e4m3_to_f32(vr[s2_off(BITS) + row]);                           // thread = (channel row, token half)
-        const __half2 sc = __float2half2_rn(s2v);
-        uint32_t W[2 * BITS];
-        load_row_half<BITS>(vr, row, half, W);
-        dequant_half<BITS, false>(W, nullptr, sc, sm.vt, row, DN_KP, half);
-        if (half == 0) *reinterpret_cast<__half2*>(sm.vt + kmaj_off(row, 128, DN_KP)) = sc;   // K columns 128, 129: s2v (zero-point term)
+        __half2 fV[PPW];
+#pragma unroll
+        for (int j = 0; j < PPW; j += 4) {
+          const uint4 f4 = *reinterpret_cast<const uint4*>(&sm.fh[st][wi * PPW + j]);
+          fV[j] = *reinterpret_cast<const __half2*>(&f4.x); fV[j + 1] = *reinterpret_cast<const __half2*>(&f4.y);
+          fV[j + 2] = *reinterpret_cast<const __half2*>(&f4.z); fV[j + 3] = *reinterpret_cast<const __half2*>(&f4.w);
+        }
+        uint32_t W[ProducerLane<BITS>::ITERS];
+#pragma unroll
+        for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i) W[i] = *reinterpret_cast<const uint32_t*>(vr + L.word_off(pw, i));
+#pragma unroll
+        for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i) {
+          const __half2 sc = __float2half2_rn(e4m3_to_f32(vr[s2_off(BITS) + L.slot(pw, i)]));   // s2v of the row's channel
+          __half2 nsc[3];
+#pragma unroll
+          for (int k = 0; k < 3; ++k) nsc[k] = __hmul2(sc, __float2half2_rn(-dq_bias<BITS>(k)));
+          dequant_word<BITS, false>(W[i], fV, fV, sc, nsc, sm.vt + vrow_off[i]);
+        }
+        if (pt < 128)                                    // K columns 128, 129 of channel row pt: s2v (zero-point term)
+          *reinterpret_cast<__half2*>(sm.vt + tile_off(pt, 128, DN_SBO_V)) = __float2half2_rn(e4m3_to_f32(vr[s2_off(BITS) + pt]));
       }
       fence_async_smem();
       mbar_arrive(&sm.vt_full);
@@ -324,7 +426,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
 #pragma unroll
           for (int ks = 0; ks < DN_KT / 16; ++ks)
             umma_f16(tmem, umma_desc(smem_u32(term ? sm.qlo : sm.qhi) + ks * 256, 128, SBO_T),
-                     umma_desc(smem_u32(sm.kt) + ks * 256, 128, SBO_T), IDESC_S, (term | ks) != 0);
+                     umma_desc(smem_u32(sm.kt) + ks * 2 * DN_LBO, DN_LBO, DN_SBO_K), IDESC_S, (term | ks) != 0);
         umma_commit(&sm.bar_s);
       };
       if (n_my > 0) issue_qk(0);
@@ -340,7 +442,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           for (int ks = 0; ks < DN_KPH / 16; ++ks) {      // 4 steps over the half's 64 tokens + 1 over the zero-point columns
             const uint32_t vcol = ks < 4 ? (uint32_t)(64 * h + 16 * ks) : 128u;
             umma_f16(tmem + O_COL + 128 * h, umma_desc(smem_u32(sm.pt[h]) + ks * 256, 128, SBO_PH),
-                     umma_desc(smem_u32(sm.vt) + (vcol >> 3) * 128, 128, SBO_P), IDESC_O, (it | ks) != 0);
+                     umma_desc(smem_u32(sm.vt) + (vcol >> 3) * DN_LBO, DN_LBO, DN_SBO_V), IDESC_O, (it | ks) != 0);
           }
           umma_commit(&sm.bar_o[h]);
         }
@@ -358,7 +460,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       mbar_wait(&sm.bar_s, par);
       mbar_wait(&sm.kt_full, par);                       // the producers' aux writes of this chunk are visible
       tc_fence_after();
-      float v[64];
+      float2 v[32];                                      // logits of the half's 64 tokens, as token pairs
       float beta;
       {
         uint32_t b0, b1;
@@ -369,19 +471,20 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         for (int c0 = 0; c0 < 64; c0 += 16) {
           tmem_ld16(t_row + 64 * h + c0, u);
 #pragma unroll
-          for (int j = 0; j < 16; ++j) v[c0 + j] = __uint_as_float(u[j]);
+          for (int j = 0; j < 16; j += 2) v[(c0 + j) >> 1] = make_float2(__uint_as_float(u[j]), __uint_as_float(u[j + 1]));
         }
       }
       tc_fence_before();
       mbar_arrive(&sm.s_free);                           // S is in registers: the next QK^T may overwrite it
-      const float2* aa = &sm.aux_a[st][64 * h];
-      const float2* ab = &sm.aux_b[st][64 * h];
+      const float2* as2 = &sm.aux_s2[st][32 * h];
+      const float2* azm = &sm.aux_zm[st][32 * h];
+      const float2 ec = sm.e_chunk[st];
+      const float2 beta2 = make_float2(beta, beta), e2 = make_float2(ec.x, ec.x);
       float mx = -INFINITY;
 #pragma unroll
-      for (int j = 0; j < 64; ++j) {
-        const float2 a = aa[j];
-        v[j] = fmaf(a.x, v[j] + beta, a.y);
-        mx = fmaxf(mx, v[j]);
+      for (int k = 0; k < 32; ++k) {
+        v[k] = __ffma2_rn(as2[k], __fadd2_rn(v[k], beta2), e2);        // log2-domain logit of p~ = p 2^E
+        mx = fmaxf(mx, fmaxf(v[k].x, v[k].y));
       }
       const float m_new = fmaxf(m_ref, mx - P_OFF);
       const float f_old = ex2_approx(m_ref - m_new);     // 0 for the first chunk (m_ref = -inf)
@@ -401,22 +504,23 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         }
       }
       m_ref = m_new;
-      float lsum = 0.f, zsum = 0.f;
+      const float2 nm2 = make_float2(-m_new, -m_new);
+      float2 l2 = make_float2(0.f, 0.f), z2 = make_float2(0.f, 0.f);
 #pragma unroll
-      for (int c0 = 0; c0 < 64; c0 += 8) {
+      for (int c0 = 0; c0 < 32; c0 += 4) {               // 4 token pairs = one 16-byte unit of the Pt row
         uint32_t o[4];
 #pragma unroll
-        for (int j = 0; j < 8; j += 2) {
-          const float2 b0 = ab[c0 + j], b1 = ab[c0 + j + 1];
-          const float p0 = ex2_approx(v[c0 + j] - m_new), p1 = ex2_approx(v[c0 + j + 1] - m_new);
-          const __half2 ph = __floats2half2_rn(p0, p1);
+        for (int k = 0; k < 4; ++k) {
+          const float2 d = __fadd2_rn(v[c0 + k], nm2);
+          const __half2 ph = __floats2half2_rn(ex2_approx(d.x), ex2_approx(d.y));
           const float2 pf = __half22float2(ph);                 // the rounded values: numerator and denominator agree
-          lsum = fmaf(pf.x, b0.x, fmaf(pf.y, b1.x, lsum));
-          zsum = fmaf(pf.x, b0.y, fmaf(pf.y, b1.y, zsum));
-          o[j >> 1] = *reinterpret_cast<const uint32_t*>(&ph);
+          l2 = __fadd2_rn(l2, pf);
+          z2 = __ffma2_rn(pf, azm[c0 + k], z2);
+          o[k] = *reinterpret_cast<const uint32_t*>(&ph);
         }
-        *reinterpret_cast<uint4*>(prow + (c0 >> 3) * 128) = make_uint4(o[0], o[1], o[2], o[3]);
+        *reinterpret_cast<uint4*>(prow + (c0 >> 2) * 128) = make_uint4(o[0], o[1], o[2], o[3]);
       }
+      const float lsum = (l2.x + l2.y) * ec.y, zsum = z2.x + z2.y;   // l in units of p = p~ 2^-E
       l_run = fmaf(l_run, f_old, lsum);
       {
         const __half zh = __float2half_rn(zsum), zl = __float2half_rn(zsum - __half2float(zh));
