@@ -59,6 +59,11 @@ __device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t da, uint64_t 
   asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
                ::"r"(d_tmem), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
 }
+// A operand from tensor memory (lane = row, one 32-bit column = two consecutive K elements)
+__device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+               ::"r"(d_tmem), "r"(a_tmem), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -72,6 +77,10 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16
   asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
                ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
                  "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]) : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -119,7 +128,6 @@ struct DenseSmem {
   alignas(1024) uint8_t qlo[128 * DN_KT * 2];      // second fp16 term
   alignas(1024) uint8_t kt[18 * DN_SBO_K];         // rows 0..127: token rho(t); 128, 129: hi / lo of s1 z; 130..143: zero
   alignas(1024) uint8_t vt[16 * DN_SBO_V];         // rows: channels; columns 0..127 tokens (rho order), 128, 129: s2v, rest zero
-  alignas(1024) uint8_t pt[2][128 * DN_KPH * 2];   // [token half] rows: query rows; columns 0..63 p~, 64, 65: hi / lo of zsum
   alignas(128) uint8_t rec_k[2][RB];               // [chunk parity]
   alignas(128) uint8_t rec_v[2][RB];
   alignas(16) __half2 s1h[64];                     // s1 of the K record as fp16 pairs in K-position order
@@ -216,8 +224,10 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   using SM = DenseSmem<BITS>;
   constexpr int RB = SM::RB;
   constexpr int PPW = 16 / BITS, CPW = 32 / BITS;
-  constexpr uint32_t TMEM_COLS = 512;           // S: columns [0, 144), O of token half h: columns [256 + 128 h, 384 + 128 h)
-  constexpr uint32_t O_COL = 256;
+  // tensor memory: S: columns [0, 144); p~ of token half h (fp16 pairs, the A operand of PV): [144 + 40 h, 184 + 40 h);
+  // O of token half h: [256 + 128 h, 384 + 128 h)
+  constexpr uint32_t TMEM_COLS = 512;
+  constexpr uint32_t P_COL = 144, O_COL = 256;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -252,7 +262,6 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   // zero the tiles once: rows / columns that are never rewritten (padding of N = 144 and of the K extents) stay zero
   for (int i = tid; i < (int)(sizeof(sm.kt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.kt)[i] = make_uint4(0, 0, 0, 0);
   for (int i = tid; i < (int)(sizeof(sm.vt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.vt)[i] = make_uint4(0, 0, 0, 0);
-  for (int i = tid; i < (int)(sizeof(sm.pt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.pt)[i] = make_uint4(0, 0, 0, 0);
   // q' = (q H / sqrt(128)) q_scale as two fp16 terms, columns in K-position order
   for (int r = warp; r < 128; r += DENSE_THREADS / 32) {
     const int R = rt * 128 + r;
@@ -284,7 +293,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
   constexpr uint32_t IDESC_S = umma_idesc_f16(128, DN_NS), IDESC_O = umma_idesc_f16(128, 128);
-  constexpr uint32_t SBO_T = (DN_KT / 8) * 128, SBO_PH = (DN_KPH / 8) * 128;
+  constexpr uint32_t SBO_T = (DN_KT / 8) * 128;
   constexpr float P_OFF = 8.f;                  // p~ = 2^(logit - max + 8): probabilities down to 2^-32 of the maximum survive fp16
   float m_ref = -INFINITY, l_run = 0.f;         // softmax warps: reference exponent of the (row, token half), running l
 
@@ -441,8 +450,8 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
 #pragma unroll
           for (int ks = 0; ks < DN_KPH / 16; ++ks) {      // 4 steps over the half's 64 tokens + 1 over the zero-point columns
             const uint32_t vcol = ks < 4 ? (uint32_t)(64 * h + 16 * ks) : 128u;
-            umma_f16(tmem + O_COL + 128 * h, umma_desc(smem_u32(sm.pt[h]) + ks * 256, 128, SBO_PH),
-                     umma_desc(smem_u32(sm.vt) + (vcol >> 3) * DN_LBO, DN_LBO, DN_SBO_V), IDESC_O, (it | ks) != 0);
+            umma_f16_ts(tmem + O_COL + 128 * h, tmem + P_COL + (DN_KPH / 2) * h + 8 * ks,
+                        umma_desc(smem_u32(sm.vt) + (vcol >> 3) * DN_LBO, DN_LBO, DN_SBO_V), IDESC_O, (it | ks) != 0);
           }
           umma_commit(&sm.bar_o[h]);
         }
@@ -453,7 +462,8 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
     const int h = warp >> 2, r = (warp & 3) * 32 + lane;
     const uint32_t t_row = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t t_o = t_row + O_COL + 128 * h;
-    uint8_t* prow = sm.pt[h] + (r >> 3) * SBO_PH + (r & 7) * 16;
+    const uint32_t t_p = t_row + P_COL + (DN_KPH / 2) * h;
+    (void)r;
     for (int it = 0; it < n_my; ++it) {
       const int st = it & 1;
       const uint32_t par = it & 1;
@@ -507,10 +517,10 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       const float2 nm2 = make_float2(-m_new, -m_new);
       float2 l2 = make_float2(0.f, 0.f), z2 = make_float2(0.f, 0.f);
 #pragma unroll
-      for (int c0 = 0; c0 < 32; c0 += 4) {               // 4 token pairs = one 16-byte unit of the Pt row
-        uint32_t o[4];
+      for (int c0 = 0; c0 < 32; c0 += 16) {              // 16 token pairs = 16 columns of the row's p~ in tensor memory
+        uint32_t o[16];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
+        for (int k = 0; k < 16; ++k) {
           const float2 d = __fadd2_rn(v[c0 + k], nm2);
           const __half2 ph = __floats2half2_rn(ex2_approx(d.x), ex2_approx(d.y));
           const float2 pf = __half22float2(ph);                 // the rounded values: numerator and denominator agree
@@ -518,15 +528,17 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           z2 = __ffma2_rn(pf, azm[c0 + k], z2);
           o[k] = *reinterpret_cast<const uint32_t*>(&ph);
         }
-        *reinterpret_cast<uint4*>(prow + (c0 >> 2) * 128) = make_uint4(o[0], o[1], o[2], o[3]);
+        tmem_st16(t_p + c0, o);
       }
       const float lsum = (l2.x + l2.y) * ec.y, zsum = z2.x + z2.y;   // l in units of p = p~ 2^-E
       l_run = fmaf(l_run, f_old, lsum);
       {
         const __half zh = __float2half_rn(zsum), zl = __float2half_rn(zsum - __half2float(zh));
-        *reinterpret_cast<__half2*>(prow + 8 * 128) = __halves2half2(zh, zl);              // K columns 64, 65
+        const __half2 zz = __halves2half2(zh, zl);                                         // K columns 64, 65; 66..79: zero
+        const uint32_t o8[8] = {*reinterpret_cast<const uint32_t*>(&zz), 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+        tmem_st8(t_p + 32, o8);
       }
-      fence_async_smem();
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       tc_fence_before();
       mbar_arrive(&sm.p_full[h]);
     }
