@@ -207,6 +207,11 @@ __device__ __forceinline__ void dequant_word(uint32_t W, const __half2 (&s)[16 /
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// one arrival per warp: the lanes' writes are ordered before it by the warp barrier
+__device__ __forceinline__ void mbar_arrive_warp(uint64_t* bar, int lane) {
+  __syncwarp();
+  if (lane == 0) mbar_arrive(bar);
+}
 __device__ __forceinline__ void producer_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 __device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t& a, uint32_t& b) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(a), "=r"(b) : "r"(taddr));
@@ -246,9 +251,9 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
 
   // ---- setup: barriers, TMEM, first records, q ------------------------------------------------------------------
   if (tid == 256) {
-    for (int s = 0; s < 2; ++s) { mbar_init(&sm.full_k[s], 1); mbar_init(&sm.full_v[s], 1); mbar_init(&sm.bar_o[s], 1); mbar_init(&sm.p_full[s], 128); }
+    for (int s = 0; s < 2; ++s) { mbar_init(&sm.full_k[s], 1); mbar_init(&sm.full_v[s], 1); mbar_init(&sm.bar_o[s], 1); mbar_init(&sm.p_full[s], 4); }
     mbar_init(&sm.bar_s, 1);
-    mbar_init(&sm.kt_full, 256); mbar_init(&sm.vt_full, 256); mbar_init(&sm.s_free, 256);
+    mbar_init(&sm.kt_full, 8); mbar_init(&sm.vt_full, 8); mbar_init(&sm.s_free, 8);     // one arrival per warp
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     for (int c = 0; c < 2 && c < n_my; ++c) {
       mbar_expect_tx(&sm.full_k[c], RB); bulk_g2s(sm.rec_k[c], krec + (size_t)c * RB, RB, &sm.full_k[c]);
@@ -376,7 +381,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           dequant_word<BITS, true>(W[i], sK, aK, __half2(), nsc0, sm.kt + krow_off[i]);
       }
       fence_async_smem();
-      mbar_arrive(&sm.kt_full);
+      mbar_arrive_warp(&sm.kt_full, lane);
       producer_sync();                                   // every producer has left rec_k[st], s1h, s1n, e_warp
       if (pt == 0 && c + 2 < n_my) {
         mbar_expect_tx(&sm.full_k[st], RB); bulk_g2s(sm.rec_k[st], krec + (size_t)(c + 2) * RB, RB, &sm.full_k[st]);
@@ -417,7 +422,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           *reinterpret_cast<__half2*>(sm.vt + tile_off(pt, 128, DN_SBO_V)) = __float2half2_rn(e4m3_to_f32(vr[s2_off(BITS) + pt]));
       }
       fence_async_smem();
-      mbar_arrive(&sm.vt_full);
+      mbar_arrive_warp(&sm.vt_full, lane);
       producer_sync();                                   // every producer has left rec_v[st]
       if (pt == 0 && it + 2 < n_my) {
         mbar_expect_tx(&sm.full_v[st], RB); bulk_g2s(sm.rec_v[st], vrec + (size_t)(it + 2) * RB, RB, &sm.full_v[st]);
@@ -485,7 +490,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         }
       }
       tc_fence_before();
-      mbar_arrive(&sm.s_free);                           // S is in registers: the next QK^T may overwrite it
+      mbar_arrive_warp(&sm.s_free, lane);                         // S is in registers: the next QK^T may overwrite it
       const float2* as2 = &sm.aux_s2[st][32 * h];
       const float2* azm = &sm.aux_zm[st][32 * h];
       const float2 ec = sm.e_chunk[st];
@@ -540,7 +545,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       }
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       tc_fence_before();
-      mbar_arrive(&sm.p_full[h]);
+      mbar_arrive_warp(&sm.p_full[h], lane);
     }
   }
   // ---- epilogue, once per token half: O rows -> shared memory (the q tiles are dead: every QK^T has completed),
