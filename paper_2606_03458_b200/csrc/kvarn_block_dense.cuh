@@ -127,20 +127,21 @@ struct DenseSmem {
   alignas(1024) uint8_t qhi[128 * DN_KT * 2];      // q' (rotated, scaled), first fp16 term; later: staging of O (with qlo)
   alignas(1024) uint8_t qlo[128 * DN_KT * 2];      // second fp16 term
   alignas(1024) uint8_t kt[18 * DN_SBO_K];         // rows 0..127: token rho(t); 128, 129: hi / lo of s1 z; 130..143: zero
-  alignas(1024) uint8_t vt[16 * DN_SBO_V];         // rows: channels; columns 0..127 tokens (rho order), 128, 129: s2v, rest zero
+  alignas(1024) uint8_t vt[2][16 * DN_SBO_V];      // [chunk parity] rows: channels; columns 0..127 tokens (rho order), 128, 129: s2v, rest zero
   alignas(128) uint8_t rec_k[2][RB];               // [chunk parity]
   alignas(128) uint8_t rec_v[2][RB];
   alignas(16) __half2 s1h[64];                     // s1 of the K record as fp16 pairs in K-position order
   alignas(16) __half2 s1n[64];                     // the addends -dq_bias s1 of the same pairs
   alignas(16) __half2 fh[2][64];                   // [chunk parity] f_t = s1v[t] 2^-E of the V record, pairs in K-position order
-  alignas(16) float2 aux_s2[2][64];                // [chunk parity] per token pair (rho order): s2 of the K record
-  alignas(16) float2 aux_zm[2][64];                //                                            f_t zv[t] of the V record
-  alignas(8) float2 e_chunk[2];                    // [chunk parity] {E, 2^-E}: E = largest binary exponent of the chunk's s1v
+  alignas(16) float2 aux_s2[3][64];                // [chunk % 3] per token pair (rho order): s2 of the K record
+  alignas(16) float2 aux_zm[3][64];                //                                         f_t zv[t] of the V record
+  alignas(8) float2 e_chunk[3];                    // [chunk % 3] {E, 2^-E}: E = largest binary exponent of the chunk's s1v
   int e_warp[4];
   alignas(16) float2 ml[128];                      // epilogue: {m, l} of the rows
   alignas(8) uint64_t full_k[2], full_v[2];        // TMA arrival [chunk parity]
   alignas(8) uint64_t bar_s, bar_o[2];             // MMA completion (tcgen05.commit): S ready, O of a token half accumulated
-  alignas(8) uint64_t kt_full, vt_full;            // producers -> issuer (and softmax warps: aux) (256 arrivals each)
+  alignas(8) uint64_t kt_full, vt_full[2];         // producers -> issuer (and softmax warps: aux), one arrival per warp
+  alignas(8) uint64_t v_free[2];                   // tcgen05.commit: the PV that read vt[parity] has completed
   alignas(8) uint64_t s_free, p_full[2];           // softmax warps -> issuer (256 / 128 arrivals)
   uint32_t tmem_base;
 };
@@ -221,7 +222,14 @@ __device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t& a, uint32_t& 
 
 
 
-constexpr int DENSE_THREADS = 544;          // warps 0-7 softmax, 8-15 producers, 16 MMA issuer
+static_assert(sizeof(DenseSmem<2>) <= 231424 && sizeof(DenseSmem<4>) <= 231424, "dense tiles exceed the shared memory of one SM");
+constexpr int DENSE_THREADS = 640;          // warps 0-7 softmax, 8-15 producers, 16 MMA issuer (17-19 idle: whole warpgroups
+                                            // for setmaxnreg)
+// 96 registers per thread at launch (640 threads), re-divided: the softmax warps keep 64 logits plus prefetched aux live
+constexpr int DENSE_REGS_SOFTMAX = 120, DENSE_REGS_PRODUCER = 72;
+template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+__device__ __forceinline__ void softmax_sync() { asm volatile("bar.sync 2, 256;" ::: "memory"); }
 constexpr int DENSE_SETS = 2;               // partial sets per CTA: one per token half (independent online softmax streams)
 
 template <int BITS, typename InT>
@@ -251,9 +259,10 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
 
   // ---- setup: barriers, TMEM, first records, q ------------------------------------------------------------------
   if (tid == 256) {
-    for (int s = 0; s < 2; ++s) { mbar_init(&sm.full_k[s], 1); mbar_init(&sm.full_v[s], 1); mbar_init(&sm.bar_o[s], 1); mbar_init(&sm.p_full[s], 4); }
+    for (int s = 0; s < 2; ++s) { mbar_init(&sm.full_k[s], 1); mbar_init(&sm.full_v[s], 1); mbar_init(&sm.bar_o[s], 1); mbar_init(&sm.p_full[s], 4);
+                                  mbar_init(&sm.vt_full[s], 8); mbar_init(&sm.v_free[s], 1); }
     mbar_init(&sm.bar_s, 1);
-    mbar_init(&sm.kt_full, 8); mbar_init(&sm.vt_full, 8); mbar_init(&sm.s_free, 8);     // one arrival per warp
+    mbar_init(&sm.kt_full, 8); mbar_init(&sm.s_free, 8);                                 // one arrival per warp
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     for (int c = 0; c < 2 && c < n_my; ++c) {
       mbar_expect_tx(&sm.full_k[c], RB); bulk_g2s(sm.rec_k[c], krec + (size_t)c * RB, RB, &sm.full_k[c]);
@@ -307,6 +316,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   // the waits marked (*) below are there for that reason alone.
   if (warp >= 8 && warp < 16) {
     // =============================== producers ======================================================================
+    setmaxnreg_dec<DENSE_REGS_PRODUCER>();
     const int pt = tid - 256, pw = warp - 8;
     const ProducerLane<BITS> L(lane);
     const int wi = L.wi();
@@ -326,7 +336,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
     }
     // chunk c: aux of both records, then Kt; afterwards the K record of chunk c + 2 is requested
     auto expand_k = [&](int c) {
-      const int st = c & 1;
+      const int st = c & 1, s3 = c % 3;
       const uint32_t par_rec = (c >> 1) & 1;
       mbar_wait(&sm.full_k[st], par_rec);
       mbar_wait(&sm.full_v[st], par_rec);
@@ -357,9 +367,9 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         const float f = s1v * two_mE;                    // in [0, 2): the V tile carries s2v f, the logits carry E
         const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[slot_tok]);
         reinterpret_cast<__half*>(sm.fh[st])[n_ax] = __float2half_rn(f);
-        reinterpret_cast<float*>(&sm.aux_s2[st][n_ax >> 1])[n_ax & 1] = e4m3_to_f32(kr[s2_off(BITS) + slot_tok]);
-        reinterpret_cast<float*>(&sm.aux_zm[st][n_ax >> 1])[n_ax & 1] = f * zv;
-        if (pt == 0) sm.e_chunk[st] = make_float2((float)max(E, -64), two_mE);
+        reinterpret_cast<float*>(&sm.aux_s2[s3][n_ax >> 1])[n_ax & 1] = e4m3_to_f32(kr[s2_off(BITS) + slot_tok]);
+        reinterpret_cast<float*>(&sm.aux_zm[s3][n_ax >> 1])[n_ax & 1] = f * zv;
+        if (pt == 0) sm.e_chunk[s3] = make_float2((float)max(E, -64), two_mE);
       }
       {
         __half2 sK[PPW], aK[PPW];
@@ -391,14 +401,15 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
     for (int it = 0; it < n_my; ++it) {
       const int st = it & 1;
       const uint32_t par = it & 1;
-      if (it > 0) mbar_wait(&sm.bar_o[1], par ^ 1);      // PV of chunk it - 1 complete: Vt is free, softmax of it - 1 is over
       if (it + 1 < n_my) {                               // K of the NEXT chunk first: its QK^T overlaps this chunk's softmax
         mbar_wait(&sm.bar_s, par);                       // QK^T of this chunk has consumed Kt
         mbar_wait(&sm.s_free, par);                      // (*) the softmax warps have looked at kt_full of this chunk
         expand_k(it + 1);
       }
       mbar_wait(&sm.full_v[st], (it >> 1) & 1);
+      if (it >= 2) mbar_wait(&sm.v_free[st], ((it >> 1) & 1) ^ 1);   // the PV of chunk it - 2 has consumed vt[st]
       {
+        uint8_t* vt = sm.vt[st];
         const uint8_t* vr = sm.rec_v[st];
         __half2 fV[PPW];
 #pragma unroll
@@ -416,21 +427,21 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           __half2 nsc[3];
 #pragma unroll
           for (int k = 0; k < 3; ++k) nsc[k] = __hmul2(sc, __float2half2_rn(-dq_bias<BITS>(k)));
-          dequant_word<BITS, false>(W[i], fV, fV, sc, nsc, sm.vt + vrow_off[i]);
+          dequant_word<BITS, false>(W[i], fV, fV, sc, nsc, vt + vrow_off[i]);
         }
         if (pt < 128)                                    // K columns 128, 129 of channel row pt: s2v (zero-point term)
-          *reinterpret_cast<__half2*>(sm.vt + tile_off(pt, 128, DN_SBO_V)) = __float2half2_rn(e4m3_to_f32(vr[s2_off(BITS) + pt]));
+          *reinterpret_cast<__half2*>(vt + tile_off(pt, 128, DN_SBO_V)) = __float2half2_rn(e4m3_to_f32(vr[s2_off(BITS) + pt]));
       }
       fence_async_smem();
-      mbar_arrive_warp(&sm.vt_full, lane);
+      mbar_arrive_warp(&sm.vt_full[st], lane);
       producer_sync();                                   // every producer has left rec_v[st]
       if (pt == 0 && it + 2 < n_my) {
         mbar_expect_tx(&sm.full_v[st], RB); bulk_g2s(sm.rec_v[st], vrec + (size_t)(it + 2) * RB, RB, &sm.full_v[st]);
       }
     }
-  } else if (warp == 16) {
+  } else if (warp >= 16) {
     // =============================== MMA issuer: one thread =========================================================
-    if (lane == 0) {
+    if (warp == 16 && lane == 0) {
       auto issue_qk = [&](int c) {
         mbar_wait(&sm.kt_full, c & 1);
         if (c > 0) mbar_wait(&sm.s_free, (c & 1) ^ 1);    // the softmax warps have read S of the previous chunk
@@ -447,7 +458,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       for (int it = 0; it < n_my; ++it) {
         const uint32_t par = it & 1;
         if (it + 1 < n_my) issue_qk(it + 1);              // runs while the softmax warps work on chunk it
-        mbar_wait(&sm.vt_full, par);
+        mbar_wait(&sm.vt_full[par], (it >> 1) & 1);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           mbar_wait(&sm.p_full[h], par);
@@ -456,21 +467,22 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           for (int ks = 0; ks < DN_KPH / 16; ++ks) {      // 4 steps over the half's 64 tokens + 1 over the zero-point columns
             const uint32_t vcol = ks < 4 ? (uint32_t)(64 * h + 16 * ks) : 128u;
             umma_f16_ts(tmem + O_COL + 128 * h, tmem + P_COL + (DN_KPH / 2) * h + 8 * ks,
-                        umma_desc(smem_u32(sm.vt) + (vcol >> 3) * DN_LBO, DN_LBO, DN_SBO_V), IDESC_O, (it | ks) != 0);
+                        umma_desc(smem_u32(sm.vt[par]) + (vcol >> 3) * DN_LBO, DN_LBO, DN_SBO_V), IDESC_O, (it | ks) != 0);
           }
           umma_commit(&sm.bar_o[h]);
         }
+        umma_commit(&sm.v_free[par]);
       }
     }
   } else {
     // =============================== softmax warps: thread = (query row = TMEM lane, token half) =====================
+    setmaxnreg_inc<DENSE_REGS_SOFTMAX>();
     const int h = warp >> 2, r = (warp & 3) * 32 + lane;
     const uint32_t t_row = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t t_o = t_row + O_COL + 128 * h;
     const uint32_t t_p = t_row + P_COL + (DN_KPH / 2) * h;
-    (void)r;
     for (int it = 0; it < n_my; ++it) {
-      const int st = it & 1;
+      const int st = it % 3;
       const uint32_t par = it & 1;
       mbar_wait(&sm.bar_s, par);
       mbar_wait(&sm.kt_full, par);                       // the producers' aux writes of this chunk are visible
@@ -495,12 +507,31 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       const float2* azm = &sm.aux_zm[st][32 * h];
       const float2 ec = sm.e_chunk[st];
       const float2 beta2 = make_float2(beta, beta), e2 = make_float2(ec.x, ec.x);
-      float mx = -INFINITY;
+      float mxa[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+      {
+        // aux in batches of 8 pairs, the next batch requested before this one is used
+        const float4* as4 = reinterpret_cast<const float4*>(as2);
+        float4 cur[4], nxt[4];
 #pragma unroll
-      for (int k = 0; k < 32; ++k) {
-        v[k] = __ffma2_rn(as2[k], __fadd2_rn(v[k], beta2), e2);        // log2-domain logit of p~ = p 2^E
-        mx = fmaxf(mx, fmaxf(v[k].x, v[k].y));
+        for (int i = 0; i < 4; ++i) cur[i] = as4[i];
+#pragma unroll
+        for (int bq = 0; bq < 4; ++bq) {
+          if (bq < 3) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) nxt[i] = as4[4 * (bq + 1) + i];
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int k = 8 * bq + 2 * i;
+            v[k] = __ffma2_rn(make_float2(cur[i].x, cur[i].y), __fadd2_rn(v[k], beta2), e2);   // log2-domain logit of p~ = p 2^E
+            v[k + 1] = __ffma2_rn(make_float2(cur[i].z, cur[i].w), __fadd2_rn(v[k + 1], beta2), e2);
+            mxa[i] = fmaxf(mxa[i], fmaxf(fmaxf(v[k].x, v[k].y), fmaxf(v[k + 1].x, v[k + 1].y)));
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) cur[i] = nxt[i];
+        }
       }
+      const float mx = fmaxf(fmaxf(mxa[0], mxa[1]), fmaxf(mxa[2], mxa[3]));
       const float m_new = fmaxf(m_ref, mx - P_OFF);
       const float f_old = ex2_approx(m_ref - m_new);     // 0 for the first chunk (m_ref = -inf)
       if (it > 0) {
@@ -547,55 +578,55 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       tc_fence_before();
       mbar_arrive_warp(&sm.p_full[h], lane);
     }
-  }
-  // ---- epilogue, once per token half: O rows -> shared memory (the q tiles are dead: every QK^T has completed),
-  //      inverse Hadamard, partial {m, l, o[128]} per query row into set DENSE_SETS * split + half ----------------------
-  float* stage = reinterpret_cast<float*>(sm.qhi);       // [128][128] fp32 = qhi + qlo
+    // ---- epilogue (softmax warps), once per token half: O rows -> shared memory (the q tiles are dead: every QK^T has
+    //      completed), inverse Hadamard, partial {m, l, o[128]} per query row into set DENSE_SETS * split + half --------
+    float* stage = reinterpret_cast<float*>(sm.qhi);     // [128][128] fp32 = qhi + qlo
 #pragma unroll 1
-  for (int hh = 0; hh < DENSE_SETS; ++hh) {
-    if (warp < 8 && (warp >> 2) == hh) {
-      const int r = (warp & 3) * 32 + lane;
-      if (n_my > 0) {
-        mbar_wait(&sm.bar_o[hh], (n_my - 1) & 1);
-        tc_fence_after();
-        const uint32_t t_o = tmem + ((uint32_t)((warp & 3) * 32) << 16) + O_COL + 128 * hh;
+    for (int hh = 0; hh < DENSE_SETS; ++hh) {
+      if (h == hh) {
+        if (n_my > 0) {
+          mbar_wait(&sm.bar_o[hh], (n_my - 1) & 1);
+          tc_fence_after();
 #pragma unroll 1
-        for (int c0 = 0; c0 < 128; c0 += 16) {
-          uint32_t u[16];
-          tmem_ld16(t_o + c0, u);
+          for (int c0 = 0; c0 < 128; c0 += 16) {
+            uint32_t u[16];
+            tmem_ld16(t_o + c0, u);
 #pragma unroll
-          for (int j = 0; j < 16; j += 4)
-            *reinterpret_cast<uint4*>(&stage[r * 128 + ((c0 + j) ^ ((r & 7) << 2))]) = make_uint4(u[j], u[j + 1], u[j + 2], u[j + 3]);
+            for (int j = 0; j < 16; j += 4)
+              *reinterpret_cast<uint4*>(&stage[r * 128 + ((c0 + j) ^ ((r & 7) << 2))]) = make_uint4(u[j], u[j + 1], u[j + 2], u[j + 3]);
+          }
+        }
+        sm.ml[r] = make_float2(m_ref, l_run);
+        tc_fence_before();
+      }
+      softmax_sync();
+      for (int rr = warp; rr < 128; rr += 8) {
+        const int R = rt * 128 + rr;
+        if (R >= n_rows) break;
+        const int i = R / g, hq = R - i * g;
+        const size_t row = ((size_t)b * A.n_q + i) * A.Hq + hkv * g + hq;
+        float* prow = A.parts + ((size_t)(DENSE_SETS * split + hh) * ((size_t)A.B * A.n_q * A.Hq) + row) * PART_STRIDE;
+        float v[4] = {0.f, 0.f, 0.f, 0.f};
+        if (n_my > 0) {
+          const float4 s4 = *reinterpret_cast<const float4*>(&stage[rr * 128 + ((4 * lane) ^ ((rr & 7) << 2))]);
+          v[0] = s4.x; v[1] = s4.y; v[2] = s4.z; v[3] = s4.w;
+          if (A.rotate_v) {
+            fwht128_lane4(v, lane);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
+          }
+        }
+        *reinterpret_cast<float4*>(prow + 4 + 4 * lane) = make_float4(v[0], v[1], v[2], v[3]);
+        if (lane == 0) {
+          const float2 ml = sm.ml[rr];
+          *reinterpret_cast<float4*>(prow) = make_float4(n_my > 0 ? ml.x : -INFINITY, n_my > 0 ? ml.y : 0.f, 0.f, 0.f);
         }
       }
-      sm.ml[r] = make_float2(m_ref, l_run);
-      tc_fence_before();
+      softmax_sync();
     }
-    __syncthreads();
-    for (int r = warp; r < 128; r += DENSE_THREADS / 32) {
-      const int R = rt * 128 + r;
-      if (R >= n_rows) break;
-      const int i = R / g, h = R - i * g;
-      const size_t row = ((size_t)b * A.n_q + i) * A.Hq + hkv * g + h;
-      float* prow = A.parts + ((size_t)(DENSE_SETS * split + hh) * ((size_t)A.B * A.n_q * A.Hq) + row) * PART_STRIDE;
-      float v[4] = {0.f, 0.f, 0.f, 0.f};
-      if (n_my > 0) {
-        const float4 s4 = *reinterpret_cast<const float4*>(&stage[r * 128 + ((4 * lane) ^ ((r & 7) << 2))]);
-        v[0] = s4.x; v[1] = s4.y; v[2] = s4.z; v[3] = s4.w;
-        if (A.rotate_v) {
-          fwht128_lane4(v, lane);
-#pragma unroll
-          for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
-        }
-      }
-      *reinterpret_cast<float4*>(prow + 4 + 4 * lane) = make_float4(v[0], v[1], v[2], v[3]);
-      if (lane == 0) {
-        const float2 ml = sm.ml[r];
-        *reinterpret_cast<float4*>(prow) = make_float4(n_my > 0 ? ml.x : -INFINITY, n_my > 0 ? ml.y : 0.f, 0.f, 0.f);
-      }
-    }
-    __syncthreads();
   }
+  tc_fence_before();
+  __syncthreads();
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
 }
 
