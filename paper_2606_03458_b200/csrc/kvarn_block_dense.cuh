@@ -126,10 +126,11 @@ struct DenseSmem {
   static constexpr int RB = record_bytes(BITS);
   alignas(1024) uint8_t qhi[128 * DN_KT * 2];      // q' (rotated, scaled), first fp16 term; later: staging of O (with qlo)
   alignas(1024) uint8_t qlo[128 * DN_KT * 2];      // second fp16 term
-  alignas(1024) uint8_t kt[18 * DN_SBO_K];         // rows 0..127: token rho(t); 128, 129: hi / lo of s1 z; 130..143: zero
-  alignas(1024) uint8_t vt[2][16 * DN_SBO_V];      // [chunk parity] rows: channels; columns 0..127 tokens (rho order), 128, 129: s2v, rest zero
+  alignas(128) uint8_t kt[2][18 * DN_SBO_K];       // [chunk parity] rows 0..127: token rho(t); 128, 129: hi / lo of s1 z; 130..143: zero
+  alignas(128) uint8_t vt[16 * DN_SBO_V];          // rows: channels; columns 0..127 tokens (rho order), 128, 129: s2v, rest zero
   alignas(128) uint8_t rec_k[2][RB];               // [chunk parity]
-  alignas(128) uint8_t rec_v[2][RB];
+  alignas(128) uint8_t rec_v[2][RB - 512];         // the codes of the V record
+  alignas(128) uint8_t aux_v[3][512];              // [chunk % 3] its s1 | s2 | z (requested two chunks earlier than the codes)
   alignas(16) __half2 s1h[64];                     // s1 of the K record as fp16 pairs in K-position order
   alignas(16) __half2 s1n[64];                     // the addends -dq_bias s1 of the same pairs
   alignas(16) __half2 fh[2][64];                   // [chunk parity] f_t = s1v[t] 2^-E of the V record, pairs in K-position order
@@ -137,11 +138,13 @@ struct DenseSmem {
   alignas(16) float2 aux_zm[3][64];                //                                         f_t zv[t] of the V record
   alignas(8) float2 e_chunk[3];                    // [chunk % 3] {E, 2^-E}: E = largest binary exponent of the chunk's s1v
   int e_warp[4];
-  alignas(16) float2 ml[128];                      // epilogue: {m, l} of the rows
+  __device__ float2* ml() { return reinterpret_cast<float2*>(rec_k[0]); }   // epilogue: {m, l} of the rows (records are dead)
   alignas(8) uint64_t full_k[2], full_v[2];        // TMA arrival [chunk parity]
+  alignas(8) uint64_t full_va[3];                  // TMA arrival of aux_v [chunk % 3]
   alignas(8) uint64_t bar_s, bar_o[2];             // MMA completion (tcgen05.commit): S ready, O of a token half accumulated
-  alignas(8) uint64_t kt_full, vt_full[2];         // producers -> issuer (and softmax warps: aux), one arrival per warp
-  alignas(8) uint64_t v_free[2];                   // tcgen05.commit: the PV that read vt[parity] has completed
+  alignas(8) uint64_t kt_full[2], vt_full;         // producers -> issuer, one arrival per warp
+  alignas(8) uint64_t aux_full[3];                 // producers -> softmax warps: aux of chunk c in slot c % 3
+  alignas(8) uint64_t k_free[2];                   // tcgen05.commit: the QK^T that read kt[parity] has completed
   alignas(8) uint64_t s_free, p_full[2];           // softmax warps -> issuer (256 / 128 arrivals)
   uint32_t tmem_base;
 };
@@ -260,13 +263,17 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   // ---- setup: barriers, TMEM, first records, q ------------------------------------------------------------------
   if (tid == 256) {
     for (int s = 0; s < 2; ++s) { mbar_init(&sm.full_k[s], 1); mbar_init(&sm.full_v[s], 1); mbar_init(&sm.bar_o[s], 1); mbar_init(&sm.p_full[s], 4);
-                                  mbar_init(&sm.vt_full[s], 8); mbar_init(&sm.v_free[s], 1); }
+                                  mbar_init(&sm.kt_full[s], 8); mbar_init(&sm.k_free[s], 1); }
+    for (int s = 0; s < 3; ++s) { mbar_init(&sm.full_va[s], 1); mbar_init(&sm.aux_full[s], 8); }
     mbar_init(&sm.bar_s, 1);
-    mbar_init(&sm.kt_full, 8); mbar_init(&sm.s_free, 8);                                 // one arrival per warp
+    mbar_init(&sm.vt_full, 8); mbar_init(&sm.s_free, 8);                                 // one arrival per warp
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     for (int c = 0; c < 2 && c < n_my; ++c) {
       mbar_expect_tx(&sm.full_k[c], RB); bulk_g2s(sm.rec_k[c], krec + (size_t)c * RB, RB, &sm.full_k[c]);
-      mbar_expect_tx(&sm.full_v[c], RB); bulk_g2s(sm.rec_v[c], vrec + (size_t)c * RB, RB, &sm.full_v[c]);
+      mbar_expect_tx(&sm.full_v[c], RB - 512); bulk_g2s(sm.rec_v[c], vrec + (size_t)c * RB, RB - 512, &sm.full_v[c]);
+    }
+    for (int c = 0; c < 3 && c < n_my; ++c) {
+      mbar_expect_tx(&sm.full_va[c], 512); bulk_g2s(sm.aux_v[c], vrec + (size_t)c * RB + (RB - 512), 512, &sm.full_va[c]);
     }
   }
   if (warp == 0) {
@@ -339,13 +346,15 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       const int st = c & 1, s3 = c % 3;
       const uint32_t par_rec = (c >> 1) & 1;
       mbar_wait(&sm.full_k[st], par_rec);
-      mbar_wait(&sm.full_v[st], par_rec);
+      mbar_wait(&sm.full_va[s3], (c / 3) & 1);
+      if (c >= 2) mbar_wait(&sm.k_free[st], par_rec ^ 1);  // the QK^T of chunk c - 2 has consumed kt[st]
       const uint8_t* kr = sm.rec_k[st];
-      const uint8_t* vr = sm.rec_v[st];
+      const uint8_t* va = sm.aux_v[s3];                    // s1 at 0, s2 at 128, z at 256
+      uint8_t* kt = sm.kt[st];
       float s1v = 0.f;
       if (pt < 128) {
         // binary exponent of s1v[token]; E = the largest of the chunk (through e_warp)
-        s1v = e4m3_to_f32(vr[s1_off(BITS) + slot_tok]);
+        s1v = e4m3_to_f32(va[slot_tok]);
         const int e = s1v > 0.f ? (int)((__float_as_uint(s1v) >> 23) & 0xFF) - 127 : -64;
         const int em = __reduce_max_sync(0xffffffffu, e);
         if (lane == 0) sm.e_warp[pw] = em;
@@ -357,15 +366,15 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         reinterpret_cast<__half*>(sm.s1n)[n_ax] = __float2half_rn(-dq_bias<BITS>((n_ax >> 1) % PPW) * s1);
         const float sz = s1 * z;
         const __half hi = __float2half_rn(sz), lo = __float2half_rn(sz - __half2float(hi));
-        *reinterpret_cast<__half*>(sm.kt + tile_off(128, n_ax, DN_SBO_K)) = hi;
-        *reinterpret_cast<__half*>(sm.kt + tile_off(129, n_ax, DN_SBO_K)) = lo;
+        *reinterpret_cast<__half*>(kt + tile_off(128, n_ax, DN_SBO_K)) = hi;
+        *reinterpret_cast<__half*>(kt + tile_off(129, n_ax, DN_SBO_K)) = lo;
       }
       producer_sync();                                   // s1h, s1n, e_warp complete
       if (pt < 128) {
         const int E = max(max(sm.e_warp[0], sm.e_warp[1]), max(sm.e_warp[2], sm.e_warp[3]));
         const float two_mE = __uint_as_float((uint32_t)(127 - max(E, -64)) << 23);        // 2^-E
         const float f = s1v * two_mE;                    // in [0, 2): the V tile carries s2v f, the logits carry E
-        const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(vr + z_off(BITS))[slot_tok]);
+        const float zv = f16_bits_to_f32(reinterpret_cast<const uint16_t*>(va + 256)[slot_tok]);
         reinterpret_cast<__half*>(sm.fh[st])[n_ax] = __float2half_rn(f);
         reinterpret_cast<float*>(&sm.aux_s2[s3][n_ax >> 1])[n_ax & 1] = e4m3_to_f32(kr[s2_off(BITS) + slot_tok]);
         reinterpret_cast<float*>(&sm.aux_zm[s3][n_ax >> 1])[n_ax & 1] = f * zv;
@@ -388,10 +397,11 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i) W[i] = *reinterpret_cast<const uint32_t*>(kr + L.word_off(pw, i));
 #pragma unroll
         for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i)
-          dequant_word<BITS, true>(W[i], sK, aK, __half2(), nsc0, sm.kt + krow_off[i]);
+          dequant_word<BITS, true>(W[i], sK, aK, __half2(), nsc0, kt + krow_off[i]);
       }
       fence_async_smem();
-      mbar_arrive_warp(&sm.kt_full, lane);
+      __syncwarp();
+      if (lane == 0) { mbar_arrive(&sm.kt_full[st]); mbar_arrive(&sm.aux_full[s3]); }
       producer_sync();                                   // every producer has left rec_k[st], s1h, s1n, e_warp
       if (pt == 0 && c + 2 < n_my) {
         mbar_expect_tx(&sm.full_k[st], RB); bulk_g2s(sm.rec_k[st], krec + (size_t)(c + 2) * RB, RB, &sm.full_k[st]);
@@ -401,16 +411,13 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
     for (int it = 0; it < n_my; ++it) {
       const int st = it & 1;
       const uint32_t par = it & 1;
-      if (it + 1 < n_my) {                               // K of the NEXT chunk first: its QK^T overlaps this chunk's softmax
-        mbar_wait(&sm.bar_s, par);                       // QK^T of this chunk has consumed Kt
-        mbar_wait(&sm.s_free, par);                      // (*) the softmax warps have looked at kt_full of this chunk
-        expand_k(it + 1);
-      }
+      if (it + 1 < n_my) expand_k(it + 1);               // K of the NEXT chunk first: its QK^T overlaps this chunk's softmax
       mbar_wait(&sm.full_v[st], (it >> 1) & 1);
-      if (it >= 2) mbar_wait(&sm.v_free[st], ((it >> 1) & 1) ^ 1);   // the PV of chunk it - 2 has consumed vt[st]
+      if (it > 0) mbar_wait(&sm.bar_o[1], par ^ 1);      // PV of chunk it - 1 complete: Vt is free, softmax of it - 1 is over
       {
-        uint8_t* vt = sm.vt[st];
+        uint8_t* vt = sm.vt;
         const uint8_t* vr = sm.rec_v[st];
+        const uint8_t* va = sm.aux_v[it % 3];
         __half2 fV[PPW];
 #pragma unroll
         for (int j = 0; j < PPW; j += 4) {
@@ -423,27 +430,31 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i) W[i] = *reinterpret_cast<const uint32_t*>(vr + L.word_off(pw, i));
 #pragma unroll
         for (int i = 0; i < ProducerLane<BITS>::ITERS; ++i) {
-          const __half2 sc = __float2half2_rn(e4m3_to_f32(vr[s2_off(BITS) + L.slot(pw, i)]));   // s2v of the row's channel
+          const __half2 sc = __float2half2_rn(e4m3_to_f32(va[128 + L.slot(pw, i)]));   // s2v of the row's channel
           __half2 nsc[3];
 #pragma unroll
           for (int k = 0; k < 3; ++k) nsc[k] = __hmul2(sc, __float2half2_rn(-dq_bias<BITS>(k)));
           dequant_word<BITS, false>(W[i], fV, fV, sc, nsc, vt + vrow_off[i]);
         }
         if (pt < 128)                                    // K columns 128, 129 of channel row pt: s2v (zero-point term)
-          *reinterpret_cast<__half2*>(vt + tile_off(pt, 128, DN_SBO_V)) = __float2half2_rn(e4m3_to_f32(vr[s2_off(BITS) + pt]));
+          *reinterpret_cast<__half2*>(vt + tile_off(pt, 128, DN_SBO_V)) = __float2half2_rn(e4m3_to_f32(va[128 + pt]));
       }
       fence_async_smem();
-      mbar_arrive_warp(&sm.vt_full[st], lane);
-      producer_sync();                                   // every producer has left rec_v[st]
+      mbar_arrive_warp(&sm.vt_full, lane);
+      producer_sync();                                   // every producer has left rec_v[st] and aux_v[it % 3]
       if (pt == 0 && it + 2 < n_my) {
-        mbar_expect_tx(&sm.full_v[st], RB); bulk_g2s(sm.rec_v[st], vrec + (size_t)(it + 2) * RB, RB, &sm.full_v[st]);
+        mbar_expect_tx(&sm.full_v[st], RB - 512); bulk_g2s(sm.rec_v[st], vrec + (size_t)(it + 2) * RB, RB - 512, &sm.full_v[st]);
+      }
+      if (pt == 0 && it + 3 < n_my) {
+        mbar_expect_tx(&sm.full_va[it % 3], 512);
+        bulk_g2s(sm.aux_v[it % 3], vrec + (size_t)(it + 3) * RB + (RB - 512), 512, &sm.full_va[it % 3]);
       }
     }
   } else if (warp >= 16) {
     // =============================== MMA issuer: one thread =========================================================
     if (warp == 16 && lane == 0) {
       auto issue_qk = [&](int c) {
-        mbar_wait(&sm.kt_full, c & 1);
+        mbar_wait(&sm.kt_full[c & 1], (c >> 1) & 1);
         if (c > 0) mbar_wait(&sm.s_free, (c & 1) ^ 1);    // the softmax warps have read S of the previous chunk
         tc_fence_after();
 #pragma unroll
@@ -451,14 +462,15 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
 #pragma unroll
           for (int ks = 0; ks < DN_KT / 16; ++ks)
             umma_f16(tmem, umma_desc(smem_u32(term ? sm.qlo : sm.qhi) + ks * 256, 128, SBO_T),
-                     umma_desc(smem_u32(sm.kt) + ks * 2 * DN_LBO, DN_LBO, DN_SBO_K), IDESC_S, (term | ks) != 0);
+                     umma_desc(smem_u32(sm.kt[c & 1]) + ks * 2 * DN_LBO, DN_LBO, DN_SBO_K), IDESC_S, (term | ks) != 0);
         umma_commit(&sm.bar_s);
+        umma_commit(&sm.k_free[c & 1]);
       };
       if (n_my > 0) issue_qk(0);
       for (int it = 0; it < n_my; ++it) {
         const uint32_t par = it & 1;
         if (it + 1 < n_my) issue_qk(it + 1);              // runs while the softmax warps work on chunk it
-        mbar_wait(&sm.vt_full[par], (it >> 1) & 1);
+        mbar_wait(&sm.vt_full, par);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           mbar_wait(&sm.p_full[h], par);
@@ -467,11 +479,10 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           for (int ks = 0; ks < DN_KPH / 16; ++ks) {      // 4 steps over the half's 64 tokens + 1 over the zero-point columns
             const uint32_t vcol = ks < 4 ? (uint32_t)(64 * h + 16 * ks) : 128u;
             umma_f16_ts(tmem + O_COL + 128 * h, tmem + P_COL + (DN_KPH / 2) * h + 8 * ks,
-                        umma_desc(smem_u32(sm.vt[par]) + (vcol >> 3) * DN_LBO, DN_LBO, DN_SBO_V), IDESC_O, (it | ks) != 0);
+                        umma_desc(smem_u32(sm.vt) + (vcol >> 3) * DN_LBO, DN_LBO, DN_SBO_V), IDESC_O, (it | ks) != 0);
           }
           umma_commit(&sm.bar_o[h]);
         }
-        umma_commit(&sm.v_free[par]);
       }
     }
   } else {
@@ -485,7 +496,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       const int st = it % 3;
       const uint32_t par = it & 1;
       mbar_wait(&sm.bar_s, par);
-      mbar_wait(&sm.kt_full, par);                       // the producers' aux writes of this chunk are visible
+      mbar_wait(&sm.aux_full[st], (it / 3) & 1);         // the producers' aux writes of this chunk are visible
       tc_fence_after();
       float2 v[32];                                      // logits of the half's 64 tokens, as token pairs
       float beta;
@@ -596,7 +607,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
               *reinterpret_cast<uint4*>(&stage[r * 128 + ((c0 + j) ^ ((r & 7) << 2))]) = make_uint4(u[j], u[j + 1], u[j + 2], u[j + 3]);
           }
         }
-        sm.ml[r] = make_float2(m_ref, l_run);
+        sm.ml()[r] = make_float2(m_ref, l_run);
         tc_fence_before();
       }
       softmax_sync();
@@ -618,7 +629,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         }
         *reinterpret_cast<float4*>(prow + 4 + 4 * lane) = make_float4(v[0], v[1], v[2], v[3]);
         if (lane == 0) {
-          const float2 ml = sm.ml[rr];
+          const float2 ml = sm.ml()[rr];
           *reinterpret_cast<float4*>(prow) = make_float4(n_my > 0 ? ml.x : -INFINITY, n_my > 0 ? ml.y : 0.f, 0.f, 0.f);
         }
       }
