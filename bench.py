@@ -56,6 +56,16 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def tensor_peak():
+    """Dense bf16 / fp16 tensor throughput in TFLOP/s: the measured burst figure, else the guide's nominal 2250."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        if d.get("bf16_tflops"):
+            return float(d["bf16_tflops"]), "measured burst (MEASURED_PEAKS.json bf16_tflops; fp16 = bf16 rate)"
+    return 2250.0, "fallback (nominal dense bf16, B200_PROFILING.md)"
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
 
@@ -312,8 +322,11 @@ def run_extras(kv, W, dev, hbm_peak, only=frozenset()):
                         torch.cuda.synchronize()
                         medd, _ = _time_launches(lambda i: kv.block_attention(p, cache, qb, kb, vb, out=ob, dense=True, ws=wsd), 5, stream)
                         flop = 4.0 * sh.B * sh.Hq * n_q * sh.ctx * D                      # QK^T + PV, 2 flop per MAC
+                        tf = flop / (medd * 1e-3) / 1e12
                         ex[f"block_dense_long_g4_2bit_nq{n_q}"] = {"us": medd * 1e3, "us_per_query_token": medd * 1e3 / n_q, "x_decode": medd / med,
-                                                                   "TFLOPs": flop / (medd * 1e-3) / 1e12}
+                                                                   "TFLOPs": tf, "tensor_frac": tf / tensor_peak()[0],
+                                                                   "note": "whole call: block_dense_kernel + raw-window decode + merge; "
+                                                                           "flop = 4 B Hq n_q ctx 128 (the hi / lo q terms are not counted twice)"}
                         del qb, kb, vb, ob, wsd
                 del cache, q, ws, out
                 torch.cuda.empty_cache()
@@ -715,6 +728,9 @@ def main():
             "cfg4_2bit_frac": frac("decode_cfg4_2bit"), "cfg4_4bit_frac": frac("decode_cfg4_4bit"),
             "long_g4_2bit_frac": frac("decode_long_g4_2bit"), "long_g4_4bit_frac": frac("decode_long_g4_4bit"),
             "quantize_alu_frac": q_tflops / FP32_PEAK_TFLOPS_NOMINAL, "quantize_hbm_frac": q_gbs / hbm_peak,
+            "block_dense_nq32_us_per_token": (ex.get("block_dense_long_g4_2bit_nq32") or {}).get("us_per_query_token"),
+            "block_dense_nq32_tensor_frac": (ex.get("block_dense_long_g4_2bit_nq32") or {}).get("tensor_frac"),
+            "block_int_nq8_us_per_token": (ex.get("block_long_g4_2bit_nq8") or {}).get("us_per_query_token"),
             "target": "north_star: decode >= 0.70 of HBM on every config, quantize >= 0.60 of HBM (ALU-bound: DESIGN 6.1)"}
     rl_dec = {"kernel": "decode_kernel<2,4,2,bf16> (configs[1])", "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak,
               "unit": "GB/s", "frac": dec_gbs / hbm_peak, "traffic": tr.get("decode_kernel"),
@@ -726,6 +742,11 @@ def main():
                 "traffic": tr.get("quantize_kernel"), "algorithmic_bytes": q_bytes,
                 "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "hbm_achieved_GBps": q_gbs, "hbm_frac": q_gbs / hbm_peak, "ms": q_ms}
+    dn = ex.get("block_dense_long_g4_2bit_nq128") or {}
+    tp, tp_src = tensor_peak()
+    rl_dense = {"kernel": "block_dense_kernel<2,bf16> (+ raw-window decode + merge), B16 32/8 ctx 65536, n_q = 128", "bound": "tensor",
+                "achieved": dn.get("TFLOPs"), "peak": tp, "unit": "TFLOP/s", "frac": dn.get("tensor_frac"), "traffic": None,
+                "peak_source": tp_src, "us": dn.get("us")} if dn else None
     line = {
         "metric": "kvarn_2bit_decode_attn_GBps", "value": world * dec_gbs, "unit": "GB/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
@@ -733,7 +754,7 @@ def main():
         "config": workload_config(shape, L),
         "decode_us_per_step": d_ms * 1e3, "quantize_ms_per_step": q_ms,
         "quantize_tokens_per_s": world * tok_s, "quantize_tiles_per_s": world * 2 * n_tiles / (q_ms * 1e-3),
-        "extras": extras, "rooflines": {"quantize": rl_quant},
+        "extras": extras, "rooflines": {"quantize": rl_quant, "block_dense": rl_dense},
         "roofline": rl_dec, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": 2 * args.steps, "clocks": clocks,
         "headline": {k: v for k, v in also.items() if k != "target"} | {"cfg1_decode_frac": dec_gbs / hbm_peak, "cfg1_decode_us": d_ms * 1e3},
     }
