@@ -13,9 +13,9 @@
  * without ever materialising a dequantised cache.
  *
  * Entry points: kvarn_quantize_chunk / kvarn_prefill (bulk write path), kvarn_append / kvarn_append_block
- * (on-the-fly compression while decoding), kvarn_decode_attention (read path), kvarn_block_attention (a block of
- * new tokens against the cache, Fig. 4), kvarn_decode_attention_partial + kvarn_merge_partials (a sequence
- * spread over several caches / GPUs), kvarn_rope_hadamard / kvarn_hadamard_rows / kvarn_hadamard_row_groups (the
+ * (on-the-fly compression while decoding), kvarn_decode_attention (read path), kvarn_block_attention /
+ * kvarn_block_attention_dense (a block of new tokens against the cache, Fig. 4),
+ * kvarn_decode_attention_partial + kvarn_merge_partials (a sequence spread over several caches / GPUs), kvarn_rope_hadamard / kvarn_hadamard_rows / kvarn_hadamard_row_groups (the
  * Hadamard arrangement of App. A), the *_host forms, layout queries and the record pack / unpack test hooks.
  *
  * Conventions
@@ -291,7 +291,13 @@ KVARN_API int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* ca
  * (code x scale is exact in fp16) and the block's 128-row tiles of (query token, head) pairs run S = Q K^T and
  * O += P V as M = 128 MMAs; the raw windows go through the decode kernel and the pieces are LSE-merged.  The right
  * form for blocks with >= ~32 (token, head) rows per KV head (blocks of b tokens); kvarn_block_attention is the
- * right one for a few speculative tokens.  ws: DEVICE scratch of >= kvarn_block_dense_workspace_bytes(...) bytes.
+ * right one for a few speculative tokens.  ws: DEVICE scratch of >= kvarn_block_dense_workspace_bytes(...) bytes
+ * (16-byte aligned; owned by the caller, may be reused by the next call on the same stream).
+ * Precision: the query enters as two fp16 terms (22 bits), the tiles are exact (the V row scale s1v[t] enters as its
+ * exact mantissa part in the tile and a per-chunk power of two in the logits; a token whose s1v is more than 2^9 below
+ * the largest of its chunk loses low bits), probabilities are fp16 relative to 2^8 times the running row maximum, with
+ * numerator and denominator from the same rounded values; accumulation in fp32.  Same tolerance as
+ * kvarn_block_attention (2e-3 of the output scale).  Errors: as kvarn_block_attention, + KVARN_WORKSPACE_TOO_SMALL.
  */
 KVARN_API size_t kvarn_block_dense_workspace_bytes(const kvarn_params* p, int32_t B, int32_t Hq, int32_t Hkv, int32_t n_q,
                                          int32_t max_chunks);
