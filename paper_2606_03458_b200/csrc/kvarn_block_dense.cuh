@@ -3,19 +3,21 @@
 // for blocks with many (query token, head) rows per KV head; the raw windows (sink, residual, the block's own causal
 // tokens) are left to decode_kernel_w (skip_chunks = 1, partial = 1) and everything is merged by merge_partials_kernel.
 //
-// One CTA = one (sequence, KV head), one tile of 128 query rows r = (token i, head h), one range of chunks; 9 warps in
-// three roles that meet only through mbarriers: warps 4-7 expand the records (producers), one thread of warp 8 issues
-// the MMAs, warps 0-3 own the softmax (thread = query row = TMEM lane).  While the softmax warps work on chunk i the
-// producers already expand V of chunk i and K of chunk i + 1 and the tensor core runs QK^T of chunk i + 1.  Per chunk:
-//   K record --TMA--> shared memory --128 threads--> Kt = code x s1[c] as fp16 (EXACT: a 2-/4-bit code times an E4M3
+// One CTA = one (sequence, KV head), one tile of 128 query rows r = (token i, head h), one range of chunks; three roles
+// that meet only through mbarriers: warps 8-15 expand the records (producers), one thread of warp 16 issues the MMAs,
+// warps 0-7 own the softmax (thread = (query row = TMEM lane, token half)).  Per chunk:
+//   K record --TMA--> shared memory --producers--> Kt = code x s1[c] as fp16 (EXACT: a 2-/4-bit code times an E4M3
 //     scale has <= 8 significant bits), K-major UMMA tile [token][channel], + two rows hi / lo of (s1 z)[c] for beta
 //   S[r][t] = sum_c (q'_hi + q'_lo)[r][c] Kt[t][c]          tcgen05.mma kind::f16, M = 128, N = 144, K = 128, twice (hi, lo)
-//   logit = s2[t] (S + beta_r) + log2 s1v[t];  online softmax per ROW inside one thread (TMEM lane = row)
-//   Pt = p~ as fp16 (+ hi / lo of the zero-point sum as two extra K columns)
-//   V record --> Vt = codeV x s2v[c] as fp16 (exact), [channel][token] (+ s2v[c] in the two extra K columns)
-//   O[r][c] += sum_t Pt[r][t] Vt[c][t]                      tcgen05.mma, M = 128, N = 128, K = 144, accumulator in TMEM
-// The accumulator is rescaled in TMEM (tcgen05.ld / st) only when a row's maximum rises.  Finally O is un-rotated
-// (inverse Hadamard) and written as the partial {m, l, o[128]} of its rows.
+//   logit = s2[t] (S + beta_r) + E;  online softmax per (row, token half) inside one thread; the two halves are
+//     independent streams (own reference exponent, l, accumulator) and leave two partial sets
+//   p~ = 2^(logit - m + 8) as fp16 pairs, written to tensor memory (+ hi / lo of the zero-point sum as two extra K columns)
+//   V record --> Vt = (codeV x s2v[c]) x f_t as fp16 (exact; f_t = s1v[t] 2^-E, E = largest s1v exponent of the chunk),
+//     [channel][token] (+ s2v[c] in the extra K columns)
+//   O_h[r][c] += sum_t p~[r][t] Vt[c][t]                    tcgen05.mma, A from tensor memory, M = 128, N = 128, K = 80
+// The accumulators are rescaled in TMEM (tcgen05.ld / st) only when a row's maximum rises.  Finally each O_h is
+// un-rotated (inverse Hadamard) and written as the partial {m, l, o[128]} of its rows.  While the softmax warps work on
+// chunk i the producers expand K of chunk i + 1 (second Kt buffer) and V of chunk i, and QK^T of chunk i + 1 runs.
 //
 // Precision: q' enters as two fp16 terms (22 bits), codes x scales exactly, beta through the same MMA; p~ is fp16
 // relative to 2^-8 of the row's running maximum (so probabilities down to 2^-32 of it survive) and l is accumulated
@@ -546,7 +548,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       const float m_new = fmaxf(m_ref, mx - P_OFF);
       const float f_old = ex2_approx(m_ref - m_new);     // 0 for the first chunk (m_ref = -inf)
       if (it > 0) {
-        mbar_wait(&sm.bar_o[h], par ^ 1);                // PV of the previous chunk is complete: Pt is free, O is consistent
+        mbar_wait(&sm.bar_o[h], par ^ 1);                // PV of the previous chunk is complete: p~ of it may be overwritten, O is consistent
         tc_fence_after();
         if (__any_sync(0xffffffffu, m_new > m_ref)) {    // some row of the warp rises: rescale the accumulator rows in TMEM
 #pragma unroll 1
