@@ -329,10 +329,14 @@ static cudaError_t launch_decode_k(DK, const DecodeArgs& A, cudaStream_t st) {
   cfg.blockDim = dim3(128, 1, 1);
   cfg.dynamicSmemBytes = DK::smem;
   cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = 1; attr[0].val.clusterDim.y = (unsigned)A.cluster; attr[0].val.clusterDim.z = 1;
-  cfg.attrs = attr; cfg.numAttrs = A.cluster > 1 ? 1 : 0;
+  // attr[0]: programmatic dependent launch (the kernel waits with griddepcontrol.wait before its first global access:
+  // launch latency and CTA scheduling overlap the tail of the previous kernel of the stream); attr[1]: the cluster
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[1].id = cudaLaunchAttributeClusterDimension;
+  attr[1].val.clusterDim.x = 1; attr[1].val.clusterDim.y = (unsigned)A.cluster; attr[1].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = A.cluster > 1 ? 2 : 1;
   return cudaLaunchKernelEx(&cfg, kern, A);
 }
 

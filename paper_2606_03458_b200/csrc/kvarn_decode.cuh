@@ -706,6 +706,13 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
   const int fg = lane >> 2, ft = lane & 3;
   const int g = A.g;
   WS& ws = sm.w[warp];
+  // Programmatic dependent launch (the launch carries cudaLaunchAttributeProgrammaticStreamSerialization): the next
+  // kernel of the stream may be made resident as soon as every CTA of this grid has started, and this grid's CTAs may
+  // have become resident while the previous kernel was still running -- nothing of global memory is touched before
+  // the wait (seq_lens, records, q, out, workspace and ticket all belong to earlier kernels until then).  Both
+  // instructions are no-ops in a launch without the attribute.
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 
   const Where w0 = where_am_i<false>(A);
   const ColMap cm0 = col_map<false>(A);
