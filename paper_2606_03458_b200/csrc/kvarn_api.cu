@@ -227,7 +227,10 @@ struct SplitPlan { int cluster, nclus; };
 #ifndef KVARN_SPLIT_FEW_SLOTS
 #define KVARN_SPLIT_FEW_SLOTS 2
 #endif
-constexpr int KVARN_MAX_CLUSTER = 8;    // portable maximum; 9..16 (non-portable) measured slower: 25 -> 27..31 us on config 1
+#ifndef KVARN_MAX_CLUSTER_OVERRIDE
+#define KVARN_MAX_CLUSTER_OVERRIDE 8
+#endif
+constexpr int KVARN_MAX_CLUSTER = KVARN_MAX_CLUSTER_OVERRIDE;    // portable maximum; 9..16 (non-portable) measured slower: 25 -> 27..31 us on config 1
 
 // DQ, DP = digit planes of q~ / p~ (kvarn_decode.cuh)
 template <int BITS, int GP, int DQ, int DP, typename InT>
@@ -302,6 +305,9 @@ static SplitPlan split_plan(const kvarn_params* p, int B, int Hkv, int g, int ma
   if (want < 1) want = 1;
   if (want > max_chunks) want = max_chunks;
   sp.cluster = want < KVARN_MAX_CLUSTER ? want : KVARN_MAX_CLUSTER;
+  // at least one chunk per warp of every CTA: below that the cluster's launch and merge cost more than they spread
+  // (B = 8, 8 KV heads, 1024 tokens: 11.2 us with 8 CTAs per unit, 8.6 with 2)
+  if (sp.cluster > 1 && max_chunks < 4 * sp.cluster) sp.cluster = max_chunks >= 8 ? max_chunks / 4 : 1;
   // about one CTA per slot and long CTAs: halve them, so that the CTAs of the second half-wave balance the SMs that
   // got one CTA more (config 4, 512 units on 444 slots: 1 / 2 / 3 / 4 / 6 CTAs per unit measured in DESIGN.md 6.2)
   if (sp.cluster == 1 && max_chunks >= 32) sp.cluster = KVARN_SPLIT_FEW_SLOTS;

@@ -494,10 +494,18 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
     const uint32_t t_row = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t t_o = t_row + O_COL + 128 * h;
     const uint32_t t_p = t_row + P_COL + (DN_KPH / 2) * h;
+    // a warp whose 32 rows lie beyond the block's rows only keeps the barriers moving (its rows of P and O are never read)
+    const bool live = rt * 128 + (warp & 3) * 32 < n_rows;
     for (int it = 0; it < n_my; ++it) {
       const int st = it % 3;
       const uint32_t par = it & 1;
       mbar_wait(&sm.bar_s, par);
+      if (!live) {
+        mbar_arrive_warp(&sm.s_free, lane);
+        if (it > 0) mbar_wait(&sm.bar_o[h], par ^ 1);
+        mbar_arrive_warp(&sm.p_full[h], lane);
+        continue;
+      }
       mbar_wait(&sm.aux_full[st], (it / 3) & 1);         // the producers' aux writes of this chunk are visible
       tc_fence_after();
       float2 v[32];                                      // logits of the half's 64 tokens, as token pairs
