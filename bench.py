@@ -237,9 +237,10 @@ def workload_config(shape, layers):
     return {"workload": "BASELINE.json configs[1]: Llama-3.1-8B-shaped decode layer",
             "B": shape.B, "Hq": shape.Hq, "Hkv": shape.Hkv, "head_dim": D, "ctx": shape.ctx,
             "chunks": shape.n_chunks, "resid": shape.resid, "bits": shape.bits,
-            "step": "kvarn_quantize_chunk(2x%d tiles) + kvarn_decode_attention" % (shape.B * shape.Hkv * shape.n_chunks),
-            "l2": "inputs larger than L2: %d rotating layer copies, decode reads the cache written %d steps earlier"
-                  % (layers, layers // 2),
+            "step": "kvarn_quantize_chunk(2x%d tiles) of one layer + kvarn_decode_attention of all %d layers (one launch per layer)"
+                    % (shape.B * shape.Hkv * shape.n_chunks, layers),
+            "l2": "inputs larger than L2: %d layer caches read in rotation (%d MB of records per step)"
+                  % (layers, layers * 2 * shape.B * shape.Hkv * shape.n_chunks * 4608 // 1000000),
             "parallelism": "replicas"}
 
 
@@ -630,12 +631,16 @@ def main():
     stream = torch.cuda.current_stream()
 
     def step(i, ev=None):
-        lq, ld = i % L, (i + L // 2) % L
+        # one layer's context quantised (write path), then the decode attention of every layer of an L-layer model
+        # (read path: one launch per layer, each over its own cache -- L x 37.9 MB of records, larger than L2)
+        lq = i % L
         c = caches[lq]
         if ev: ev[0].record(stream)
         kv.quantize_chunk(p, Ks[lq], Vs[lq], c.k_records.view(n_tiles, rb), c.v_records.view(n_tiles, rb))
         if ev: ev[1].record(stream)
-        kv.decode_attention(p, caches[ld], qs[ld], out=out, ws=ws)
+        for l in range(L):
+            ld = (lq + 1 + l) % L
+            kv.decode_attention(p, caches[ld], qs[ld], out=out, ws=ws)
         if ev: ev[2].record(stream)
 
     for l in range(L):   # fill every cache once (untimed) so decode always reads real records
@@ -657,12 +662,13 @@ def main():
     if dist: dist.barrier()
     total_ms = t0.elapsed_time(t1)
     q_ms = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
-    d_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
+    d_ms = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps / L       # per decode launch: L launches between the two events
+    d1_ms, _ = _time_launches(lambda i: kv.decode_attention(p, caches[i % L], qs[i % L], out=out, ws=ws), 16, stream)  # one launch per event pair
     # the decode launch alone, back to back over the rotating caches (3 x L launches = 24 at the default, 906 MB of
     # records > L2) inside one CUDA graph: no event pair, no host launch gap (SURVEY 8(d) "Timing")
     dg_ms = _time_graph([(lambda l=l: kv.decode_attention(p, caches[l % L], qs[l % L], out=out, ws=ws)) for l in range(3 * L)], stream)
     clocks = sampler.stop() if sampler else None
-    total_ms, q_ms, d_ms, dg_ms = max_over_ranks([total_ms, q_ms, d_ms, dg_ms], dist, dev)
+    total_ms, q_ms, d_ms, dg_ms, d1_ms = max_over_ranks([total_ms, q_ms, d_ms, dg_ms, d1_ms], dist, dev)
 
     # ---- algorithmic bytes --------------------------------------
     dec_bytes = BH * shape.n_chunks * 2 * rb + shape.B * shape.Hq * (D * 2 + D * 4)
@@ -724,6 +730,7 @@ def main():
     # the metric's kernel is the decode kernel: its roofline is `roofline`; the other kernels' fractions ride inside it
     # (the driver's record keeps the contract keys only) and, once more, at the very end of the line
     also = {"cfg1_decode_graph_frac": dec_gbs_graph / hbm_peak, "cfg1_decode_graph_us": dg_ms * 1e3,
+            "cfg1_decode_single_launch_us": d1_ms * 1e3,
             "cfg2_ctx32k_decode_frac": (ex.get("cfg2_incremental") or {}).get("decode_hbm_frac"),
             "cfg4_2bit_frac": frac("decode_cfg4_2bit"), "cfg4_4bit_frac": frac("decode_cfg4_4bit"),
             "long_g4_2bit_frac": frac("decode_long_g4_2bit"), "long_g4_4bit_frac": frac("decode_long_g4_4bit"),
@@ -735,7 +742,8 @@ def main():
     rl_dec = {"kernel": "decode_kernel<2,4,2,bf16> (configs[1])", "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak,
               "unit": "GB/s", "frac": dec_gbs / hbm_peak, "traffic": tr.get("decode_kernel"),
               "algorithmic_bytes": dec_bytes, "peak_source": peak_src, "us": d_ms * 1e3,
-              "timing": "CUDA events around each launch inside the step; also.cfg1_decode_graph_*: 24 launches in one CUDA graph",
+              "timing": "CUDA events around the step's L decode launches, divided by L; also.cfg1_decode_single_launch_us: one launch "
+                        "per event pair; also.cfg1_decode_graph_*: 24 launches in one CUDA graph",
               "also": also}
     rl_quant = {"kernel": "quantize_kernel<2,bf16>", "bound": "alu", "achieved": q_tflops,
                 "peak": FP32_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s", "frac": q_tflops / FP32_PEAK_TFLOPS_NOMINAL,
@@ -755,7 +763,7 @@ def main():
         "decode_us_per_step": d_ms * 1e3, "quantize_ms_per_step": q_ms,
         "quantize_tokens_per_s": world * tok_s, "quantize_tiles_per_s": world * 2 * n_tiles / (q_ms * 1e-3),
         "extras": extras, "rooflines": {"quantize": rl_quant, "block_dense": rl_dense},
-        "roofline": rl_dec, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": 2 * args.steps, "clocks": clocks,
+        "roofline": rl_dec, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": (1 + L) * args.steps, "clocks": clocks,
         "headline": {k: v for k, v in also.items() if k != "target"} | {"cfg1_decode_frac": dec_gbs / hbm_peak, "cfg1_decode_us": d_ms * 1e3},
     }
     print(json.dumps(compact(line)))
