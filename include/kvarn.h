@@ -239,12 +239,14 @@ KVARN_API int kvarn_append_block(const kvarn_params* p, const kvarn_cache* cache
  *   q    DEVICE [B][Hq][128] in_dtype          out  DEVICE [B][Hq][128] out_dtype
  *   ws   DEVICE scratch of >= kvarn_decode_workspace_bytes(...) bytes, 16-B aligned
  * A sequence of length 0 yields zeros.  Hq/Hkv must be in 1..8.
- * Precision: fp32 accumulation; the folded query and the probabilities enter the tensor cores as 22-bit
- * fixed-point numbers, the query relative to max_c |q~[h, c]| of its chunk, a probability relative to the largest
- * probability of the tokens that share its loop iteration (<= 256 tokens at 2-bit, <= 128 at 4-bit).  A token is
- * therefore rounded to zero only if it lies more than 2^-23 below one of its <= 255 neighbours -- a bound that does
- * not grow with the context length; numerator and denominator of the softmax use the same rounded values.  Raw
- * (sink / residual / block) tokens are handled in fp32.
+ * Precision: fp32 accumulation; the folded query and the weights pt = p[t] s1v[t] (probability times the V record's row
+ * scale) enter the tensor cores as fixed-point numbers (kvarn_params::decode_digits: 22 / 16 bits by default), the query
+ * relative to max_c |q~[h, c]| of its chunk, a weight relative to the largest weight of its own chunk (128 tokens).  A
+ * token's VALUE contribution is therefore rounded to zero only if pt lies more than 2^-17 (2^-23 with decode_digits = 4)
+ * below the largest of its 127 neighbours -- a bound that does not grow with the context length -- while the
+ * denominator takes the exact p, so a token with a tiny V row keeps its probability mass; numerator and denominator
+ * differ by at most half a fixed-point unit per token (random sign; worst case 128 x 2^-17 of the chunk's largest
+ * weight).  Raw (sink / residual / block) tokens are handled in fp32.
  */
 KVARN_API int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
                            int32_t Hq, float sm_scale, void* out, void* ws, size_t ws_bytes,

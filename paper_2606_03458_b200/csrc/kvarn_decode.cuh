@@ -610,7 +610,7 @@ struct WarpSm {
   alignas(128) uint8_t vrec[RB];
   alignas(16) uint32_t bfr[NT][2][32][4];      // B fragments: first of q~ (QK^T), then -- reused -- of p~ (value contraction)
   alignas(16) float2 aux_a[128];               // per K row slot: {s2, log2 s1v}
-  alignas(16) float2 aux_b[128];               //                 {1 / (s1v P_FIX), zv}
+  alignas(16) float2 aux_b[128];               //                 {1 / s1v, zv}
   alignas(8) __half aux_ch[4][8][4];           // per channel: s2v, [mp][fg][i] of channel slot 32 mp + 16 (i >> 1) + 8 (i & 1) + fg
   alignas(8) float2 hs[GP];                    // per column: {scale, beta}
   alignas(8) uint64_t fullk, fullv;
@@ -875,7 +875,7 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
         const float s = fmaxf(s1v[j], 9.094947e-13f);   // 2^-40: a zero scale stays harmless
         // pt = p s1v = exp2(logit + log2 s1v - m): the maximum is taken over the shifted logits, so pt <= 1
         ws.aux_a[4 * lane + j].y = lg2_approx(s);
-        ws.aux_b[4 * lane + j] = make_float2(rcp_approx(s) * (1.f / PF), zv[j]);
+        ws.aux_b[4 * lane + j] = make_float2(rcp_approx(s), zv[j]);
       }
       {   // s2v of channels 4 lane + j (exact in fp16): channel slot c -> [c >> 5][c & 7][(c >> 3) & 3]
         uint32_t h2[2];
@@ -906,7 +906,11 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
       mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 16));
       // The fixed-point probabilities refer to the maximum mx of THIS chunk: a token is dropped only if it lies
       // below the resolution relative to the largest of its 127 neighbours, whatever the context length; the chunk's
-      // sums enter the running ones with the weight wch = 2^(mx - m_new).  l uses the same rounded values as the numerator.
+      // sums enter the running ones with the weight wch = 2^(mx - m_new).  What is rounded is pt = p s1v (probability times
+      // the value row scale): the numerator (codes and zero-point sum) uses the rounded pt, the denominator l the EXACT
+      // p = pt / s1v -- a token whose V row is tiny against its neighbours' keeps its probability mass in l (its value
+      // contribution is below the resolution by construction); numerator and denominator differ by <= 1/2 unit of the
+      // fixed point per token, with random sign.
       const float m_new = fmaxf(mr[u], mx);
       corr[u] = ex2_approx(mr[u] - m_new);
       wch[u] = ex2_approx(mx - m_new);
@@ -920,11 +924,11 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
         uint32_t X[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          const float2 ab = ws.aux_b[32 * mp + 16 * (i >> 1) + 8 * (i & 1) + fg];   // {1 / (s1v PF), zv}
+          const float2 ab = ws.aux_b[32 * mp + 16 * (i >> 1) + 8 * (i & 1) + fg];   // {1 / s1v, zv}
           const float pt = ex2_approx(sraw[mp][u][i] - mx);
           const float f = fmaf(pt, PF, MAGIC_F);        // fixed-point pt; its radix-256 digits are the low bytes of f's bits
           const float pr = f - MAGIC_F;                 // PF * (rounded pt), an exact integer
-          lz = __ffma2_rn(make_float2(pr, pr), ab, lz);
+          lz = __ffma2_rn(make_float2(pt, pr), ab, lz);   // l from the exact p = pt / s1v, the zero-point sum from the rounded pt
           X[i] = DP == 4 ? __float_as_uint(f) * mul_p + add_p : __float_as_uint(f);
         }
         // column (h, d) of column h = ft + 4u: n-tile (DP / 2) u + (d >> 1), g' = 2 ft + (d & 1); word (kappa = mp, half = fg >> 2, t' = fg & 3)

@@ -232,3 +232,34 @@ def test_block_attention_dense_long_context_and_splits(kv):
     cache = _cache(kv, p, K, V)
     out = kv.block_attention(p, cache, q, kb, vb, dense=True)
     _check(kv, p, cache, q, kb, vb, out, n_tok)
+
+
+@pytest.mark.parametrize("dense", [False, True])
+@pytest.mark.parametrize("bits", [2, 4])
+def test_block_attention_token_scale_spread_and_dominant_keys(kv, bits, dense):
+    """V token norms spread over 20 binades inside a chunk (incl. all-zero V rows and half a chunk 2^-14 below the other
+    half) and keys that dominate their chunk by 10-20 log2 units for individual query rows, against the oracle on the
+    same record bytes.  Integer path: what is rounded to fixed point is p s1v[t], so the denominator must take the exact
+    p (a token with a tiny V row keeps its probability mass).  Dense path: s1v[t] enters as a per-chunk exponent in the
+    logits and an exact factor in the tile, and the TMEM accumulator is rescaled when a row's maximum rises.
+    The error is taken relative to the largest output of the (sequence, KV head) unit: rows that attend to a
+    tiny-norm token have outputs 2^-12 of the others', so R16's per-row ratio would measure nothing but that scale."""
+    n_tok, n_q, Hq, Hkv = 128 * 6 + 17, 40, 8, 2
+    K, V, kb, vb, q = _inputs(1, Hq, Hkv, n_tok, n_q, seed=190 + bits)
+    gen = torch.Generator(device="cuda").manual_seed(7)
+    e = torch.randint(-12, 9, (1, Hkv, n_tok, 1), generator=gen, device="cuda").to(torch.float32)
+    V = (V.float() * torch.exp2(e)).to(V.dtype)
+    V[:, :, 5::41] = 0                                   # whole V rows exactly zero
+    V[:, :, 128 * 3:128 * 4:2] *= 2.0 ** -14             # half of one chunk far below the other half
+    for i, t in enumerate((130, 300, 301, 640, 777)):    # keys aligned with individual queries
+        K[0, :, t] = (q[0, (7 * i) % n_q, ::Hq // Hkv].float() * (3.0 + i)).to(K.dtype)
+    p = kv.default_params(bits)
+    cache = _cache(kv, p, K, V)
+    out = kv.block_attention(p, cache, q, kb, vb, dense=dense)
+    assert torch.isfinite(out).all()
+    g = Hq // Hkv
+    o = out.to(torch.float64).cpu().numpy()
+    for h in range(Hkv):
+        ref = _oracle_block(kv, p, cache, 0, h, g, q, kb, vb, n_tok)
+        err = np.abs(o[0, :, h * g:(h + 1) * g] - ref).max() / np.abs(ref).max()
+        assert err <= P.ATTN_RTOL, (h, err)
