@@ -291,7 +291,8 @@ KVARN_API int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* ca
  * kvarn_block_attention_dense -- the same operation and arguments as kvarn_block_attention, computed by a dense
  * tensor-core kernel (tcgen05 + tensor memory): every chunk of the cache is expanded once into fp16 tiles
  * (code x scale is exact in fp16) and the block's 128-row tiles of (query token, head) pairs run S = Q K^T and
- * O += P V as M = 128 MMAs; the raw windows go through the decode kernel and the pieces are LSE-merged.  The right
+ * O += P V as M = 128 MMAs; the raw windows (sink, residual, the block's own causal tokens) pass through the same
+ * pipeline as fp16 tiles (keys in two fp16 terms, values in one: 2^-12 per element) and the pieces are LSE-merged.  The right
  * form for blocks with >= ~32 (token, head) rows per KV head (blocks of b tokens); kvarn_block_attention is the
  * right one for a few speculative tokens.  ws: DEVICE scratch of >= kvarn_block_dense_workspace_bytes(...) bytes
  * (16-byte aligned; owned by the caller, may be reused by the next call on the same stream).

@@ -588,7 +588,7 @@ int kvarn_block_attention(const kvarn_params* p, const kvarn_cache* cache, const
 }
 
 // Dense form of kvarn_block_attention for blocks with many query rows per KV head (tcgen05 + TMEM; kvarn_block_dense.cuh):
-// packed chunks by block_dense_kernel, raw windows by decode_kernel_w (skip_chunks), merged by merge_partials_kernel.
+// packed chunks and raw windows by block_dense_kernel, its partial sets merged by merge_partials_kernel.
 static int dense_splits(int B, int Hkv, int n_tiles, int max_chunks) {
   int sms = 148;
   const int dev = current_device();
@@ -623,6 +623,8 @@ int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache,
   DenseArgs E{};
   E.k_records = (const uint8_t*)cache->k_records; E.v_records = (const uint8_t*)cache->v_records; E.seq_lens = cache->seq_lens;
   E.q = q; E.parts = (float*)ws;
+  E.k_resid = cache->k_resid; E.v_resid = cache->v_resid; E.k_sink = cache->k_sink; E.v_sink = cache->v_sink;
+  E.k_blk = k_blk; E.v_blk = v_blk;
   E.B = cache->B; E.Hkv = cache->Hkv; E.Hq = Hq; E.g = g; E.max_chunks = cache->max_chunks; E.n_sink = cache->n_sink; E.n_q = n_q;
   E.n_tiles = (n_q * g + 127) / 128;
   E.splits = dense_splits(cache->B, cache->Hkv, E.n_tiles, cache->max_chunks);
@@ -643,21 +645,8 @@ int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache,
     }
     if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return KVARN_CUDA;
   }
-  // raw windows (sink, residual, the block's own causal tokens): the decode kernel without its chunks, as one more partial
-  DecodeArgs A{};
-  A.k_records = E.k_records; A.v_records = E.v_records;
-  A.k_resid = cache->k_resid; A.v_resid = cache->v_resid; A.seq_lens = cache->seq_lens;
-  A.k_sink = cache->k_sink; A.v_sink = cache->v_sink; A.n_sink = cache->n_sink;
-  A.ticket = cache->decode_ticket;
-  A.q = q; A.out = (float*)ws + (size_t)(DENSE_SETS * E.splits) * n_rows * PART_STRIDE; A.ws = nullptr;
-  A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;
-  A.n_q = n_q; A.k_blk = k_blk; A.v_blk = v_blk;
-  A.tpc = n_q * g <= 4 ? n_q : (8 / g < n_q ? 8 / g : n_q);
-  A.cluster = 1; A.nclus = 1; A.splits = 1;
-  A.q_scale = E.q_scale; A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = KVARN_F32;
-  A.partial = 1; A.skip_chunks = 1;
-  if (launch_decode(p, A, s) != cudaSuccess) return KVARN_CUDA;
-  merge_partials_kernel<<<(unsigned)n_rows, 128, 0, s>>>((const float*)ws, DENSE_SETS * E.splits + 1, n_rows, out, p->out_dtype);
+  // (the raw windows -- sink, residual, the block's own causal tokens -- ran inside the same kernel as extra chunks)
+  merge_partials_kernel<<<(unsigned)n_rows, 128, 0, s>>>((const float*)ws, DENSE_SETS * E.splits, n_rows, out, p->out_dtype);
   return last_cuda();
 }
 

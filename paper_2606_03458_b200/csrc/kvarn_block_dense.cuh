@@ -1,7 +1,8 @@
 // Dense multi-token read path on the 5th-generation tensor cores (tcgen05 + TMEM): a block of query rows against the
 // packed chunks of the cache (Fig. 4 pseudo-decode).  Used by kvarn_block_attention_dense
-// for blocks with many (query token, head) rows per KV head; the raw windows (sink, residual, the block's own causal
-// tokens) are left to decode_kernel_w (skip_chunks = 1, partial = 1) and everything is merged by merge_partials_kernel.
+// for blocks with many (query token, head) rows per KV head.  The raw windows (sink, residual, the block's own causal
+// tokens) run through the same pipeline as extra chunks after the packed ones (rotated rows as fp16 tiles, K in two
+// terms, masked in the softmax); the partial sets of all CTAs are merged by merge_partials_kernel.
 //
 // One CTA = one (sequence, KV head), one tile of 128 query rows r = (token i, head h), one range of chunks; three roles
 // that meet only through mbarriers: warps 8-15 expand the records (producers), one thread of warp 16 issues the MMAs,
@@ -33,6 +34,9 @@ struct DenseArgs {
   const uint8_t* v_records;
   const int32_t* seq_lens;
   const void* q;        // [B][n_q][Hq][128]
+  const void* k_resid; const void* v_resid;   // raw residual window [B * Hkv][128][128]
+  const void* k_sink;  const void* v_sink;    // raw sink tokens [B * Hkv][n_sink][128]
+  const void* k_blk;   const void* v_blk;     // the block's own tokens [B * Hkv][n_q][128] (causal), or null
   float* parts;         // [splits][B * n_q * Hq][PART_STRIDE]
   int B, Hkv, Hq, g, max_chunks, n_sink, n_q, splits, n_tiles;
   float q_scale;
@@ -103,6 +107,7 @@ template <int BITS> __host__ __device__ constexpr int dense_elem_of_kpos(int kp)
 // different rows.  Their core matrices are therefore spread with LBO = 144 B (K direction) and an odd number of
 // 16-byte groups per 8 rows (SBO): with the lane assignment of ProducerLane every quarter warp then stores to eight
 // different bank groups, and its record loads are one contiguous 128 B line per warp (no bank conflict on either side).
+constexpr int DN_NO_MASK = 1 << 20;
 constexpr int DN_LBO = 144;
 constexpr int DN_SBO_K = (16 * 9 + 1) * 16;      // 2320 B per 8 rows of Kt (16 units of 144 B + 16 B)
 constexpr int DN_SBO_V = (18 * 9 + 1) * 16;      // 2608 B per 8 rows of Vt (18 units + 16 B)
@@ -139,6 +144,8 @@ struct DenseSmem {
   alignas(16) float2 aux_s2[3][64];                // [chunk % 3] per token pair (rho order): s2 of the K record
   alignas(16) float2 aux_zm[3][64];                //                                         f_t zv[t] of the V record
   alignas(8) float2 e_chunk[3];                    // [chunk % 3] {E, 2^-E}: E = largest binary exponent of the chunk's s1v
+  alignas(8) int2 mask[3];                         // [chunk % 3] {tokens in the chunk, vis0}: column n is visible to query token i
+                                                   // iff n < tokens and n <= vis0 + i (raw chunks; packed: {128, DN_NO_MASK})
   int e_warp[4];
   __device__ float2* ml() { return reinterpret_cast<float2*>(rec_k[0]); }   // epilogue: {m, l} of the rows (records are dead)
   alignas(8) uint64_t full_k[2], full_v[2];        // TMA arrival [chunk parity]
@@ -258,6 +265,31 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   const int per = (n_chunks + A.splits - 1) / A.splits;
   const int c_begin = min(split * per, n_chunks), c_end = min(c_begin + per, n_chunks);
   const int n_my = c_end - c_begin;
+  // Raw windows run through the same pipeline as extra chunks after the packed ones: their K / V rows are rotated and
+  // rounded to fp16 by the producers (one term: 2^-12 per element, below the other terms of the tolerance), s2 = 1, no
+  // zero point, and the softmax masks by count and causality.  Sink: split 0; residual window and the block's own
+  // tokens: the last split.
+  const InT* raw_k[3]; const InT* raw_v[3]; int raw_cnt[3], raw_vis[3];
+  int n_raw = 0;
+  {
+    const int ns_tok = min(len, A.n_sink), resid = body & 127;
+    if (split == 0 && ns_tok > 0) {
+      raw_k[n_raw] = reinterpret_cast<const InT*>(A.k_sink) + (size_t)unit * A.n_sink * D;
+      raw_v[n_raw] = reinterpret_cast<const InT*>(A.v_sink) + (size_t)unit * A.n_sink * D;
+      raw_cnt[n_raw] = ns_tok; raw_vis[n_raw] = DN_NO_MASK; ++n_raw;
+    }
+    if (split == A.splits - 1 && resid > 0) {
+      raw_k[n_raw] = reinterpret_cast<const InT*>(A.k_resid) + (size_t)unit * G * D;
+      raw_v[n_raw] = reinterpret_cast<const InT*>(A.v_resid) + (size_t)unit * G * D;
+      raw_cnt[n_raw] = resid; raw_vis[n_raw] = DN_NO_MASK; ++n_raw;
+    }
+    if (split == A.splits - 1 && A.k_blk != nullptr) {
+      raw_k[n_raw] = reinterpret_cast<const InT*>(A.k_blk) + (size_t)unit * A.n_q * D;
+      raw_v[n_raw] = reinterpret_cast<const InT*>(A.v_blk) + (size_t)unit * A.n_q * D;
+      raw_cnt[n_raw] = A.n_q; raw_vis[n_raw] = 0; ++n_raw;
+    }
+  }
+  const int n_tot = n_my + n_raw;
   const int n_rows = A.n_q * g;                                                     // query rows of this (b, kv head)
   const uint8_t* krec = A.k_records + ((size_t)unit * A.max_chunks + c_begin) * RB;
   const uint8_t* vrec = A.v_records + ((size_t)unit * A.max_chunks + c_begin) * RB;
@@ -347,6 +379,50 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
     auto expand_k = [&](int c) {
       const int st = c & 1, s3 = c % 3;
       const uint32_t par_rec = (c >> 1) & 1;
+      if (c >= n_my) {
+        // raw chunk: Kt row n = token n (identity order), columns in the K-position order of q'
+        // The rotated row enters as TWO fp16 terms (keys have outlier channels of several hundred: one term would cost
+        // 1e-2 of a logit): the first in kt[st], the second in the Vt buffer laid out as a 128-row K tile -- which is why
+        // raw chunks are not prefetched: Vt is free only when PV of the previous chunk has completed.
+        const int j = c - n_my;
+        if (c >= 2) mbar_wait(&sm.k_free[st], par_rec ^ 1);
+        if (c >= 1) mbar_wait(&sm.bar_o[1], (c & 1) ^ 1);
+        uint8_t* kt = sm.kt[st];
+        if (pt < 128) {
+          reinterpret_cast<float*>(&sm.aux_s2[s3][n_ax >> 1])[n_ax & 1] = 1.f;
+          reinterpret_cast<float*>(&sm.aux_zm[s3][n_ax >> 1])[n_ax & 1] = 0.f;
+          if (pt == 0) { sm.e_chunk[s3] = make_float2(0.f, 1.f); sm.mask[s3] = make_int2(raw_cnt[j], raw_vis[j]); }
+        } else {
+          *reinterpret_cast<__half*>(kt + tile_off(128, n_ax, DN_SBO_K)) = __float2half_rn(0.f);   // no beta
+          *reinterpret_cast<__half*>(kt + tile_off(129, n_ax, DN_SBO_K)) = __float2half_rn(0.f);
+        }
+        const InT* kp = raw_k[j];
+        const int cnt = raw_cnt[j];
+        for (int t = pw; t < 128; t += 8) {
+          float x[4] = {0.f, 0.f, 0.f, 0.f};
+          if (t < cnt) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) x[e] = ld_in<InT>(kp + (size_t)t * D + 4 * lane + e);
+            if (A.rotate_k) {
+              fwht128_lane4(x, lane);
+#pragma unroll
+              for (int e = 0; e < 4; ++e) x[e] *= 0.08838834764831845f;
+            }
+          }
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int off = tile_off(t, dense_kpos<BITS>(4 * lane + e), DN_SBO_K);
+            const __half hi = __float2half_rn(x[e]);
+            *reinterpret_cast<__half*>(kt + off) = hi;
+            *reinterpret_cast<__half*>(sm.vt + off) = __float2half_rn(x[e] - __half2float(hi));
+          }
+        }
+        fence_async_smem();
+        __syncwarp();
+        if (lane == 0) { mbar_arrive(&sm.kt_full[st]); mbar_arrive(&sm.aux_full[s3]); }
+        producer_sync();
+        return;
+      }
       mbar_wait(&sm.full_k[st], par_rec);
       mbar_wait(&sm.full_va[s3], (c / 3) & 1);
       if (c >= 2) mbar_wait(&sm.k_free[st], par_rec ^ 1);  // the QK^T of chunk c - 2 has consumed kt[st]
@@ -380,7 +456,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         reinterpret_cast<__half*>(sm.fh[st])[n_ax] = __float2half_rn(f);
         reinterpret_cast<float*>(&sm.aux_s2[s3][n_ax >> 1])[n_ax & 1] = e4m3_to_f32(kr[s2_off(BITS) + slot_tok]);
         reinterpret_cast<float*>(&sm.aux_zm[s3][n_ax >> 1])[n_ax & 1] = f * zv;
-        if (pt == 0) sm.e_chunk[s3] = make_float2((float)max(E, -64), two_mE);
+        if (pt == 0) { sm.e_chunk[s3] = make_float2((float)max(E, -64), two_mE); sm.mask[s3] = make_int2(128, DN_NO_MASK); }
       }
       {
         __half2 sK[PPW], aK[PPW];
@@ -410,13 +486,38 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       }
     };
     if (n_my > 0) expand_k(0);
-    for (int it = 0; it < n_my; ++it) {
+    for (int it = 0; it < n_tot; ++it) {
       const int st = it & 1;
       const uint32_t par = it & 1;
-      if (it + 1 < n_my) expand_k(it + 1);               // K of the NEXT chunk first: its QK^T overlaps this chunk's softmax
-      mbar_wait(&sm.full_v[st], (it >> 1) & 1);
-      if (it > 0) mbar_wait(&sm.bar_o[1], par ^ 1);      // PV of chunk it - 1 complete: Vt is free, softmax of it - 1 is over
-      {
+      if (it >= n_my) expand_k(it);                      // raw chunk: expanded in its own turn (it waits for PV of chunk it - 1)
+      else if (it + 1 < n_my) expand_k(it + 1);          // K of the NEXT chunk first: its QK^T overlaps this chunk's softmax
+      if (it < n_my) {
+        mbar_wait(&sm.full_v[st], (it >> 1) & 1);
+        if (it > 0) mbar_wait(&sm.bar_o[1], par ^ 1);    // PV of chunk it - 1 complete: Vt is free, softmax of it - 1 is over
+      } else {
+        mbar_wait(&sm.bar_s, par);                       // QK^T of this chunk has consumed the second K term in the Vt buffer
+      }
+      if (it >= n_my) {
+        // raw chunk: Vt[channel][token n] = fp16 of the rotated V row n
+        const int j = it - n_my;
+        const InT* vp = raw_v[j];
+        const int cnt = raw_cnt[j];
+        for (int t = pw; t < 128; t += 8) {
+          float x[4] = {0.f, 0.f, 0.f, 0.f};
+          if (t < cnt) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) x[e] = ld_in<InT>(vp + (size_t)t * D + 4 * lane + e);
+            if (A.rotate_v) {
+              fwht128_lane4(x, lane);
+#pragma unroll
+              for (int e = 0; e < 4; ++e) x[e] *= 0.08838834764831845f;
+            }
+          }
+#pragma unroll
+          for (int e = 0; e < 4; ++e)
+            *reinterpret_cast<__half*>(sm.vt + tile_off(4 * lane + e, t, DN_SBO_V)) = __float2half_rn(x[e]);
+        }
+      } else {
         uint8_t* vt = sm.vt;
         const uint8_t* vr = sm.rec_v[st];
         const uint8_t* va = sm.aux_v[it % 3];
@@ -465,13 +566,20 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           for (int ks = 0; ks < DN_KT / 16; ++ks)
             umma_f16(tmem, umma_desc(smem_u32(term ? sm.qlo : sm.qhi) + ks * 256, 128, SBO_T),
                      umma_desc(smem_u32(sm.kt[c & 1]) + ks * 2 * DN_LBO, DN_LBO, DN_SBO_K), IDESC_S, (term | ks) != 0);
+        if (c >= n_my) {                                  // raw chunk: + q'_hi x (second fp16 term of K, in the Vt buffer), N = 128
+#pragma unroll
+          for (int ks = 0; ks < DN_KT / 16; ++ks)
+            umma_f16(tmem, umma_desc(smem_u32(sm.qhi) + ks * 256, 128, SBO_T),
+                     umma_desc(smem_u32(sm.vt) + ks * 2 * DN_LBO, DN_LBO, DN_SBO_K), umma_idesc_f16(128, 128), 1u);
+        }
         umma_commit(&sm.bar_s);
         umma_commit(&sm.k_free[c & 1]);
       };
-      if (n_my > 0) issue_qk(0);
-      for (int it = 0; it < n_my; ++it) {
+      if (n_tot > 0) issue_qk(0);
+      for (int it = 0; it < n_tot; ++it) {
         const uint32_t par = it & 1;
-        if (it + 1 < n_my) issue_qk(it + 1);              // runs while the softmax warps work on chunk it
+        const bool next_packed = it + 1 < n_my;           // a raw chunk's tiles exist only after this chunk's PV (see expand_k)
+        if (next_packed) issue_qk(it + 1);                // runs while the softmax warps work on chunk it
         mbar_wait(&sm.vt_full, par);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
@@ -485,6 +593,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           }
           umma_commit(&sm.bar_o[h]);
         }
+        if (!next_packed && it + 1 < n_tot) issue_qk(it + 1);
       }
     }
   } else {
@@ -496,7 +605,8 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
     const uint32_t t_p = t_row + P_COL + (DN_KPH / 2) * h;
     // a warp whose 32 rows lie beyond the block's rows only keeps the barriers moving (its rows of P and O are never read)
     const bool live = rt * 128 + (warp & 3) * 32 < n_rows;
-    for (int it = 0; it < n_my; ++it) {
+    const int i_tok = (rt * 128 + r) / g;                // query token of this row (causal mask of the block's own tokens)
+    for (int it = 0; it < n_tot; ++it) {
       const int st = it % 3;
       const uint32_t par = it & 1;
       mbar_wait(&sm.bar_s, par);
@@ -552,8 +662,21 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           for (int i = 0; i < 4; ++i) cur[i] = nxt[i];
         }
       }
-      const float mx = fmaxf(fmaxf(mxa[0], mxa[1]), fmaxf(mxa[2], mxa[3]));
-      const float m_new = fmaxf(m_ref, mx - P_OFF);
+      float mx = fmaxf(fmaxf(mxa[0], mxa[1]), fmaxf(mxa[2], mxa[3]));
+      const int2 mk = sm.mask[st];
+      if (mk.x < 128 || mk.y != DN_NO_MASK) {            // raw chunk (CTA-uniform): masked columns leave the softmax
+        const int n_vis = min(mk.x, mk.y == DN_NO_MASK ? 128 : mk.y + i_tok + 1) - 64 * h;   // visible: columns 64 h + [0, n_vis)
+        mx = -INFINITY;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+          if (2 * k >= n_vis) v[k].x = -INFINITY;
+          if (2 * k + 1 >= n_vis) v[k].y = -INFINITY;
+          mx = fmaxf(mx, fmaxf(v[k].x, v[k].y));
+        }
+      }
+      // (a row that has seen nothing yet keeps m_ref = -inf: every p~ is 2^(-inf - 0) = 0 and nothing is rescaled)
+      const float m_cand = fmaxf(m_ref, mx - P_OFF);
+      const float m_new = m_cand == -INFINITY ? 0.f : m_cand;
       const float f_old = ex2_approx(m_ref - m_new);     // 0 for the first chunk (m_ref = -inf)
       if (it > 0) {
         mbar_wait(&sm.bar_o[h], par ^ 1);                // PV of the previous chunk is complete: p~ of it may be overwritten, O is consistent
@@ -570,7 +693,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
           asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         }
       }
-      m_ref = m_new;
+      m_ref = m_cand;
       const float2 nm2 = make_float2(-m_new, -m_new);
       float2 l2 = make_float2(0.f, 0.f), z2 = make_float2(0.f, 0.f);
 #pragma unroll
@@ -605,8 +728,8 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
 #pragma unroll 1
     for (int hh = 0; hh < DENSE_SETS; ++hh) {
       if (h == hh) {
-        if (n_my > 0) {
-          mbar_wait(&sm.bar_o[hh], (n_my - 1) & 1);
+        if (n_tot > 0) {
+          mbar_wait(&sm.bar_o[hh], (n_tot - 1) & 1);
           tc_fence_after();
 #pragma unroll 1
           for (int c0 = 0; c0 < 128; c0 += 16) {
@@ -628,7 +751,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         const size_t row = ((size_t)b * A.n_q + i) * A.Hq + hkv * g + hq;
         float* prow = A.parts + ((size_t)(DENSE_SETS * split + hh) * ((size_t)A.B * A.n_q * A.Hq) + row) * PART_STRIDE;
         float v[4] = {0.f, 0.f, 0.f, 0.f};
-        if (n_my > 0) {
+        if (n_tot > 0) {
           const float4 s4 = *reinterpret_cast<const float4*>(&stage[rr * 128 + ((4 * lane) ^ ((rr & 7) << 2))]);
           v[0] = s4.x; v[1] = s4.y; v[2] = s4.z; v[3] = s4.w;
           if (A.rotate_v) {
@@ -640,7 +763,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         *reinterpret_cast<float4*>(prow + 4 + 4 * lane) = make_float4(v[0], v[1], v[2], v[3]);
         if (lane == 0) {
           const float2 ml = sm.ml()[rr];
-          *reinterpret_cast<float4*>(prow) = make_float4(n_my > 0 ? ml.x : -INFINITY, n_my > 0 ? ml.y : 0.f, 0.f, 0.f);
+          *reinterpret_cast<float4*>(prow) = make_float4(n_tot > 0 ? ml.x : -INFINITY, n_tot > 0 ? ml.y : 0.f, 0.f, 0.f);
         }
       }
       softmax_sync();
