@@ -311,8 +311,9 @@ def run_extras(kv, W, dev, hbm_peak, only=frozenset()):
                             meda, _ = _time_launches(lambda i: kv.append_block(p, cache, kb, vb), 13, stream)
                             ex["append_block_nq8"] = {"us": meda * 1e3, "note": "8 tokens x 16 sequences, one launch"}
                         del qb, kb, vb, ob
+                if name == "decode_long_g4":
                     # the dense tcgen05 form of the same call (kvarn_block_attention_dense) on blocks of 8, 32 and 128 tokens
-                    for n_q in (8, 32, 128):
+                    for n_q in ((8, 32, 128) if bits == 2 else (32,)):
                         qb = torch.stack([W.queries(sh.B, sh.Hq, seed=sh.seed + 100 + i, device=dev) for i in range(n_q)], dim=1).contiguous()
                         kb, vb = W.kv_tokens(sh.B, sh.Hkv, n_q, seed=sh.seed + 200, device=dev, sink_first=False)
                         ob = torch.empty((sh.B, n_q, sh.Hq, D), dtype=torch.float32, device=dev)
@@ -324,9 +325,9 @@ def run_extras(kv, W, dev, hbm_peak, only=frozenset()):
                         medd, _ = _time_launches(lambda i: kv.block_attention(p, cache, qb, kb, vb, out=ob, dense=True, ws=wsd), 5, stream)
                         flop = 4.0 * sh.B * sh.Hq * n_q * sh.ctx * D                      # QK^T + PV, 2 flop per MAC
                         tf = flop / (medd * 1e-3) / 1e12
-                        ex[f"block_dense_long_g4_2bit_nq{n_q}"] = {"us": medd * 1e3, "us_per_query_token": medd * 1e3 / n_q, "x_decode": medd / med,
+                        ex[f"block_dense_long_g4_{bits}bit_nq{n_q}"] = {"us": medd * 1e3, "us_per_query_token": medd * 1e3 / n_q, "x_decode": medd / med,
                                                                    "TFLOPs": tf, "tensor_frac": tf / tensor_peak()[0],
-                                                                   "note": "whole call: block_dense_kernel + raw-window decode + merge; "
+                                                                   "note": "whole call: block_dense_kernel (packed chunks + raw windows) + merge; "
                                                                            "flop = 4 B Hq n_q ctx 128 (the hi / lo q terms are not counted twice)"}
                         del qb, kb, vb, ob, wsd
                 del cache, q, ws, out

@@ -187,6 +187,8 @@ KVARN_API size_t kvarn_decode_workspace_bytes(const kvarn_params* p, int32_t B, 
  * four standard deviations take pivoted single-pass sums, so the 1e-5 agreement of the scales with a float64
  * evaluation holds up to channel offsets of ~100 standard deviations; beyond that the fp32 rotation of the input
  * itself (rounding of order |offset| x 2^-24 per butterfly stage) is the limit, not the variance passes.
+ * Range: the squares of the values must stay inside fp32 (|x| between ~2^-60 and 2^60); below that the variances
+ * underflow to the clamp and the choice of the iterate is no longer the float64 one (the record stays finite).
  */
 KVARN_API int kvarn_quantize_chunk(const kvarn_params* p, const void* k, const void* v, int64_t n_tiles,
                          int64_t tile_stride, int64_t tok_stride, void* k_rec, void* v_rec,

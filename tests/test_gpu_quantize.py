@@ -237,3 +237,26 @@ def test_round_before_decode_matches_oracle_on_its_records(kv):
                                                   np.zeros((0, 128)), np.zeros((0, 128)), P.tile_f64(q[0, 4 * h:4 * h + 4]))
             worst = max(worst, P.attn_rel_err(out[0, 4 * h:4 * h + 4], ref))
         assert worst <= P.ATTN_RTOL, worst
+
+
+@pytest.mark.parametrize("bits", [2, 4])
+def test_adversarial_tiles_vs_oracle(kv, bits):
+    """Tiles built to stress the normaliser and the storage formats, against the oracle at the iterate the kernel kept:
+    token norms over 16 binades, channel norms over 12 binades (the log clamps of Alg. 1 bind), one element 2^14 above
+    the rest, exact-zero rows and columns, and a tile of magnitude 2^-40."""
+    g = torch.Generator(device="cuda").manual_seed(31 + bits)
+    base = torch.randn((5, 128, 128), generator=g, device="cuda")
+    T = base.clone()
+    T[0] *= torch.exp2(torch.randint(-8, 9, (128, 1), generator=g, device="cuda").float())      # token norms
+    T[1] *= torch.exp2(torch.randint(-6, 7, (1, 128), generator=g, device="cuda").float())      # channel norms
+    T[2, 17, 93] = 2.0 ** 14                                                                       # one massive element
+    T[3, 5::19, :] = 0; T[3, :, 7::23] = 0                                                         # zero rows and columns
+    T[4] *= 2.0 ** -40            # small magnitudes (fp32 variances: below ~2^-60 the squares underflow, kvarn.h states the bound)
+    X = T.to(torch.bfloat16)
+    p = kv.default_params(bits)
+    stats, recs, kb = _run_and_check(kv, p, X, X.flip(0).contiguous())
+    P.assert_mismatch_budget(stats, aux_frac=3e-4)
+    for kind in (0, 1):
+        for rec in recs[kind]:
+            codes, s1, s2, z = kv.unpack_record(p, kind, rec)
+            assert np.isfinite(s1).all() and np.isfinite(s2).all() and np.isfinite(z).all()
