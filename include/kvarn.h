@@ -15,13 +15,15 @@
  * Entry points: kvarn_quantize_chunk / kvarn_prefill (bulk write path), kvarn_append / kvarn_append_block
  * (on-the-fly compression while decoding), kvarn_decode_attention (read path), kvarn_block_attention /
  * kvarn_block_attention_dense (a block of new tokens against the cache, Fig. 4),
- * kvarn_decode_attention_partial + kvarn_merge_partials (a sequence spread over several caches / GPUs), kvarn_rope_hadamard / kvarn_hadamard_rows / kvarn_hadamard_row_groups (the
- * Hadamard arrangement of App. A), the *_host forms, layout queries and the record pack / unpack test hooks.
+ * kvarn_decode_attention_partial + kvarn_merge_partials (a sequence spread over several caches / GPUs),
+ * kvarn_decode_attention_static (the read path with its scratch inside the library: allocates nothing),
+ * kvarn_rope_hadamard / kvarn_hadamard_rows / kvarn_hadamard_row_groups (the Hadamard arrangement of App. A), the *_host forms, layout queries and the record pack / unpack test hooks.
  *
  * Conventions
  *   - "DEVICE" pointers are CUDA device memory owned by the caller; "HOST"
  *     pointers are ordinary (preferably pinned) host memory.  The library
- *     allocates no device memory, keeps no global state and never synchronises
+ *     allocates no device memory, keeps no global state (one exception: the static
+ *     scratch array of kvarn_decode_attention_static) and never synchronises
  *     the device: every call only enqueues work on the caller's `stream`
  *     (a cudaStream_t passed as void*; NULL = the legacy default stream).
  *   - All calls return a kvarn_status (0 = OK, negative = error); nothing is
@@ -253,6 +255,24 @@ KVARN_API int kvarn_append_block(const kvarn_params* p, const kvarn_cache* cache
 KVARN_API int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* cache, const void* q,
                            int32_t Hq, float sm_scale, void* out, void* ws, size_t ws_bytes,
                            void* stream);
+
+/*
+ * kvarn_decode_attention_static -- kvarn_decode_attention for callers that cannot allocate device memory (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): same operation, arguments, precision and
+ * result, but the split-K scratch (arrival counters + workspace partials; cache->decode_ticket is not used and may be
+ * NULL) lives in a static device array of KVARN_STATIC_SCRATCH_BYTES (1 MiB) inside the library, which every GPU that
+ * loads the library holds until the process exits.  The call allocates nothing (no cudaMalloc / cudaFree / allocating
+ * library routine).  Limits: a split plan that needs more than 1 MiB - 4 KiB of partials (B * Hq * clusters-per-sequence
+ * * 1040 B; every plan the library chooses itself for <= 8 KV-head groups stays below 0.4 MiB, only caller-chosen
+ * kvarn_params::splits can exceed it) or more than 1024 (sequence, KV head) units on the workspace route returns
+ * KVARN_WORKSPACE_TOO_SMALL.  ALL calls on one GPU share the array: calls that may overlap on the GPU (different streams
+ * without ordering) race; order them on one stream or use kvarn_decode_attention with separate workspaces.  The array
+ * keeps the previous call's contents; the call clears the counters it needs on `stream` before the launch.
+ * The device of `stream` must be current.
+ */
+#define KVARN_STATIC_SCRATCH_BYTES (1u << 20)
+KVARN_API int kvarn_decode_attention_static(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                                  int32_t Hq, float sm_scale, void* out, void* stream);
 
 /*
  * Context-parallel building block ("Splitting one sequence's chunks across GPUs needs exactly one

@@ -543,6 +543,67 @@ int kvarn_decode_attention_partial(const kvarn_params* p, const kvarn_cache* cac
   return decode_impl(p, cache, q, Hq, sm_scale, part, ws, ws_bytes, stream, 1);
 }
 
+// ---- kvarn_decode_attention_static: the read path for callers that cannot allocate -------------------------------
+// The split-K scratch of the decode kernel (arrival counters + workspace partials, touched only when a sequence's
+// chunks are spread over several clusters) lives in ONE file-scope device array of KVARN_STATIC_SCRATCH_BYTES per GPU,
+// held from the moment the library is loaded on that GPU until the process exits.  In host code the array's NAME is a
+// host-side stand-in, not a device address: its device address is taken once per device with cudaGetSymbolAddress
+// (that device current) and passed to the kernel.  Layout: [0, 4096) bytes = 1024 int32 arrival counters,
+// [4096, KVARN_STATIC_SCRATCH_BYTES) = partials.
+static __device__ __align__(256) unsigned char g_static_scratch[KVARN_STATIC_SCRATCH_BYTES];
+constexpr size_t STATIC_TICKET_BYTES = 4096;
+
+static cudaError_t static_scratch_ptr(unsigned char** out) {
+  static std::atomic<unsigned char*> cached[KVARN_MAX_DEVICES] = {};
+  const int dev = current_device();
+  if (dev < 0) return cudaErrorInvalidDevice;
+  if (dev < KVARN_MAX_DEVICES) { unsigned char* c = cached[dev].load(std::memory_order_acquire); if (c) { *out = c; return cudaSuccess; } }
+  unsigned char* ptr = nullptr;
+  const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_static_scratch);   // the current device's copy of the array
+  if (e != cudaSuccess || !ptr) { cudaGetLastError(); return e != cudaSuccess ? e : cudaErrorInvalidSymbol; }
+  if (dev < KVARN_MAX_DEVICES) cached[dev].store(ptr, std::memory_order_release);
+  *out = ptr;
+  return cudaSuccess;
+}
+
+int kvarn_decode_attention_static(const kvarn_params* p, const kvarn_cache* cache, const void* q,
+                                  int32_t Hq, float sm_scale, void* out, void* stream) {
+  int st = check_params(p);
+  if (st) return st;
+  if ((st = check_cache(cache))) return st;
+  if (!q || !out || Hq <= 0 || (Hq % cache->Hkv) != 0) return KVARN_INVALID_ARG;
+  const int g = Hq / cache->Hkv;
+  if (g > 8) return KVARN_UNSUPPORTED;
+  if (!aligned16(q) || !aligned16(out)) return KVARN_MISALIGNED;
+  const SplitPlan sp = split_plan(p, cache->B, cache->Hkv, g, cache->max_chunks);
+  const size_t need = sp.nclus > 1 ? (size_t)cache->B * Hq * sp.nclus * WS_STRIDE * sizeof(float) : 0;
+  if (need > KVARN_STATIC_SCRATCH_BYTES - STATIC_TICKET_BYTES ||
+      (sp.nclus > 1 && (size_t)cache->B * cache->Hkv * sizeof(int32_t) > STATIC_TICKET_BYTES))
+    return KVARN_WORKSPACE_TOO_SMALL;       // the plan needs more scratch than the static array holds
+  unsigned char* scratch = nullptr;
+  if (static_scratch_ptr(&scratch) != cudaSuccess) return KVARN_CUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  // The array keeps the last call's contents.  The partials are written before they are read; the arrival counters must
+  // start at zero (a kernel leaves them zero, an aborted or overlapping call may not have): cleared on the stream.
+  if (sp.nclus > 1 && cudaMemsetAsync(scratch, 0, (size_t)cache->B * cache->Hkv * sizeof(int32_t), s) != cudaSuccess) {
+    cudaGetLastError();
+    return KVARN_CUDA;
+  }
+  DecodeArgs A{};
+  A.k_records = (const uint8_t*)cache->k_records; A.v_records = (const uint8_t*)cache->v_records;
+  A.k_resid = cache->k_resid; A.v_resid = cache->v_resid; A.seq_lens = cache->seq_lens;
+  A.k_sink = cache->k_sink; A.v_sink = cache->v_sink; A.n_sink = cache->n_sink;
+  A.ticket = (int32_t*)scratch;
+  A.q = q; A.out = out; A.ws = (float*)(scratch + STATIC_TICKET_BYTES);
+  A.B = cache->B; A.Hkv = cache->Hkv; A.Hq = Hq; A.g = g; A.max_chunks = cache->max_chunks;
+  A.cluster = sp.cluster; A.nclus = sp.nclus; A.splits = sp.cluster * sp.nclus;
+  A.q_scale = sm_scale * 1.4426950408889634f;
+  A.rotate_k = p->rotate_k; A.rotate_v = p->rotate_v; A.out_dtype = p->out_dtype;
+  A.n_q = 1; A.tpc = 1; A.k_blk = nullptr; A.v_blk = nullptr; A.partial = 0;
+  const cudaError_t e = launch_decode(p, A, s);
+  return e == cudaSuccess ? KVARN_OK : KVARN_CUDA;
+}
+
 int kvarn_merge_partials(const float* parts, int32_t n_parts, int64_t n_rows, void* out, int32_t out_dtype,
                          void* stream) {
   if (!parts || !out || n_parts < 1 || n_rows < 0) return KVARN_INVALID_ARG;

@@ -59,6 +59,8 @@ EXPORTS = {
     "kvarn_version": (C.c_int, []),
     "kvarn_layout": (C.c_int, [C.POINTER(Params), C.POINTER(LayoutInfo)]),
     "kvarn_decode_workspace_bytes": (C.c_size_t, [C.POINTER(Params), C.c_int32, C.c_int32, C.c_int32, C.c_int32]),
+    "kvarn_decode_attention_static": (C.c_int, [C.POINTER(Params), C.POINTER(CacheDesc), C.c_void_p, C.c_int32, C.c_float,
+                                                C.c_void_p, C.c_void_p]),
     "kvarn_quantize_chunk": (C.c_int, [C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int64, C.c_int64,
                                        C.c_int64, C.c_void_p, C.c_void_p, C.c_int64,
                                        C.POINTER(DebugDesc), C.c_void_p]),
@@ -285,6 +287,28 @@ def decode_attention(p: Params, cache: Cache, q: torch.Tensor, sm_scale: float |
     st = lib.kvarn_decode_attention(C.byref(p), C.byref(cache.desc), _ptr(q), Hq, sm_scale, _ptr(out),
                                     _ptr(ws), ws.numel(), _stream(stream))
     _check(st, "kvarn_decode_attention")
+    return out
+
+
+STATIC_SCRATCH_BYTES = 1 << 20
+
+
+def decode_attention_static(p: Params, cache: Cache, q: torch.Tensor, sm_scale: float | None = None,
+                            out: torch.Tensor | None = None, stream=None):
+    """kvarn_decode_attention_static: decode_attention with the split-K scratch in the library's static device array
+    (1 MiB per GPU; nothing is allocated by the call -- pass `out` to keep the binding allocation-free too).  Calls
+    that overlap on the GPU race on that array."""
+    assert q.is_cuda and q.is_contiguous() and q.shape[0] == cache.B and q.shape[2] == HEAD_DIM
+    Hq = q.shape[1]
+    p.in_dtype = _dtype_code(q)
+    assert cache.k_resid.dtype == q.dtype
+    if sm_scale is None:
+        sm_scale = 1.0 / float(np.sqrt(HEAD_DIM))
+    if out is None:
+        out = torch.empty((cache.B, Hq, HEAD_DIM), device=q.device,
+                          dtype=torch.float32 if p.out_dtype == F32 else torch.bfloat16)
+    st = lib.kvarn_decode_attention_static(C.byref(p), C.byref(cache.desc), _ptr(q), Hq, sm_scale, _ptr(out), _stream(stream))
+    _check(st, "kvarn_decode_attention_static")
     return out
 
 
