@@ -293,6 +293,16 @@ def run_extras(kv, W, dev, hbm_peak, only=frozenset()):
                 byts = cache.nbytes_read_by_decode(sh.ctx) + sh.B * sh.Hq * (D * 2 + D * 4)
                 ex[f"{name}_{bits}bit"] = {"us": med * 1e3, "GBps": byts / med / 1e6, "hbm_frac": byts / med / 1e6 / hbm_peak,
                                            "MB": byts / 1e6, "shape": f"B{sh.B} {sh.Hq}/{sh.Hkv} ctx{sh.ctx}"}
+                if bits == 2:
+                    # the same launch with 16-bit q~ (kvarn_params::decode_digits = 2: half the QK^T tensor-core work; its
+                    # error is statistically ~3e-4 but has no deterministic bound below the 2e-3 tolerance: not the default)
+                    p2 = kv.default_params(bits)
+                    p2.decode_digits = 2
+                    for _ in range(3):
+                        kv.decode_attention(p2, cache, q, out=out, ws=ws)
+                    torch.cuda.synchronize()
+                    med2, _ = _time_launches(lambda i: kv.decode_attention(p2, cache, q, out=out, ws=ws), 10, stream)
+                    ex[f"{name}_{bits}bit_digits2"] = {"us": med2 * 1e3, "GBps": byts / med2 / 1e6, "hbm_frac": byts / med2 / 1e6 / hbm_peak}
                 if name == "decode_long_g4" and bits == 2:
                     # multi-token read path (Fig. 4): a block of n_q new tokens against the same cache
                     for n_q in (2, 8):
@@ -735,6 +745,7 @@ def main():
             "cfg2_ctx32k_decode_frac": (ex.get("cfg2_incremental") or {}).get("decode_hbm_frac"),
             "cfg4_2bit_frac": frac("decode_cfg4_2bit"), "cfg4_4bit_frac": frac("decode_cfg4_4bit"),
             "long_g4_2bit_frac": frac("decode_long_g4_2bit"), "long_g4_4bit_frac": frac("decode_long_g4_4bit"),
+            "long_g4_2bit_digits2_frac": frac("decode_long_g4_2bit_digits2"), "cfg4_2bit_digits2_frac": frac("decode_cfg4_2bit_digits2"),
             "quantize_alu_frac": q_tflops / FP32_PEAK_TFLOPS_NOMINAL, "quantize_hbm_frac": q_gbs / hbm_peak,
             "block_dense_nq32_us_per_token": (ex.get("block_dense_long_g4_2bit_nq32") or {}).get("us_per_query_token"),
             "block_dense_nq32_tensor_frac": (ex.get("block_dense_long_g4_2bit_nq32") or {}).get("tensor_frac"),
