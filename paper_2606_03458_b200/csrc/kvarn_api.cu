@@ -7,6 +7,7 @@
 #include "kvarn_common.cuh"
 #include "kvarn_decode.cuh"
 #include "kvarn_block_dense.cuh"
+#include <cstdlib>
 #include "kvarn_rotate.cuh"
 #include "kvarn_quantize.cuh"
 
@@ -230,6 +231,8 @@ struct SplitPlan { int cluster, nclus; };
 #ifndef KVARN_MAX_CLUSTER_OVERRIDE
 #define KVARN_MAX_CLUSTER_OVERRIDE 8
 #endif
+constexpr int KVARN_DENSE_CTA_COST = 18;    // fixed cost of a dense CTA / of the merge launch, in chunk-times (~2 us each)
+constexpr int KVARN_DENSE_MERGE_COST = 12;
 constexpr int KVARN_MAX_CLUSTER = KVARN_MAX_CLUSTER_OVERRIDE;    // portable maximum; 9..16 (non-portable) measured slower: 25 -> 27..31 us on config 1
 
 // DQ, DP = digit planes of q~ / p~ (kvarn_decode.cuh)
@@ -654,17 +657,32 @@ static int dense_splits(int B, int Hkv, int n_tiles, int max_chunks) {
   int sms = 148;
   const int dev = current_device();
   if (dev >= 0 && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); sms = 148; }
-  int s = sms / (B * Hkv * n_tiles);            // one CTA per SM (197 KB of shared memory, 512 TMEM columns)
-  if (s > max_chunks / 4) s = max_chunks / 4;   // at least 4 chunks per CTA
-  if (s > 32) s = 32;
-  return s < 1 ? 1 : s;
+#ifdef KVARN_DENSE_SPLITS_ENV
+  if (const char* e = getenv("KVARN_DENSE_SPLITS")) { const int v = atoi(e); if (v > 0) return v > 32 ? 32 : v; }
+#endif
+  // One CTA per SM (210 KB of shared memory, 512 TMEM columns), so the CTAs run in waves of `sms`.  Cost of a plan in
+  // chunk-times: waves x (chunks per CTA + the fixed cost of a CTA: prologue, pipeline fill and drain, epilogue), plus
+  // the merge launch when a row tile is spread over several CTAs -- fitted to measured splits 1..16 on the 64k-context
+  // cache.  Few units: the chunks spread over the idle SMs; many units: the split that fills the
+  // last wave (512 CTAs on 148 SMs: 2 per row tile make 7 full waves of 256 chunks instead of 4 of 512).
+  const long long ctas = (long long)B * Hkv * n_tiles;
+  int best = 1;
+  long long best_cost = -1;
+  for (int s = 1; s <= 32; ++s) {
+    const int per = (max_chunks + s - 1) / s;
+    if (s > 1 && per < 4) break;                 // at least 4 chunks per CTA
+    const long long waves = (ctas * s + sms - 1) / sms;
+    const long long cost = waves * (per + KVARN_DENSE_CTA_COST) + (s > 1 ? KVARN_DENSE_MERGE_COST : 0);
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = s; }
+  }
+  return best;
 }
 
 size_t kvarn_block_dense_workspace_bytes(const kvarn_params* p, int32_t B, int32_t Hq, int32_t Hkv, int32_t n_q,
                                          int32_t max_chunks) {
   if (!p || B <= 0 || Hq <= 0 || Hkv <= 0 || n_q <= 0 || (Hq % Hkv) != 0) return 0;
   const int g = Hq / Hkv, n_tiles = (n_q * g + 127) / 128;
-  return (size_t)(DENSE_SETS * dense_splits(B, Hkv, n_tiles, max_chunks) + 1) * B * n_q * Hq * PART_STRIDE * sizeof(float);
+  return (size_t)dense_splits(B, Hkv, n_tiles, max_chunks) * B * n_q * Hq * PART_STRIDE * sizeof(float);   // touched only when > 1 split
 }
 
 int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache, const void* q,
@@ -683,7 +701,7 @@ int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache,
   const long long n_rows = (long long)cache->B * n_q * Hq;
   DenseArgs E{};
   E.k_records = (const uint8_t*)cache->k_records; E.v_records = (const uint8_t*)cache->v_records; E.seq_lens = cache->seq_lens;
-  E.q = q; E.parts = (float*)ws;
+  E.q = q; E.parts = (float*)ws; E.out = out; E.out_dtype = p->out_dtype;
   E.k_resid = cache->k_resid; E.v_resid = cache->v_resid; E.k_sink = cache->k_sink; E.v_sink = cache->v_sink;
   E.k_blk = k_blk; E.v_blk = v_blk;
   E.B = cache->B; E.Hkv = cache->Hkv; E.Hq = Hq; E.g = g; E.max_chunks = cache->max_chunks; E.n_sink = cache->n_sink; E.n_q = n_q;
@@ -707,7 +725,7 @@ int kvarn_block_attention_dense(const kvarn_params* p, const kvarn_cache* cache,
     if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return KVARN_CUDA;
   }
   // (the raw windows -- sink, residual, the block's own causal tokens -- ran inside the same kernel as extra chunks)
-  merge_partials_kernel<<<(unsigned)n_rows, 128, 0, s>>>((const float*)ws, DENSE_SETS * E.splits, n_rows, out, p->out_dtype);
+  if (E.splits > 1) merge_partials_kernel<<<(unsigned)n_rows, 128, 0, s>>>((const float*)ws, E.splits, n_rows, out, p->out_dtype);
   return last_cuda();
 }
 

@@ -37,7 +37,9 @@ struct DenseArgs {
   const void* k_resid; const void* v_resid;   // raw residual window [B * Hkv][128][128]
   const void* k_sink;  const void* v_sink;    // raw sink tokens [B * Hkv][n_sink][128]
   const void* k_blk;   const void* v_blk;     // the block's own tokens [B * Hkv][n_q][128] (causal), or null
-  float* parts;         // [splits][B * n_q * Hq][PART_STRIDE]
+  float* parts;         // [splits][B * n_q * Hq][PART_STRIDE] (splits > 1)
+  void* out;            // splits == 1: the normalised result [B][n_q][Hq][128] is written directly
+  int out_dtype;
   int B, Hkv, Hq, g, max_chunks, n_sink, n_q, splits, n_tiles;
   float q_scale;
   int rotate_k, rotate_v;
@@ -242,7 +244,7 @@ constexpr int DENSE_REGS_SOFTMAX = 120, DENSE_REGS_PRODUCER = 72;
 template <int N> __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void softmax_sync() { asm volatile("bar.sync 2, 256;" ::: "memory"); }
-constexpr int DENSE_SETS = 2;               // partial sets per CTA: one per token half (independent online softmax streams)
+constexpr int DENSE_SETS = 1;               // partial sets per CTA (the two token-half streams are merged in the epilogue)
 
 template <int BITS, typename InT>
 __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const DenseArgs A) {
@@ -318,16 +320,26 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
   for (int i = tid; i < (int)(sizeof(sm.kt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.kt)[i] = make_uint4(0, 0, 0, 0);
   for (int i = tid; i < (int)(sizeof(sm.vt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.vt)[i] = make_uint4(0, 0, 0, 0);
   // q' = (q H / sqrt(128)) q_scale as two fp16 terms, columns in K-position order
-  for (int r = warp; r < 128; r += DENSE_THREADS / 32) {
-    const int R = rt * 128 + r;
-    float v[4] = {0.f, 0.f, 0.f, 0.f};
-    if (R < n_rows) {
+  constexpr int QROWS = (128 + DENSE_THREADS / 32 - 1) / (DENSE_THREADS / 32);   // rows per warp: all loads in flight together
+  float qv[QROWS][4];
+#pragma unroll
+  for (int k = 0; k < QROWS; ++k) {
+    const int r = warp + k * (DENSE_THREADS / 32), R = rt * 128 + r;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) qv[k][j] = 0.f;
+    if (r < 128 && R < n_rows) {
       const int i = R / g, h = R - i * g;
       const size_t row = ((size_t)b * A.n_q + i) * A.Hq + hkv * g + h;
       const InT* qp = reinterpret_cast<const InT*>(A.q) + row * D + 4 * lane;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) v[j] = ld_in<InT>(qp + j) * A.q_scale;
+      for (int j = 0; j < 4; ++j) qv[k][j] = ld_in<InT>(qp + j) * A.q_scale;
     }
+  }
+#pragma unroll
+  for (int k = 0; k < QROWS; ++k) {
+    const int r = warp + k * (DENSE_THREADS / 32);
+    if (r >= 128) break;
+    float v[4] = {qv[k][0], qv[k][1], qv[k][2], qv[k][3]};
     if (A.rotate_k) {
       fwht128_lane4(v, lane);
 #pragma unroll
@@ -375,6 +387,29 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       krow_off[i] = tile_off(kr_, 0, DN_SBO_K) + wi * (CPW / 8) * DN_LBO;
       vrow_off[i] = tile_off(sl, 0, DN_SBO_V) + wi * (CPW / 8) * DN_LBO;
     }
+    // rows pw, pw + 8, ... < cnt of a raw window, rotated, four rows' loads in flight together
+    auto raw_rows = [&](const InT* base, int cnt, int rotate, auto store) {
+      for (int t0 = pw; t0 < cnt; t0 += 32) {
+        float x[4][4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const int t = t0 + 8 * k;
+#pragma unroll
+          for (int e = 0; e < 4; ++e) x[k][e] = t < cnt ? ld_in<InT>(base + (size_t)t * D + 4 * lane + e) : 0.f;
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const int t = t0 + 8 * k;
+          if (t >= cnt) break;
+          if (rotate) {
+            fwht128_lane4(x[k], lane);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) x[k][e] *= 0.08838834764831845f;
+          }
+          store(t, x[k]);
+        }
+      }
+    };
     // chunk c: aux of both records, then Kt; afterwards the K record of chunk c + 2 is requested
     auto expand_k = [&](int c) {
       const int st = c & 1, s3 = c % 3;
@@ -398,17 +433,8 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         }
         const InT* kp = raw_k[j];
         const int cnt = raw_cnt[j];
-        for (int t = pw; t < 128; t += 8) {
-          float x[4] = {0.f, 0.f, 0.f, 0.f};
-          if (t < cnt) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) x[e] = ld_in<InT>(kp + (size_t)t * D + 4 * lane + e);
-            if (A.rotate_k) {
-              fwht128_lane4(x, lane);
-#pragma unroll
-              for (int e = 0; e < 4; ++e) x[e] *= 0.08838834764831845f;
-            }
-          }
+        // only the rows of real tokens: rows >= cnt keep stale (finite) tile contents and are masked in the softmax
+        raw_rows(kp, cnt, A.rotate_k, [&](int t, const float (&x)[4]) {
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             const int off = tile_off(t, dense_kpos<BITS>(4 * lane + e), DN_SBO_K);
@@ -416,7 +442,7 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
             *reinterpret_cast<__half*>(kt + off) = hi;
             *reinterpret_cast<__half*>(sm.vt + off) = __float2half_rn(x[e] - __half2float(hi));
           }
-        }
+        });
         fence_async_smem();
         __syncwarp();
         if (lane == 0) { mbar_arrive(&sm.kt_full[st]); mbar_arrive(&sm.aux_full[s3]); }
@@ -502,21 +528,12 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
         const int j = it - n_my;
         const InT* vp = raw_v[j];
         const int cnt = raw_cnt[j];
-        for (int t = pw; t < 128; t += 8) {
-          float x[4] = {0.f, 0.f, 0.f, 0.f};
-          if (t < cnt) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) x[e] = ld_in<InT>(vp + (size_t)t * D + 4 * lane + e);
-            if (A.rotate_v) {
-              fwht128_lane4(x, lane);
-#pragma unroll
-              for (int e = 0; e < 4; ++e) x[e] *= 0.08838834764831845f;
-            }
-          }
+        // (columns >= cnt keep stale finite values: their p~ is exactly zero)
+        raw_rows(vp, cnt, A.rotate_v, [&](int t, const float (&x)[4]) {
 #pragma unroll
           for (int e = 0; e < 4; ++e)
             *reinterpret_cast<__half*>(sm.vt + tile_off(4 * lane + e, t, DN_SBO_V)) = __float2half_rn(x[e]);
-        }
+        });
       } else {
         uint8_t* vt = sm.vt;
         const uint8_t* vr = sm.rec_v[st];
@@ -722,51 +739,84 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
       tc_fence_before();
       mbar_arrive_warp(&sm.p_full[h], lane);
     }
-    // ---- epilogue (softmax warps), once per token half: O rows -> shared memory (the q tiles are dead: every QK^T has
-    //      completed), inverse Hadamard, partial {m, l, o[128]} per query row into set DENSE_SETS * split + half --------
+    // ---- epilogue (softmax warps): the two token halves of a row are LSE-merged here (m = max, weights 2^(m_h - m)),
+    //      O rows -> shared memory (the q tiles are dead: every QK^T has completed), inverse Hadamard; then either the
+    //      normalised result (one CTA per row tile: splits == 1) or the partial {m, l, o[128]} of set `split` -----------
     float* stage = reinterpret_cast<float*>(sm.qhi);     // [128][128] fp32 = qhi + qlo
+    float2* ml = sm.ml();                                // [0, 256): {m, l} of (half, row); [256, 384): merged
+    ml[128 * h + r] = make_float2(m_ref, l_run);
+    if (n_tot > 0) {
+      mbar_wait(&sm.bar_o[h], (n_tot - 1) & 1);
+      tc_fence_after();
+    }
+    softmax_sync();
+    const float2 a0 = ml[r], a1 = ml[128 + r];
+    const float m_row = fmaxf(a0.x, a1.x);
+    const float w0 = a0.x == -INFINITY ? 0.f : ex2_approx(a0.x - m_row), w1 = a1.x == -INFINITY ? 0.f : ex2_approx(a1.x - m_row);
+    const float w_me = h ? w1 : w0;
+    if (h == 0) {
+      ml[256 + r] = make_float2(m_row, fmaf(w0, a0.y, w1 * a1.y));
 #pragma unroll 1
-    for (int hh = 0; hh < DENSE_SETS; ++hh) {
-      if (h == hh) {
-        if (n_tot > 0) {
-          mbar_wait(&sm.bar_o[hh], (n_tot - 1) & 1);
-          tc_fence_after();
-#pragma unroll 1
-          for (int c0 = 0; c0 < 128; c0 += 16) {
-            uint32_t u[16];
-            tmem_ld16(t_o + c0, u);
+      for (int c0 = 0; c0 < 128; c0 += 16) {
+        uint32_t u[16];
+        if (n_tot > 0) tmem_ld16(t_o + c0, u);
 #pragma unroll
-            for (int j = 0; j < 16; j += 4)
-              *reinterpret_cast<uint4*>(&stage[r * 128 + ((c0 + j) ^ ((r & 7) << 2))]) = make_uint4(u[j], u[j + 1], u[j + 2], u[j + 3]);
-          }
+        for (int j = 0; j < 16; j += 4) {
+          float4 o4 = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (w_me > 0.f) o4 = make_float4(w_me * __uint_as_float(u[j]), w_me * __uint_as_float(u[j + 1]),
+                                           w_me * __uint_as_float(u[j + 2]), w_me * __uint_as_float(u[j + 3]));
+          *reinterpret_cast<float4*>(&stage[r * 128 + ((c0 + j) ^ ((r & 7) << 2))]) = o4;
         }
-        sm.ml()[r] = make_float2(m_ref, l_run);
-        tc_fence_before();
       }
-      softmax_sync();
-      for (int rr = warp; rr < 128; rr += 8) {
-        const int R = rt * 128 + rr;
-        if (R >= n_rows) break;
-        const int i = R / g, hq = R - i * g;
-        const size_t row = ((size_t)b * A.n_q + i) * A.Hq + hkv * g + hq;
-        float* prow = A.parts + ((size_t)(DENSE_SETS * split + hh) * ((size_t)A.B * A.n_q * A.Hq) + row) * PART_STRIDE;
-        float v[4] = {0.f, 0.f, 0.f, 0.f};
-        if (n_tot > 0) {
-          const float4 s4 = *reinterpret_cast<const float4*>(&stage[rr * 128 + ((4 * lane) ^ ((rr & 7) << 2))]);
-          v[0] = s4.x; v[1] = s4.y; v[2] = s4.z; v[3] = s4.w;
-          if (A.rotate_v) {
-            fwht128_lane4(v, lane);
+    }
+    softmax_sync();
+    if (h == 1 && n_tot > 0) {                           // (warp-uniform: tcgen05.ld is a warp-wide instruction)
+#pragma unroll 1
+      for (int c0 = 0; c0 < 128; c0 += 16) {
+        uint32_t u[16];
+        tmem_ld16(t_o + c0, u);
+        if (w_me > 0.f) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
+          for (int j = 0; j < 16; j += 4) {
+            float4* sp = reinterpret_cast<float4*>(&stage[r * 128 + ((c0 + j) ^ ((r & 7) << 2))]);
+            float4 o4 = *sp;
+            o4.x = fmaf(w_me, __uint_as_float(u[j]), o4.x); o4.y = fmaf(w_me, __uint_as_float(u[j + 1]), o4.y);
+            o4.z = fmaf(w_me, __uint_as_float(u[j + 2]), o4.z); o4.w = fmaf(w_me, __uint_as_float(u[j + 3]), o4.w);
+            *sp = o4;
           }
         }
+      }
+    }
+    tc_fence_before();
+    softmax_sync();
+    const bool direct = A.splits == 1;
+    for (int rr = warp; rr < 128; rr += 8) {
+      const int R = rt * 128 + rr;
+      if (R >= n_rows) break;
+      const int i = R / g, hq = R - i * g;
+      const size_t row = ((size_t)b * A.n_q + i) * A.Hq + hkv * g + hq;
+      const float4 s4 = *reinterpret_cast<const float4*>(&stage[rr * 128 + ((4 * lane) ^ ((rr & 7) << 2))]);
+      float v[4] = {s4.x, s4.y, s4.z, s4.w};
+      if (A.rotate_v) {
+        fwht128_lane4(v, lane);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
+      }
+      const float2 mlr = ml[256 + rr];
+      if (direct) {
+        const float inv = mlr.y > 0.f ? 1.f / mlr.y : 0.f;     // an empty cache and an empty block: zeros
+        if (A.out_dtype == KVARN_F32) {
+          *reinterpret_cast<float4*>(reinterpret_cast<float*>(A.out) + row * D + 4 * lane) = make_float4(v[0] * inv, v[1] * inv, v[2] * inv, v[3] * inv);
+        } else {
+          const __nv_bfloat162 o01 = __floats2bfloat162_rn(v[0] * inv, v[1] * inv), o23 = __floats2bfloat162_rn(v[2] * inv, v[3] * inv);
+          *reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(A.out) + row * D + 4 * lane) =
+              make_uint2(*reinterpret_cast<const uint32_t*>(&o01), *reinterpret_cast<const uint32_t*>(&o23));
+        }
+      } else {
+        float* prow = A.parts + ((size_t)split * ((size_t)A.B * A.n_q * A.Hq) + row) * PART_STRIDE;
         *reinterpret_cast<float4*>(prow + 4 + 4 * lane) = make_float4(v[0], v[1], v[2], v[3]);
-        if (lane == 0) {
-          const float2 ml = sm.ml()[rr];
-          *reinterpret_cast<float4*>(prow) = make_float4(n_tot > 0 ? ml.x : -INFINITY, n_tot > 0 ? ml.y : 0.f, 0.f, 0.f);
-        }
+        if (lane == 0) *reinterpret_cast<float4*>(prow) = make_float4(mlr.x, mlr.y, 0.f, 0.f);
       }
-      softmax_sync();
     }
   }
   tc_fence_before();

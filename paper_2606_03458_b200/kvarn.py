@@ -210,6 +210,7 @@ class Cache:
     def slice(self, b0: int, b1: int) -> "Cache":
         """A cache over sequences b0..b1-1 that shares this cache's buffers (views, no copy):
         lets a large cache be filled or read a few sequences at a time."""
+        assert 0 <= b0 < b1 <= self.B, (b0, b1, self.B)
         c = Cache.__new__(Cache)
         c.B, c.Hkv, c.max_chunks, c.rb, c.n_sink = b1 - b0, self.Hkv, self.max_chunks, self.rb, self.n_sink
         c.k_sink, c.v_sink = self.k_sink[b0:b1], self.v_sink[b0:b1]
