@@ -838,28 +838,8 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
       ws.aux_a[4 * lane + 0].x = a01.x; ws.aux_a[4 * lane + 1].x = a01.y;
       ws.aux_a[4 * lane + 2].x = a23.x; ws.aux_a[4 * lane + 3].x = a23.y;
     }
-    __syncwarp();
-    // ---- D3: QK^T over the 8 m-tiles: raw integer sums -> float (the scales follow once V's aux is there) ----
-    float sraw[4][HPW][4];
-    {
-      uint4 bf[2][NTQ];
-#pragma unroll
-      for (int hk = 0; hk < 2; ++hk)
-#pragma unroll
-        for (int nu = 0; nu < NTQ; ++nu) bf[hk][nu] = *reinterpret_cast<const uint4*>(&ws.bfr[nu][hk][b_slot(lane, hk)][0]);
-#pragma unroll
-      for (int mp = 0; mp < 4; ++mp) {
-        int32_t dd[2][NTQ][4];
-        contract_mp<BITS, NTQ, NTQ, true, DQ == 2, DQ == 2>(ws.krec, bf, mp, lane, dd, A.shl_mul);
-#pragma unroll
-        for (int u = 0; u < HPW; ++u)
-#pragma unroll
-          for (int i = 0; i < 4; ++i) sraw[mp][u][i] = undigit_w<DQ, NTQ>(dd, i >> 1, u, 2 * (i & 1));   // i = 2 mt + rho
-      }
-    }
-    __syncwarp();
-    // the K slot is free (codes consumed, aux read in phase A): request the next chunk's K record
-    if (lane == 0 && more) { mbar_expect_tx(&ws.fullk, RB); bulk_g2s(ws.krec, krec + (size_t)(4 * (it + 1)) * RB, RB, &ws.fullk); }
+    // (the V record's aux conversions sit here, ahead of the QK^T contraction they do not depend on: independent work
+    //  for the scheduler while the tensor-core chains run; the V record was requested a whole iteration ago)
     mbar_wait(&ws.fullv, par);
     {   // aux of the V record: per-token (row-slot order) s1v, zv; per-channel s2v
       const uint8_t* vr = ws.vrec;
@@ -887,6 +867,27 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
       }
     }
     __syncwarp();
+    // ---- D3: QK^T over the 8 m-tiles: raw integer sums -> float (the scales follow once V's aux is there) ----
+    float sraw[4][HPW][4];
+    {
+      uint4 bf[2][NTQ];
+#pragma unroll
+      for (int hk = 0; hk < 2; ++hk)
+#pragma unroll
+        for (int nu = 0; nu < NTQ; ++nu) bf[hk][nu] = *reinterpret_cast<const uint4*>(&ws.bfr[nu][hk][b_slot(lane, hk)][0]);
+#pragma unroll
+      for (int mp = 0; mp < 4; ++mp) {
+        int32_t dd[2][NTQ][4];
+        contract_mp<BITS, NTQ, NTQ, true, DQ == 2, DQ == 2>(ws.krec, bf, mp, lane, dd, A.shl_mul);
+#pragma unroll
+        for (int u = 0; u < HPW; ++u)
+#pragma unroll
+          for (int i = 0; i < 4; ++i) sraw[mp][u][i] = undigit_w<DQ, NTQ>(dd, i >> 1, u, 2 * (i & 1));   // i = 2 mt + rho
+      }
+    }
+    __syncwarp();
+    // the K slot is free (codes consumed, aux read in phase A): request the next chunk's K record
+    if (lane == 0 && more) { mbar_expect_tx(&ws.fullk, RB); bulk_g2s(ws.krec, krec + (size_t)(4 * (it + 1)) * RB, RB, &ws.fullk); }
     // ---- D3 (scales) + D4: logits of this thread's 16 tokens x HPW columns, maximum over the chunk -----------
     float corr[HPW], wch[HPW], zsum[HPW];
 #pragma unroll
