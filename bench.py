@@ -764,7 +764,7 @@ def main():
                 "hbm_achieved_GBps": q_gbs, "hbm_frac": q_gbs / hbm_peak, "ms": q_ms}
     dn = ex.get("block_dense_long_g4_2bit_nq128") or {}
     tp, tp_src = tensor_peak()
-    rl_dense = {"kernel": "block_dense_kernel<2,bf16> (+ raw-window decode + merge), B16 32/8 ctx 65536, n_q = 128", "bound": "tensor",
+    rl_dense = {"kernel": "block_dense_kernel<2,bf16> (packed chunks + raw windows; + merge_partials_kernel), B16 32/8 ctx 65536, n_q = 128", "bound": "tensor",
                 "achieved": dn.get("TFLOPs"), "peak": tp, "unit": "TFLOP/s", "frac": dn.get("tensor_frac"), "traffic": None,
                 "peak_source": tp_src, "us": dn.get("us")} if dn else None
     line = {
