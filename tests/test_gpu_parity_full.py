@@ -265,3 +265,50 @@ def test_storage_rounding_tie_rate_over_2000_tiles(kv):
         print(f"{bits}-bit: {stats}; aux tie rate {rate:.2e}, code tie rate {stats['code_mismatch'] / stats['codes']:.2e}")
         assert stats["tiles"] == 4096 and rate <= P.AUX_MISMATCH_FRAC
         P.assert_mismatch_budget(stats)
+
+
+def _fill(kv, p, B, Hkv, ctx, seed):
+    cache = kv.Cache(p, B, Hkv, ctx // 128 + 1, device="cuda")
+    for b0 in range(0, B, 4):
+        K, V = W.kv_tokens(min(4, B - b0), Hkv, ctx, seed=seed + b0, device="cuda")
+        kv.prefill(p, cache.slice(b0, min(b0 + 4, B)), K, V)
+        del K, V
+    return cache
+
+
+@pytest.mark.parametrize("n_q", [32, 128])
+def test_block_attention_at_64k_context_in_the_bench_configuration(kv, n_q):
+    """Both block-attention forms in the launch configuration bench.py times (B = 16, 32 / 8 heads, 65 536 + 37 tokens,
+    2-bit; n_q = 32: one row tile per CTA, direct output; n_q = 128: four row tiles x two chunk ranges + merge for the
+    dense kernel): sampled (sequence, KV head, query token) triples against the oracle's plain-definition attention of
+    that query over the GPU's records, the raw residual tokens and the block tokens it may see (causal); the dense and
+    the integer form against each other on every row."""
+    B, Hq, Hkv, ctx = 16, 32, 8, 65536 + 37
+    g = Hq // Hkv
+    p = kv.default_params(2)
+    cache = _fill(kv, p, B, Hkv, ctx, seed=77)
+    q = torch.stack([W.queries(B, Hq, seed=900 + i, device="cuda") for i in range(n_q)], dim=1).contiguous()
+    kb, vb = W.kv_tokens(B, Hkv, n_q, seed=950, device="cuda", sink_first=False)
+    dense = kv.block_attention(p, cache, q, kb, vb, dense=True)
+    triples = [(0, 0, 0), (7, 3, n_q // 2), (15, 7, n_q - 1)]
+    jobs = []
+    for b, h, i in triples:
+        ns, nc, r = O.cache_partition(ctx, cache.n_sink)
+        kt = [kv.unpack_record(p, 0, rec) for rec in cache.k_records[b, h, :nc].cpu().numpy()]
+        vt = [kv.unpack_record(p, 1, rec) for rec in cache.v_records[b, h, :nc].cpu().numpy()]
+        kraw = np.concatenate([P.tile_f64(cache.k_resid[b, h, :r]), P.tile_f64(kb[b, h, :i + 1])])
+        vraw = np.concatenate([P.tile_f64(cache.v_resid[b, h, :r]), P.tile_f64(vb[b, h, :i + 1])])
+        jobs.append((P.tile_f64(q[b, i, h * g:(h + 1) * g]), kt, vt, kraw, vraw, None, True, True))
+    refs = fanout.pmap("decode", jobs)
+    forms = {"dense": dense}
+    if n_q == 32:                                   # the integer form costs 140 us per query token: only on the smaller block
+        forms["integer"] = kv.block_attention(p, cache, q, kb, vb)
+    for name, out in forms.items():
+        o = out.to(torch.float64).cpu().numpy()
+        for (b, h, i), ref in zip(triples, refs):
+            err = P.attn_rel_err(o[b, i, h * g:(h + 1) * g], ref)
+            assert err <= P.ATTN_RTOL, (name, b, h, i, err)
+    if n_q == 32:
+        d = (forms["dense"].double() - forms["integer"].double()).abs().amax(dim=-1)
+        scale = forms["integer"].double().abs().amax(dim=-1).clamp_min(1e-30)
+        assert float((d / scale).max()) <= P.ATTN_RTOL
