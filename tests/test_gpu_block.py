@@ -263,3 +263,26 @@ def test_block_attention_token_scale_spread_and_dominant_keys(kv, bits, dense):
         ref = _oracle_block(kv, p, cache, 0, h, g, q, kb, vb, n_tok)
         err = np.abs(o[0, :, h * g:(h + 1) * g] - ref).max() / np.abs(ref).max()
         assert err <= P.ATTN_RTOL, (h, err)
+
+
+@pytest.mark.parametrize("dense", [False, True])
+def test_block_attention_ragged_lengths_in_one_batch(kv, dense):
+    """Sequences of very different lengths in one call (41 chunks, 3 chunks + a residual window, 5 raw tokens, an empty
+    cache): the dense kernel's chunk ranges are planned from the cache's capacity, so most CTAs of the short sequences
+    own no chunk at all and the last one owns only the raw windows."""
+    lens = [128 * 41 + 9, 128 * 3 + 70, 5, 0]
+    B, Hq, Hkv, n_q = len(lens), 4, 1, 32
+    p = kv.default_params(2)
+    cache = kv.Cache(p, B, Hkv, 42, device="cuda")
+    q = torch.stack([W.queries(B, Hq, seed=700 + i, device="cuda") for i in range(n_q)], dim=1).contiguous()
+    kb, vb = W.kv_tokens(B, Hkv, n_q, seed=701, device="cuda", sink_first=False)
+    for b, n in enumerate(lens):
+        K, V = W.kv_tokens(1, Hkv, max(n, 1), seed=710 + b, device="cuda")
+        kv.prefill(p, cache.slice(b, b + 1), K[:, :, :n].contiguous(), V[:, :, :n].contiguous())
+    assert cache.seq_lens.tolist() == lens
+    out = kv.block_attention(p, cache, q, kb, vb, dense=dense).to(torch.float64).cpu().numpy()
+    g = Hq // Hkv
+    for b, n in enumerate(lens):
+        ref = _oracle_block(kv, p, cache, b, 0, g, q, kb, vb, n)
+        err = P.attn_rel_err(out[b, :, 0:g].reshape(-1, 128), ref.reshape(-1, 128))
+        assert err <= P.ATTN_RTOL, (b, n, err)
