@@ -233,12 +233,12 @@ def replica_seed(base: int, layer: int, rank: int) -> int:
     return base + 100 * layer + 1000 * rank
 
 
-def workload_config(shape, layers):
+def workload_config(shape, layers, eager=False):
     return {"workload": "BASELINE.json configs[1]: Llama-3.1-8B-shaped decode layer",
             "B": shape.B, "Hq": shape.Hq, "Hkv": shape.Hkv, "head_dim": D, "ctx": shape.ctx,
             "chunks": shape.n_chunks, "resid": shape.resid, "bits": shape.bits,
-            "step": "kvarn_quantize_chunk(2x%d tiles) of one layer + kvarn_decode_attention of all %d layers (one launch per layer)"
-                    % (shape.B * shape.Hkv * shape.n_chunks, layers),
+            "step": "kvarn_quantize_chunk(2x%d tiles) of one layer + kvarn_decode_attention of all %d layers (one launch per layer%s)"
+                    % (shape.B * shape.Hkv * shape.n_chunks, layers, "" if eager else ", replayed as one CUDA graph"),
             "l2": "inputs larger than L2: %d layer caches read in rotation (%d MB of records per step)"
                   % (layers, layers * 2 * shape.B * shape.Hkv * shape.n_chunks * 4608 // 1000000),
             "parallelism": "replicas"}
@@ -576,6 +576,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--extras-only", action="store_true",
                     help="run only the configs[2] / [3] / [4] measurements (profiling aid)")
+    ap.add_argument("--eager-step", action="store_true",
+                    help="launch the step's L decode kernels one by one instead of replaying their CUDA graph")
     ap.add_argument("--only", default="", help="with --extras-only: comma-separated extras groups to run")
     ap.add_argument("--mode", default="replicas", choices=["replicas", "cp"],
                     help="replicas (default): N independent replicas of the configs[1] step; cp: configs[4] decode with every "
@@ -649,13 +651,35 @@ def main():
         if ev: ev[0].record(stream)
         kv.quantize_chunk(p, Ks[lq], Vs[lq], c.k_records.view(n_tiles, rb), c.v_records.view(n_tiles, rb))
         if ev: ev[1].record(stream)
-        for l in range(L):
-            ld = (lq + 1 + l) % L
-            kv.decode_attention(p, caches[ld], qs[ld], out=out, ws=ws)
+        if dec_graphs is not None:
+            dec_graphs[lq].replay()            # the same L launches, captured once (what a serving loop replays per step)
+        else:
+            for l in range(L):
+                ld = (lq + 1 + l) % L
+                kv.decode_attention(p, caches[ld], qs[ld], out=out, ws=ws)
         if ev: ev[2].record(stream)
 
+    dec_graphs = None
     for l in range(L):   # fill every cache once (untimed) so decode always reads real records
         step(l)
+    if not args.eager_step:
+        # the L decode launches of a step as one CUDA graph per rotation (the layer quantised in the step is decoded
+        # last, after the other L - 1 caches have gone through L2)
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        graphs = []
+        for r in range(L):
+            g = torch.cuda.CUDAGraph()
+            side.wait_stream(stream)
+            with torch.cuda.stream(side):
+                with torch.cuda.graph(g, stream=side):
+                    for l in range(L):
+                        ld = (r + 1 + l) % L
+                        kv.decode_attention(p, caches[ld], qs[ld], out=out, ws=ws, stream=side)
+            stream.wait_stream(side)
+            graphs.append(g)
+        torch.cuda.synchronize()
+        dec_graphs = graphs
     for i in range(args.warmup):
         step(i)
     torch.cuda.synchronize()
@@ -754,8 +778,8 @@ def main():
     rl_dec = {"kernel": "decode_kernel<2,4,2,bf16> (configs[1])", "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak,
               "unit": "GB/s", "frac": dec_gbs / hbm_peak, "traffic": tr.get("decode_kernel"),
               "algorithmic_bytes": dec_bytes, "peak_source": peak_src, "us": d_ms * 1e3,
-              "timing": "CUDA events around the step's L decode launches, divided by L; also.cfg1_decode_single_launch_us: one launch "
-                        "per event pair; also.cfg1_decode_graph_*: 24 launches in one CUDA graph",
+              "timing": "CUDA events around the step's L decode launches (replayed as one CUDA graph unless --eager-step), divided by L; "
+                        "also.cfg1_decode_single_launch_us: one launch per event pair; also.cfg1_decode_graph_*: 24 launches in one CUDA graph",
               "also": also}
     rl_quant = {"kernel": "quantize_kernel<2,bf16>", "bound": "alu", "achieved": q_tflops,
                 "peak": FP32_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s", "frac": q_tflops / FP32_PEAK_TFLOPS_NOMINAL,
@@ -771,7 +795,7 @@ def main():
         "metric": "kvarn_2bit_decode_attn_GBps", "value": world * dec_gbs, "unit": "GB/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": workload_config(shape, L),
+        "config": workload_config(shape, L, args.eager_step),
         "decode_us_per_step": d_ms * 1e3, "quantize_ms_per_step": q_ms,
         "quantize_tokens_per_s": world * tok_s, "quantize_tiles_per_s": world * 2 * n_tiles / (q_ms * 1e-3),
         "extras": extras, "rooflines": {"quantize": rl_quant, "block_dense": rl_dense},
