@@ -309,7 +309,23 @@ __device__ __forceinline__ void decode_finish(const DecodeArgs& A, SM& sm, float
   const int bh = w1.bh, b = w1.b, hkv = w1.hkv, split = w1.split, n_sink_tok = w1.n_sink_tok, resid = w1.resid;
   const int lg = cm.lg, tok0 = cm.tok0, ncols = cm.ncols, n_q = cm.n_q, blk_cnt = cm.blk_cnt;
   const bool has_blk = A.k_blk != nullptr;
-  const bool do_blk = (split == A.splits - 1) && has_blk;
+  // Every raw window (sink, residual, the block's own tokens) is cut into A.splits slices of >= RAW_SLICE_MIN tokens, one
+  // per CTA of the (sequence, KV head): a window's cost is the latency of its dependent global loads (thread = token, few
+  // warps), so slices run side by side instead of one CTA walking 128 tokens; the partials merge like the chunks'.
+  constexpr int RAW_SLICE_MIN = 16;
+  auto slice = [&](int cnt, int& t0, int& n) {
+    int per_w = (cnt + A.splits - 1) / A.splits;
+    per_w = per_w < RAW_SLICE_MIN ? RAW_SLICE_MIN : per_w;
+    t0 = split * per_w;
+    n = min(max(cnt - t0, 0), per_w);
+  };
+  int sink_t0, sink_n, res_t0, res_n, blk_t0, blk_n;
+  slice(n_sink_tok, sink_t0, sink_n);
+  slice(resid, res_t0, res_n);
+  slice(has_blk ? blk_cnt : 0, blk_t0, blk_n);
+  const bool ran_raw = (sink_n | res_n | blk_n) > 0;                 // CTA-uniform
+  const bool any_raw = n_sink_tok > 0 || resid > 0 || has_blk;       // uniform over the CTAs of this (sequence, KV head)
+  (void)do_resid; (void)do_sink;
   auto qrow = [&](int j) -> size_t { return ((size_t)b * n_q + tok0 + (j >> lg)) * A.Hq + hkv * g + (j - ((j >> lg) << lg)); };
   // ---- D6: raw windows (sink tokens of split 0, residual window of the last split; un-rotated space) ----
   float acc_res[GP];
@@ -365,9 +381,11 @@ __device__ __forceinline__ void decode_finish(const DecodeArgs& A, SM& sm, float
     for (int h = 0; h < GP; ++h) {
       const float mc = fmaxf(fmaxf(sm.wmax[0][h], sm.wmax[1][h]), fmaxf(sm.wmax[2][h], sm.wmax[3][h]));
       const float m_new = fmaxf(m_run[h], mc);
-      const float corr = exp2f(m_run[h] - m_new);
+      // (a column that has seen nothing yet and sees nothing of this slice either -- a causal slice beyond its query
+      //  token in a CTA without chunks -- keeps m = -inf: no NaN from -inf - -inf)
+      const float corr = m_new == -INFINITY ? 1.f : exp2f(m_run[h] - m_new);
       m_run[h] = m_new;
-      p[h] = exp2f(logit[h] - m_new);        // exp2(-inf) = 0 for masked tokens
+      p[h] = m_new == -INFINITY ? 0.f : exp2f(logit[h] - m_new);        // exp2(-inf) = 0 for masked tokens
       l_part[h] = fmaf(l_part[h], corr, p[h]);
       acc[h] *= corr;
       acc_res[h] *= corr;
@@ -395,18 +413,18 @@ __device__ __forceinline__ void decode_finish(const DecodeArgs& A, SM& sm, float
     }
     __syncthreads();   // psm and wmax are free again
   };
-  if (do_sink)
-    raw_window(reinterpret_cast<const InT*>(A.k_sink) + (size_t)bh * A.n_sink * D,
-               reinterpret_cast<const InT*>(A.v_sink) + (size_t)bh * A.n_sink * D, n_sink_tok, NO_MASK);
-  if (do_resid)
-    raw_window(reinterpret_cast<const InT*>(A.k_resid) + (size_t)bh * G * D,
-               reinterpret_cast<const InT*>(A.v_resid) + (size_t)bh * G * D, resid, NO_MASK);
-  if (do_blk)
-    raw_window(reinterpret_cast<const InT*>(A.k_blk) + (size_t)bh * n_q * D,
-               reinterpret_cast<const InT*>(A.v_blk) + (size_t)bh * n_q * D, blk_cnt, tok0);
+  if (sink_n > 0)
+    raw_window(reinterpret_cast<const InT*>(A.k_sink) + ((size_t)bh * A.n_sink + sink_t0) * D,
+               reinterpret_cast<const InT*>(A.v_sink) + ((size_t)bh * A.n_sink + sink_t0) * D, sink_n, NO_MASK);
+  if (res_n > 0)
+    raw_window(reinterpret_cast<const InT*>(A.k_resid) + ((size_t)bh * G + res_t0) * D,
+               reinterpret_cast<const InT*>(A.v_resid) + ((size_t)bh * G + res_t0) * D, res_n, NO_MASK);
+  if (blk_n > 0)       // causal: block token blk_t0 + tid is visible to query token i iff blk_t0 + tid <= i
+    raw_window(reinterpret_cast<const InT*>(A.k_blk) + ((size_t)bh * n_q + blk_t0) * D,
+               reinterpret_cast<const InT*>(A.v_blk) + ((size_t)bh * n_q + blk_t0) * D, blk_n, tok0 - blk_t0);
 
   // ---- l: reduce the per-thread partial sums (only a CTA that ran a raw window has any beyond the chunks') ----
-  if (do_sink || do_resid || do_blk) {   // CTA-uniform
+  if (ran_raw) {   // CTA-uniform
     __syncthreads();
     {
       float v[GP];
@@ -438,12 +456,10 @@ __device__ __forceinline__ void decode_finish(const DecodeArgs& A, SM& sm, float
         const uint32_t dst = mapa_shared(land_addr + (uint32_t)(j * CS + crank) * (WS_STRIDE * 4), (uint32_t)d);
         if (tid == 0) { st_cluster_f32(dst, m_run[h]); st_cluster_f32(dst + 4, l_tot[h]); }
         st_cluster_f32(dst + 16 + 4 * tid, acc[h]);
-        if (do_resid || do_sink || do_blk) st_cluster_f32(dst + 16 + 512 + 4 * tid, acc_res[h]);
+        if (any_raw) st_cluster_f32(dst + 16 + 512 + 4 * tid, acc_res[h]);
       }
     }
     cluster_sync_all();
-    const bool res_here = (resid > 0 || has_blk) && split / CS == NC - 1;   // this cluster's last rank ran the residual window
-    const bool sink_here = n_sink_tok > 0 && split / CS == 0;    // this cluster's rank 0 ran the sink window
 #pragma unroll
     for (int j = 0; j < GP; ++j) {
       const int h = crank + j * CS;
@@ -456,7 +472,7 @@ __device__ __forceinline__ void decode_finish(const DecodeArgs& A, SM& sm, float
           const float w = (sl[0] == -INFINITY) ? 0.f : ex2_approx(sl[0] - mj);
           lj = fmaf(w, sl[1], lj);
           aj = fmaf(w, sl[4 + tid], aj);
-          if ((res_here && r == CS - 1) || (sink_here && r == 0)) rj = fmaf(w, sl[132 + tid], rj);
+          if (any_raw) rj = fmaf(w, sl[132 + tid], rj);
         }
       }
       m_run[j] = mj; l_tot[j] = lj; acc[j] = aj; acc_res[j] = rj;
@@ -718,10 +734,8 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
   const ColMap cm0 = col_map<false>(A);
   const bool do_resid = (w0.split == A.splits - 1) && w0.resid > 0;
   const bool do_sink = (w0.split == 0) && w0.n_sink_tok > 0;
-  // ---- chunk range of this split (balanced against the raw windows as in the CTA-cooperative variant) ----
-  // (a raw window of n tokens keeps its CTA as long as ~n / 8 chunks do -- measured on the 64k-context cache with
-  //  a 128-token sink and a 64-token residual window --, so the splits that own one get that many chunks fewer)
-  const int w_sink = (w0.n_sink_tok + 7) / 8, w_res = (w0.resid + cm0.blk_cnt + 7) / 8;
+  // ---- chunk range of this split (the raw windows are sliced over all the CTAs of the unit: decode_finish) ----
+  const int w_sink = 0, w_res = 0;
   const int nch = A.skip_chunks ? 0 : w0.n_chunks;
   const int per = (nch + w_sink + w_res + A.splits - 1) / A.splits;
   const int c_begin = min(max(w0.split * per - w_sink, 0), nch);
@@ -1013,7 +1027,7 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
   // dead slots: [0, 16 x WS_STRIDE floats) landing area of the peers' partials, w[2] un-rotated q of the raw windows, w[3] merge weights
   static_assert(sizeof(WS) * 2 >= 16 * WS_STRIDE * sizeof(float) && sizeof(WS) >= GP * 128 * sizeof(float), "landing / scratch areas");
   float* qraw = reinterpret_cast<float*>(&sm.w[2]);
-  if (do_resid || do_sink || (A.k_blk != nullptr && w0.split == A.splits - 1)) {   // CTA-uniform: this CTA runs a raw window
+  if (w0.n_sink_tok > 0 || w0.resid > 0 || A.k_blk != nullptr) {   // CTA-uniform: this CTA may run a slice of a raw window
     for (int hh = warp; hh < GP; hh += 4) {
       float v[4] = {0.f, 0.f, 0.f, 0.f};
       if (hh < cm0.ncols) {
