@@ -294,6 +294,23 @@ __device__ __forceinline__ ColMap col_map(const DecodeArgs& A) {
   return c;
 }
 
+// Slice `split` of a raw window of cnt tokens cut over n_splits CTAs (>= RAW_SLICE_MIN tokens per slice): first token, count.
+constexpr int RAW_SLICE_MIN = 16;
+__device__ __forceinline__ void raw_slice(int cnt, int split, int n_splits, int& t0, int& n) {
+  int per_w = (cnt + n_splits - 1) / n_splits;
+  per_w = per_w < RAW_SLICE_MIN ? RAW_SLICE_MIN : per_w;
+  t0 = split * per_w;
+  n = min(max(cnt - t0, 0), per_w);
+}
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// the n rows (128 values each) at `base` towards L2: one 128-byte line per thread and step
+template <typename InT>
+__device__ __forceinline__ void prefetch_rows(const InT* base, int n, int tid) {
+  const char* p = reinterpret_cast<const char*>(base);
+  const int bytes = n * D * (int)sizeof(InT);
+  for (int o = tid * 128; o < bytes; o += 128 * 128) prefetch_l2(p + o);
+}
+
 // ---- D6 + D7 of one CTA, shared by both main-loop variants: raw windows, merge of the split partials, finish.
 // On entry thread tid = channel tid holds, per column h: m_run[h] (running maximum of the chunks, CTA-wide),
 // l_tot[h] (l of the chunks, CTA-wide), l_part[h] (thread 0: l_tot, others 0) and acc[h] (its channel of the
@@ -312,17 +329,10 @@ __device__ __forceinline__ void decode_finish(const DecodeArgs& A, SM& sm, float
   // Every raw window (sink, residual, the block's own tokens) is cut into A.splits slices of >= RAW_SLICE_MIN tokens, one
   // per CTA of the (sequence, KV head): a window's cost is the latency of its dependent global loads (thread = token, few
   // warps), so slices run side by side instead of one CTA walking 128 tokens; the partials merge like the chunks'.
-  constexpr int RAW_SLICE_MIN = 16;
-  auto slice = [&](int cnt, int& t0, int& n) {
-    int per_w = (cnt + A.splits - 1) / A.splits;
-    per_w = per_w < RAW_SLICE_MIN ? RAW_SLICE_MIN : per_w;
-    t0 = split * per_w;
-    n = min(max(cnt - t0, 0), per_w);
-  };
   int sink_t0, sink_n, res_t0, res_n, blk_t0, blk_n;
-  slice(n_sink_tok, sink_t0, sink_n);
-  slice(resid, res_t0, res_n);
-  slice(has_blk ? blk_cnt : 0, blk_t0, blk_n);
+  raw_slice(n_sink_tok, split, A.splits, sink_t0, sink_n);
+  raw_slice(resid, split, A.splits, res_t0, res_n);
+  raw_slice(has_blk ? blk_cnt : 0, split, A.splits, blk_t0, blk_n);
   const bool ran_raw = (sink_n | res_n | blk_n) > 0;                 // CTA-uniform
   const bool any_raw = n_sink_tok > 0 || resid > 0 || has_blk;       // uniform over the CTAs of this (sequence, KV head)
   (void)do_resid; (void)do_sink;
@@ -744,6 +754,25 @@ __global__ void __launch_bounds__(128, BITS == 2 ? (GP == 4 ? KVARN_DECW_OCC4 : 
   const uint8_t* krec = A.k_records + ((size_t)w0.bh * A.max_chunks + c_begin + warp) * RB;
   const uint8_t* vrec = A.v_records + ((size_t)w0.bh * A.max_chunks + c_begin + warp) * RB;
 
+  // this CTA's slices of the raw windows go towards L2 now: decode_finish reads them with dependent loads, long after
+  {
+    int t0, n;
+    raw_slice(w0.n_sink_tok, w0.split, A.splits, t0, n);
+    if (n > 0) {
+      prefetch_rows(reinterpret_cast<const InT*>(A.k_sink) + ((size_t)w0.bh * A.n_sink + t0) * D, n, tid);
+      prefetch_rows(reinterpret_cast<const InT*>(A.v_sink) + ((size_t)w0.bh * A.n_sink + t0) * D, n, tid);
+    }
+    raw_slice(w0.resid, w0.split, A.splits, t0, n);
+    if (n > 0) {
+      prefetch_rows(reinterpret_cast<const InT*>(A.k_resid) + ((size_t)w0.bh * G + t0) * D, n, tid);
+      prefetch_rows(reinterpret_cast<const InT*>(A.v_resid) + ((size_t)w0.bh * G + t0) * D, n, tid);
+    }
+    raw_slice(A.k_blk != nullptr ? cm0.blk_cnt : 0, w0.split, A.splits, t0, n);
+    if (n > 0) {
+      prefetch_rows(reinterpret_cast<const InT*>(A.k_blk) + ((size_t)w0.bh * cm0.n_q + t0) * D, n, tid);
+      prefetch_rows(reinterpret_cast<const InT*>(A.v_blk) + ((size_t)w0.bh * cm0.n_q + t0) * D, n, tid);
+    }
+  }
   // ---- setup: the warp's barriers and first loads; q ---------------------------------------------------
   if (lane == 0) {
     mbar_init(&ws.fullk, 1); mbar_init(&ws.fullv, 1);
