@@ -297,6 +297,8 @@ __device__ __forceinline__ ColMap col_map(const DecodeArgs& A) {
 // Slice `split` of a raw window of cnt tokens cut over n_splits CTAs (>= RAW_SLICE_MIN tokens per slice): first token, count.
 constexpr int RAW_SLICE_MIN = 16;
 __device__ __forceinline__ void raw_slice(int cnt, int split, int n_splits, int& t0, int& n) {
+  t0 = 0; n = 0;
+  if (cnt <= 0) return;                      // (no window: no integer division either)
   int per_w = (cnt + n_splits - 1) / n_splits;
   per_w = per_w < RAW_SLICE_MIN ? RAW_SLICE_MIN : per_w;
   t0 = split * per_w;
