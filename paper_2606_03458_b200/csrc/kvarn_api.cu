@@ -231,7 +231,7 @@ struct SplitPlan { int cluster, nclus; };
 #ifndef KVARN_MAX_CLUSTER_OVERRIDE
 #define KVARN_MAX_CLUSTER_OVERRIDE 8
 #endif
-constexpr int KVARN_DENSE_CTA_COST = 18;    // fixed cost of a dense CTA / of the merge launch, in chunk-times (~2 us each)
+constexpr int KVARN_DENSE_CTA_COST = 14;    // fixed cost of a dense CTA / of the merge launch, in chunk-times (~2 us each)
 constexpr int KVARN_DENSE_MERGE_COST = 12;
 constexpr int KVARN_MAX_CLUSTER = KVARN_MAX_CLUSTER_OVERRIDE;    // portable maximum; 9..16 (non-portable) measured slower: 25 -> 27..31 us on config 1
 

@@ -316,10 +316,14 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sm.tmem_base)), "n"(TMEM_COLS));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
-  // zero the tiles once: rows / columns that are never rewritten (padding of N = 144 and of the K extents) stay zero
-  for (int i = tid; i < (int)(sizeof(sm.kt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.kt)[i] = make_uint4(0, 0, 0, 0);
-  for (int i = tid; i < (int)(sizeof(sm.vt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.vt)[i] = make_uint4(0, 0, 0, 0);
-  // q' = (q H / sqrt(128)) q_scale as two fp16 terms, columns in K-position order
+  // q' = (q H / sqrt(128)) q_scale as two fp16 terms, columns in K-position order.  Two steps, so that both sides of shared
+  // memory are conflict-free: (1) a warp rotates a row (lane = 4 channels) and writes it as fp32 into a scratch
+  // [128][132] that borrows the Kt buffers; (2) lane = (row of an 8-row group, unit of 8 K positions) reads its eight values
+  // and stores them as one 16-byte piece of the hi and of the lo tile: a quarter warp covers 128 contiguous bytes.
+  // (Writing 2-byte pieces straight from step 1 cost 16-way conflicts: 10 us per CTA.)
+  constexpr int QS = 132;                                                        // scratch row stride in floats
+  float* qscr = reinterpret_cast<float*>(sm.kt);
+  static_assert(sizeof(sm.kt) >= 128 * QS * sizeof(float), "q scratch borrows the Kt buffers");
   constexpr int QROWS = (128 + DENSE_THREADS / 32 - 1) / (DENSE_THREADS / 32);   // rows per warp: all loads in flight together
   float qv[QROWS][4];
 #pragma unroll
@@ -345,15 +349,30 @@ __global__ void __launch_bounds__(DENSE_THREADS, 1) block_dense_kernel(const Den
 #pragma unroll
       for (int j = 0; j < 4; ++j) v[j] *= 0.08838834764831845f;
     }
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const int kp = dense_kpos<BITS>(4 * lane + j);
-      const __half hi = __float2half_rn(v[j]);
-      const __half lo = __float2half_rn(v[j] - __half2float(hi));
-      *reinterpret_cast<__half*>(sm.qhi + kmaj_off(r, kp, DN_KT)) = hi;
-      *reinterpret_cast<__half*>(sm.qlo + kmaj_off(r, kp, DN_KT)) = lo;
-    }
+    *reinterpret_cast<float4*>(&qscr[r * QS + 4 * lane]) = make_float4(v[0], v[1], v[2], v[3]);
   }
+  __syncthreads();
+  for (int w = warp; w < 16 * 4; w += DENSE_THREADS / 32) {                      // (row group, quarter of the 16 units)
+    const int r = (w >> 2) * 8 + (lane & 7), u = (w & 3) * 4 + (lane >> 3);
+    const int e0 = dense_elem_of_kpos<BITS>(8 * u), e1 = dense_elem_of_kpos<BITS>(8 * u + 1);   // K positions 8u + 2i / + 2i + 1 = elements e0 + i / e1 + i
+    const float4 a = *reinterpret_cast<const float4*>(&qscr[r * QS + e0]);
+    const float4 c = *reinterpret_cast<const float4*>(&qscr[r * QS + e1]);
+    const float x[8] = {a.x, c.x, a.y, c.y, a.z, c.z, a.w, c.w};
+    uint32_t hi[4], lo[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const __half2 h2 = __floats2half2_rn(x[2 * i], x[2 * i + 1]);
+      const float2 hf = __half22float2(h2);
+      const __half2 l2 = __floats2half2_rn(x[2 * i] - hf.x, x[2 * i + 1] - hf.y);
+      hi[i] = *reinterpret_cast<const uint32_t*>(&h2); lo[i] = *reinterpret_cast<const uint32_t*>(&l2);
+    }
+    *reinterpret_cast<uint4*>(sm.qhi + kmaj_off(r, 8 * u, DN_KT)) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    *reinterpret_cast<uint4*>(sm.qlo + kmaj_off(r, 8 * u, DN_KT)) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+  }
+  __syncthreads();
+  // zero the tiles once: rows / columns that are never rewritten (padding of N = 144 and of the K extents) stay zero
+  for (int i = tid; i < (int)(sizeof(sm.kt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.kt)[i] = make_uint4(0, 0, 0, 0);
+  for (int i = tid; i < (int)(sizeof(sm.vt) / 16); i += DENSE_THREADS) reinterpret_cast<uint4*>(sm.vt)[i] = make_uint4(0, 0, 0, 0);
   fence_async_smem();
   tc_fence_before();
   __syncthreads();
