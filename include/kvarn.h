@@ -268,7 +268,8 @@ KVARN_API int kvarn_decode_attention(const kvarn_params* p, const kvarn_cache* c
  * KVARN_WORKSPACE_TOO_SMALL.  ALL calls on one GPU share the array: calls that may overlap on the GPU (different streams
  * without ordering) race; order them on one stream or use kvarn_decode_attention with separate workspaces.  The array
  * keeps the previous call's contents; the call clears the counters it needs on `stream` before the launch.
- * The device of `stream` must be current.
+ * The device of `stream` must be current.  The first call on a device does the one-time set-up (the array's device address,
+ * the kernel's shared-memory attribute): make it once before capturing the stream into a graph.
  */
 #define KVARN_STATIC_SCRATCH_BYTES (1u << 20)
 KVARN_API int kvarn_decode_attention_static(const kvarn_params* p, const kvarn_cache* cache, const void* q,
