@@ -76,3 +76,26 @@ def test_static_scratch_allocates_nothing_and_rejects_oversized_plans(kv):
     with pytest.raises(kv.KvarnError, match="KVARN_WORKSPACE_TOO_SMALL"):
         kv.decode_attention_static(pb, cb, qb)
     assert kv.decode_attention(pb, cb, qb).isfinite().all()        # the workspace path still serves that plan
+
+
+def test_static_scratch_under_cuda_graph_capture(kv):
+    """The use the entry point exists for: after one warm call, the call is captured into a CUDA graph (the counter
+    clear becomes a memset node, the kernel a kernel node) and the replays reproduce the workspace path's bits."""
+    p, cache, q = _case(kv, 2, 32, 8, 128 * 26 + 77, 16, seed=306)
+    ref = kv.decode_attention(p, cache, q)
+    out = torch.empty_like(ref)
+    kv.decode_attention_static(p, cache, q, out=out)              # one-time set-up outside the capture
+    torch.cuda.synchronize()
+    out.zero_()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            kv.decode_attention_static(p, cache, q, out=out, stream=side)
+    torch.cuda.current_stream().wait_stream(side)
+    for _ in range(2):
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref)
