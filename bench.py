@@ -773,7 +773,10 @@ def main():
             "quantize_alu_frac": q_tflops / FP32_PEAK_TFLOPS_NOMINAL, "quantize_hbm_frac": q_gbs / hbm_peak,
             "block_dense_nq32_us_per_token": (ex.get("block_dense_long_g4_2bit_nq32") or {}).get("us_per_query_token"),
             "block_dense_nq32_tensor_frac": (ex.get("block_dense_long_g4_2bit_nq32") or {}).get("tensor_frac"),
+            "block_dense_nq128_us_per_token": (ex.get("block_dense_long_g4_2bit_nq128") or {}).get("us_per_query_token"),
+            "block_dense_nq128_tensor_frac": (ex.get("block_dense_long_g4_2bit_nq128") or {}).get("tensor_frac"),
             "block_int_nq8_us_per_token": (ex.get("block_long_g4_2bit_nq8") or {}).get("us_per_query_token"),
+            "sink128_frac": frac("decode_long_g4_2bit_sink128"),
             "target": "north_star: decode >= 0.70 of HBM on every config, quantize >= 0.60 of HBM (ALU-bound: DESIGN 6.1)"}
     rl_dec = {"kernel": "decode_kernel<2,4,2,bf16> (configs[1])", "bound": "hbm", "achieved": dec_gbs, "peak": hbm_peak,
               "unit": "GB/s", "frac": dec_gbs / hbm_peak, "traffic": tr.get("decode_kernel"),
